@@ -1,0 +1,439 @@
+"""Pins of the CPU oracle (oracle/pwa_oracle.c) against what the paper and mathematics fix.
+
+No GPU.  The paper prints no worked numbers (P0), so each pin is a closed form, an
+invariant, an exact-rational brute force, or a reduction to a numpy/BLAS routine, chosen so
+that a dropped term, wrong sign/conjugation, factor 2 or transposed index fails one of them.
+Pin numbers follow SURVEY.md section 8(c) / DESIGN.md section 5.
+P:n = /root/reference/PAPER.md line n (cited, never read at run time).
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def cplx(x):
+    x = np.asarray(x)
+    return x[..., 0] + 1j * x[..., 1]
+
+
+def ri(z):
+    z = np.asarray(z)
+    return np.ascontiguousarray(np.stack([z.real, z.imag], axis=-1))
+
+
+def rand_amps(rng, N, n, scale=0.35):
+    return rng.normal(size=(N, n, 2)) * scale
+
+
+def full_eval(oracle, A, B, n_gen, V):
+    M = oracle.norm_matrix(B, n_gen)
+    return oracle.nll_grad(A, M, V), M
+
+
+# ---------------------------------------------------------------- P0 / storage remark
+def test_paper_storage_remark():
+    """n^2 fp32 reals per event: 1e6 * 20^2 * 4 B = 1.49 GiB ~ '1.5 GB'."""
+    kv = {}
+    for line in open(os.path.join(GOLD, "paper_storage_remark.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        kv[k] = float(v)
+    gib = kv["events"] * kv["waves"] ** 2 * kv["bytes_per_real"] / 2 ** 30
+    assert abs(gib - kv["quoted_gib"]) < 0.05
+    # the streamed N x n complex matrix of this build is n/2 times smaller in fp32
+    assert kv["events"] * kv["waves"] * 8 * (kv["waves"] / 2) == kv["events"] * kv["waves"] ** 2 * 4
+
+
+# ---------------------------------------------------------------- P1 single-wave closed form
+def test_p1_single_wave_constant_amplitudes(oracle):
+    N, Nacc, Ngen = 1000, 700, 1000
+    A = np.zeros((N, 1, 2)); A[..., 0] = 1.0
+    B = np.zeros((Nacc, 1, 2)); B[..., 0] = 1.0
+    V = np.array([[0.8, -1.3]])
+    (nll, g, parts, bad), M = full_eval(oracle, A, B, Ngen, V)
+    v2 = 0.8 ** 2 + 1.3 ** 2
+    lnL = N * math.log(v2) - v2 * Nacc / Ngen
+    assert bad == 0
+    assert nll == pytest.approx(-lnL, rel=1e-15)
+    assert cplx(M)[0, 0] == pytest.approx(Nacc / Ngen, rel=1e-15)
+    gexp = -2 * N * cplx(V)[0] / v2 + 2 * (Nacc / Ngen) * cplx(V)[0]
+    assert cplx(g)[0] == pytest.approx(gexp, rel=1e-14)
+    # stationary point of eq. 3 at |V|^2 = N / M11 (P7 corollary): gradient vanishes there
+    Vs = np.array([[math.sqrt(N / (Nacc / Ngen)), 0.0]])
+    nll_s, g_s, parts_s, _ = oracle.nll_grad(A, M, Vs)
+    assert np.abs(g_s).max() < 1e-10
+    assert parts_s[1] == pytest.approx(N, rel=1e-14)
+
+
+def test_p1_single_wave_random_amplitudes(oracle):
+    rng = np.random.default_rng(11)
+    N, Nacc, Ngen = 513, 901, 1300
+    A, B = rand_amps(rng, N, 1), rand_amps(rng, Nacc, 1)
+    V = np.array([[-0.4, 0.9]])
+    (nll, g, parts, _), M = full_eval(oracle, A, B, Ngen, V)
+    v2 = float(np.abs(cplx(V)[0]) ** 2)
+    M11 = float((np.abs(cplx(B)[:, 0]) ** 2).sum() / Ngen)
+    lnL = N * math.log(v2) + float(np.log(np.abs(cplx(A)[:, 0]) ** 2).sum()) - v2 * M11
+    assert nll == pytest.approx(-lnL, rel=1e-13)
+    gexp = -2 * N * cplx(V)[0] / v2 + 2 * M11 * cplx(V)[0]
+    assert cplx(g)[0] == pytest.approx(gexp, rel=1e-12)
+
+
+# ---------------------------------------------------------------- P2 global phase
+def test_p2_global_phase(oracle):
+    rng = np.random.default_rng(2)
+    n = 5
+    A, B = rand_amps(rng, 400, n), rand_amps(rng, 700, n)
+    V = rng.normal(size=(n, 2))
+    (nll, g, parts, _), M = full_eval(oracle, A, B, 900, V)
+    for th in (0.3, 1.7, math.pi):
+        Vr = ri(np.exp(1j * th) * cplx(V))
+        nll2, g2, parts2, _ = oracle.nll_grad(A, M, Vr)
+        assert nll2 == pytest.approx(nll, rel=1e-13)
+        assert np.allclose(cplx(g2), np.exp(1j * th) * cplx(g), rtol=1e-11, atol=1e-11 * np.abs(g).max())
+    # infinitesimal form, separately for data and norm terms: Im(V^H g) = 0
+    L, T, _ = oracle.data_term(A, V)
+    g_data = 2 * np.conj(cplx(T))
+    Nv, gN = oracle.norm_explicit(B, 900, V)
+    Vc = cplx(V)
+    assert abs(np.imag(np.vdot(Vc, g_data))) < 1e-10 * np.abs(g_data).max()
+    assert abs(np.imag(np.vdot(Vc, cplx(gN)))) < 1e-12 * np.abs(gN).max()
+
+
+# ---------------------------------------------------------------- P3 M Hermitian PSD
+def test_p3_norm_matrix_hermitian_psd(oracle):
+    rng = np.random.default_rng(3)
+    n = 6
+    B = rand_amps(rng, 2000, n)
+    M = cplx(oracle.norm_matrix(B, 2500))
+    assert np.allclose(M, M.conj().T, rtol=0, atol=1e-16)
+    assert np.all(M.diagonal().real >= 0) and np.abs(M.diagonal().imag).max() == 0.0
+    ev = np.linalg.eigvalsh(M)
+    assert ev.min() >= -1e-13 * np.trace(M).real
+    for _ in range(5):
+        x = rng.normal(size=n) + 1j * rng.normal(size=n)
+        assert np.vdot(x, M @ x).real >= 0
+
+
+# ---------------------------------------------------------------- P4 M <-> explicit MC sum (C1)
+def test_p4_norm_index_convention(oracle):
+    rng = np.random.default_rng(4)
+    n, Ngen = 4, 1234
+    B = rand_amps(rng, 1000, n)
+    V = rng.normal(size=(n, 2))
+    M = cplx(oracle.norm_matrix(B, Ngen))
+    Vc = cplx(V)
+    Nprime, gN = oracle.norm_explicit(B, Ngen, V)
+    # independent third opinion of the explicit sum
+    Nnp = float((np.abs(cplx(B) @ Vc) ** 2).sum() / Ngen)
+    assert Nprime == pytest.approx(Nnp, rel=1e-13)
+    assert np.vdot(Vc, M @ Vc).real == pytest.approx(Nprime, rel=1e-13)
+    assert np.allclose(2 * M @ Vc, cplx(gN), rtol=1e-12)
+    # the transposed pairing V^T M conj(V) (eq. 3's bracket read literally, C1) is a different number
+    wrong = (Vc @ M @ Vc.conj()).real
+    assert abs(wrong - Nprime) > 1e-3 * abs(Nprime)
+    # assemble() uses the same convention
+    nll, g, parts = oracle.assemble(0.0, np.zeros((n, 2)), ri(M), V)
+    assert parts[1] == pytest.approx(Nprime, rel=1e-13)
+    assert np.allclose(cplx(g), cplx(gN), rtol=1e-12)
+
+
+# ---------------------------------------------------------------- P5 gradient vs differences
+@pytest.mark.parametrize("n", [1, 3, 8])
+def test_p5_gradient_central_differences(oracle, n):
+    rng = np.random.default_rng(50 + n)
+    A, B = rand_amps(rng, 300, n), rand_amps(rng, 500, n)
+    V = rng.normal(size=(n, 2))
+    (nll, g, parts, _), M = full_eval(oracle, A, B, 800, V)
+    num = np.zeros_like(V)
+    for a in range(n):
+        for c in range(2):
+            h = 1e-6 * max(1.0, abs(V[a, c]))
+            Vp, Vm = V.copy(), V.copy()
+            Vp[a, c] += h; Vm[a, c] -= h
+            fp = oracle.nll_grad(A, M, Vp)[0]
+            fm = oracle.nll_grad(A, M, Vm)[0]
+            num[a, c] = (fp - fm) / (2 * h)
+    assert np.abs(num - g).max() <= 2e-8 * np.abs(g).max()
+
+
+# ---------------------------------------------------------------- P6 + brute force (exact rationals)
+def _load_tiny():
+    A, V, ngen = [], None, None
+    for line in open(os.path.join(GOLD, "tiny_dyadic_case.txt")):
+        t = line.split()
+        if not t or t[0].startswith("#"):
+            continue
+        if t[0] == "A":
+            A.append([float(x) for x in t[1:]])
+        elif t[0] == "V":
+            V = [float(x) for x in t[1:]]
+        elif t[0] == "NGEN":
+            ngen = int(t[1])
+    return np.array(A).reshape(3, 2, 2), np.array(V).reshape(2, 2), ngen
+
+
+def _fc(re, im):
+    return (Fraction(re), Fraction(im))
+
+
+def _fmul(x, y):
+    return (x[0] * y[0] - x[1] * y[1], x[0] * y[1] + x[1] * y[0])
+
+
+def _fconj(x):
+    return (x[0], -x[1])
+
+
+def test_p6_eq1_equals_eq3_and_exact_bruteforce(oracle):
+    """eq. 1 == eq. 3's double sum with zero imaginary part, checked in exact
+    rational arithmetic; L_data, T, M, Norm, gradient brute-forced from the definitions."""
+    A, V, ngen = _load_tiny()
+    N, n = A.shape[0], A.shape[1]
+    Af = [[_fc(A[i, a, 0], A[i, a, 1]) for a in range(n)] for i in range(N)]
+    Vf = [_fc(V[a, 0], V[a, 1]) for a in range(n)]
+    L_exact, T_exact = 0.0, [(Fraction(0), Fraction(0)) for _ in range(n)]
+    for i in range(N):
+        S = (Fraction(0), Fraction(0))
+        for a in range(n):
+            p = _fmul(Vf[a], Af[i][a]); S = (S[0] + p[0], S[1] + p[1])
+        I1 = S[0] ** 2 + S[1] ** 2
+        dbl = (Fraction(0), Fraction(0))
+        for a in range(n):
+            for b in range(n):
+                t = _fmul(_fmul(Vf[a], _fconj(Vf[b])), _fmul(Af[i][a], _fconj(Af[i][b])))
+                dbl = (dbl[0] + t[0], dbl[1] + t[1])
+        assert dbl[1] == 0 and dbl[0] == I1                    # exact identity
+        # oracle's two forms (all products exact in binary floating point for this fixture)
+        assert oracle.intensity_eq1(A[i], V) == float(I1)
+        e3 = oracle.intensity_eq3(A[i], V)
+        assert e3.real == float(I1) and e3.imag == 0.0
+        L_exact += math.log(float(I1))
+        for a in range(n):   # A/S = A conj(S)/I
+            q = _fmul(Af[i][a], _fconj(S))
+            T_exact[a] = (T_exact[a][0] + q[0] / I1, T_exact[a][1] + q[1] / I1)
+    L, T, bad = oracle.data_term(A, V)
+    assert bad == 0 and L == pytest.approx(L_exact, rel=1e-15)
+    for a in range(n):
+        assert T[a, 0] == pytest.approx(float(T_exact[a][0]), rel=1e-15)
+        assert T[a, 1] == pytest.approx(float(T_exact[a][1]), rel=1e-15)
+    # use the same 3 events as "MC": M_ab = sum_j conj(B_ja) B_jb / ngen exactly
+    M = oracle.norm_matrix(A, ngen)
+    for a in range(n):
+        for b in range(n):
+            acc = (Fraction(0), Fraction(0))
+            for j in range(N):
+                t = _fmul(_fconj(Af[j][a]), Af[j][b]); acc = (acc[0] + t[0], acc[1] + t[1])
+            assert M[a, b, 0] == float(acc[0] / ngen) and M[a, b, 1] == float(acc[1] / ngen)
+    # Norm = (1/ngen) sum_j |S_j|^2 exactly, gradient = -2 conj(T) + (2/ngen) sum_j conj(B_ja) S_j
+    Nx = Fraction(0)
+    gN = [(Fraction(0), Fraction(0)) for _ in range(n)]
+    for j in range(N):
+        S = (Fraction(0), Fraction(0))
+        for a in range(n):
+            p = _fmul(Vf[a], Af[j][a]); S = (S[0] + p[0], S[1] + p[1])
+        Nx += S[0] ** 2 + S[1] ** 2
+        for a in range(n):
+            t = _fmul(_fconj(Af[j][a]), S); gN[a] = (gN[a][0] + 2 * t[0] / ngen, gN[a][1] + 2 * t[1] / ngen)
+    nll, g, parts, _ = oracle.nll_grad(A, M, V)
+    assert parts[1] == pytest.approx(float(Nx / ngen), rel=1e-15)
+    assert nll == pytest.approx(-(L_exact - float(Nx / ngen)), rel=1e-14)
+    for a in range(n):
+        assert g[a, 0] == pytest.approx(-2 * float(T_exact[a][0]) + float(gN[a][0]), rel=1e-13)
+        assert g[a, 1] == pytest.approx(+2 * float(T_exact[a][1]) + float(gN[a][1]), rel=1e-13)
+
+
+# ---------------------------------------------------------------- P7 Euler / scale identity
+def test_p7_euler_identity(oracle):
+    rng = np.random.default_rng(7)
+    n, N = 7, 1500
+    A, B = rand_amps(rng, N, n), rand_amps(rng, 900, n)
+    V = rng.normal(size=(n, 2))
+    L, T, _ = oracle.data_term(A, V)
+    assert np.sum(cplx(V) * cplx(T)) == pytest.approx(N, rel=1e-13)       # sum_a V_a T_a = N exactly
+    Nv, gN = oracle.norm_explicit(B, 1000, V)
+    assert np.vdot(cplx(V), cplx(gN)).real == pytest.approx(2 * Nv, rel=1e-13)
+    # scaling law: L(sV) = L(V) + N ln s^2 ; Norm(sV) = s^2 Norm(V)
+    s = 1.7
+    L2, _, _ = oracle.data_term(A, s * V)
+    assert L2 == pytest.approx(L + N * math.log(s * s), rel=1e-13)
+    assert oracle.norm_explicit(B, 1000, s * V)[0] == pytest.approx(s * s * Nv, rel=1e-13)
+
+
+# ---------------------------------------------------------------- P8 numpy / BLAS third opinion
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_p8_reduces_to_blas(oracle, dtype):
+    rng = np.random.default_rng(8)
+    n, N, Nacc, Ngen = 12, 3000, 4000, 5000
+    A = rand_amps(rng, N, n).astype(dtype)
+    B = rand_amps(rng, Nacc, n).astype(dtype)
+    V = rng.normal(size=(n, 2))
+    Ac, Bc, Vc = cplx(A.astype(np.float64)), cplx(B.astype(np.float64)), cplx(V)
+    M = oracle.norm_matrix(B, Ngen)
+    assert np.allclose(cplx(M), Bc.conj().T @ Bc / Ngen, rtol=1e-13, atol=1e-15)
+    S = Ac @ Vc
+    L, T, _ = oracle.data_term(A, V)
+    assert L == pytest.approx(np.log(np.abs(S) ** 2).sum(), rel=1e-13)
+    assert np.allclose(cplx(T), (Ac / S[:, None]).sum(0), rtol=1e-12, atol=1e-12 * np.abs(T).max())
+    # batched = loop (step 9)
+    Vk = rng.normal(size=(3, n, 2))
+    nllk, gk, partsk, _ = oracle.nll_grad_batch(A, M, Vk)
+    Sk = Ac @ cplx(Vk).T
+    assert np.allclose(partsk[:, 0], np.log(np.abs(Sk) ** 2).sum(0), rtol=1e-13)
+    for k in range(3):
+        one = oracle.nll_grad(A, M, Vk[k])
+        assert one[0] == nllk[k] and np.array_equal(one[1], gk[k])
+
+
+def test_fp32_storage_is_exact_widening(oracle):
+    """C16: fp32-stored amplitudes are widened exactly; same bits as the widened fp64 array."""
+    rng = np.random.default_rng(16)
+    A32 = rand_amps(rng, 700, 5).astype(np.float32)
+    B32 = rand_amps(rng, 900, 5).astype(np.float32)
+    V = rng.normal(size=(5, 2))
+    M32, M64 = oracle.norm_matrix(B32, 1000), oracle.norm_matrix(B32.astype(np.float64), 1000)
+    assert np.array_equal(M32, M64)
+    r32, r64 = oracle.nll_grad(A32, M32, V), oracle.nll_grad(A32.astype(np.float64), M64, V)
+    assert r32[0] == r64[0] and np.array_equal(r32[1], r64[1])
+
+
+# ---------------------------------------------------------------- P9 structural invariances
+def test_p9_invariances(oracle):
+    rng = np.random.default_rng(9)
+    n, N = 4, 2000
+    A = rand_amps(rng, N, n)
+    V = rng.normal(size=(n, 2))
+    L, T, _ = oracle.data_term(A, V)
+    # permutation
+    perm = rng.permutation(N)
+    Lp, Tp, _ = oracle.data_term(A[perm], V)
+    assert Lp == pytest.approx(L, rel=1e-14) and np.allclose(Tp, T, rtol=1e-12, atol=1e-13)
+    # duplication doubles L and T
+    Ld, Td, _ = oracle.data_term(np.concatenate([A, A]), V)
+    assert Ld == pytest.approx(2 * L, rel=1e-14) and np.allclose(Td, 2 * T, rtol=1e-12, atol=1e-13)
+    # A -> cA: S -> cS, so L + N ln|c|^2 and T = sum A/S is UNCHANGED
+    # (SURVEY.md P9 says 'T/c'; that is a slip: the c cancels in A_ia / S_i)
+    c = 0.7 - 1.9j
+    Lc, Tc, _ = oracle.data_term(ri(c * cplx(A)), V)
+    assert Lc == pytest.approx(L + N * math.log(abs(c) ** 2), rel=1e-13)
+    assert np.allclose(cplx(Tc), cplx(T), rtol=1e-11, atol=1e-12)
+    # two identical columns -> depends on V_0 + V_1 only
+    A2 = A.copy(); A2[:, 1] = A2[:, 0]
+    V2 = V.copy(); V2[0] = V[0] + V[1] - np.array([0.3, -0.2]); V2[1] = np.array([0.3, -0.2])
+    assert oracle.data_term(A2, V2)[0] == pytest.approx(oracle.data_term(A2, V)[0], rel=1e-13)
+    # thread-count independence to rounding
+    from oracle import oracle as o
+    nt = o.threads()
+    o.set_threads(1)
+    L1, T1, _ = o.data_term(A, V)
+    o.set_threads(nt)
+    assert L1 == pytest.approx(L, rel=1e-15) and np.allclose(T1, T, rtol=1e-14, atol=1e-15)
+
+
+# ---------------------------------------------------------------- P10 Breit-Wigner (C3)
+def test_p10_breit_wigner(oracle):
+    M, G = 1.71, 0.14
+    assert oracle.bw(M, M, G) == pytest.approx(1j / (M * G), rel=1e-15)       # pure imaginary on the pole
+    for m in (1.0, 1.6, 1.71, 2.4):
+        bw = oracle.bw(m, M, G)
+        assert bw == pytest.approx(1.0 / (M * M - m * m - 1j * M * G), rel=1e-15)
+        assert abs(bw) ** 2 == pytest.approx(1.0 / ((M * M - m * m) ** 2 + (M * G) ** 2), rel=1e-14)
+    # half maximum of |BW|^2 at m^2 = M^2 +- M G
+    peak = abs(oracle.bw(M, M, G)) ** 2
+    for sgn in (+1, -1):
+        m = math.sqrt(M * M + sgn * M * G)
+        assert abs(oracle.bw(m, M, G)) ** 2 == pytest.approx(peak / 2, rel=1e-13)
+    # derivatives vs central differences
+    for m in (1.2, 1.7, 2.2):
+        dM, dG = oracle.bw_deriv(m, M, G)
+        h = 1e-6
+        nM = (oracle.bw(m, M + h, G) - oracle.bw(m, M - h, G)) / (2 * h)
+        nG = (oracle.bw(m, M, G + h) - oracle.bw(m, M, G - h)) / (2 * h)
+        assert dM == pytest.approx(nM, rel=1e-7) and dG == pytest.approx(nG, rel=1e-7)
+
+
+def test_factored_expansion_matches_generator(oracle, synth):
+    """Oracle step 1 (A = BW * Z, own BW code) vs the generator's own line-shape code."""
+    w = synth.make_workload(3, n_data=2000, n_mc=3000)
+    A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, w.Mr, w.Gr)
+    assert np.allclose(A, w.A_data, rtol=1e-13, atol=1e-15)
+    # explicit complex formula, third opinion
+    m = w.mass_data[:, None]
+    bw = 1.0 / (w.Mr[None, :] ** 2 - m ** 2 - 1j * w.Mr[None, :] * w.Gr[None, :])
+    ref = bw[:, w.res_of_wave] * cplx(w.Z_data)[:, w.ang_of_wave]
+    assert np.allclose(cplx(A), ref, rtol=1e-13, atol=1e-15)
+
+
+def test_res_grad_vs_differences(oracle, synth):
+    """Reading A9: d L_data / d(M_r, G_r) and d Norm / d(M_r, G_r) vs central differences."""
+    w = synth.make_workload(3, n_data=1500, n_mc=2500)
+    V = synth.eval_points(w, 1)[0]
+    Mr, Gr = w.Mr.copy(), w.Gr.copy()
+    dM, dG = oracle.res_grad(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 0)
+    nM, nG = oracle.res_grad(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 1, w.n_gen)
+
+    def L_of(Mx, Gx):
+        A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mx, Gx)
+        return oracle.data_term(A, V)[0]
+
+    def N_of(Mx, Gx):
+        B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mx, Gx)
+        return oracle.norm_explicit(B, w.n_gen, V)[0]
+
+    h = 1e-6
+    for r in range(w.n_res):
+        for which, (aL, aN) in enumerate(((dM, nM), (dG, nG))):
+            P, Q = (Mr.copy(), Gr.copy()), (Mr.copy(), Gr.copy())
+            P[which][r] += h; Q[which][r] -= h
+            numL = (L_of(*P) - L_of(*Q)) / (2 * h)
+            numN = (N_of(*P) - N_of(*Q)) / (2 * h)
+            assert aL[r] == pytest.approx(numL, rel=2e-6, abs=1e-6 * np.abs(dM).max())
+            assert aN[r] == pytest.approx(numN, rel=2e-6, abs=1e-6 * max(np.abs(nM).max(), 1e-12))
+
+
+# ---------------------------------------------------------------- C14 non-finite propagation
+def test_c14_zero_intensity(oracle):
+    A = np.zeros((3, 2, 2)); A[0, 0, 0] = 1.0; A[2, 1, 1] = 0.5     # event 1 has S = 0
+    V = np.array([[1.0, 0.0], [0.0, 1.0]])
+    L, T, bad = oracle.data_term(A, V)
+    assert bad == 1 and L == -math.inf
+
+
+# ---------------------------------------------------------------- configs 0/1 sanity (P11, P12-lite)
+def test_cfg0_sanity_and_orthogonality(oracle, synth):
+    w = synth.make_workload(0)
+    assert w.n == 4 and w.n_gen == w.n_acc == 50_000 and w.n_over == 0
+    # P11: over a flat full-acceptance MC, 4 pi <conj(Z^s) Z^s'> -> delta_ss'
+    Z = cplx(synth.angular(w, w.kin_mc))
+    G = 4 * math.pi * (Z.conj().T @ Z) / Z.shape[0]
+    assert np.abs(G - np.eye(3)).max() < 5.0 / math.sqrt(Z.shape[0])
+    M = oracle.norm_matrix(w.A_mc, w.n_gen)
+    nll, g, parts, bad = oracle.nll_grad(w.A_data, M, w.V_true)
+    assert bad == 0 and np.isfinite(nll)
+    # the data were generated from V_true: lnL at truth beats a random point after optimal rescaling
+    # (scale-profiled: max_s lnL(sV) = L - N ln(Norm/N) - N), P7
+    def profiled(V):
+        _, _, p, _ = oracle.nll_grad(w.A_data, M, V)
+        return p[0] - w.n_data * math.log(p[1] / w.n_data) - w.n_data
+    assert profiled(w.V_true) > profiled(synth.eval_points(w, 1)[0])
+
+
+def test_cfg1_generator_recipe(synth):
+    w = synth.make_workload(1, n_data=20_000, n_mc=50_000)
+    assert w.n == 16 and w.n_res == 8 and w.storage == "f64"
+    assert 1.2 <= w.Mr.min() and w.Mr.max() <= 2.8 and 0.05 <= w.Gr.min() and w.Gr.max() <= 0.3
+    assert abs(w.n_acc / w.n_gen - 0.7) < 0.01            # C9: mean efficiency 0.700
+    m, c, p = w.kin_mc
+    assert m.min() >= 0.988 and m.max() <= 3.0 and abs(c).max() <= 1 and 0 <= p.min() and p.max() < 2 * math.pi
+    # determinism / order independence of the counter-based RNG
+    w2 = synth.make_workload(1, n_data=20_000, n_mc=50_000)
+    assert np.array_equal(w.A_data, w2.A_data) and w.n_gen == w2.n_gen
+    # a shorter request is a prefix of a longer one
+    w3 = synth.make_workload(1, n_data=5_000, n_mc=10_000)
+    assert np.array_equal(w3.A_data, w.A_data[:5000]) and np.array_equal(w3.A_mc, w.A_mc[:10000])

@@ -1,0 +1,185 @@
+/*
+ * pwa.h — C ABI of libpwa.so: the per-iteration extended log-likelihood and gradient of an
+ * unbinned partial-wave-analysis fit (arXiv 1108.5882, N. Berger, "Partial Wave Analysis
+ * using Graphics Cards"), computed on one NVIDIA B200 (sm_100a).
+ *
+ * Citations: "P:n" = line n of the paper text; "C<k>" = reading k in DESIGN.md
+ * section 3 (where the paper is silent).  Notation:
+ *   n waves (index a), N data events (i), N_acc accepted MC events (j), N_gen generated MC;
+ *   A[i][a] = A_a(Omega_i), B[j][a] = A_a(Omega_j);  V_a = x_a + i y_a;
+ *   S_i = sum_a V_a A_ia,  I_i = |S_i|^2                                  (eq. 1)
+ *   L_data = sum_i ln I_i                                                  (eq. 3 first term)
+ *   Norm   = (1/N_gen) sum_j |sum_a V_a B_ja|^2 = V^H M V,  M = B^H B / N_gen   (eq. 3 second term; C1)
+ *   nll    = -(L_data - Norm)                                              (P:55 fn. 3)
+ *   T_a    = sum_i A_ia / S_i;   grad_a = d nll/d x_a + i d nll/d y_a = -2 conj(T_a) + 2 (M V)_a   (C6)
+ *
+ * General rules.  All symbols are extern "C"; no exception, abort() or stdout output
+ * crosses the ABI.  Every call returns a pwa_status; on PWA_ERR_* the outputs are
+ * untouched and pwa_last_error() describes the failure.  The library never frees or keeps
+ * caller memory except as stated for PWA_BORROW.  One context = one CUDA stream = one host
+ * thread at a time.  All scratch is owned by the context and allocated at create / upload
+ * time, never inside an evaluation call.  There is no CPU fallback: without a CUDA device
+ * pwa_create fails with PWA_ERR_CUDA.
+ *
+ * Pointer kinds are stated per argument: HOST = ordinary host memory, DEVICE = CUDA device
+ * memory of the context's device, ANY = either (detected with cudaPointerGetAttributes).
+ * Complex numbers are interleaved (re, im).  Matrices are row-major.
+ */
+#ifndef PWA_H_
+#define PWA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pwa_ctx pwa_ctx; /* opaque, library-owned */
+
+typedef enum {
+    PWA_OK = 0,
+    PWA_ERR_INVALID_ARG = 1,
+    PWA_ERR_STATE = 2,        /* call order wrong: data not uploaded, M missing or stale, ... */
+    PWA_ERR_OOM = 3,
+    PWA_ERR_CUDA = 4,
+    PWA_ERR_UNSUPPORTED = 5,
+    PWA_WARN_NONFINITE = 6    /* results written, but some I_i was 0 or non-finite (C14) */
+} pwa_status;
+
+typedef enum { PWA_F64 = 0, PWA_F32 = 1 } pwa_dtype;   /* amplitude STORAGE type (C16) */
+typedef enum { PWA_DATA = 0, PWA_MC = 1 } pwa_sample;
+
+#define PWA_COPY   0u   /* library copies the events into its own device buffer (default) */
+#define PWA_BORROW 1u   /* DEVICE pointer in native layout is used in place; caller keeps it
+                           alive and unchanged until the next upload of that sample or destroy */
+
+/* ---- life cycle ----------------------------------------------------------------------- */
+
+/* n_waves >= 1.  storage: element type of every amplitude array given to this context
+ * (arithmetic and accumulation are always fp64).  device: CUDA ordinal.
+ * cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for
+ * the legacy default stream.  All work of the context is enqueued on that stream.       */
+pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t device,
+                      void *cuda_stream);
+void pwa_destroy(pwa_ctx *ctx);                       /* NULL-safe; frees library memory only */
+const char *pwa_last_error(const pwa_ctx *ctx);       /* ctx-owned string, valid until next call */
+const char *pwa_status_string(pwa_status s);          /* static string */
+
+/* ---- event upload --------------------------------------------------------------------- */
+
+/* Constant-resonance mode (amplitudes pre-calculated once per fit).
+ * amps: ANY pointer, row-major [n_events][n_waves] complex, element type = ctx storage.
+ * n_generated: N_gen of eq. 3, used for which == PWA_MC only and must then be
+ * >= n_events (C9); ignored for PWA_DATA.  n_events may be 0.
+ * flags: PWA_COPY or PWA_BORROW (BORROW requires a DEVICE pointer, 16-byte aligned).
+ * Uploading PWA_MC marks M stale.                                                        */
+pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps,
+                             int64_t n_events, int64_t n_generated, uint32_t flags);
+
+/* Floating-resonance mode (when masses/widths float nothing can be pre-calculated):
+ *   A_ia = BW(mass_i; M_r(a), G_r(a)) * ang[i][s(a)],  BW(m; M, G) = 1/(M^2 - m^2 - i M G)  (C3)
+ * and the Breit-Wigner factors are recomputed inside every kernel that reads the sample.
+ * mass: ANY, [n_events] doubles (always fp64).  ang: ANY, [n_events][n_ang] complex of the
+ * ctx storage type.  1 <= n_ang <= 4.  Needs pwa_set_wave_map + pwa_set_resonances before
+ * any evaluation.                                                                        */
+pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const double *mass,
+                                      const void *ang, int32_t n_ang, int64_t n_events,
+                                      int64_t n_generated, uint32_t flags);
+
+/* res_of_wave[a] in [0, n_res), ang_of_wave[a] in [0, n_ang): HOST int32 [n_waves].
+ * 1 <= n_res <= 64.  Each (resonance, angular structure) pair may belong to at most one
+ * wave.                                                                                   */
+pwa_status pwa_set_wave_map(pwa_ctx *ctx, int32_t n_res, const int32_t *res_of_wave,
+                            const int32_t *ang_of_wave);
+
+/* mass0, width0: HOST [n_res] doubles (GeV).  Marks M stale (it must be rebuilt).  */
+pwa_status pwa_set_resonances(pwa_ctx *ctx, const double *mass0, const double *width0);
+
+/* ---- normalisation matrix (P:41 inner bracket) ----------------------------------- */
+
+/* Builds M = B^H B / N_gen over the uploaded MC sample (Breit-Wigner fused in factored
+ * mode) and keeps it on the device for the evaluation calls.  M_out: optional HOST buffer
+ * [n][n][2] doubles, M_out[a][b] = M_ab = (1/N_gen) sum_j conj(B_ja) B_jb (C1); may be NULL.
+ * Synchronous when M_out != NULL.  PWA_ERR_STATE if no MC sample was uploaded.           */
+pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out);
+
+/* Installs an externally computed M (HOST [n][n][2]), e.g. the sum over ranks of per-shard
+ * matrices in an event-sharded multi-GPU run.                                      */
+pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M);
+
+/* ---- evaluation: the per-iteration hot path -------------------------------------------- */
+
+/* V: HOST [n][2] doubles.  Outputs (HOST): *nll = -(L_data - V^H M V);
+ * grad[n][2] = (d nll / d Re V_a, d nll / d Im V_a);  parts (may be NULL): [0] = L_data,
+ * [1] = Norm.  One pass over the data amplitudes in HBM; synchronous (returns after the
+ * results are in host memory).  PWA_ERR_STATE if DATA is missing or M is missing / stale.
+ * PWA_WARN_NONFINITE if some I_i was 0 or not finite (IEEE values are still written).     */
+pwa_status pwa_nll_grad(pwa_ctx *ctx, const double *V, double *nll, double *grad,
+                        double *parts);
+
+/* K starting points in one pass over the data.  V: HOST [K][n][2];
+ * nll: [K]; grad: [K][n][2]; parts: [K][2] or NULL.  Column k equals pwa_nll_grad(V_k)
+ * to floating-point tolerance (not necessarily bitwise).  1 <= K <= 1024.                */
+pwa_status pwa_nll_grad_batch(pwa_ctx *ctx, int32_t K, const double *V, double *nll,
+                              double *grad, double *parts);
+
+/* Asynchronous pair: enqueue one evaluation (V is copied before return) / wait and fetch
+ * the results of the most recent enqueue.  Used for device-side timing.                  */
+pwa_status pwa_nll_grad_enqueue(pwa_ctx *ctx, const double *V);
+pwa_status pwa_nll_grad_batch_enqueue(pwa_ctx *ctx, int32_t K, const double *V);
+pwa_status pwa_fetch(pwa_ctx *ctx, int32_t K, double *nll, double *grad, double *parts);
+
+/* Data term only, for event-sharded multi-GPU runs ("treat different subsets of
+ * events on different ... machines ... then ... perform a synthesis"): enqueues one pass
+ * and writes out_dev (DEVICE, [2 + 2n] doubles) = { L_data, n_nonfinite, Re T_0, Im T_0,
+ * ... } of THIS context's events.  The caller sums out_dev over ranks and finishes with
+ * pwa_assemble_host.  Asynchronous.                                                      */
+pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev);
+
+/* Host-only step A7: Norm = V^H M V, nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V.
+ * All pointers HOST; T [n][2], M [n][n][2], V [n][2]; parts [2] or NULL.  No GPU needed. */
+pwa_status pwa_assemble_host(int32_t n_waves, double L_data, const double *T, const double *M,
+                             const double *V, double *nll, double *grad, double *parts);
+
+/* Floating mode: gradient of nll w.r.t. the resonance parameters at the current
+ * (mass0, width0) and the given V (reading A9):  d nll / d M_r and d nll / d G_r, HOST
+ * [n_res] each.  Needs factored DATA and MC uploads.  One extra pass over data and MC.   */
+pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dnll_dmass, double *dnll_dwidth);
+
+/* ---- host minimiser (a quasi-Newton in real parameters stays on the host) --- */
+
+/* Plain BFGS with backtracking line search on the 2n reals of V (constant-resonance mode).
+ * V_inout: HOST [n][2], start in / result out.  Stops after max_iter iterations or when
+ * max|grad| < gtol.  n_evals_out / nll_out may be NULL.                                  */
+pwa_status pwa_minimize_bfgs(pwa_ctx *ctx, double *V_inout, int32_t max_iter, double gtol,
+                             double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out);
+
+/* K independent BFGS fits run in lock-step on pwa_nll_grad_batch.  V_inout [K][n][2].    */
+pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V_inout, int32_t max_iter,
+                                   double gtol, double *nll_out /* [K] */,
+                                   int32_t *n_evals_out);
+
+/* ---- introspection / measurement ------------------------------------------------------- */
+
+/* n_waves the context was created with.                                                  */
+int32_t pwa_n_waves(const pwa_ctx *ctx);
+
+/* Number of CUDA kernels this context has launched since creation.                        */
+uint64_t pwa_launch_count(const pwa_ctx *ctx);
+
+/* Waits for all enqueued work of the context.                                             */
+pwa_status pwa_sync(pwa_ctx *ctx);
+
+/* Selects a kernel variant for experiments (0 = default).  Returns PWA_ERR_INVALID_ARG for
+ * unknown keys.  Keys: "data_term", "norm", "batch".                                      */
+pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
+
+/* Register-resident peak probes used as roofline denominators:
+ * which = 0: fp64 FMA (result TFLOP/s), 1: fp64 mma.sync m8n8k4 (TFLOP/s),
+ * 2: HBM read-only stream over `bytes` of scratch (GB/s).  Synchronous; result HOST.     */
+pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PWA_H_ */

@@ -1,0 +1,299 @@
+"""Thin ctypes binding of include/pwa.h — argument marshalling only.
+
+Every step of the hot path runs inside libpwa.so's CUDA kernels; there is no Python or CPU
+fallback: if the shared library is missing, import of this module raises, and if no CUDA
+device is present pwa_create raises PwaError(PWA_ERR_CUDA).
+
+Functions carry the same names as the C entry points.  Amplitude arrays are numpy arrays
+(host) of shape [N, n, 2] or torch CUDA tensors / raw device pointers (device); V is a
+float64 numpy array [n, 2] (or [K, n, 2] for the batched call).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libpwa.so")
+
+PWA_OK, PWA_ERR_INVALID_ARG, PWA_ERR_STATE, PWA_ERR_OOM, PWA_ERR_CUDA, PWA_ERR_UNSUPPORTED, \
+    PWA_WARN_NONFINITE = range(7)
+PWA_F64, PWA_F32 = 0, 1
+PWA_DATA, PWA_MC = 0, 1
+PWA_COPY, PWA_BORROW = 0, 1
+
+SYMBOLS = [
+    "pwa_create", "pwa_destroy", "pwa_last_error", "pwa_status_string", "pwa_upload_events",
+    "pwa_upload_events_factored", "pwa_set_wave_map", "pwa_set_resonances", "pwa_build_norm",
+    "pwa_set_norm", "pwa_nll_grad", "pwa_nll_grad_batch", "pwa_nll_grad_enqueue",
+    "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
+    "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
+    "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench",
+]
+
+
+class PwaError(RuntimeError):
+    def __init__(self, status, msg=""):
+        self.status = int(status)
+        super().__init__(f"{_status_name(status)}: {msg}")
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} not found: build it with `python -m paper_1108_5882_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, u32, dp = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.POINTER(C.c_double)
+    sig = {
+        "pwa_create": (C.c_int, [C.POINTER(vp), i32, C.c_int, i32, vp]),
+        "pwa_destroy": (None, [vp]),
+        "pwa_last_error": (C.c_char_p, [vp]),
+        "pwa_status_string": (C.c_char_p, [C.c_int]),
+        "pwa_upload_events": (C.c_int, [vp, C.c_int, vp, i64, i64, u32]),
+        "pwa_upload_events_factored": (C.c_int, [vp, C.c_int, vp, vp, i32, i64, i64, u32]),
+        "pwa_set_wave_map": (C.c_int, [vp, i32, vp, vp]),
+        "pwa_set_resonances": (C.c_int, [vp, vp, vp]),
+        "pwa_build_norm": (C.c_int, [vp, vp]),
+        "pwa_set_norm": (C.c_int, [vp, vp]),
+        "pwa_nll_grad": (C.c_int, [vp, vp, dp, vp, vp]),
+        "pwa_nll_grad_batch": (C.c_int, [vp, i32, vp, vp, vp, vp]),
+        "pwa_nll_grad_enqueue": (C.c_int, [vp, vp]),
+        "pwa_nll_grad_batch_enqueue": (C.c_int, [vp, i32, vp]),
+        "pwa_fetch": (C.c_int, [vp, i32, vp, vp, vp]),
+        "pwa_data_term_enqueue": (C.c_int, [vp, vp, vp]),
+        "pwa_assemble_host": (C.c_int, [i32, C.c_double, vp, vp, vp, dp, vp, vp]),
+        "pwa_res_grad": (C.c_int, [vp, vp, vp, vp]),
+        "pwa_minimize_bfgs": (C.c_int, [vp, vp, i32, C.c_double, dp, C.POINTER(i32), C.POINTER(i32)]),
+        "pwa_minimize_bfgs_batch": (C.c_int, [vp, i32, vp, i32, C.c_double, vp, C.POINTER(i32)]),
+        "pwa_n_waves": (i32, [vp]),
+        "pwa_launch_count": (C.c_uint64, [vp]),
+        "pwa_sync": (C.c_int, [vp]),
+        "pwa_set_option": (C.c_int, [vp, C.c_char_p, i32]),
+        "pwa_microbench": (C.c_int, [vp, i32, i64, dp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)          # AttributeError here = header/library mismatch
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+_lib = _load()
+
+
+def _status_name(s):
+    return _lib.pwa_status_string(int(s)).decode()
+
+
+def _check(ctx, status, allow_warn=True):
+    status = int(status)
+    if status == PWA_OK or (allow_warn and status == PWA_WARN_NONFINITE):
+        return status
+    msg = _lib.pwa_last_error(ctx).decode() if ctx else ""
+    raise PwaError(status, msg)
+
+
+def _ptr_and_keep(x):
+    """-> (address, keepalive, dtype_code or None). numpy -> host ptr; torch tensor / int -> device ptr."""
+    if x is None:
+        return None, None, None
+    if isinstance(x, int):
+        return x, None, None
+    if isinstance(x, np.ndarray):
+        x = np.ascontiguousarray(x)
+        return x.ctypes.data, x, (PWA_F32 if x.dtype == np.float32 else PWA_F64 if x.dtype == np.float64 else None)
+    if hasattr(x, "data_ptr"):   # torch tensor (device or pinned host)
+        if not x.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        code = {"torch.float32": PWA_F32, "torch.float64": PWA_F64}.get(str(x.dtype))
+        return x.data_ptr(), x, code
+    raise TypeError(f"unsupported buffer type {type(x)}")
+
+
+def _f64(x, shape=None):
+    a = np.ascontiguousarray(x, dtype=np.float64)
+    if shape is not None and tuple(a.shape) != tuple(shape):
+        raise ValueError(f"expected shape {shape}, got {a.shape}")
+    return a
+
+
+def pwa_create(n_waves, storage, device=0, cuda_stream=0):
+    """storage: PWA_F64 / PWA_F32 or 'f64' / 'f32'.  Returns an opaque context handle."""
+    if isinstance(storage, str):
+        storage = {"f64": PWA_F64, "f32": PWA_F32}[storage]
+    ctx = C.c_void_p()
+    st = _lib.pwa_create(C.byref(ctx), int(n_waves), int(storage), int(device), C.c_void_p(int(cuda_stream) or None))
+    if st != PWA_OK:
+        raise PwaError(st, "pwa_create failed (no CUDA device, bad arguments or out of memory)")
+    return ctx
+
+
+def pwa_destroy(ctx):
+    _lib.pwa_destroy(ctx)
+
+
+def pwa_upload_events(ctx, which, amps, n_events=None, n_generated=0, flags=PWA_COPY):
+    ptr, keep, _ = _ptr_and_keep(amps)
+    if n_events is None:
+        n_events = amps.shape[0]
+    _check(ctx, _lib.pwa_upload_events(ctx, int(which), C.c_void_p(ptr), int(n_events), int(n_generated), int(flags)))
+    return keep
+
+
+def pwa_upload_events_factored(ctx, which, mass, ang, n_ang=None, n_events=None, n_generated=0, flags=PWA_COPY):
+    pm, km, _ = _ptr_and_keep(mass)
+    pa, ka, _ = _ptr_and_keep(ang)
+    if n_events is None:
+        n_events = ang.shape[0]
+    if n_ang is None:
+        n_ang = ang.shape[1]
+    _check(ctx, _lib.pwa_upload_events_factored(ctx, int(which), C.c_void_p(pm), C.c_void_p(pa), int(n_ang),
+                                                int(n_events), int(n_generated), int(flags)))
+    return km, ka
+
+
+def pwa_set_wave_map(ctx, n_res, res_of_wave, ang_of_wave):
+    r = np.ascontiguousarray(res_of_wave, dtype=np.int32)
+    a = np.ascontiguousarray(ang_of_wave, dtype=np.int32)
+    _check(ctx, _lib.pwa_set_wave_map(ctx, int(n_res), r.ctypes.data, a.ctypes.data))
+
+
+def pwa_set_resonances(ctx, mass0, width0):
+    m, w = _f64(mass0), _f64(width0)
+    _check(ctx, _lib.pwa_set_resonances(ctx, m.ctypes.data, w.ctypes.data))
+
+
+def pwa_build_norm(ctx, want_M=True):
+    n = _lib.pwa_n_waves(ctx)
+    if not want_M:
+        _check(ctx, _lib.pwa_build_norm(ctx, None))
+        return None
+    M = np.empty((n, n, 2))
+    _check(ctx, _lib.pwa_build_norm(ctx, M.ctypes.data))
+    return M
+
+
+def pwa_set_norm(ctx, M):
+    n = _lib.pwa_n_waves(ctx)
+    M = _f64(M, (n, n, 2))
+    _check(ctx, _lib.pwa_set_norm(ctx, M.ctypes.data))
+
+
+def pwa_nll_grad(ctx, V, want_status=False):
+    """-> (nll, grad[n, 2], parts[2]) (+ status when want_status)."""
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V, (n, 2))
+    nll = C.c_double(0.0)
+    grad, parts = np.empty((n, 2)), np.empty(2)
+    st = _check(ctx, _lib.pwa_nll_grad(ctx, V.ctypes.data, C.byref(nll), grad.ctypes.data, parts.ctypes.data))
+    return (nll.value, grad, parts, st) if want_status else (nll.value, grad, parts)
+
+
+def pwa_nll_grad_batch(ctx, V, want_status=False):
+    """V [K, n, 2] -> (nll[K], grad[K, n, 2], parts[K, 2])."""
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V)
+    K = V.shape[0]
+    if V.shape != (K, n, 2):
+        raise ValueError("V must be [K, n, 2]")
+    nll, grad, parts = np.empty(K), np.empty((K, n, 2)), np.empty((K, 2))
+    st = _check(ctx, _lib.pwa_nll_grad_batch(ctx, K, V.ctypes.data, nll.ctypes.data, grad.ctypes.data, parts.ctypes.data))
+    return (nll, grad, parts, st) if want_status else (nll, grad, parts)
+
+
+def pwa_nll_grad_enqueue(ctx, V):
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V, (n, 2))
+    _check(ctx, _lib.pwa_nll_grad_enqueue(ctx, V.ctypes.data))
+
+
+def pwa_nll_grad_batch_enqueue(ctx, V):
+    V = _f64(V)
+    _check(ctx, _lib.pwa_nll_grad_batch_enqueue(ctx, V.shape[0], V.ctypes.data))
+
+
+def pwa_fetch(ctx, K=1):
+    n = _lib.pwa_n_waves(ctx)
+    nll, grad, parts = np.empty(K), np.empty((K, n, 2)), np.empty((K, 2))
+    _check(ctx, _lib.pwa_fetch(ctx, int(K), nll.ctypes.data, grad.ctypes.data, parts.ctypes.data))
+    return nll, grad, parts
+
+
+def pwa_data_term_enqueue(ctx, V, out_dev):
+    """out_dev: torch CUDA float64 tensor with >= 2 + 2n elements (or a raw device address)."""
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V, (n, 2))
+    ptr, _, _ = _ptr_and_keep(out_dev)
+    _check(ctx, _lib.pwa_data_term_enqueue(ctx, V.ctypes.data, C.c_void_p(ptr)))
+
+
+def pwa_assemble_host(L_data, T, M, V):
+    """Host-only step A7 -> (nll, grad[n, 2], parts[2])."""
+    V = _f64(V)
+    n = V.shape[0]
+    T, M = _f64(T, (n, 2)), _f64(M, (n, n, 2))
+    nll = C.c_double(0.0)
+    grad, parts = np.empty((n, 2)), np.empty(2)
+    st = _lib.pwa_assemble_host(n, float(L_data), T.ctypes.data, M.ctypes.data, V.ctypes.data,
+                                C.byref(nll), grad.ctypes.data, parts.ctypes.data)
+    if st != PWA_OK:
+        raise PwaError(st, "pwa_assemble_host")
+    return nll.value, grad, parts
+
+
+def pwa_res_grad(ctx, V, n_res):
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V, (n, 2))
+    dM, dG = np.empty(n_res), np.empty(n_res)
+    _check(ctx, _lib.pwa_res_grad(ctx, V.ctypes.data, dM.ctypes.data, dG.ctypes.data))
+    return dM, dG
+
+
+def pwa_minimize_bfgs(ctx, V0, max_iter=200, gtol=1e-6):
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V0, (n, 2)).copy()
+    nll = C.c_double(0.0)
+    it, ev = C.c_int32(0), C.c_int32(0)
+    st = _check(ctx, _lib.pwa_minimize_bfgs(ctx, V.ctypes.data, int(max_iter), float(gtol), C.byref(nll),
+                                            C.byref(it), C.byref(ev)))
+    return V, nll.value, ev.value, st
+
+
+def pwa_minimize_bfgs_batch(ctx, V0, max_iter=300, gtol=1e-6):
+    V = _f64(V0).copy()
+    K = V.shape[0]
+    nll = np.empty(K)
+    ev = C.c_int32(0)
+    st = _check(ctx, _lib.pwa_minimize_bfgs_batch(ctx, K, V.ctypes.data, int(max_iter), float(gtol),
+                                                  nll.ctypes.data, C.byref(ev)))
+    return V, nll, ev.value, st
+
+
+def pwa_launch_count(ctx):
+    return int(_lib.pwa_launch_count(ctx))
+
+
+def pwa_sync(ctx):
+    _check(ctx, _lib.pwa_sync(ctx))
+
+
+def pwa_set_option(ctx, key, value):
+    _check(ctx, _lib.pwa_set_option(ctx, key.encode(), int(value)))
+
+
+def pwa_microbench(ctx, which, nbytes=0):
+    out = C.c_double(0.0)
+    _check(ctx, _lib.pwa_microbench(ctx, int(which), int(nbytes), C.byref(out)))
+    return out.value
+
+
+def pwa_n_waves(ctx):
+    return int(_lib.pwa_n_waves(ctx))
+
+
+def pwa_last_error(ctx):
+    return _lib.pwa_last_error(ctx).decode()
+
+
+def pwa_status_string(status):
+    return _status_name(status)

@@ -1,0 +1,448 @@
+// pwa_api.cu — the C ABI of include/pwa.h: context, uploads, call-order checks and the
+// host side of each evaluation (argument marshalling, one launch, one small D2H copy).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "pwa_internal.h"
+
+namespace pwa {
+
+pwa_status fail(pwa_ctx *ctx, pwa_status s, const std::string &msg)
+{
+    if (ctx) ctx->err = msg;
+    return s;
+}
+
+pwa_status cuda_fail(pwa_ctx *ctx, cudaError_t e, const char *what)
+{
+    std::string msg = std::string(what) + ": " + cudaGetErrorString(e);
+    pwa_status s = (e == cudaErrorMemoryAllocation) ? PWA_ERR_OOM : PWA_ERR_CUDA;
+    if (e == cudaErrorMemoryAllocation) cudaGetLastError();   // clear the sticky-free error
+    return fail(ctx, s, msg);
+}
+
+pwa_status ensure_partials(pwa_ctx *ctx, size_t doubles)
+{
+    if (doubles <= ctx->partials_cap) return PWA_OK;
+    // grows only when the launch shape changes (first evaluation after an upload)
+    if (ctx->d_partials) { PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->d_partials); ctx->d_partials = nullptr; }
+    ctx->partials_cap = 0;
+    PWA_CUDA(ctx, cudaMalloc(&ctx->d_partials, doubles * sizeof(double)));
+    ctx->partials_cap = doubles;
+    return PWA_OK;
+}
+
+pwa_status ensure_scratch(pwa_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->scratch_cap) return PWA_OK;
+    if (ctx->d_scratch) { PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->d_scratch); ctx->d_scratch = nullptr; }
+    ctx->scratch_cap = 0;
+    PWA_CUDA(ctx, cudaMalloc(&ctx->d_scratch, bytes));
+    ctx->scratch_cap = bytes;
+    return PWA_OK;
+}
+
+static bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static void free_sample(Sample &s)
+{
+    if (s.amps_owned && s.amps) cudaFree(s.amps);
+    if (s.fact_owned) { if (s.mass) cudaFree(s.mass); if (s.ang) cudaFree(s.ang); }
+    s = Sample();
+}
+
+static size_t elem_size(pwa_dtype d) { return d == PWA_F32 ? sizeof(float) : sizeof(double); }
+
+// copy (host or device source) into a fresh device buffer, or borrow a device pointer
+static pwa_status take_buffer(pwa_ctx *ctx, const void *src, size_t bytes, uint32_t flags,
+                              void **dst, bool *owned)
+{
+    *dst = nullptr; *owned = false;
+    if (bytes == 0) return PWA_OK;
+    const bool dev = is_device_ptr(src);
+    if (flags & PWA_BORROW) {
+        if (!dev) return fail(ctx, PWA_ERR_INVALID_ARG, "PWA_BORROW needs a device pointer");
+        if (((uintptr_t)src & 15u) != 0) return fail(ctx, PWA_ERR_INVALID_ARG, "PWA_BORROW pointer must be 16-byte aligned");
+        *dst = const_cast<void *>(src);
+        return PWA_OK;
+    }
+    void *buf = nullptr;
+    PWA_CUDA(ctx, cudaMalloc(&buf, bytes));
+    cudaError_t e = cudaMemcpyAsync(buf, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { cudaFree(buf); return cuda_fail(ctx, e, "upload copy"); }
+    *dst = buf; *owned = true;
+    return PWA_OK;
+}
+
+static pwa_status check_ready(pwa_ctx *ctx, bool need_M)
+{
+    if (ctx->data.n_events < 0) return fail(ctx, PWA_ERR_STATE, "no DATA sample uploaded");
+    if (need_M && !ctx->M_valid) return fail(ctx, PWA_ERR_STATE, "normalisation matrix missing or stale: call pwa_build_norm");
+    return PWA_OK;
+}
+
+static bool finite_all(const double *x, size_t k)
+{
+    for (size_t i = 0; i < k; ++i) if (!isfinite(x[i])) return false;
+    return true;
+}
+
+static pwa_status unpack_results(pwa_ctx *ctx, int K, double *nll, double *grad, double *parts)
+{
+    const int n = ctx->n, st = result_stride(n);
+    bool nonfinite = false;
+    for (int k = 0; k < K; ++k) {
+        const double *r = ctx->h_result + (size_t)k * st;
+        if (nll) nll[k] = r[0];
+        if (parts) { parts[2 * k] = r[1]; parts[2 * k + 1] = r[2]; }
+        if (grad) memcpy(grad + (size_t)k * 2 * n, r + 4, sizeof(double) * 2 * n);
+        if (r[3] != 0.0 || !finite_all(r, (size_t)st)) nonfinite = true;
+    }
+    return nonfinite ? PWA_WARN_NONFINITE : PWA_OK;
+}
+
+static pwa_status stage_V(pwa_ctx *ctx, int K, const double *V)
+{
+    const size_t cnt = (size_t)K * 2 * ctx->n;
+    if (!finite_all(V, cnt)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
+    memcpy(ctx->h_V, V, sizeof(double) * cnt);
+    return PWA_OK;
+}
+
+static pwa_status enqueue_evals(pwa_ctx *ctx, int K, bool batched)
+{
+    const int n = ctx->n;
+    const bool fast = (n == 4 || n == 8 || n == 16 || n == 32 || n == 64) && ctx->opt_data_term != 99;
+    const bool need_dV = batched || (!fast && !ctx->data.factored);
+    if (need_dV)
+        PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * (size_t)K * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
+    pwa_status s = PWA_OK;
+    if (batched) {
+        s = launch_batch(ctx, K);
+    } else {
+        for (int k = 0; k < K && s == PWA_OK; ++k)
+            s = launch_data_term(ctx, ctx->h_V + (size_t)k * 2 * n, k, nullptr);
+    }
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->h_result, ctx->d_result, sizeof(double) * (size_t)K * result_stride(n),
+                                  cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->last_K = K;
+    return PWA_OK;
+}
+
+}  // namespace pwa
+
+using namespace pwa;
+
+extern "C" {
+
+const char *pwa_status_string(pwa_status s)
+{
+    switch (s) {
+    case PWA_OK: return "PWA_OK";
+    case PWA_ERR_INVALID_ARG: return "PWA_ERR_INVALID_ARG";
+    case PWA_ERR_STATE: return "PWA_ERR_STATE";
+    case PWA_ERR_OOM: return "PWA_ERR_OOM";
+    case PWA_ERR_CUDA: return "PWA_ERR_CUDA";
+    case PWA_ERR_UNSUPPORTED: return "PWA_ERR_UNSUPPORTED";
+    case PWA_WARN_NONFINITE: return "PWA_WARN_NONFINITE";
+    }
+    return "PWA_?";
+}
+
+const char *pwa_last_error(const pwa_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t device, void *cuda_stream)
+{
+    if (!out) return PWA_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (n_waves < 1 || n_waves > 256) return PWA_ERR_INVALID_ARG;
+    if (storage != PWA_F64 && storage != PWA_F32) return PWA_ERR_INVALID_ARG;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) { cudaGetLastError(); return PWA_ERR_CUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return PWA_ERR_CUDA; }
+    pwa_ctx *ctx = new (std::nothrow) pwa_ctx();
+    if (!ctx) return PWA_ERR_OOM;
+    ctx->n = n_waves; ctx->storage = storage; ctx->device = device; ctx->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) ctx->sm_count = prop.multiProcessorCount;
+    const size_t n = (size_t)n_waves;
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_M, sizeof(double) * 2 * n * n);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_ticket, 4 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_ticket, 0, 4 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_result, sizeof(double) * kMaxK * result_stride(n_waves));
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_result, sizeof(double) * kMaxK * result_stride(n_waves));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_V, sizeof(double) * kMaxK * 2 * n);
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_V, sizeof(double) * kMaxK * 2 * n);
+    if (e != cudaSuccess) { cudaGetLastError(); pwa_destroy(ctx); return e == cudaErrorMemoryAllocation ? PWA_ERR_OOM : PWA_ERR_CUDA; }
+    ctx->h_M.assign(2 * n * n, 0.0);
+    *out = ctx;
+    return PWA_OK;
+}
+
+void pwa_destroy(pwa_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    free_sample(ctx->data);
+    free_sample(ctx->mc);
+    if (ctx->d_M) cudaFree(ctx->d_M);
+    if (ctx->d_ticket) cudaFree(ctx->d_ticket);
+    if (ctx->d_result) cudaFree(ctx->d_result);
+    if (ctx->h_result) cudaFreeHost(ctx->h_result);
+    if (ctx->d_V) cudaFree(ctx->d_V);
+    if (ctx->h_V) cudaFreeHost(ctx->h_V);
+    if (ctx->d_partials) cudaFree(ctx->d_partials);
+    if (ctx->d_scratch) cudaFree(ctx->d_scratch);
+    cudaGetLastError();
+    delete ctx;
+}
+
+pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, int64_t n_events,
+                             int64_t n_generated, uint32_t flags)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
+    if (n_events < 0 || (n_events > 0 && !amps)) return fail(ctx, PWA_ERR_INVALID_ARG, "bad amps / n_events");
+    if (flags > PWA_BORROW) return fail(ctx, PWA_ERR_INVALID_ARG, "bad flags");
+    if (which == PWA_MC && n_generated < n_events) return fail(ctx, PWA_ERR_INVALID_ARG, "n_generated < n_events");
+    if (which == PWA_MC && n_generated < 1) return fail(ctx, PWA_ERR_INVALID_ARG, "n_generated must be >= 1");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    void *buf = nullptr; bool owned = false;
+    const size_t bytes = (size_t)n_events * (size_t)ctx->n * 2 * elem_size(ctx->storage);
+    pwa_status s = take_buffer(ctx, amps, bytes, flags, &buf, &owned);
+    if (s != PWA_OK) return s;
+    Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
+    free_sample(smp);
+    smp.amps = buf; smp.amps_owned = owned; smp.factored = false;
+    smp.n_events = n_events; smp.n_gen = n_generated;
+    if (which == PWA_MC) ctx->M_valid = false;
+    return PWA_OK;
+}
+
+pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const double *mass, const void *ang,
+                                      int32_t n_ang, int64_t n_events, int64_t n_generated, uint32_t flags)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
+    if (n_ang < 1 || n_ang > kMaxAng) return fail(ctx, PWA_ERR_INVALID_ARG, "n_ang must be in [1, 4]");
+    if (n_events < 0 || (n_events > 0 && (!mass || !ang))) return fail(ctx, PWA_ERR_INVALID_ARG, "bad mass / ang / n_events");
+    if (flags > PWA_BORROW) return fail(ctx, PWA_ERR_INVALID_ARG, "bad flags");
+    if (which == PWA_MC && (n_generated < n_events || n_generated < 1)) return fail(ctx, PWA_ERR_INVALID_ARG, "bad n_generated");
+    if (ctx->n > kMaxFastWaves) return fail(ctx, PWA_ERR_UNSUPPORTED, "factored mode needs n <= 64");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    void *bm = nullptr, *ba = nullptr; bool om = false, oa = false;
+    pwa_status s = take_buffer(ctx, mass, (size_t)n_events * sizeof(double), flags, &bm, &om);
+    if (s != PWA_OK) return s;
+    s = take_buffer(ctx, ang, (size_t)n_events * (size_t)n_ang * 2 * elem_size(ctx->storage), flags, &ba, &oa);
+    if (s != PWA_OK) { if (om) cudaFree(bm); return s; }
+    Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
+    free_sample(smp);
+    smp.mass = (double *)bm; smp.ang = ba; smp.fact_owned = om || oa; smp.n_ang = n_ang; smp.factored = true;
+    smp.n_events = n_events; smp.n_gen = n_generated;
+    if (which == PWA_MC) ctx->M_valid = false;
+    return PWA_OK;
+}
+
+pwa_status pwa_set_wave_map(pwa_ctx *ctx, int32_t n_res, const int32_t *res_of_wave, const int32_t *ang_of_wave)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (n_res < 1 || n_res > kMaxRes || !res_of_wave || !ang_of_wave) return fail(ctx, PWA_ERR_INVALID_ARG, "bad wave map");
+    if (ctx->n > kMaxFastWaves) return fail(ctx, PWA_ERR_UNSUPPORTED, "factored mode needs n <= 64");
+    std::vector<int32_t> pair(n_res * kMaxAng, -1);
+    for (int a = 0; a < ctx->n; ++a) {
+        if (res_of_wave[a] < 0 || res_of_wave[a] >= n_res || ang_of_wave[a] < 0 || ang_of_wave[a] >= kMaxAng)
+            return fail(ctx, PWA_ERR_INVALID_ARG, "wave map entry out of range");
+        int32_t &slot = pair[res_of_wave[a] * kMaxAng + ang_of_wave[a]];
+        if (slot >= 0) return fail(ctx, PWA_ERR_INVALID_ARG, "two waves share one (resonance, angular structure) pair");
+        slot = a;
+    }
+    ctx->n_res = n_res;
+    ctx->res_of_wave.assign(res_of_wave, res_of_wave + ctx->n);
+    ctx->ang_of_wave.assign(ang_of_wave, ang_of_wave + ctx->n);
+    ctx->wave_of_pair = pair;
+    ctx->res_set = false;
+    ctx->M_valid = false;
+    return PWA_OK;
+}
+
+pwa_status pwa_set_resonances(pwa_ctx *ctx, const double *mass0, const double *width0)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (ctx->n_res < 1) return fail(ctx, PWA_ERR_STATE, "pwa_set_wave_map not called");
+    if (!mass0 || !width0 || !finite_all(mass0, ctx->n_res) || !finite_all(width0, ctx->n_res))
+        return fail(ctx, PWA_ERR_INVALID_ARG, "bad resonance parameters");
+    ctx->mass0.assign(mass0, mass0 + ctx->n_res);
+    ctx->width0.assign(width0, width0 + ctx->n_res);
+    ctx->res_set = true;
+    if (ctx->mc.factored) ctx->M_valid = false;
+    return PWA_OK;
+}
+
+pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "no MC sample uploaded");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    pwa_status s = launch_norm_build(ctx);
+    if (s != PWA_OK) return s;
+    ctx->M_valid = true;
+    if (M_out) {
+        const size_t cnt = 2 * (size_t)ctx->n * ctx->n;
+        PWA_CUDA(ctx, cudaMemcpyAsync(ctx->h_M.data(), ctx->d_M, sizeof(double) * cnt, cudaMemcpyDeviceToHost, ctx->stream));
+        PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        memcpy(M_out, ctx->h_M.data(), sizeof(double) * cnt);
+    }
+    return PWA_OK;
+}
+
+pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
+{
+    if (!ctx || !M) return PWA_ERR_INVALID_ARG;
+    const size_t cnt = 2 * (size_t)ctx->n * ctx->n;
+    if (!finite_all(M, cnt)) return fail(ctx, PWA_ERR_INVALID_ARG, "M contains non-finite values");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    memcpy(ctx->h_M.data(), M, sizeof(double) * cnt);
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_M, ctx->h_M.data(), sizeof(double) * cnt, cudaMemcpyHostToDevice, ctx->stream));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->M_valid = true;
+    return PWA_OK;
+}
+
+pwa_status pwa_nll_grad_enqueue(pwa_ctx *ctx, const double *V)
+{
+    if (!ctx || !V) return PWA_ERR_INVALID_ARG;
+    pwa_status s = check_ready(ctx, true);
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    s = stage_V(ctx, 1, V);
+    if (s != PWA_OK) return s;
+    return enqueue_evals(ctx, 1, false);
+}
+
+pwa_status pwa_nll_grad_batch_enqueue(pwa_ctx *ctx, int32_t K, const double *V)
+{
+    if (!ctx || !V) return PWA_ERR_INVALID_ARG;
+    if (K < 1 || K > kMaxK) return fail(ctx, PWA_ERR_INVALID_ARG, "K must be in [1, 1024]");
+    pwa_status s = check_ready(ctx, true);
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    s = stage_V(ctx, K, V);
+    if (s != PWA_OK) return s;
+    return enqueue_evals(ctx, K, true);
+}
+
+pwa_status pwa_fetch(pwa_ctx *ctx, int32_t K, double *nll, double *grad, double *parts)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (K < 1 || K != ctx->last_K) return fail(ctx, PWA_ERR_STATE, "pwa_fetch: K does not match the last enqueue");
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return unpack_results(ctx, K, nll, grad, parts);
+}
+
+pwa_status pwa_nll_grad(pwa_ctx *ctx, const double *V, double *nll, double *grad, double *parts)
+{
+    if (!ctx || !V || !nll || !grad) return ctx ? fail(ctx, PWA_ERR_INVALID_ARG, "null argument") : PWA_ERR_INVALID_ARG;
+    pwa_status s = pwa_nll_grad_enqueue(ctx, V);
+    if (s != PWA_OK) return s;
+    return pwa_fetch(ctx, 1, nll, grad, parts);
+}
+
+pwa_status pwa_nll_grad_batch(pwa_ctx *ctx, int32_t K, const double *V, double *nll, double *grad, double *parts)
+{
+    if (!ctx || !V || !nll || !grad) return ctx ? fail(ctx, PWA_ERR_INVALID_ARG, "null argument") : PWA_ERR_INVALID_ARG;
+    pwa_status s = pwa_nll_grad_batch_enqueue(ctx, K, V);
+    if (s != PWA_OK) return s;
+    return pwa_fetch(ctx, K, nll, grad, parts);
+}
+
+pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
+{
+    if (!ctx || !V || !out_dev) return PWA_ERR_INVALID_ARG;
+    pwa_status s = check_ready(ctx, false);
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    s = stage_V(ctx, 1, V);
+    if (s != PWA_OK) return s;
+    const int n = ctx->n;
+    const bool fast = (n == 4 || n == 8 || n == 16 || n == 32 || n == 64) && ctx->opt_data_term != 99;
+    if (!fast && !ctx->data.factored)
+        PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
+    return launch_data_term(ctx, ctx->h_V, 0, out_dev);
+}
+
+pwa_status pwa_assemble_host(int32_t n, double L_data, const double *T, const double *M, const double *V,
+                             double *nll, double *grad, double *parts)
+{
+    if (n < 1 || !T || !M || !V || !nll || !grad) return PWA_ERR_INVALID_ARG;
+    double norm = 0.0;
+    for (int a = 0; a < n; ++a) {
+        double mr = 0.0, mi = 0.0;
+        for (int b = 0; b < n; ++b) {
+            const double Mr = M[((size_t)a * n + b) * 2], Mi = M[((size_t)a * n + b) * 2 + 1];
+            mr += Mr * V[2 * b] - Mi * V[2 * b + 1];
+            mi += Mr * V[2 * b + 1] + Mi * V[2 * b];
+        }
+        norm += V[2 * a] * mr + V[2 * a + 1] * mi;
+        grad[2 * a] = -2.0 * T[2 * a] + 2.0 * mr;
+        grad[2 * a + 1] = 2.0 * T[2 * a + 1] + 2.0 * mi;
+    }
+    *nll = -(L_data - norm);
+    if (parts) { parts[0] = L_data; parts[1] = norm; }
+    return PWA_OK;
+}
+
+pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG)
+{
+    if (!ctx || !V || !dM || !dG) return PWA_ERR_INVALID_ARG;
+    if (ctx->data.n_events < 0 || ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "DATA and MC must be uploaded");
+    if (!ctx->data.factored || !ctx->mc.factored) return fail(ctx, PWA_ERR_STATE, "pwa_res_grad needs factored uploads");
+    if (!finite_all(V, 2 * (size_t)ctx->n)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_res_grad(ctx, V, dM, dG);
+}
+
+uint64_t pwa_launch_count(const pwa_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int32_t pwa_n_waves(const pwa_ctx *ctx) { return ctx ? ctx->n : 0; }
+
+pwa_status pwa_sync(pwa_ctx *ctx)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return PWA_OK;
+}
+
+pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
+{
+    if (!ctx || !key) return PWA_ERR_INVALID_ARG;
+    if (!strcmp(key, "data_term")) ctx->opt_data_term = value;
+    else if (!strcmp(key, "norm")) ctx->opt_norm = value;
+    else if (!strcmp(key, "batch")) ctx->opt_batch = value;
+    else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
+    return PWA_OK;
+}
+
+pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result)
+{
+    if (!ctx || !result) return PWA_ERR_INVALID_ARG;
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return run_microbench(ctx, which, bytes, result);
+}
+
+}  // extern "C"

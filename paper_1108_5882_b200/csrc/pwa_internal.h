@@ -1,0 +1,91 @@
+// pwa_internal.h — context and shared device helpers of libpwa.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/pwa.h"
+
+namespace pwa {
+
+constexpr int kMaxFastWaves = 64;     // V passed by value for n <= 64
+constexpr int kMaxRes = 64;
+constexpr int kMaxAng = 4;
+constexpr int kMaxK = 1024;
+
+// Result record of one evaluation k, written by the finishing block of the data pass:
+//   [0] nll  [1] L_data  [2] Norm  [3] n_nonfinite  [4 + 2a] d nll/d Re V_a  [5 + 2a] d nll/d Im V_a
+inline int result_stride(int n) { return 4 + 2 * n; }
+// Partial / data-term component order: [0] L_data [1] n_nonfinite [2 + 2a] Re T_a [3 + 2a] Im T_a
+inline int n_components(int n) { return 2 + 2 * n; }
+
+struct VArg { double v[2 * kMaxFastWaves]; };   // kernel-parameter copy of V (<= 1 KB)
+
+struct Sample {
+    // constant-resonance form
+    void *amps = nullptr;   bool amps_owned = false;
+    // factored form
+    double *mass = nullptr; void *ang = nullptr; bool fact_owned = false; int n_ang = 0;
+    bool factored = false;
+    int64_t n_events = -1;  // -1 = not uploaded
+    int64_t n_gen = 0;
+};
+
+struct ResParams {           // by-value kernel argument in factored mode
+    double m2[kMaxRes];      // M_r^2
+    double mg[kMaxRes];      // M_r * G_r
+};
+
+}  // namespace pwa
+
+struct pwa_ctx {
+    int n = 0;
+    pwa_dtype storage = PWA_F64;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+    pwa::Sample data, mc;
+    // floating mode
+    int n_res = 0;
+    std::vector<int32_t> res_of_wave, ang_of_wave;
+    std::vector<int32_t> wave_of_pair;        // [n_res * kMaxAng] -> wave or -1
+    std::vector<double> mass0, width0;
+    bool res_set = false;
+    // normalisation matrix
+    double *d_M = nullptr;                    // [n][n][2]
+    std::vector<double> h_M;
+    bool M_valid = false;
+    // scratch
+    double *d_partials = nullptr; size_t partials_cap = 0;   // doubles
+    unsigned *d_ticket = nullptr;
+    double *d_result = nullptr; double *h_result = nullptr;  // [kMaxK][result_stride]
+    double *d_V = nullptr; double *h_V = nullptr;            // [kMaxK][n][2]
+    double *d_scratch = nullptr; size_t scratch_cap = 0;     // bytes (M partials, batch partials)
+    int last_K = 0;
+    uint64_t launches = 0;
+    int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
+    std::string err;
+};
+
+namespace pwa {
+
+pwa_status fail(pwa_ctx *ctx, pwa_status s, const std::string &msg);
+pwa_status cuda_fail(pwa_ctx *ctx, cudaError_t e, const char *what);
+pwa_status ensure_partials(pwa_ctx *ctx, size_t doubles);
+pwa_status ensure_scratch(pwa_ctx *ctx, size_t bytes);
+
+#define PWA_CUDA(ctx, call)                                                   \
+    do {                                                                      \
+        cudaError_t e__ = (call);                                             \
+        if (e__ != cudaSuccess) return pwa::cuda_fail((ctx), e__, #call);     \
+    } while (0)
+
+// launchers (one .cu each)
+pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double *out_dev_terms);
+pwa_status launch_batch(pwa_ctx *ctx, int K);   // V already staged in h_V/d_V
+pwa_status launch_norm_build(pwa_ctx *ctx);
+pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
+pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
+
+}  // namespace pwa

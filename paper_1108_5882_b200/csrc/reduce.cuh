@@ -1,0 +1,140 @@
+// reduce.cuh — step A5 ("the final sum has to be computed in double precision ...
+// tree sums as usually implemented on GPUs perform much better here"): fixed-shape fp64
+// tree: per-thread running sums -> warp shuffles -> per-block partial in a fixed slot ->
+// the last-arriving block sums the slots in slot order.  No floating-point atomics, so a
+// launch with a fixed grid is bitwise reproducible.  The finishing block also performs step
+// A7 (Norm = V^H M V, nll, gradient assembly; P:41 second term).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace pwa {
+
+constexpr int kMaxWaves = 256;
+constexpr int kMaxComp = 2 + 2 * kMaxWaves;
+
+struct FinishArgs {
+    double *partials;      // [NC][gridDim.x]
+    unsigned *ticket;
+    const double *M;       // device [n][n][2]; nullptr -> data-term-only output
+    double *out;           // result record (M != nullptr) or [NC] components (M == nullptr)
+    int n;
+};
+
+__device__ __forceinline__ double shfl_xor_d(double x, int m)
+{
+    return __shfl_xor_sync(0xffffffffu, x, m);
+}
+
+__device__ __forceinline__ double warp_sum(double x)
+{
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) x += shfl_xor_d(x, m);
+    return x;
+}
+
+// s_tot[0..NC): this block's totals (valid for all threads after a __syncthreads by the
+// caller).  sV: V in shared memory [2n].  Must be called by every thread of the block.
+__device__ inline void block_finish(double *s_tot, const double *sV, const FinishArgs &fa)
+{
+    const int n = fa.n, NC = 2 + 2 * n;
+    const int tid = threadIdx.x, nthreads = blockDim.x;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+    __shared__ bool s_last;
+    __shared__ double s_mv[2 * kMaxWaves];
+
+    for (int c = tid; c < NC; c += nthreads) fa.partials[(size_t)c * gridDim.x + blockIdx.x] = s_tot[c];
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(fa.ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+
+    // fixed-order sum over slots: lane l takes slots l, l+32, ... then a fixed xor tree
+    for (int c = warp; c < NC; c += nwarps) {
+        const double *p = fa.partials + (size_t)c * gridDim.x;
+        double acc = 0.0;
+        for (unsigned s = lane; s < gridDim.x; s += 32) acc += __ldcg(p + s);
+        acc = warp_sum(acc);
+        if (lane == 0) s_tot[c] = acc;
+    }
+    __syncthreads();
+
+    if (fa.M == nullptr) {
+        for (int c = tid; c < NC; c += nthreads) fa.out[c] = s_tot[c];
+    } else {
+        // (M V)_a, one row per thread
+        for (int a = tid; a < n; a += nthreads) {
+            const double *row = fa.M + (size_t)a * n * 2;
+            double mr = 0.0, mi = 0.0;
+            for (int b = 0; b < n; ++b) {
+                double Mr = row[2 * b], Mi = row[2 * b + 1];
+                double vr = sV[2 * b], vi = sV[2 * b + 1];
+                mr = fma(Mr, vr, mr); mr = fma(-Mi, vi, mr);
+                mi = fma(Mr, vi, mi); mi = fma(Mi, vr, mi);
+            }
+            s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi;
+            // grad_a = -2 conj(T_a) + 2 (M V)_a
+            fa.out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + 2.0 * mr;
+            fa.out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + 2.0 * mi;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double acc = 0.0;   // Norm = sum_a Re( conj(V_a) (M V)_a )
+            for (int a = lane; a < n; a += 32) acc += sV[2 * a] * s_mv[2 * a] + sV[2 * a + 1] * s_mv[2 * a + 1];
+            acc = warp_sum(acc);
+            if (lane == 0) {
+                fa.out[0] = -(s_tot[0] - acc);
+                fa.out[1] = s_tot[0];
+                fa.out[2] = acc;
+                fa.out[3] = s_tot[1];
+            }
+        }
+    }
+    if (tid == 0) *fa.ticket = 0u;   // re-arm for the next launch on this stream
+}
+
+constexpr int kFastWaves = 64;   // == kMaxFastWaves (pwa_internal.h)
+
+// Shared tail of every grouped data-pass kernel: per-thread (L, bad, T of the lane's waves)
+// -> warp shuffles -> block totals -> block_finish.  Lanes with equal (lane % G) own the same
+// waves; wave_of(idx) maps accumulator idx -> wave (or -1: not a wave, skipped).
+template <int G, int W, int THREADS, typename WaveOf>
+__device__ __forceinline__ void reduce_and_finish(double L, double bad, double (&tr)[W], double (&ti)[W],
+                                                    WaveOf wave_of, const double *sV, const FinishArgs &fa)
+{
+    constexpr int NWARPS = THREADS / 32;
+    __shared__ double s_warp[NWARPS][2 + 2 * kFastWaves];
+    __shared__ double s_tot[2 + 2 * kFastWaves];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int NC = 2 + 2 * fa.n;
+    L = warp_sum(L);
+    bad = warp_sum(bad);
+#pragma unroll
+    for (int w = 0; w < W; ++w) {
+#pragma unroll
+        for (int m = G; m < 32; m <<= 1) {
+            tr[w] += shfl_xor_d(tr[w], m);
+            ti[w] += shfl_xor_d(ti[w], m);
+        }
+    }
+    if (lane == 0) { s_warp[warp][0] = L; s_warp[warp][1] = bad; }
+    if (lane < G) {
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            const int a = wave_of(w);
+            if (a >= 0) { s_warp[warp][2 + 2 * a] = tr[w]; s_warp[warp][3 + 2 * a] = ti[w]; }
+        }
+    }
+    __syncthreads();
+    for (int c = threadIdx.x; c < NC; c += THREADS) {
+        double acc = 0.0;
+#pragma unroll
+        for (int w = 0; w < NWARPS; ++w) acc += s_warp[w][c];
+        s_tot[c] = acc;
+    }
+    __syncthreads();
+    block_finish(s_tot, sV, fa);
+}
+
+}  // namespace pwa

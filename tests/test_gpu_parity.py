@@ -1,0 +1,301 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances (BASELINE.json north_star, reading C8), norm-wise:
+    fp64 amplitude storage : 1e-12 on nll, L_data, Norm, and on the gradient in max-norm
+    fp32 amplitude storage : 1e-6  (fp64 arithmetic and accumulation)
+M is compared entry-wise relative to max|M|.  Run with `pytest -m gpu` on a B200.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-6}
+
+
+@pytest.fixture(scope="module")
+def pwa():
+    from paper_1108_5882_b200 import binding
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return binding
+
+
+class Ctx:
+    """Small RAII helper around the binding (marshalling only)."""
+
+    def __init__(self, pwa, n, storage):
+        self.pwa, self.n, self.storage = pwa, n, storage
+        self.ctx = pwa.pwa_create(n, storage)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.pwa.pwa_destroy(self.ctx)
+
+
+def check_eval(res, ref, tol, N):
+    nll, g, parts = res[0], res[1], res[2]
+    nll_o, g_o, parts_o = ref[0], ref[1], ref[2]
+    scaleL = max(abs(parts_o[0]), 1e-2 * N, 1e-300)
+    assert abs(parts[0] - parts_o[0]) <= tol * scaleL, ("L_data", parts[0], parts_o[0])
+    assert abs(parts[1] - parts_o[1]) <= tol * max(abs(parts_o[1]), 1e-300), ("Norm", parts[1], parts_o[1])
+    assert abs(nll - nll_o) <= tol * max(abs(nll_o), scaleL), ("nll", nll, nll_o)
+    gs = np.abs(g_o).max()
+    assert np.abs(g - g_o).max() <= tol * gs, ("grad", np.abs(g - g_o).max() / gs)
+
+
+def check_M(M, M_o, tol):
+    assert np.abs(M - M_o).max() <= tol * np.abs(M_o).max(), np.abs(M - M_o).max() / np.abs(M_o).max()
+    Mc = M[..., 0] + 1j * M[..., 1]
+    assert np.array_equal(Mc, Mc.conj().T), "GPU M must be exactly Hermitian"
+
+
+def rand_case(seed, N, Nacc, n, storage):
+    rng = np.random.default_rng(seed)
+    dt = np.float64 if storage == "f64" else np.float32
+    A = (rng.normal(size=(N, n, 2)) * 0.35).astype(dt)
+    B = (rng.normal(size=(Nacc, n, 2)) * 0.35).astype(dt)
+    V = rng.normal(size=(n, 2))
+    return A, B, V
+
+
+# ------------------------------------------------------------------ configs 0 and 1 at full size
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_cfg_full_parity(pwa, oracle, synth, cfg):
+    w = synth.make_workload(cfg)
+    M_o = oracle.norm_matrix(w.A_mc, w.n_gen)
+    with Ctx(pwa, w.n, w.storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, w.A_data)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+        M = pwa.pwa_build_norm(c.ctx)
+        check_M(M, M_o, TOL[w.storage])
+        pts = [w.V_true] + list(synth.eval_points(w, 3))
+        for V in pts:
+            res = pwa.pwa_nll_grad(c.ctx, V)
+            # oracle evaluates with ITS OWN M: the whole path is compared
+            check_eval(res, oracle.nll_grad(w.A_data, M_o, V), TOL[w.storage], w.n_data)
+        # run-to-run bitwise reproducibility (fixed reduction tree, C8)
+        a = pwa.pwa_nll_grad(c.ctx, pts[1])
+        b = pwa.pwa_nll_grad(c.ctx, pts[1])
+        assert a[0] == b[0] and np.array_equal(a[1], b[1])
+
+
+# ------------------------------------------------------------------ tiles, ragged tails, every fast n and the generic path
+@pytest.mark.parametrize("storage", ["f64", "f32"])
+@pytest.mark.parametrize("n", [1, 3, 4, 5, 8, 16, 20, 32, 64])
+def test_ragged_sizes(pwa, oracle, n, storage):
+    for N, Nacc in [(1, 1), (31, 7), (33, 64), (1000, 257), (4097, 3001), (20011, 9973)]:
+        A, B, V = rand_case(100 * n + N, N, Nacc, n, storage)
+        M_o = oracle.norm_matrix(B, Nacc + 5)
+        with Ctx(pwa, n, storage) as c:
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=Nacc + 5)
+            check_M(pwa.pwa_build_norm(c.ctx), M_o, TOL[storage])
+            check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(A, M_o, V), TOL[storage], N)
+
+
+@pytest.mark.parametrize("storage,n,opt", [("f64", 16, 1), ("f64", 32, 1), ("f64", 64, 1), ("f32", 32, 1),
+                                           ("f32", 32, 2), ("f32", 64, 1), ("f32", 64, 2), ("f64", 16, 99),
+                                           ("f32", 64, 99)])
+def test_kernel_variants(pwa, oracle, storage, n, opt):
+    """Every selectable data-term variant (pwa_set_option) must meet the same bar."""
+    A, B, V = rand_case(7 + n + opt, 5003, 1201, n, storage)
+    M_o = oracle.norm_matrix(B, 1300)
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_set_option(c.ctx, "data_term", opt)
+        pwa.pwa_set_option(c.ctx, "norm", 99 if opt == 99 else 0)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=1300)
+        check_M(pwa.pwa_build_norm(c.ctx), M_o, TOL[storage])
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(A, M_o, V), TOL[storage], 5003)
+
+
+def test_empty_inputs(pwa):
+    n = 4
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.zeros((0, n, 2)), n_events=0)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, np.zeros((0, n, 2)), n_events=0, n_generated=10)
+        M = pwa.pwa_build_norm(c.ctx)
+        assert np.all(M == 0)
+        nll, g, parts = pwa.pwa_nll_grad(c.ctx, np.ones((n, 2)))
+        assert nll == 0.0 and np.all(g == 0) and parts[0] == 0.0 and parts[1] == 0.0
+
+
+def test_call_order_errors(pwa):
+    with Ctx(pwa, 4, "f64") as c:
+        with pytest.raises(pwa.PwaError) as e:
+            pwa.pwa_nll_grad(c.ctx, np.ones((4, 2)))
+        assert e.value.status == pwa.PWA_ERR_STATE
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.ones((8, 4, 2)))
+        with pytest.raises(pwa.PwaError) as e:       # M missing
+            pwa.pwa_nll_grad(c.ctx, np.ones((4, 2)))
+        assert e.value.status == pwa.PWA_ERR_STATE
+        with pytest.raises(pwa.PwaError) as e:       # N_gen < N_acc
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, np.ones((8, 4, 2)), n_generated=3)
+        assert e.value.status == pwa.PWA_ERR_INVALID_ARG
+        with pytest.raises(pwa.PwaError):            # non-finite V
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, np.ones((8, 4, 2)), n_generated=8)
+            pwa.pwa_build_norm(c.ctx)
+            pwa.pwa_nll_grad(c.ctx, np.full((4, 2), np.nan))
+
+
+def test_nonfinite_warning(pwa, oracle):
+    """C14: an event with S_i = 0 gives ln 0 = -inf; IEEE values propagate, status warns."""
+    n = 4
+    A = np.random.default_rng(1).normal(size=(40, n, 2))
+    A[17] = 0.0
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, A, n_generated=40)
+        pwa.pwa_build_norm(c.ctx)
+        nll, g, parts, st = pwa.pwa_nll_grad(c.ctx, np.ones((n, 2)), want_status=True)
+        assert st == pwa.PWA_WARN_NONFINITE and parts[0] == -math.inf and nll == math.inf
+    L, T, bad = oracle.data_term(A, np.ones((n, 2)))
+    assert bad == 1 and L == -math.inf
+
+
+# ------------------------------------------------------------------ batched == single == oracle
+@pytest.mark.parametrize("storage,n,K", [("f64", 4, 3), ("f64", 16, 8), ("f32", 32, 5), ("f32", 64, 64), ("f64", 5, 2)])
+def test_batch_matches_single_and_oracle(pwa, oracle, storage, n, K):
+    A, B, _ = rand_case(31 + n, 6007, 2003, n, storage)
+    Vk = np.random.default_rng(K).normal(size=(K, n, 2))
+    M_o = oracle.norm_matrix(B, 2100)
+    nll_o, g_o, parts_o, _ = oracle.nll_grad_batch(A, M_o, Vk)
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2100)
+        pwa.pwa_build_norm(c.ctx)
+        nll, g, parts = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        for k in range(K):
+            check_eval((nll[k], g[k], parts[k]), (nll_o[k], g_o[k], parts_o[k]), TOL[storage], 6007)
+            one = pwa.pwa_nll_grad(c.ctx, Vk[k])
+            check_eval((nll[k], g[k], parts[k]), one, TOL[storage], 6007)
+
+
+# ------------------------------------------------------------------ floating resonances (A1, fused BW)
+def _factored_ctx(pwa, w, Mr, Gr, N=None, Nacc=None):
+    c = Ctx(pwa, w.n, w.storage)
+    N = N or w.n_data
+    Nacc = Nacc or w.n_acc
+    pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_DATA, w.mass_data[:N], w.Z_data[:N])
+    pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_MC, w.mass_mc[:Nacc], w.Z_mc[:Nacc], n_generated=w.n_gen)
+    pwa.pwa_set_wave_map(c.ctx, w.n_res, w.res_of_wave, w.ang_of_wave)
+    pwa.pwa_set_resonances(c.ctx, Mr, Gr)
+    return c
+
+
+@pytest.mark.parametrize("n_data,n_mc", [(5003, 7001), (100_000, 200_000)])
+def test_factored_parity(pwa, oracle, synth, n_data, n_mc):
+    w = synth.make_workload(3, n_data=n_data, n_mc=n_mc, full_amplitudes=False)
+    Mr, Gr = synth.floating_start(w)
+    A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    M_o = oracle.norm_matrix(B, w.n_gen)
+    V = synth.eval_points(w, 1)[0]
+    with _factored_ctx(pwa, w, Mr, Gr) as c:
+        check_M(pwa.pwa_build_norm(c.ctx), M_o, 1e-12)
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(A, M_o, V), 1e-12, n_data)
+        # moving the resonances makes M stale: evaluation must refuse until rebuilt
+        pwa.pwa_set_resonances(c.ctx, w.Mr, w.Gr)
+        with pytest.raises(pwa.PwaError) as e:
+            pwa.pwa_nll_grad(c.ctx, V)
+        assert e.value.status == pwa.PWA_ERR_STATE
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        A2 = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, w.Mr, w.Gr)
+        B2 = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, w.Mr, w.Gr)
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(A2, oracle.norm_matrix(B2, w.n_gen), V), 1e-12, n_data)
+        # factored result == constant-mode result on the generator's own full matrix
+        assert np.allclose(A2, synth.amplitudes(w, w.kin_data), rtol=1e-13, atol=1e-15)
+
+
+def test_factored_three_angular_structures(pwa, oracle, synth):
+    """cfg-0 style wave map (4 resonances, 3 angular structures, 4 of the 12 pairs used)."""
+    w = synth.make_workload(0, n_data=3001, n_mc=4001)
+    Zd, Zm = synth.angular(w, w.kin_data), synth.angular(w, w.kin_mc)
+    V = synth.eval_points(w, 1)[0]
+    M_o = oracle.norm_matrix(w.A_mc, w.n_gen)
+    with Ctx(pwa, w.n, "f64") as c:
+        pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_DATA, w.mass_data, Zd)
+        pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_MC, w.mass_mc, Zm, n_generated=w.n_gen)
+        pwa.pwa_set_wave_map(c.ctx, w.n_res, w.res_of_wave, w.ang_of_wave)
+        pwa.pwa_set_resonances(c.ctx, w.Mr, w.Gr)
+        check_M(pwa.pwa_build_norm(c.ctx), M_o, 1e-12)
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(w.A_data, M_o, V), 1e-12, w.n_data)
+
+
+def test_res_grad_parity(pwa, oracle, synth):
+    w = synth.make_workload(3, n_data=20_011, n_mc=30_011, full_amplitudes=False)
+    Mr, Gr = synth.floating_start(w)
+    V = synth.eval_points(w, 1)[0]
+    dLM, dLG = oracle.res_grad(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 0)
+    dNM, dNG = oracle.res_grad(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 1, w.n_gen)
+    with _factored_ctx(pwa, w, Mr, Gr) as c:
+        dM, dG = pwa.pwa_res_grad(c.ctx, V, w.n_res)
+    ref = np.concatenate([-dLM + dNM, -dLG + dNG])
+    got = np.concatenate([dM, dG])
+    assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------ device-resident (BORROW) path and the multi-GPU building block
+def test_borrowed_device_buffers_and_data_term_only(pwa, oracle):
+    import torch
+    n, N = 16, 30_001
+    A, B, V = rand_case(3, N, 5000, n, "f64")
+    M_o = oracle.norm_matrix(B, 6000)
+    At = torch.from_numpy(A).cuda()
+    with Ctx(pwa, n, "f64") as c:
+        keep = pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, At, n_events=N, flags=pwa.PWA_BORROW)
+        assert keep is At
+        pwa.pwa_set_norm(c.ctx, M_o)
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), oracle.nll_grad(A, M_o, V), 1e-12, N)
+        out = torch.zeros(2 + 2 * n, dtype=torch.float64, device="cuda")
+        pwa.pwa_data_term_enqueue(c.ctx, V, out)
+        pwa.pwa_sync(c.ctx)
+        terms = out.cpu().numpy()
+        L_o, T_o, _ = oracle.data_term(A, V)
+        assert abs(terms[0] - L_o) <= 1e-12 * abs(L_o) and terms[1] == 0
+        assert np.abs(terms[2:].reshape(n, 2) - T_o).max() <= 1e-12 * np.abs(T_o).max()
+        res = pwa.pwa_assemble_host(terms[0], terms[2:].reshape(n, 2), M_o, V)
+        check_eval(res, oracle.nll_grad(A, M_o, V), 1e-12, N)
+        assert pwa.pwa_launch_count(c.ctx) >= 2
+
+
+# ------------------------------------------------------------------ host minimiser drives the GPU path (P12)
+def test_bfgs_converges_on_cfg0(pwa, oracle, synth):
+    w = synth.make_workload(0)
+    with Ctx(pwa, w.n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, w.A_data)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+        M = pwa.pwa_build_norm(c.ctx)
+        V0 = synth.eval_points(w, 1, stream=synth.S_START)[0]
+        Vfit, nll, evals, st = pwa.pwa_minimize_bfgs(c.ctx, V0, max_iter=300, gtol=1e-5)
+        nll_fit, g_fit, parts = pwa.pwa_nll_grad(c.ctx, Vfit)
+        nll_true = pwa.pwa_nll_grad(c.ctx, w.V_true)[0]
+    assert nll == nll_fit and np.abs(g_fit).max() < 1e-2
+    # P7: at a stationary point of eq. 3, Norm(V_hat) = N_data
+    assert parts[1] == pytest.approx(w.n_data, rel=1e-6)
+    # the fit at least matches the scale-profiled truth
+    _, _, p_true, _ = oracle.nll_grad(w.A_data, M, w.V_true)
+    prof_true = -(p_true[0] - w.n_data * math.log(p_true[1] / w.n_data) - w.n_data)
+    assert nll_fit <= prof_true + 1e-6 * abs(prof_true)
+    assert nll_fit <= nll_true
+    # the oracle agrees with the GPU at the fitted point
+    check_eval((nll_fit, g_fit, parts), oracle.nll_grad(w.A_data, M, Vfit), 1e-12, w.n_data)
+
+
+def test_bfgs_batch_lockstep(pwa, synth):
+    w = synth.make_workload(0)
+    K = 4
+    with Ctx(pwa, w.n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, w.A_data)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        V0 = synth.eval_points(w, K, stream=synth.S_START)
+        Vfit, nll, evals, st = pwa.pwa_minimize_bfgs_batch(c.ctx, V0, max_iter=200, gtol=1e-5)
+        for k in range(K):
+            one = pwa.pwa_nll_grad(c.ctx, Vfit[k])
+            assert one[0] == pytest.approx(nll[k], rel=1e-12)
+            assert one[2][1] == pytest.approx(w.n_data, rel=1e-5)

@@ -1,0 +1,552 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the PWA likelihood hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload (default cfg4 = BASELINE.json configs[4], the largest config and the one the
+north_star's HBM target is stated on): n = 64 waves, N_data = 5e6 events, fp32 amplitude storage
+(2.56 GB, >> the 126 MB L2, so nothing is cache-resident between steps), fp64 arithmetic.
+A STEP is one lnL + gradient evaluation at a fresh random V over all data events of the rank:
+steps A2-A5 + A7 of DESIGN.md section 2 (one pass over the amplitude matrix in HBM); with
+N > 1 ranks the events are sharded (weak scaling: every rank holds a full cfg-sized shard) and
+the step adds the rank-ordered sum of the (2 + 2n)-double data-term record.  The normalisation
+matrix M (step A6) is built once per fit at constant resonances and is
+therefore outside the step; its build, the batched K-start path (A8) and the floating-resonance
+iteration (A1, cfg3) are timed separately and reported under "extra" on the same JSON line.
+
+value = event-waves/s = (events x waves evaluated by all ranks) / time, device-timed with CUDA
+events on the library's stream, max over ranks.  e2e = the same through the synchronous C-ABI
+call pwa_nll_grad with HOST V in and HOST results out (wall clock).
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on the box's host cores on
+a bounded sample of the same workload; it is a deliberately plain program, reported as context.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+WORKLOADS = {"cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg0": 0}
+SAMPLE_TARGET_S = 0.6          # reference arm: aim for this much oracle time per step
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-extra", action="store_true", help="skip the M-build / batched / cfg3 side measurements")
+    ap.add_argument("--n-data", type=int, default=0, help="override N_data (debugging only; makes the line invalid)")
+    ap.add_argument("--n-mc", type=int, default=0, help="override N_MC accepted (debugging only)")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)", d
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)", {}
+
+
+def load_traffic(kernel_key):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture
+    (profiles/traffic.csv: key,dram_bytes_per_launch,source) or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = line.strip().split(",")
+        if len(f) >= 2 and f[0] == kernel_key:
+            try:
+                return float(f[1])
+            except ValueError:
+                return None
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    BAD = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown"}
+    NOTE = {0x4: "sw_power_cap", 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _once(self):
+        nv = self.nv
+        self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+        try:
+            r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        for bit, name in list(self.BAD.items()) + list(self.NOTE.items()):
+            if r & bit:
+                self.reasons.add(name)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._once()
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def start(self):
+        if self.ok:
+            self._stop.clear()
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+            self._thr = None
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, ws, local
+
+
+def sizes_for(args, spec):
+    n_data = args.n_data or spec["n_data"]
+    n_mc = args.n_mc or spec["n_mc"]
+    return int(n_data), int(n_mc)
+
+
+# --------------------------------------------------------------------------- reference arm
+def oracle_sample_size(oracle, A, M, V, n_total, target_s):
+    """Largest prefix of the data whose oracle evaluation takes about target_s seconds."""
+    probe = min(n_total, 20_000)
+    oracle.nll_grad(A[:probe], M, V)                     # page in / warm up threads
+    t0 = time.perf_counter()
+    oracle.nll_grad(A[:probe], M, V)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    s = int(probe * target_s / dt)
+    return max(1000, min(n_total, s))
+
+
+def small_oracle_norm(synth, oracle, cfg, n_mc=50_000):
+    wm = synth.make_workload(cfg, n_data=1, n_mc=n_mc, want_data=False)
+    A_mc = wm.A_mc
+    if A_mc is None:   # factored config
+        A_mc = synth.amplitudes(wm, wm.kin_mc)
+    return oracle.norm_matrix(A_mc, wm.n_gen)
+
+
+def run_reference(args):
+    rank, ws, _ = dist_env()
+    if rank != 0:
+        return 0
+    from oracle import oracle
+    from paper_1108_5882_b200.inputs import synth
+    cfg = WORKLOADS[args.workload]
+    spec = synth._CFG[cfg]
+    n_data, _ = sizes_for(args, spec)
+    K, W = args.steps, args.warmup
+    target = min(SAMPLE_TARGET_S, 150.0 / max(1, K + W))
+    # generate a bounded prefix of the data sample (the generator is sequential in candidate
+    # order, so the first S accepted events of the full workload are exactly these)
+    cap = min(n_data, 400_000)
+    w = synth.make_workload(cfg, n_data=cap, n_mc=1, want_mc=False)
+    A = w.A_data if w.A_data is not None else synth.amplitudes(w, w.kin_data)
+    M = small_oracle_norm(synth, oracle, cfg)
+    Vs = synth.eval_points(w, K + W)
+    S = oracle_sample_size(oracle, A, M, Vs[0], cap, target)
+    A = np.ascontiguousarray(A[:S])
+    for i in range(W):
+        oracle.nll_grad(A, M, Vs[i])
+    t0 = time.perf_counter()
+    for i in range(K):
+        oracle.nll_grad(A, M, Vs[W + i])
+    dt = time.perf_counter() - t0
+    value = S * w.n * K / dt
+    sample = f"first {S} of {n_data} data events of {args.workload} (n={w.n}, {w.storage} storage), full lnL+gradient per step"
+    line = {
+        "impl": "reference", "metric": "event-waves/s (lnL+gradient evaluation)", "value": value,
+        "unit": "event-waves/s", "n_gpus": args.gpus, "steps": K, "warmup": W,
+        "ms_per_step": dt / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "n_waves": w.n, "n_data": n_data, "storage": w.storage,
+                   "sample_events": S},
+        "evals_per_s": K / dt * (S / n_data),
+        "cpu_baseline": {"value": value, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "event-waves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------- our arm
+class Timer:
+    """CUDA-event timing on torch's current stream (the stream every pwa context here uses)."""
+
+    def __init__(self, torch):
+        self.torch = torch
+
+    def run(self, fn, steps, warmup, barrier=None):
+        torch = self.torch
+        for i in range(warmup):
+            fn(i)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if barrier:
+            barrier()
+            torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0.record()
+        for i in range(steps):
+            fn(warmup + i)
+        e1.record()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        if barrier:
+            barrier()
+        return e0.elapsed_time(e1) / steps, wall / steps * 1e3      # ms per step (device, wall)
+
+
+def upload_constant(pwa, ctx, w):
+    t0 = time.perf_counter()
+    pwa.pwa_upload_events(ctx, pwa.PWA_DATA, w.A_data)
+    pwa.pwa_sync(ctx)
+    return time.perf_counter() - t0
+
+
+def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
+    """Single-rank side measurement of a constant-resonance config -> dict."""
+    tm = Timer(torch)
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = pwa.pwa_create(w.n, w.storage, torch.cuda.current_device(), stream)
+    out = {}
+    try:
+        up_s = upload_constant(pwa, ctx, w)
+        n = w.n
+        M0 = np.zeros((n, n, 2)); M0[np.arange(n), np.arange(n), 0] = 1.0
+        if w.A_mc is not None:
+            pwa.pwa_upload_events(ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+            ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), 3, 1)
+            flops = 8.0 * n * n * w.n_acc
+            out["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": flops / ms_m * 1e-6,
+                              "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
+        else:
+            pwa.pwa_set_norm(ctx, M0)
+        Vs = synth.eval_points(w, steps + warmup)
+        ms, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i]), steps, warmup)
+        t0 = time.perf_counter()
+        for i in range(steps):
+            pwa.pwa_nll_grad(ctx, Vs[warmup + i])
+        wall = (time.perf_counter() - t0) / steps * 1e3
+        nbytes = w.n_data * n * 2 * elem
+        out.update({"n_waves": n, "n_data": w.n_data, "storage": w.storage, "ms_per_eval": ms,
+                    "evals_per_s": 1e3 / ms, "event_waves_per_s": w.n_data * n / ms * 1e3,
+                    "algorithmic_gbs": nbytes / ms * 1e-6, "e2e_ms_per_eval": wall,
+                    "e2e_evals_per_s": 1e3 / wall, "upload_s": up_s,
+                    "l2_resident": bool(nbytes < 100e6)})
+        if w.K > 1:
+            Vk = synth.eval_points(w, w.K, stream=synth.S_START)
+            ms_b, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
+            out["batch"] = {"K": w.K, "ms_per_call": ms_b, "evals_per_s": w.K / ms_b * 1e3,
+                            "event_waves_per_s": w.n_data * n * w.K / ms_b * 1e3,
+                            "gflops": 16.0 * w.n_data * n * w.K / ms_b * 1e-6}
+    finally:
+        pwa.pwa_destroy(ctx)
+    return out
+
+
+def bench_floating(torch, pwa, synth, w, steps, warmup):
+    """cfg3: per quasi-Newton iteration = set_resonances + build_norm (fused BW over MC) +
+    nll_grad (fused BW over data) + res_grad (analytic d/dM_r, d/dG_r; reading A9)."""
+    tm = Timer(torch)
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = pwa.pwa_create(w.n, w.storage, torch.cuda.current_device(), stream)
+    try:
+        pwa.pwa_upload_events_factored(ctx, pwa.PWA_DATA, w.mass_data, w.Z_data)
+        pwa.pwa_upload_events_factored(ctx, pwa.PWA_MC, w.mass_mc, w.Z_mc, n_generated=w.n_gen)
+        pwa.pwa_set_wave_map(ctx, w.n_res, w.res_of_wave, w.ang_of_wave)
+        Mr0, Gr0 = synth.floating_start(w)
+        Vs = synth.eval_points(w, steps + warmup)
+        jit = synth.cnormal(w.seed, synth.S_START + 1, steps + warmup)
+
+        def params(i):
+            Mr, Gr = Mr0.copy(), Gr0.copy()
+            Mr[: w.n_free] *= 1.0 + 1e-3 * jit[i, 0]
+            Gr[: w.n_free] *= 1.0 + 1e-3 * jit[i, 1]
+            return Mr, Gr
+
+        def it_dev(i):
+            Mr, Gr = params(i)
+            pwa.pwa_set_resonances(ctx, Mr, Gr)
+            pwa.pwa_build_norm(ctx, want_M=False)
+            pwa.pwa_nll_grad_enqueue(ctx, Vs[i])
+
+        def it_full(i):
+            Mr, Gr = params(i)
+            pwa.pwa_set_resonances(ctx, Mr, Gr)
+            pwa.pwa_build_norm(ctx, want_M=False)
+            pwa.pwa_nll_grad(ctx, Vs[i])
+            pwa.pwa_res_grad(ctx, Vs[i], w.n_res)
+
+        def only_norm(i):
+            Mr, Gr = params(i)
+            pwa.pwa_set_resonances(ctx, Mr, Gr)
+            pwa.pwa_build_norm(ctx, want_M=False)
+
+        ms_it, _ = tm.run(it_dev, steps, warmup)
+        ms_norm, _ = tm.run(only_norm, steps, warmup)
+        _, wall_full = tm.run(it_full, steps, warmup)
+        return {"n_waves": w.n, "n_data": w.n_data, "n_mc": w.n_acc, "storage": w.storage,
+                "ms_per_iteration_nll_grad_plus_norm": ms_it, "ms_norm_build_fused_bw": ms_norm,
+                "ms_data_term_fused_bw": ms_it - ms_norm,
+                "e2e_ms_per_iteration_with_res_grad": wall_full,
+                "iterations_per_s": 1e3 / ms_it,
+                "event_waves_per_s": (w.n_data + w.n_acc) * w.n / ms_it * 1e3}
+    finally:
+        pwa.pwa_destroy(ctx)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, ws, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if ws > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.gpus != ws and rank == 0:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={ws}; using {ws}\n")
+    import __graft_entry__
+    if rank == 0:
+        __graft_entry__.build()
+    if ws > 1:
+        dist.barrier()
+    from paper_1108_5882_b200 import binding as pwa
+    from paper_1108_5882_b200 import sharded
+    from paper_1108_5882_b200.inputs import synth
+
+    cfg = WORKLOADS[args.workload]
+    spec = synth._CFG[cfg]
+    n_data, n_mc = sizes_for(args, spec)
+    K, W = args.steps, args.warmup
+    if W < 3:
+        raise SystemExit("bench.py: --warmup must be >= 3")
+    peak, peak_src, _ = load_peaks()
+    elem = 8 if spec["storage"] == "f64" else 4
+    extra_on = (not args.no_extra) and ws == 1
+    tm = Timer(torch)
+    barrier = (lambda: dist.barrier()) if ws > 1 else None
+    stream = torch.cuda.current_stream().cuda_stream
+    dev = torch.device("cuda", local)
+    t_gen = time.perf_counter()
+
+    if spec["factored"]:
+        # cfg3 as the main workload: a step is one floating-resonance iteration
+        w = synth.make_workload(cfg, n_data=n_data, n_mc=n_mc, full_amplitudes=False, shard=rank)
+        if ws > 1:
+            raise SystemExit("bench.py: the cfg3 step is single-GPU here; use the default workload for N > 1")
+        clk = ClockSampler(local); clk.start()
+        r = bench_floating(torch, pwa, synth, w, K, W)
+        clk.stop()
+        ms = r["ms_per_iteration_nll_grad_plus_norm"]
+        line = {"metric": "event-waves/s (floating-resonance iteration: M rebuild + lnL+gradient)",
+                "value": r["event_waves_per_s"], "unit": "event-waves/s", "n_gpus": ws, "steps": K, "warmup": W,
+                "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "n_waves": w.n, "n_data": w.n_data, "n_mc": w.n_acc,
+                           "storage": w.storage, "l2": "factored inputs 200 MB > L2 126 MB"},
+                "e2e": {"value": (w.n_data + w.n_acc) * w.n / r["e2e_ms_per_iteration_with_res_grad"] * 1e3,
+                        "unit": "event-waves/s", "h2d_bytes_per_step": 16 * w.n + 16 * w.n_res,
+                        "d2h_bytes_per_step": 8 * (4 + 2 * w.n) + 16 * w.n_res},
+                "roofline": {"bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None,
+                             "traffic": None, "note": "see DESIGN.md section 7 (fused Breit-Wigner passes are fp64-ALU bound)"},
+                "clocks": clk.summary(), "extra": {"cfg3": r}, "gpu_launches": None}
+        print(json.dumps(line), flush=True)
+        return 0
+
+    w = synth.make_workload(cfg, n_data=n_data, n_mc=(n_mc if extra_on or ws > 1 else 1),
+                            want_mc=(extra_on or ws > 1), shard=rank)
+    gen_s = time.perf_counter() - t_gen
+    n = w.n
+    ctx = pwa.pwa_create(n, w.storage, local, stream)
+    extra = {"generate_s": gen_s}
+    try:
+        up_s = upload_constant(pwa, ctx, w)
+        bytes_data = w.n_data * n * 2 * elem
+        extra["upload_data_s"] = up_s
+        # ---- normalisation matrix (once per fit; not part of the step)
+        if w.A_mc is not None:
+            pwa.pwa_upload_events(ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+            ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), 3, 1)
+            extra["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": 8.0 * n * n * w.n_acc / ms_m * 1e-6,
+                                "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
+            M_local = pwa.pwa_build_norm(ctx)
+            if ws > 1:
+                M_all, _ = sharded.combine_norm(M_local, w.n_gen, device=dev)
+                pwa.pwa_set_norm(ctx, M_all)
+            else:
+                M_all = M_local
+            w.A_mc = None   # free 10 GB of host memory
+        else:
+            M_all = np.zeros((n, n, 2)); M_all[np.arange(n), np.arange(n), 0] = 1.0
+            pwa.pwa_set_norm(ctx, M_all)
+        Vs = synth.eval_points(w, 2 * (K + W))
+        out_dev = torch.zeros(2 + 2 * n, dtype=torch.float64, device=dev)
+
+        # ---- the timed region: K steps, device-timed
+        if ws == 1:
+            step = lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i])          # noqa: E731
+        else:
+            def step(i):
+                pwa.pwa_data_term_enqueue(ctx, Vs[i], out_dev)
+                sharded.reduce_terms(out_dev)
+        clk = ClockSampler(local)
+        l0 = pwa.pwa_launch_count(ctx)
+        for i in range(W):
+            step(i)
+        torch.cuda.synchronize()
+        l0 = pwa.pwa_launch_count(ctx)
+        clk.start()
+        ms, _ = tm.run(step, K, 0, barrier)
+        clk.stop()
+        launches = pwa.pwa_launch_count(ctx) - l0
+        # kernel-only loop for the roofline when the step also holds a collective
+        if ws > 1:
+            ms_kernel, _ = tm.run(lambda i: pwa.pwa_data_term_enqueue(ctx, Vs[i], out_dev), K, W)
+        else:
+            ms_kernel = ms
+        # ---- end to end: synchronous C-ABI call, host V in, host results out
+        def e2e_step(i):
+            if ws == 1:
+                return pwa.pwa_nll_grad(ctx, Vs[K + W + i])
+            pwa.pwa_data_term_enqueue(ctx, Vs[K + W + i], out_dev)
+            t = sharded.reduce_terms(out_dev).cpu().numpy()
+            return pwa.pwa_assemble_host(t[0], t[2:].reshape(n, 2), M_all, Vs[K + W + i])
+        for i in range(W):
+            e2e_step(i)
+        torch.cuda.synchronize()
+        if barrier:
+            barrier()
+        t0 = time.perf_counter()
+        for i in range(K):
+            e2e_step(W + i)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) / K * 1e3
+        if ws > 1:
+            t = torch.tensor([ms, wall_ms, ms_kernel], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms, wall_ms, ms_kernel = (float(x) for x in t.tolist())
+    finally:
+        pwa.pwa_destroy(ctx)
+
+    if rank != 0:
+        if ws > 1:
+            dist.barrier(); dist.destroy_process_group()
+        return 0
+
+    units = w.n_data * n * ws                      # event-waves per step, all ranks (weak scaling)
+    achieved = bytes_data / ms_kernel * 1e-6       # GB/s, algorithmic bytes of one launch
+    kernel_key = f"k_data_term_{w.storage}_n{n}"
+    line = {
+        "metric": "event-waves/s (lnL+gradient evaluation)", "value": units / ms * 1e3, "unit": "event-waves/s",
+        "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "n_waves": n, "n_data_per_gpu": w.n_data, "storage": w.storage,
+                   "parallelism": f"event-sharded x{ws}" if ws > 1 else "single GPU",
+                   "l2": f"input {bytes_data / 1e6:.0f} MB per step vs 126 MB L2: "
+                         + ("larger than L2, no flush needed" if bytes_data > 2.5e8 else "L2-RESIDENT (latency-bound config)")},
+        "evals_per_s": 1e3 / ms,
+        "e2e": {"value": units / wall_ms * 1e3, "unit": "event-waves/s", "ms_per_step": wall_ms,
+                "evals_per_s": 1e3 / wall_ms, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 8 * (4 + 2 * n),
+                "note": "events are uploaded once per fit (upload_data_s in extra), V and results cross every step"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": load_traffic(kernel_key), "peak_source": peak_src, "kernel": kernel_key,
+                     "algorithmic_bytes_per_launch": bytes_data},
+        "clocks": clk.summary(), "gpu_launches": int(launches),
+    }
+    if extra_on:
+        line["cpu_baseline"] = cpu_baseline(synth, w, M_all, Vs[0], args.workload)
+        line["extra"] = side_measurements(torch, pwa, synth, args, extra)
+    else:
+        line["extra"] = extra
+        if ws == 1:
+            line["cpu_baseline"] = cpu_baseline(synth, w, M_all, Vs[0], args.workload)
+    print(json.dumps(line), flush=True)
+    if ws > 1:
+        dist.barrier(); dist.destroy_process_group()
+    return 0
+
+
+def cpu_baseline(synth, w, M, V, name):
+    """The oracle as it stands on this box's host cores, on a prefix of the same data."""
+    from oracle import oracle
+    S = oracle_sample_size(oracle, w.A_data, M, V, w.n_data, 5.0)
+    A = np.ascontiguousarray(w.A_data[:S])
+    reps, t0 = 3, time.perf_counter()
+    for _ in range(reps):
+        oracle.nll_grad(A, M, V)
+    dt = (time.perf_counter() - t0) / reps
+    return {"value": S * w.n / dt, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"first {S} of {w.n_data} data events of {name}, {reps} full lnL+gradient evaluations, {dt:.2f} s each"}
+
+
+def side_measurements(torch, pwa, synth, args, extra):
+    """Other configs of BASELINE.json, single GPU, each in the launch configuration the tests check."""
+    try:
+        w2 = synth.make_workload(2)
+        extra["cfg2"] = bench_constant(torch, pwa, synth, w2, 50, 5, 4)
+        del w2
+        w1 = synth.make_workload(1)
+        extra["cfg1"] = bench_constant(torch, pwa, synth, w1, 100, 5, 8)
+        del w1
+        w3 = synth.make_workload(3, full_amplitudes=False)
+        extra["cfg3"] = bench_floating(torch, pwa, synth, w3, 20, 3)
+        del w3
+        if args.workload == "cfg4":
+            w4 = synth.make_workload(4, n_mc=1, want_mc=False)
+            w4.A_mc = None
+            r = bench_constant(torch, pwa, synth, w4, 3, 3, 4)
+            extra["cfg4_batch"] = r.get("batch")
+    except Exception as e:   # side measurements must never lose the main line
+        extra["error"] = repr(e)
+    return extra
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

@@ -170,12 +170,17 @@ def _accept(w, seed, s0, n_want, mode, i_max, V):
 def make_workload(cfg: int, seed: int = DEFAULT_SEED, n_data: Optional[int] = None,
                   n_mc: Optional[int] = None, storage: Optional[str] = None,
                   want_data: bool = True, want_mc: bool = True,
-                  full_amplitudes: bool = True) -> Workload:
+                  full_amplitudes: bool = True, shard: int = 0) -> Workload:
     """Build configs[cfg] (optionally with reduced event counts for CPU-side tests).
 
     want_data / want_mc = False skip generating that sample (bench legs that need one only).
     full_amplitudes=False skips the [N, n, 2] matrices for a factored workload.
+    shard: index of an event-sharded rank (0..23).  The model (resonances, V_true, I_max) is
+    the same for every shard; only the candidate streams of the data and MC kinematics differ,
+    so shards are disjoint, independent samples of the same distribution.
     """
+    if not 0 <= shard < 24:
+        raise ValueError("shard must be in [0, 24)")
     spec = _CFG[cfg]
     n_res = spec["n_res"]
     if spec["fixed"] is not None:
@@ -205,9 +210,9 @@ def make_workload(cfg: int, seed: int = DEFAULT_SEED, n_data: Optional[int] = No
                                         C.c_int(eff), C.c_int(n_res), _p(Mr), _p(Gr), C.c_int(n),
                                         _p(res_of_wave), _p(yw), _p(V_true))
         w.i_max = 1.5 * float(pilot)                                  # C11
-        w.kin_data, _, w.n_over = _accept(w, seed, S_DATA, w.n_data, 2 | eff, w.i_max, V_true)
+        w.kin_data, _, w.n_over = _accept(w, seed, S_DATA + 4 * shard, w.n_data, 2 | eff, w.i_max, V_true)
     if want_mc:
-        w.kin_mc, w.n_gen, _ = _accept(w, seed, S_MC, w.n_acc, eff, 1.0, V_true)   # C9
+        w.kin_mc, w.n_gen, _ = _accept(w, seed, S_MC + 4 * shard, w.n_acc, eff, 1.0, V_true)   # C9
     factored = spec["factored"]
     if factored:
         if want_data:

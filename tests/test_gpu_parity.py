@@ -36,14 +36,17 @@ class Ctx:
         self.pwa.pwa_destroy(self.ctx)
 
 
-def check_eval(res, ref, tol, N):
+def check_eval(res, ref, tol, N, gscale=0.0):
+    """gscale: extra gradient scale for points where the data and norm gradients cancel
+    (near a stationary point |g| -> 0 while each term stays O(N); C8: the tolerance is
+    norm-wise on the terms that are actually summed)."""
     nll, g, parts = res[0], res[1], res[2]
     nll_o, g_o, parts_o = ref[0], ref[1], ref[2]
     scaleL = max(abs(parts_o[0]), 1e-2 * N, 1e-300)
     assert abs(parts[0] - parts_o[0]) <= tol * scaleL, ("L_data", parts[0], parts_o[0])
     assert abs(parts[1] - parts_o[1]) <= tol * max(abs(parts_o[1]), 1e-300), ("Norm", parts[1], parts_o[1])
     assert abs(nll - nll_o) <= tol * max(abs(nll_o), scaleL), ("nll", nll, nll_o)
-    gs = np.abs(g_o).max()
+    gs = max(np.abs(g_o).max(), gscale)
     assert np.abs(g - g_o).max() <= tol * gs, ("grad", np.abs(g - g_o).max() / gs)
 
 
@@ -283,7 +286,10 @@ def test_bfgs_converges_on_cfg0(pwa, oracle, synth):
     assert nll_fit <= prof_true + 1e-6 * abs(prof_true)
     assert nll_fit <= nll_true
     # the oracle agrees with the GPU at the fitted point
-    check_eval((nll_fit, g_fit, parts), oracle.nll_grad(w.A_data, M, Vfit), 1e-12, w.n_data)
+    # (there g = -2 conj(T) + 2 M V cancels to ~1e-6 of either term: scale by |2 M V|)
+    g_norm = oracle.assemble(0.0, np.zeros((w.n, 2)), M, Vfit)[1]
+    check_eval((nll_fit, g_fit, parts), oracle.nll_grad(w.A_data, M, Vfit), 1e-12, w.n_data,
+               gscale=np.abs(g_norm).max())
 
 
 def test_bfgs_batch_lockstep(pwa, synth):

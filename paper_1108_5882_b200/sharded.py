@@ -36,11 +36,11 @@ def sum_in_rank_order(x: torch.Tensor, group=None) -> torch.Tensor:
     if ws == 1:
         return x.clone()
     x = x.contiguous()
-    buf = torch.empty((ws,) + tuple(x.shape), dtype=x.dtype, device=x.device)
-    dist.all_gather_into_tensor(buf, x, group=group)
-    out = buf[0].clone()
+    parts = [torch.empty_like(x) for _ in range(ws)]
+    dist.all_gather(parts, x, group=group)
+    out = parts[0].clone()
     for r in range(1, ws):
-        out += buf[r]
+        out += parts[r]
     return out
 
 

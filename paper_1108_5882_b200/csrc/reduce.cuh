@@ -32,6 +32,50 @@ __device__ __forceinline__ double warp_sum(double x)
     return x;
 }
 
+// Step A7 from block totals s_tot[0..2+2n) = {L_data, n_nonfinite, Re T_0, Im T_0, ...} and V in
+// shared memory: M == nullptr -> copy the data-term components to out[0..2+2n); otherwise write
+// the result record {nll, L_data, Norm, n_nonfinite, grad[2n]} (P:41 second term).
+// Must be called by every thread of the block; s_tot and sV valid for all threads on entry.
+__device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
+                                            double *out, int n)
+{
+    const int NC = 2 + 2 * n;
+    const int tid = threadIdx.x, nthreads = blockDim.x;
+    const int lane = tid & 31, warp = tid >> 5;
+    __shared__ double s_mv[2 * kMaxWaves];
+    if (M == nullptr) {
+        for (int c = tid; c < NC; c += nthreads) out[c] = s_tot[c];
+        return;
+    }
+    // (M V)_a, one row per thread
+    for (int a = tid; a < n; a += nthreads) {
+        const double *row = M + (size_t)a * n * 2;
+        double mr = 0.0, mi = 0.0;
+        for (int b = 0; b < n; ++b) {
+            double Mr = row[2 * b], Mi = row[2 * b + 1];
+            double vr = sV[2 * b], vi = sV[2 * b + 1];
+            mr = fma(Mr, vr, mr); mr = fma(-Mi, vi, mr);
+            mi = fma(Mr, vi, mi); mi = fma(Mi, vr, mi);
+        }
+        s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi;
+        // grad_a = -2 conj(T_a) + 2 (M V)_a
+        out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + 2.0 * mr;
+        out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + 2.0 * mi;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        double acc = 0.0;   // Norm = sum_a Re( conj(V_a) (M V)_a )
+        for (int a = lane; a < n; a += 32) acc += sV[2 * a] * s_mv[2 * a] + sV[2 * a + 1] * s_mv[2 * a + 1];
+        acc = warp_sum(acc);
+        if (lane == 0) {
+            out[0] = -(s_tot[0] - acc);
+            out[1] = s_tot[0];
+            out[2] = acc;
+            out[3] = s_tot[1];
+        }
+    }
+}
+
 // s_tot[0..NC): this block's totals (valid for all threads after a __syncthreads by the
 // caller).  sV: V in shared memory [2n].  Must be called by every thread of the block.
 __device__ inline void block_finish(double *s_tot, const double *sV, const FinishArgs &fa)
@@ -40,7 +84,6 @@ __device__ inline void block_finish(double *s_tot, const double *sV, const Finis
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
     __shared__ bool s_last;
-    __shared__ double s_mv[2 * kMaxWaves];
 
     for (int c = tid; c < NC; c += nthreads) fa.partials[(size_t)c * gridDim.x + blockIdx.x] = s_tot[c];
     __threadfence();
@@ -60,37 +103,7 @@ __device__ inline void block_finish(double *s_tot, const double *sV, const Finis
     }
     __syncthreads();
 
-    if (fa.M == nullptr) {
-        for (int c = tid; c < NC; c += nthreads) fa.out[c] = s_tot[c];
-    } else {
-        // (M V)_a, one row per thread
-        for (int a = tid; a < n; a += nthreads) {
-            const double *row = fa.M + (size_t)a * n * 2;
-            double mr = 0.0, mi = 0.0;
-            for (int b = 0; b < n; ++b) {
-                double Mr = row[2 * b], Mi = row[2 * b + 1];
-                double vr = sV[2 * b], vi = sV[2 * b + 1];
-                mr = fma(Mr, vr, mr); mr = fma(-Mi, vi, mr);
-                mi = fma(Mr, vi, mi); mi = fma(Mi, vr, mi);
-            }
-            s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi;
-            // grad_a = -2 conj(T_a) + 2 (M V)_a
-            fa.out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + 2.0 * mr;
-            fa.out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + 2.0 * mi;
-        }
-        __syncthreads();
-        if (warp == 0) {
-            double acc = 0.0;   // Norm = sum_a Re( conj(V_a) (M V)_a )
-            for (int a = lane; a < n; a += 32) acc += sV[2 * a] * s_mv[2 * a] + sV[2 * a + 1] * s_mv[2 * a + 1];
-            acc = warp_sum(acc);
-            if (lane == 0) {
-                fa.out[0] = -(s_tot[0] - acc);
-                fa.out[1] = s_tot[0];
-                fa.out[2] = acc;
-                fa.out[3] = s_tot[1];
-            }
-        }
-    }
+    assemble_from_totals(s_tot, sV, fa.M, fa.out, n);
     if (tid == 0) *fa.ticket = 0u;   // re-arm for the next launch on this stream
 }
 

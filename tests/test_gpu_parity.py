@@ -161,13 +161,18 @@ def test_nonfinite_warning(pwa, oracle):
 
 
 # ------------------------------------------------------------------ batched == single == oracle
-@pytest.mark.parametrize("storage,n,K", [("f64", 4, 3), ("f64", 16, 8), ("f32", 32, 5), ("f32", 64, 64), ("f64", 5, 2)])
-def test_batch_matches_single_and_oracle(pwa, oracle, storage, n, K):
+@pytest.mark.parametrize("storage,n,K,opt", [
+    ("f64", 4, 3, 0), ("f64", 16, 8, 0), ("f32", 32, 5, 0), ("f32", 64, 64, 0), ("f64", 5, 2, 0),
+    # opt 1 forces the tensor-core (DMMA) chained-GEMM path for any K; 99 forces K streaming passes
+    ("f64", 4, 3, 1), ("f64", 5, 2, 1), ("f32", 3, 33, 1), ("f64", 8, 40, 1), ("f64", 16, 65, 1),
+    ("f32", 20, 7, 1), ("f64", 32, 31, 1), ("f64", 64, 33, 1), ("f32", 64, 64, 99), ("f64", 1, 9, 1)])
+def test_batch_matches_single_and_oracle(pwa, oracle, storage, n, K, opt):
     A, B, _ = rand_case(31 + n, 6007, 2003, n, storage)
     Vk = np.random.default_rng(K).normal(size=(K, n, 2))
     M_o = oracle.norm_matrix(B, 2100)
     nll_o, g_o, parts_o, _ = oracle.nll_grad_batch(A, M_o, Vk)
     with Ctx(pwa, n, storage) as c:
+        pwa.pwa_set_option(c.ctx, "batch", opt)
         pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
         pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2100)
         pwa.pwa_build_norm(c.ctx)

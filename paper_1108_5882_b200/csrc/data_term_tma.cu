@@ -1,0 +1,355 @@
+// data_term_tma.cu — steps A2-A5, TMA-tiled two-phase kernel.  Used for
+// rows that are a whole number of 128-byte lines (fp32: n = 16, 32, 64; fp64: n = 8 ... 64).
+//
+//   S_i = sum_a V_a A_ia, I_i = |S_i|^2                eq. 1
+//   L_data = sum_i ln I_i                              eq. 3 first term
+//   T_a = sum_i A_ia / S_i                             gradient of L_data
+//
+// Warps work in groups of GW; a group owns a ring of NS shared-memory stages and its tiles are
+// taken round-robin (tile t of the group: warp t % GW, stage t % NS), so GW tiles are being
+// processed while NS-GW are in flight.  A stage is a tile of TR = 32/LPR
+// consecutive events, fetched by the TMA unit (cp.async.bulk.tensor.2d, SASS UTMALDG) as CB column
+// boxes of [TR rows x 128 bytes] with the 128-byte swizzle: the 16-byte chunk c of row r lands at
+// slot c ^ (r & 7) of its 128-byte line.  That makes BOTH access patterns conflict-free:
+//   phase 1 (lane = event, LPR lanes per row): every lane walks its own row; the 8 lanes of a
+//            quarter-warp sit on 8 consecutive rows and hit 8 different slots.  S_i is formed with
+//            no cross-lane traffic (LPR = 1) or one shuffle-add (LPR > 1); V comes from the constant
+//            bank (kernel parameter, LPR = 1) or shared memory (LPR > 1).  ONE log and ONE
+//            reciprocal per event (no redundancy); r_i = 1/S_i goes to a 16-byte smem slot.
+//   phase 2 (lane = 16-byte chunk of the row = 1 or 2 waves): the warp walks the tile's rows, each
+//            lane accumulates A_ia * r_i for its own waves (r_i is a broadcast load).
+// The tile is read from HBM once and from shared memory twice.  Out-of-range rows of the last
+// tile are zero-filled by the TMA unit and masked (r_i = 0, not counted).  Lane 0 re-arms a stage
+// (with the group's tile t + NS) right after its warp has finished phase 2 of tile t and bumps the
+// stage's issue counter; the next owner of the stage waits for that counter and then for the TMA
+// completion barrier (no block barrier inside the loop).
+// ln I_i is accumulated as a running product of mantissas plus an integer exponent sum, with one
+// log per 256 events per lane (P:47 leaves the summation algorithm open; the error of the product,
+// <= 256 * 2^-53 relative, is of the same order as the rounding of 256 separate logs); 1/I_i is a
+// MUFU seed plus two Newton steps.  Abnormal intensities (0, denormal, inf, nan: reading C14)
+// take the plain IEEE log / division path.  Reduction: reduce.cuh (A5, A7).
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
+#include "pwa_internal.h"
+#include "reduce.cuh"
+#include "stream_common.cuh"
+
+namespace pwa {
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *tmap, int x, int y, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(tmap), "r"(x), "r"(y), "r"(bar) : "memory");
+}
+
+__device__ __forceinline__ double2 lds_d2(uint32_t addr)
+{
+    double2 r;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ void sts_d2(uint32_t addr, double x, double y)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(x), "d"(y) : "memory");
+}
+
+template <typename ST, int CB, int LPR, int THREADS, int GW, int NS>
+struct TmaCfg {
+    static constexpr int WPC = Chunk<ST>::WPC;
+    static constexpr int CPR = CB * 8;                  // 16-byte chunks per row
+    static constexpr int NW = CPR * WPC;                // waves
+    static constexpr int TR = 32 / LPR;                 // rows per warp tile
+    static constexpr int BOXB = TR * 128;               // bytes per column box
+    static constexpr int STAGE = CB * BOXB;             // bytes per stage
+    static constexpr int CPL1 = CPR / LPR;              // chunks per lane, phase 1
+    static constexpr int CK2 = CPR > 32 ? CPR / 32 : 1; // chunks per lane, phase 2
+    static constexpr int G2 = CPR / CK2;                // lanes per row, phase 2
+    static constexpr int RPI = 32 / G2;                 // rows per phase-2 iteration
+    static constexpr int NWARPS = THREADS / 32;
+    static constexpr int NGRP = NWARPS / GW;              // warp groups per CTA
+    static constexpr size_t SMEM = (size_t)NGRP * NS * STAGE + 1024;
+    static_assert(NWARPS % GW == 0 && NS > GW - 1 && NS >= 2, "ring shape");
+    static_assert(CPL1 % 8 == 0 || LPR == 1, "a lane's phase-1 share must be whole column boxes");
+    static_assert(TR % 8 == 0, "swizzle atom is 8 rows");
+};
+
+// Fast 1/x for normal positive x well inside the exponent range: MUFU.RCP64H seed (~2^-20)
+// + two Newton steps (error <= ~1 ulp).
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
+template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS>
+__global__ void __launch_bounds__(THREADS, MINB)
+k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, const __grid_constant__ VArg varg, FinishArgs fa)
+{
+    using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
+    constexpr int WPC = C::WPC, NW = C::NW, TR = C::TR, BOXB = C::BOXB, STAGE = C::STAGE;
+    constexpr int CPL1 = C::CPL1, CK2 = C::CK2, G2 = C::G2, RPI = C::RPI, NWARPS = C::NWARPS, NGRP = C::NGRP;
+    constexpr int W2 = CK2 * WPC;
+    constexpr int BOX_ELEMS = 128 / (int)sizeof(ST);
+    constexpr int NIT2 = TR / RPI;                     // phase-2 iterations per tile
+    constexpr int U2 = (NIT2 % 2 == 0) ? 2 : 1;        // independent accumulator sets in phase 2
+    constexpr int FLUSH = 256;                         // tiles between two logs of the mantissa product
+
+    extern __shared__ unsigned char tma_smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[NGRP][NS];
+    __shared__ volatile int issued[NGRP][NS];          // number of tiles issued into each stage so far (GW > 1)
+    __shared__ __align__(16) double rbuf[NWARPS][32][2];
+    __shared__ __align__(16) double sV[2 * NW];
+    for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = varg.v[t];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = warp / GW, wig = warp % GW;        // group in the CTA, warp in the group
+    const uint32_t ring0 = ((smem_u32(tma_smem_raw) + 1023u) & ~1023u) + (uint32_t)(grp * NS) * STAGE;
+    const uint32_t bar0 = smem_u32(&bars[grp][0]);
+    const uint32_t rb0 = smem_u32(&rbuf[warp][0][0]);
+    const uint32_t sv0 = smem_u32(sV);
+    if (wig == 0 && lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) { mbar_init(bar0 + 8 * s, 1); issued[grp][s] = 0; }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    // tile t of this group is global tile g0 + t * gstride; warp t % GW takes it in stage t % NS
+    const long long ntiles = (N + TR - 1) / TR;
+    const long long gstride = (long long)gridDim.x * NGRP;
+    const long long g0 = (long long)blockIdx.x * NGRP + grp;
+    const long long nt_grp = (ntiles > g0) ? (ntiles - g0 + gstride - 1) / gstride : 0;   // tiles of this group
+    auto issue = [&](long long t) {                              // lane 0 of the warp that owns tile t (or t - NS)
+        const int slot = (int)(t % NS);
+        mbar_expect_tx(bar0 + 8 * slot, STAGE);                  // OOB rows are zero-filled and still counted
+        const int y = (int)((g0 + t * gstride) * TR);
+#pragma unroll
+        for (int cb = 0; cb < CB; ++cb)
+            tma_load_2d(ring0 + (uint32_t)slot * STAGE + cb * BOXB, &tmap, cb * BOX_ELEMS, y, bar0 + 8 * slot);
+        if (GW > 1) { __threadfence_block(); issued[grp][slot] = (int)(t / NS) + 1; }
+    };
+    if (lane == 0) {
+        for (long long t = wig; t < NS && t < nt_grp; t += GW) issue(t);
+    }
+
+    // phase-1 coordinates: lane -> (row, part)
+    const int row1 = lane % TR, part = lane / TR;
+    uint32_t a1[8];                                               // per-slot address offsets of this lane's row
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+        a1[c] = (uint32_t)row1 * 128u + (uint32_t)((c ^ (row1 & 7)) << 4) + (LPR > 1 ? (uint32_t)(part * (CPL1 / 8)) * BOXB : 0u);
+    // phase-2 coordinates: lane -> (chunk(s), row selector)
+    const int g2 = lane % G2, rsel = lane / G2;
+    uint32_t a2[CK2]; int c2[CK2];
+#pragma unroll
+    for (int k = 0; k < CK2; ++k) {
+        const int ch = g2 + G2 * k;
+        a2[k] = (uint32_t)(ch >> 3) * BOXB;
+        c2[k] = (ch & 7) << 4;
+    }
+
+    double tr[U2][W2], ti[U2][W2];
+#pragma unroll
+    for (int u = 0; u < U2; ++u)
+#pragma unroll
+        for (int w = 0; w < W2; ++w) { tr[u][w] = 0.0; ti[u][w] = 0.0; }
+    double L = 0.0, bad = 0.0, P = 1.0;                          // P: running product of mantissas in [1, 2)
+    int esum = 0, since = 0;                                     // sum of unbiased exponents; tiles since the last flush
+
+    for (long long t = wig; t < nt_grp; t += GW) {
+        const int slot = (int)(t % NS);
+        const uint32_t parity = (uint32_t)((t / NS) & 1);
+        const uint32_t tile = ring0 + (uint32_t)slot * STAGE;
+        const long long row0 = (g0 + t * gstride) * TR;
+        // A stage is re-armed by the warp that consumed its previous tile, which may be another warp
+        // of the group: a parity wait is only unambiguous once that re-arm has happened (before it the
+        // barrier can still be one phase behind, and the flipped parity would read as "complete").
+        if (GW > 1) { const int need = (int)(t / NS) + 1; while (issued[grp][slot] < need) { } }
+        mbar_wait(bar0 + 8 * slot, parity);
+
+        // ---------------- phase 1: S_i, ln I_i, r_i
+        double sre[4] = {0.0, 0.0, 0.0, 0.0}, sim[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int i = 0; i < CPL1; ++i) {
+            const uint4 q = lds128(tile + a1[i & 7] + (uint32_t)(i >> 3) * BOXB);
+            double ar[WPC], ai[WPC];
+            Chunk<ST>::unpack(q, ar, ai);
+#pragma unroll
+            for (int w = 0; w < WPC; ++w) {
+                double vr, vi;
+                if (LPR == 1) { vr = varg.v[2 * (i * WPC + w)]; vi = varg.v[2 * (i * WPC + w) + 1]; }
+                else { const double2 v = lds_d2(sv0 + (uint32_t)((part * CPL1 + i) * WPC + w) * 16u); vr = v.x; vi = v.y; }
+                const int c = (i * WPC + w) & 1;                  // 2 x 2 independent chains per component
+                sre[c] = fma(vr, ar[w], sre[c]); sre[2 + c] = fma(-vi, ai[w], sre[2 + c]);
+                sim[c] = fma(vr, ai[w], sim[c]); sim[2 + c] = fma(vi, ar[w], sim[2 + c]);
+            }
+        }
+        double sr = (sre[0] + sre[1]) + (sre[2] + sre[3]), si = (sim[0] + sim[1]) + (sim[2] + sim[3]);
+#pragma unroll
+        for (int m = TR; m < 32; m <<= 1) { sr += shfl_xor_d(sr, m); si += shfl_xor_d(si, m); }
+        {
+            const bool valid = (row0 + row1) < N;
+            const bool counted = valid && part == 0;
+            const double I = sr * sr + si * si;
+            const int hi = __double2hiint(I);
+            const unsigned ex = ((unsigned)hi >> 20) & 0x7ffu;   // I >= 0 or nan: biased exponent (sign ignored)
+            const bool normal = (ex - 1u) < 0x7feu && hi > 0;    // not 0 / denormal / inf / nan / negative
+            double rr, rim;
+            if (__all_sync(0xffffffffu, normal || !valid)) {
+                const double inv = fast_rcp(valid ? I : 1.0);
+                rr = sr * inv; rim = -si * inv;                   // r = conj(S) / I
+                if (counted) {
+                    P *= __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(I));
+                    esum += (int)ex - 1023;
+                }
+            } else {                                              // reading C14: plain IEEE values
+                const double l = log(I);
+                const double inv = 1.0 / I;
+                rr = sr * inv; rim = -si * inv;
+                if (counted) { L += l; if (!(I > 0.0) || !isfinite(l)) bad += 1.0; }
+            }
+            if (!valid) { rr = 0.0; rim = 0.0; }
+            if (part == 0) sts_d2(rb0 + (uint32_t)row1 * 16u, rr, rim);
+            if (++since == FLUSH) { L += log(P); P = 1.0; since = 0; }
+        }
+        __syncwarp();
+
+        // ---------------- phase 2: T_a += A_ia r_i
+#pragma unroll 2
+        for (int it = 0; it < NIT2; it += U2) {
+#pragma unroll
+            for (int u = 0; u < U2; ++u) {
+                const int r = (it + u) * RPI + rsel;
+                const double2 rv = lds_d2(rb0 + (uint32_t)r * 16u);
+                const uint32_t rowa = tile + (uint32_t)r * 128u;
+                const int xr = (r & 7) << 4;
+#pragma unroll
+                for (int k = 0; k < CK2; ++k) {
+                    const uint4 q = lds128(rowa + a2[k] + (uint32_t)(c2[k] ^ xr));
+                    double ar[WPC], ai[WPC];
+                    Chunk<ST>::unpack(q, ar, ai);
+#pragma unroll
+                    for (int w = 0; w < WPC; ++w) {
+                        tr[u][k * WPC + w] = fma(ar[w], rv.x, tr[u][k * WPC + w]); tr[u][k * WPC + w] = fma(-ai[w], rv.y, tr[u][k * WPC + w]);
+                        ti[u][k * WPC + w] = fma(ar[w], rv.y, ti[u][k * WPC + w]); ti[u][k * WPC + w] = fma(ai[w], rv.x, ti[u][k * WPC + w]);
+                    }
+                }
+            }
+        }
+        __syncwarp();                                             // tile and rbuf fully consumed
+        if (lane == 0 && t + NS < nt_grp) issue(t + NS);
+    }
+    L += log(P) + 0.6931471805599453094 * (double)esum;
+    double trs[W2], tis[W2];
+#pragma unroll
+    for (int w = 0; w < W2; ++w) { trs[w] = tr[0][w]; tis[w] = ti[0][w]; if (U2 > 1) { trs[w] += tr[U2 - 1][w]; tis[w] += ti[U2 - 1][w]; } }
+    auto wave_of = [&](int idx) { return (g2 + G2 * (idx / WPC)) * WPC + (idx % WPC); };
+    reduce_and_finish<G2, W2, THREADS>(L, bad, trs, tis, wave_of, sV, fa);
+}
+
+// ---- host side: tensor map (driver entry point fetched through the runtime; no -lcuda) ----------
+static PFN_cuTensorMapEncodeTiled_v12000 get_encode()
+{
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+static pwa_status make_tmap(pwa_ctx *ctx, CUtensorMap *out, const void *base, bool f32, int n, long long N, int box_rows)
+{
+    PFN_cuTensorMapEncodeTiled_v12000 enc = get_encode();
+    if (!enc) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    const cuuint64_t gdim[2] = {(cuuint64_t)(2 * n), (cuuint64_t)N};
+    const cuuint64_t gstride[1] = {(cuuint64_t)(2 * n) * (f32 ? 4u : 8u)};
+    const cuuint32_t box[2] = {(cuuint32_t)(f32 ? 32 : 16), (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(out, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base),
+                     gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled failed (code " + std::to_string((int)r) + ")");
+    return PWA_OK;
+}
+
+template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS>
+static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa_in)
+{
+    using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
+    auto kern = k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS>;
+    const long long N = ctx->data.n_events;
+    CUtensorMap tmap;
+    pwa_status s = make_tmap(ctx, &tmap, ctx->data.amps, sizeof(ST) == 4, ctx->n, N, C::TR);
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+    int occ = 0;
+    PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, C::SMEM));
+    if (occ < 1) occ = 1;
+    const long long ntiles = (N + C::TR - 1) / C::TR;
+    long long want = (ntiles + C::NGRP - 1) / C::NGRP;
+    long long grid = (long long)ctx->sm_count * occ;
+    if (want < grid) grid = want;
+    if (grid < 1) grid = 1;
+    FinishArgs fa = fa_in;
+    s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
+    if (s != PWA_OK) return s;
+    fa.partials = ctx->d_partials;
+    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(tmap, N, varg, fa);
+    ctx->launches++;
+    PWA_CUDA(ctx, cudaGetLastError());
+    return PWA_OK;
+}
+
+// opt: 0 = default configuration of this kernel; 1.. = tuning variants (see the table below).
+pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, int opt, bool *handled)
+{
+    *handled = false;
+    const int n = ctx->n;
+    const bool f32 = ctx->storage == PWA_F32;
+    const long long N = ctx->data.n_events;
+    if (N < 1 || N > 0x7fffffffLL || ((uintptr_t)ctx->data.amps & 15u) != 0) return PWA_OK;
+    const int row_bytes = 2 * n * (f32 ? 4 : 8);
+    if (row_bytes % 128 != 0 || row_bytes > 1024 || (n & (n - 1)) != 0) return PWA_OK;
+    *handled = true;
+    //                                   ST    CB LPR THREADS MINB GW NS     stage bytes, notes
+    if (f32) {
+        switch (n) {
+        case 16: return launch_tma<float, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);                    //  4 KB
+        case 32: return opt == 1 ? launch_tma<float, 2, 2, 512, 1, 2, 3>(ctx, varg, fa)          //  4 KB
+                      : opt == 2 ? launch_tma<float, 2, 1, 512, 1, 2, 3>(ctx, varg, fa)          //  8 KB, 16 warps
+                                 : launch_tma<float, 2, 1, 256, 1, 1, 3>(ctx, varg, fa);         //  8 KB
+        case 64: return opt == 1 ? launch_tma<float, 4, 1, 256, 1, 2, 3>(ctx, varg, fa)          // 16 KB, V in the constant bank, 8 warps
+                      : opt == 2 ? launch_tma<float, 4, 2, 384, 1, 1, 2>(ctx, varg, fa)          //  8 KB, 12 warps, private rings
+                      : opt == 3 ? launch_tma<float, 4, 2, 512, 1, 4, 6>(ctx, varg, fa)          //  8 KB, 16 warps, groups of 4
+                      : opt == 4 ? launch_tma<float, 4, 1, 320, 1, 5, 6>(ctx, varg, fa)          // 16 KB, 10 warps, groups of 5
+                                 : launch_tma<float, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);         //  8 KB, 16 warps, groups of 2
+        }
+    } else {
+        switch (n) {
+        case 8:  return launch_tma<double, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);
+        case 16: return opt == 1 ? launch_tma<double, 2, 2, 512, 1, 2, 3>(ctx, varg, fa)
+                      : opt == 2 ? launch_tma<double, 2, 1, 512, 1, 2, 3>(ctx, varg, fa)
+                                 : launch_tma<double, 2, 1, 256, 1, 1, 3>(ctx, varg, fa);
+        case 32: return opt == 1 ? launch_tma<double, 4, 1, 256, 1, 2, 3>(ctx, varg, fa)
+                      : opt == 2 ? launch_tma<double, 4, 2, 384, 1, 1, 2>(ctx, varg, fa)
+                                 : launch_tma<double, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);
+        case 64: return opt == 1 ? launch_tma<double, 8, 2, 256, 1, 2, 3>(ctx, varg, fa)
+                      : opt == 2 ? launch_tma<double, 8, 4, 384, 1, 1, 2>(ctx, varg, fa)
+                                 : launch_tma<double, 8, 4, 512, 1, 2, 3>(ctx, varg, fa);
+        }
+    }
+    *handled = false;
+    return PWA_OK;
+}
+
+}  // namespace pwa

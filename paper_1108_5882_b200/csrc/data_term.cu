@@ -297,7 +297,7 @@ k_data_term_generic(const ST *__restrict__ A, long long N, const double *__restr
     const int n = fa.n, NC = 2 + 2 * n;
     double *sV = dyn;                         // [2n]
     double *s_acc = dyn + 2 * n;              // [NWARPS][NC]
-    double *s_tot = s_acc + NWARPS * NC;      // [NC]
+    double *s_tot = s_acc + (NWARPS * NC > THREADS ? NWARPS * NC : THREADS);   // [NC]; s_acc doubles as block_finish scratch (>= THREADS)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int t = tid; t < 2 * n; t += THREADS) sV[t] = Vdev[t];
     for (int t = tid; t < NWARPS * NC; t += THREADS) s_acc[t] = 0.0;
@@ -335,7 +335,7 @@ k_data_term_generic(const ST *__restrict__ A, long long N, const double *__restr
         s_tot[c] = t;
     }
     __syncthreads();
-    block_finish(s_tot, sV, fa);
+    block_finish(s_tot, s_acc, sV, fa);
 }
 
 template <typename ST, int G, int CK, int E, int THREADS, int MINB>
@@ -393,7 +393,7 @@ static pwa_status launch_generic(pwa_ctx *ctx, const double *Vdev, const FinishA
 {
     constexpr int THREADS = 128, NWARPS = THREADS / 32;
     const int n = ctx->n, NC = 2 + 2 * n;
-    size_t smem = sizeof(double) * (size_t)(2 * n + NWARPS * NC + NC);
+    size_t smem = sizeof(double) * (size_t)(2 * n + (NWARPS * NC > THREADS ? NWARPS * NC : THREADS) + NC);
     auto kern = k_data_term_generic<ST, THREADS>;
     if (smem > 48 * 1024)
         PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -112,6 +112,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, const __g
     const uint32_t bar0 = smem_u32(&bars[grp][0]);
     const uint32_t rb0 = smem_u32(&rbuf[warp][0][0]);
     const uint32_t sv0 = smem_u32(sV);
+    if (threadIdx.x == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     if (wig == 0 && lane == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(bar0 + 8 * s, 1); issued[grp][s] = 0; }
@@ -288,23 +289,32 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
     auto kern = k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS>;
     const long long N = ctx->data.n_events;
-    CUtensorMap tmap;
-    pwa_status s = make_tmap(ctx, &tmap, ctx->data.amps, sizeof(ST) == 4, ctx->n, N, C::TR);
-    if (s != PWA_OK) return s;
-    PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-    int occ = 0;
-    PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, C::SMEM));
-    if (occ < 1) occ = 1;
+    // per-instantiation, per-device launch plan: attribute + occupancy are queried once
+    static int s_occ[64] = {0};
+    int &occ = s_occ[ctx->device & 63];
+    if (occ == 0) {
+        PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        int o = 0;
+        PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, THREADS, C::SMEM));
+        occ = o < 1 ? 1 : o;
+    }
+    static_assert(sizeof(CUtensorMap) <= sizeof(ctx->tmap_cache.map), "tensor map cache too small");
+    auto &tc = ctx->tmap_cache;
+    if (!tc.valid || tc.base != ctx->data.amps || tc.n_events != N || tc.box_rows != C::TR) {
+        pwa_status s = make_tmap(ctx, reinterpret_cast<CUtensorMap *>(tc.map), ctx->data.amps, sizeof(ST) == 4, ctx->n, N, C::TR);
+        if (s != PWA_OK) return s;
+        tc.base = ctx->data.amps; tc.n_events = N; tc.box_rows = C::TR; tc.valid = true;
+    }
     const long long ntiles = (N + C::TR - 1) / C::TR;
     long long want = (ntiles + C::NGRP - 1) / C::NGRP;
     long long grid = (long long)ctx->sm_count * occ;
     if (want < grid) grid = want;
     if (grid < 1) grid = 1;
     FinishArgs fa = fa_in;
-    s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
+    pwa_status s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
     if (s != PWA_OK) return s;
     fa.partials = ctx->d_partials;
-    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(tmap, N, varg, fa);
+    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(*reinterpret_cast<const CUtensorMap *>(tc.map), N, varg, fa);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;

@@ -228,6 +228,7 @@ pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, i
     Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
     free_sample(smp);
     smp.amps = buf; smp.amps_owned = owned; smp.factored = false;
+    if (which == PWA_DATA) ctx->tmap_cache.valid = false;
     smp.n_events = n_events; smp.n_gen = n_generated;
     if (which == PWA_MC) ctx->M_valid = false;
     return PWA_OK;

@@ -63,6 +63,9 @@ struct pwa_ctx {
     double *d_V = nullptr; double *h_V = nullptr;            // [kMaxK][n][2]
     double *d_scratch = nullptr; size_t scratch_cap = 0;     // bytes (M partials, batch partials)
     int last_K = 0;
+    // cached TMA descriptor of the DATA sample (data_term_tma.cu); rebuilt when the key changes
+    struct { const void *base = nullptr; long long n_events = -1; int box_rows = 0; bool valid = false;
+             alignas(64) unsigned char map[128]; } tmap_cache;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     std::string err;

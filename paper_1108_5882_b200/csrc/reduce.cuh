@@ -13,7 +13,7 @@ constexpr int kMaxWaves = 256;
 constexpr int kMaxComp = 2 + 2 * kMaxWaves;
 
 struct FinishArgs {
-    double *partials;      // [NC][gridDim.x]
+    double *partials;      // [gridDim.x][NC]
     unsigned *ticket;
     const double *M;       // device [n][n][2]; nullptr -> data-term-only output
     double *out;           // result record (M != nullptr) or [NC] components (M == nullptr)
@@ -47,20 +47,32 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
         for (int c = tid; c < NC; c += nthreads) out[c] = s_tot[c];
         return;
     }
-    // (M V)_a, one row per thread
-    for (int a = tid; a < n; a += nthreads) {
-        const double *row = M + (size_t)a * n * 2;
+    // (M V)_a: `slices` adjacent lanes share a row (coalesced reads of M, all loads independent),
+    // partial dot products are combined with a fixed xor tree
+    int slices = 1;
+    while (slices * 2 <= 32 && slices * 2 * n <= nthreads && slices * 2 <= n) slices *= 2;
+    const int rows_per_pass = nthreads / slices;
+    const int sl = tid % slices, ra = tid / slices;
+    for (int a0 = 0; a0 < n; a0 += rows_per_pass) {          // uniform trip count
+        const int a = a0 + ra;
         double mr = 0.0, mi = 0.0;
-        for (int b = 0; b < n; ++b) {
-            double Mr = row[2 * b], Mi = row[2 * b + 1];
-            double vr = sV[2 * b], vi = sV[2 * b + 1];
-            mr = fma(Mr, vr, mr); mr = fma(-Mi, vi, mr);
-            mi = fma(Mr, vi, mi); mi = fma(Mi, vr, mi);
+        if (a < n) {
+            const double2 *row = reinterpret_cast<const double2 *>(M) + (size_t)a * n;
+#pragma unroll 4
+            for (int b = sl; b < n; b += slices) {
+                const double2 m = __ldg(row + b);
+                const double vr = sV[2 * b], vi = sV[2 * b + 1];
+                mr = fma(m.x, vr, mr); mr = fma(-m.y, vi, mr);
+                mi = fma(m.x, vi, mi); mi = fma(m.y, vr, mi);
+            }
         }
-        s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi;
-        // grad_a = -2 conj(T_a) + 2 (M V)_a
-        out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + 2.0 * mr;
-        out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + 2.0 * mi;
+        for (int m = 1; m < slices; m <<= 1) { mr += shfl_xor_d(mr, m); mi += shfl_xor_d(mi, m); }
+        if (a < n && sl == 0) {
+            s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi;
+            // grad_a = -2 conj(T_a) + 2 (M V)_a
+            out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + 2.0 * mr;
+            out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + 2.0 * mi;
+        }
     }
     __syncthreads();
     if (warp == 0) {
@@ -77,15 +89,18 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
 }
 
 // s_tot[0..NC): this block's totals (valid for all threads after a __syncthreads by the
-// caller).  sV: V in shared memory [2n].  Must be called by every thread of the block.
-__device__ inline void block_finish(double *s_tot, const double *sV, const FinishArgs &fa)
+// caller).  s_red: shared scratch of at least blockDim.x doubles.  sV: V in shared
+// memory [2n].  Must be called by every thread of the block.  Per-block partials live in fixed
+// slots [slot][NC]; the last-arriving block (ticket) adds them in a fixed order (strided slot
+// subsets per thread group, then the groups in group order).  No floating-point atomics: bitwise reproducible for a fixed launch shape.
+__device__ inline void block_finish(double *s_tot, double *s_red, const double *sV, const FinishArgs &fa)
 {
     const int n = fa.n, NC = 2 + 2 * n;
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
     __shared__ bool s_last;
 
-    for (int c = tid; c < NC; c += nthreads) fa.partials[(size_t)c * gridDim.x + blockIdx.x] = s_tot[c];
+    for (int c = tid; c < NC; c += nthreads) fa.partials[(size_t)blockIdx.x * NC + c] = s_tot[c];
     __threadfence();
     __syncthreads();
     if (tid == 0) s_last = (atomicAdd(fa.ticket, 1u) == gridDim.x - 1);
@@ -93,13 +108,44 @@ __device__ inline void block_finish(double *s_tot, const double *sV, const Finis
     if (!s_last) return;
     __threadfence();
 
-    // fixed-order sum over slots: lane l takes slots l, l+32, ... then a fixed xor tree
-    for (int c = warp; c < NC; c += nwarps) {
-        const double *p = fa.partials + (size_t)c * gridDim.x;
-        double acc = 0.0;
-        for (unsigned s = lane; s < gridDim.x; s += 32) acc += __ldcg(p + s);
-        acc = warp_sum(acc);
-        if (lane == 0) s_tot[c] = acc;
+    // `ngroups` groups of NC adjacent threads: group g adds slots g, g + ngroups, ... of its
+    // component (coalesced across the group); loads are issued in independent batches of FB
+    const int nslots = (int)gridDim.x;
+    constexpr int FB = 24;
+    const int ngroups = nthreads / NC;
+    if (ngroups >= 1) {
+        const int g = tid / NC, c = tid - g * NC;
+        if (g < ngroups) {
+            const double *p = fa.partials + c;
+            double acc = 0.0;
+            for (int base = g; base < nslots; base += FB * ngroups) {
+                double x[FB];
+#pragma unroll
+                for (int k = 0; k < FB; ++k) { const int sl = base + k * ngroups; x[k] = (sl < nslots) ? __ldcg(p + (size_t)sl * NC) : 0.0; }
+#pragma unroll
+                for (int k = 0; k < FB; ++k) acc += x[k];
+            }
+            s_red[tid] = acc;                     // == s_red[g * NC + c]
+        }
+        __syncthreads();
+        for (int c2 = tid; c2 < NC; c2 += nthreads) {
+            double t = 0.0;
+            for (int g2 = 0; g2 < ngroups; ++g2) t += s_red[g2 * NC + c2];
+            s_tot[c2] = t;
+        }
+    } else {                                      // more components than threads (generic kernel, n > 63)
+        for (int c = tid; c < NC; c += nthreads) {
+            const double *p = fa.partials + c;
+            double acc = 0.0;
+            for (int base = 0; base < nslots; base += FB) {
+                double x[FB];
+#pragma unroll
+                for (int k = 0; k < FB; ++k) { const int sl = base + k; x[k] = (sl < nslots) ? __ldcg(p + (size_t)sl * NC) : 0.0; }
+#pragma unroll
+                for (int k = 0; k < FB; ++k) acc += x[k];
+            }
+            s_tot[c] = acc;
+        }
     }
     __syncthreads();
 
@@ -147,7 +193,7 @@ __device__ __forceinline__ void reduce_and_finish(double L, double bad, double (
         s_tot[c] = acc;
     }
     __syncthreads();
-    block_finish(s_tot, sV, fa);
+    block_finish(s_tot, &s_warp[0][0], sV, fa);
 }
 
 }  // namespace pwa

@@ -80,7 +80,7 @@ k_res_grad(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs fa)
         s_tot[c] = t;
     }
     __syncthreads();
-    block_finish(s_tot, sV, fa);
+    block_finish(s_tot, &s_acc[0][0], sV, fa);
 }
 
 static pwa_status run_pass(pwa_ctx *ctx, const Sample &smp, int mode, const VArg &varg, double *out_dev)

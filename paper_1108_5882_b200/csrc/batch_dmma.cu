@@ -233,33 +233,54 @@ k_batch_dmma(const void *__restrict__ Av, long long N, int n, const double *__re
     }
 }
 
-// One block per column: slot-ordered sums, Q -> T, then step A7 -> result record k0 + column.
-__global__ void __launch_bounds__(128)
+// One block per column: sums over the per-CTA slots in a fixed tree, Q -> T, then step A7 ->
+// result record k0 + column.  1024 threads = 4 slot phases x 256 values (wave a, which of
+// Q[2a][2k], Q[2a][2k+1], Q[2a+1][2k], Q[2a+1][2k+1]); warps 0 and 1 of phase 0 also add L and the
+// non-finite count (lanes stride the slots, xor tree).
+constexpr int BF_THREADS = 1024;
+__global__ void __launch_bounds__(BF_THREADS)
 k_batch_finalize(const double *__restrict__ scratch, int nslots, int NB, int n, const double *__restrict__ Vdev,
                  int k0, const double *__restrict__ M, double *__restrict__ results, int result_stride)
 {
+    __shared__ double s_val[4][256];
     __shared__ double s_tot[2 + 2 * kFastWaves];
     __shared__ double sV[2 * kFastWaves];
     const int kl = blockIdx.x, k = k0 + kl, tid = threadIdx.x;
     const size_t sd = bd_slot_doubles(NB);
-    for (int a = tid; a < n; a += blockDim.x) {
-        const int rbk = a >> 2, cbk = kl >> 2, rr = (2 * a) & 7, cc = (2 * kl) & 7;
-        const double *blk = scratch + ((size_t)rbk * 8 + cbk) * 64;
-        double q00 = 0.0, q01 = 0.0, q10 = 0.0, q11 = 0.0;
-        for (int s = 0; s < nslots; ++s) {
-            const double *b = blk + (size_t)s * sd;
-            q00 += b[rr * 8 + cc];       q01 += b[rr * 8 + cc + 1];
-            q10 += b[(rr + 1) * 8 + cc]; q11 += b[(rr + 1) * 8 + cc + 1];
+    const int v = tid & 255, ph = tid >> 8;
+    {
+        const int a = v >> 2, w = v & 3;
+        double acc = 0.0;
+        if (a < n) {
+            const int rbk = a >> 2, cbk = kl >> 2, rr = ((2 * a) & 7) + (w >> 1), cc = ((2 * kl) & 7) + (w & 1);
+            const double *src = scratch + ((size_t)rbk * 8 + cbk) * 64 + rr * 8 + cc;
+            for (int s0 = ph; s0 < nslots; s0 += 16) {
+                double x[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { const int sl = s0 + 4 * u; x[u] = (sl < nslots) ? __ldcg(src + (size_t)sl * sd) : 0.0; }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) acc += x[u];
+            }
         }
-        s_tot[2 + 2 * a] = q00 - q11;
-        s_tot[3 + 2 * a] = q01 + q10;
+        s_val[ph][v] = acc;
+    }
+    if (tid < 64) {                                  // warp 0: L, warp 1: non-finite count
+        const int which = tid >> 5, lane = tid & 31;
+        double acc = 0.0;
+        for (int s = lane; s < nslots; s += 32) acc += __ldcg(scratch + (size_t)s * sd + (size_t)NB * 8 * 64 + which * BD_KC + kl);
+        acc = warp_sum(acc);
+        if (lane == 0) s_tot[which] = acc;
+    }
+    __syncthreads();
+    if (tid < n) {
+        const int a = tid;
+        double q[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) q[w] = ((s_val[0][4 * a + w] + s_val[1][4 * a + w]) + s_val[2][4 * a + w]) + s_val[3][4 * a + w];
+        s_tot[2 + 2 * a] = q[0] - q[3];              // Re T = Q[2a][2k] - Q[2a+1][2k+1]
+        s_tot[3 + 2 * a] = q[1] + q[2];              // Im T = Q[2a][2k+1] + Q[2a+1][2k]
         sV[2 * a] = Vdev[((size_t)k * n + a) * 2];
         sV[2 * a + 1] = Vdev[((size_t)k * n + a) * 2 + 1];
-    }
-    if (tid < 2) {
-        double v = 0.0;
-        for (int s = 0; s < nslots; ++s) v += scratch[(size_t)s * sd + (size_t)NB * 8 * 64 + tid * BD_KC + kl];
-        s_tot[tid] = v;
     }
     __syncthreads();
     assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n);
@@ -283,7 +304,7 @@ static pwa_status launch_bd(pwa_ctx *ctx, int K)
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
         const int cols = (K - k0 < BD_KC) ? (K - k0) : BD_KC;
-        k_batch_finalize<<<cols, 128, 0, ctx->stream>>>(ctx->d_scratch, (int)grid, NB, ctx->n, ctx->d_V, k0, ctx->d_M,
+        k_batch_finalize<<<cols, BF_THREADS, 0, ctx->stream>>>(ctx->d_scratch, (int)grid, NB, ctx->n, ctx->d_V, k0, ctx->d_M,
                                                         ctx->d_result, result_stride(ctx->n));
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());

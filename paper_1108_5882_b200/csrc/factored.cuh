@@ -28,11 +28,37 @@ __device__ __forceinline__ double2 bw_eval(double m2, double M2, double MG)
     return make_double2(d * inv, MG * inv);
 }
 
+// 1/x for normal positive x: MUFU.RCP64H seed + two Newton steps (<= ~1 ulp); anything else
+// (0, denormal, inf, nan, negative) takes the IEEE division.
+__device__ __forceinline__ double rcp_pos(double x)
+{
+    const unsigned ex = ((unsigned)__double2hiint(x) >> 20) & 0xfffu;   // sign + biased exponent
+    if (ex - 1u >= 0x7feu) return 1.0 / x;
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
+__device__ __forceinline__ double2 bw_eval_fast(double m2, double M2, double MG)
+{
+    const double d = M2 - m2;
+    const double inv = rcp_pos(fma(d, d, MG * MG));
+    return make_double2(d * inv, MG * inv);
+}
+
+// one complex angular factor, one vector load (the array is 16-byte aligned: upload contract)
 template <typename ST>
 __device__ __forceinline__ double2 load_ang(const void *ang, long long ev, int n_ang, int s)
 {
-    const ST *p = reinterpret_cast<const ST *>(ang) + (ev * n_ang + s) * 2;
-    return make_double2((double)p[0], (double)p[1]);
+    if (sizeof(ST) == 8) {
+        return __ldg(reinterpret_cast<const double2 *>(ang) + (ev * n_ang + s));
+    } else {
+        const float2 z = __ldg(reinterpret_cast<const float2 *>(ang) + (ev * n_ang + s));
+        return make_double2((double)z.x, (double)z.y);
+    }
 }
 
 template <typename ST>

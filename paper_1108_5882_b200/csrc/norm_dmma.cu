@@ -11,9 +11,10 @@
 // is at the same time the A operand (8x4, row) of row-block cb and the B operand (4x8, col) of
 // column-block cb, so a warp loads D/8 fragments per quad from the shared-memory tile and issues
 // one DMMA per block pair (i <= j) it owns.  Accumulators (8x8 per pair, 2 doubles per lane) stay
-// in registers for the CTA's whole event range (split-K); every (CTA, warp group) writes its
-// partial upper-triangle blocks to a fixed slot and k_norm_dmma_finalize sums the slots in slot
-// order (bitwise reproducible), scales by 1/N_gen and writes both triangles (exactly Hermitian).
+// in registers for the CTA's whole event range (split-K); the CTA's warp groups are summed in group
+// order, every CTA writes its partial upper-triangle blocks to a fixed slot and k_norm_dmma_finalize
+// sums the slots in a fixed tree (bitwise reproducible), scales by 1/N_gen and writes both
+// triangles (exactly Hermitian).
 //
 // Tile rows are padded to DP = D + 4 doubles (DP mod 16 in {4, 12}) so that the fragment load
 // LDS.64 is bank-conflict free.  fp32-stored amplitudes are widened when the tile is written
@@ -66,10 +67,10 @@ struct NormCfg {
     static constexpr int CH = 16 / (int)sizeof(ST);          // elements per 16-byte chunk
     static constexpr int RC = D / CH;                          // chunks per (unpadded) row
     static constexpr int CPT = (ET * RC + THREADS - 1) / THREADS;
-    static constexpr size_t SMEM = sizeof(double) * 2 * ET * DP;
+    static constexpr size_t SMEM = sizeof(double) * (2 * ET * DP > NPAIRS * 64 ? 2 * ET * DP : NPAIRS * 64);   // tiles, then the CTA partial
 };
 
-template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S>
+template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S, int NANG>
 __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long N, int n, const FactArgs &f,
                                           double *__restrict__ scratch, double *smem)
 {
@@ -85,6 +86,35 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
 
     const long long ntiles = (N + ET - 1) / ET;
     uint4 stage[CPT];   // FILL_STAGED only (dead otherwise)
+    // FILL_FACTORED: thread -> (event e = tid % ET, resonance subset part, part + TPE, ...); the mass
+    // and the angular factors of the NEXT tile are fetched into registers before the DMMAs of the
+    // current one, so their latency is hidden (the event's TPE threads load the same 8 + 16 n_ang bytes)
+    constexpr int TPE = THREADS / ET;
+    static_assert(THREADS % ET == 0, "whole threads per event");
+    double pm = 0.0;
+    double2 pz[NANG];
+    auto fact_load = [&](long long t) {
+        const long long ev = t * ET + (tid % ET);
+        const bool valid = ev < N;
+        pm = valid ? __ldg(f.mass + ev) : 0.0;
+#pragma unroll
+        for (int s = 0; s < NANG; ++s)
+            pz[s] = (valid && s < f.n_ang) ? load_ang<ST>(f.ang, ev, f.n_ang, s) : make_double2(0.0, 0.0);
+    };
+    auto fact_store = [&](double *dst) {                       // A1: BW(m_j; M_r, G_r) * Z_js -> tile (fp64)
+        double *row = dst + (tid % ET) * DP;
+        const double m2 = pm * pm;
+        for (int r = tid / ET; r < f.n_res; r += TPE) {        // warp-uniform r: parameters come from the constant bank
+            const double2 bw = bw_eval_fast(m2, f.rp.m2[r], f.rp.mg[r]);
+#pragma unroll
+            for (int s = 0; s < NANG; ++s) {
+                const int w = f.wave_of_pair[r * kMaxAng + s];
+                if (w >= 0)
+                    *reinterpret_cast<double2 *>(row + 2 * w) =
+                        make_double2(bw.x * pz[s].x - bw.y * pz[s].y, bw.x * pz[s].y + bw.y * pz[s].x);
+            }
+        }
+    };
 
     auto load_tile = [&](long long t) {                       // FILL_STAGED: global -> registers
 #pragma unroll
@@ -121,25 +151,6 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
                 const long long ev = t * ET + e;
                 dst[e * DP + c] = (ev < N && c < d2) ? (double)B[ev * d2 + c] : 0.0;
             }
-        } else {
-            const int nres = f.n_res;
-            for (int idx = tid; idx < ET * nres; idx += THREADS) {
-                const int e = idx / nres, r = idx % nres;
-                const long long ev = t * ET + e;
-                const bool valid = ev < N;
-                double2 bw = make_double2(0.0, 0.0);
-                if (valid) { const double m = f.mass[ev]; bw = bw_eval(m * m, f.rp.m2[r], f.rp.mg[r]); }
-                for (int s = 0; s < f.n_ang; ++s) {
-                    const int w = f.wave_of_pair[r * kMaxAng + s];
-                    if (w < 0) continue;
-                    double2 a = make_double2(0.0, 0.0);
-                    if (valid) {
-                        const double2 z = load_ang<ST>(f.ang, ev, f.n_ang, s);
-                        a = make_double2(bw.x * z.x - bw.y * z.y, bw.x * z.y + bw.y * z.x);
-                    }
-                    *reinterpret_cast<double2 *>(dst + e * DP + 2 * w) = a;
-                }
-            }
         }
     };
     auto compute = [&](const double *src) {
@@ -155,6 +166,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
     int cur = 0;
     if (t < ntiles) {
         if constexpr (MODE == FILL_STAGED) { load_tile(t); store_tile(buf[0]); }
+        else if constexpr (MODE == FILL_FACTORED) { fact_load(t); fact_store(buf[0]); }
         else fill_tile(buf[0], t);
     }
     __syncthreads();
@@ -164,6 +176,10 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
             if (nxt < ntiles) load_tile(nxt);
             compute(buf[cur]);
             if (nxt < ntiles) store_tile(buf[cur ^ 1]);
+        } else if constexpr (MODE == FILL_FACTORED) {
+            if (nxt < ntiles) fact_load(nxt);
+            compute(buf[cur]);
+            if (nxt < ntiles) fact_store(buf[cur ^ 1]);
         } else {
             compute(buf[cur]);
             if (nxt < ntiles) fill_tile(buf[cur ^ 1], nxt);
@@ -171,106 +187,131 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
         __syncthreads();
         cur ^= 1;
     }
-    // partial blocks of this (CTA, group) -> fixed slot, [pair][8][8] doubles
-    const size_t slot = (size_t)blockIdx.x * NG + group;
-    double *dst = scratch + slot * (size_t)NPAIRS * 64 + (lane >> 2) * 8 + (lane & 3) * 2;
+    // the CTA's groups are summed in group order in shared memory (the tile buffers are free after
+    // the loop's last barrier), then ONE partial per CTA goes to its fixed slot, [pair][8][8] doubles
+    double *red = smem;
+    for (int g = 0; g < NG; ++g) {
+        if (group == g) {
+            double *dst = red + (lane >> 2) * 8 + (lane & 3) * 2;
 #pragma unroll
-    for (int pl = 0; pl < PPW; ++pl) {
-        const int p = pl * SPLIT + S;
-        if (p < NPAIRS) *reinterpret_cast<double2 *>(dst + (size_t)p * 64) = make_double2(acc[pl][0], acc[pl][1]);
+            for (int pl = 0; pl < PPW; ++pl) {
+                const int p = pl * SPLIT + S;
+                if (p < NPAIRS) {
+                    double2 v = make_double2(acc[pl][0], acc[pl][1]);
+                    if (g > 0) { const double2 o = *reinterpret_cast<double2 *>(dst + p * 64); v.x += o.x; v.y += o.y; }
+                    *reinterpret_cast<double2 *>(dst + p * 64) = v;
+                }
+            }
+        }
+        __syncthreads();
     }
+    double *slot = scratch + (size_t)blockIdx.x * NPAIRS * 64;
+    for (int idx = tid; idx < NPAIRS * 64; idx += THREADS) slot[idx] = red[idx];
 }
 
-template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET>
+template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET, int NANG>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_norm_dmma(const void *__restrict__ Bv, long long N, int n, FactArgs f, double *__restrict__ scratch)
 {
     extern __shared__ double nd_smem[];
     const int S = (threadIdx.x >> 5) % SPLIT;
-    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0>(Bv, N, n, f, scratch, nd_smem); return; }
+    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem); return; }
     switch (S) {        // warp-uniform: each sub-id owns a compile-time list of block pairs
-    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0>(Bv, N, n, f, scratch, nd_smem); break;
-    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0)>(Bv, N, n, f, scratch, nd_smem); break;
-    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0)>(Bv, N, n, f, scratch, nd_smem); break;
-    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0)>(Bv, N, n, f, scratch, nd_smem); break;
+    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem); break;
+    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
+    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
+    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
     }
 }
 
-// One warp per complex entry (a <= b): lanes stride over the slots, fixed xor tree.
+// Final sum over the per-CTA slots and P -> M.  One block per (block pair p, row pair k): its 16
+// elements are rows 2k, 2k+1 of the 8 x 8 block = one wave a (re, im rows) against the 4 waves of
+// the column block.  256 threads = 16 elements x 16 slot phases: thread (el, ph) adds slots ph,
+// ph + 16, ... (coalesced 128-byte reads, independent loads), the phases are then added in phase
+// order: a fixed tree, bitwise reproducible for a fixed grid.
 __global__ void __launch_bounds__(256)
 k_norm_dmma_finalize(const double *__restrict__ scratch, int nslots, int n, int NB, double inv_ngen,
                      double *__restrict__ M)
 {
-    const int lane = threadIdx.x & 31;
-    const long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nent = (long long)n * (n + 1) / 2;
-    if (wid >= nent) return;
-    int a = 0; long long q = wid;
-    while (q >= n - a) { q -= n - a; ++a; }
-    const int b = a + (int)q;
-    const int i = a >> 2, j = b >> 2;
-    const int p = i * NB - i * (i - 1) / 2 + (j - i);
-    const int rr = (2 * a) & 7, cc = (2 * b) & 7;
-    const int npairs = NB * (NB + 1) / 2;
-    double p00 = 0.0, p11 = 0.0, p01 = 0.0, p10 = 0.0;
-    for (int s = lane; s < nslots; s += 32) {
-        const double *blk = scratch + ((size_t)s * npairs + p) * 64;
-        p00 += blk[rr * 8 + cc];       p01 += blk[rr * 8 + cc + 1];
-        p10 += blk[(rr + 1) * 8 + cc]; p11 += blk[(rr + 1) * 8 + cc + 1];
-    }
+    __shared__ double s_ph[16][17];
+    __shared__ double s_tot[16];
+    const int p = blockIdx.x >> 2, k = blockIdx.x & 3;
+    const int el = threadIdx.x & 15, ph = threadIdx.x >> 4;
+    const size_t stride = (size_t)NB * (NB + 1) / 2 * 64;
+    const double *src = scratch + (size_t)p * 64 + k * 16 + el;
+    double acc = 0.0;
+    for (int s0 = ph; s0 < nslots; s0 += 64) {
+        double x[4];
 #pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) {
-        p00 += __shfl_xor_sync(0xffffffffu, p00, m); p01 += __shfl_xor_sync(0xffffffffu, p01, m);
-        p10 += __shfl_xor_sync(0xffffffffu, p10, m); p11 += __shfl_xor_sync(0xffffffffu, p11, m);
+        for (int u = 0; u < 4; ++u) { const int sl = s0 + 16 * u; x[u] = (sl < nslots) ? __ldcg(src + (size_t)sl * stride) : 0.0; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc += x[u];
     }
-    if (lane == 0) {
-        const double re = (p00 + p11) * inv_ngen;
-        const double im = (a == b) ? 0.0 : (p01 - p10) * inv_ngen;      // |B_ja|^2 is real
-        M[((size_t)a * n + b) * 2] = re;  M[((size_t)a * n + b) * 2 + 1] = im;
-        if (a != b) { M[((size_t)b * n + a) * 2] = re;  M[((size_t)b * n + a) * 2 + 1] = -im; }
+    s_ph[ph][el] = acc;
+    __syncthreads();
+    if (threadIdx.x < 16) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) t += s_ph[q][threadIdx.x];
+        s_tot[threadIdx.x] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        int i = 0, q = p;
+        while (q >= NB - i) { q -= NB - i; ++i; }
+        const int j = i + q;
+        const int a = 4 * i + k, b = 4 * j + (int)threadIdx.x, cc = 2 * (int)threadIdx.x;
+        if (a < n && b < n && a <= b) {
+            const double re = (s_tot[cc] + s_tot[8 + cc + 1]) * inv_ngen;                       // P[2a][2b] + P[2a+1][2b+1]
+            const double im = (a == b) ? 0.0 : (s_tot[cc + 1] - s_tot[8 + cc]) * inv_ngen;      // P[2a][2b+1] - P[2a+1][2b]
+            M[((size_t)a * n + b) * 2] = re;  M[((size_t)a * n + b) * 2 + 1] = im;
+            if (a != b) { M[((size_t)b * n + a) * 2] = re;  M[((size_t)b * n + a) * 2 + 1] = -im; }
+        }
     }
 }
 
-template <typename ST, int NB, int SPLIT, int MODE, int MINB, int ET>
+template <typename ST, int NB, int SPLIT, int MODE, int MINB, int ET, int NANG>
 static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs)
 {
     constexpr int THREADS = 256;
     using C = NormCfg<ST, NB, SPLIT, MODE, THREADS, ET>;
-    auto kern = k_norm_dmma<ST, NB, SPLIT, MODE, THREADS, MINB, ET>;
-    PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-    int occ = 0;
-    PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, C::SMEM));
-    if (occ < 1) occ = 1;
+    auto kern = k_norm_dmma<ST, NB, SPLIT, MODE, THREADS, MINB, ET, NANG>;
+    static int s_occ[64] = {0};                                 // per instantiation and device
+    int &occ = s_occ[ctx->device & 63];
+    if (occ == 0) {
+        PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        int o = 0;
+        PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, THREADS, C::SMEM));
+        occ = o < 1 ? 1 : o;
+    }
     const long long N = ctx->mc.n_events;
     const long long ntiles = (N + ET - 1) / ET;
     long long grid = (long long)ctx->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
     if (grid < 1) grid = 1;
-    const int nslots = (int)grid * C::NG;
+    const int nslots = (int)grid;
     pwa_status s = ensure_scratch(ctx, sizeof(double) * (size_t)nslots * C::NPAIRS * 64);
     if (s != PWA_OK) return s;
     kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(ctx->mc.factored ? nullptr : ctx->mc.amps, N, ctx->n, fargs, ctx->d_scratch);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
-    const long long nent = (long long)ctx->n * (ctx->n + 1) / 2;
-    const int fblocks = (int)((nent * 32 + 255) / 256);
-    k_norm_dmma_finalize<<<fblocks, 256, 0, ctx->stream>>>(ctx->d_scratch, nslots, ctx->n, NB,
-                                                          1.0 / (double)ctx->mc.n_gen, ctx->d_M);
+    k_norm_dmma_finalize<<<C::NPAIRS * 4, 256, 0, ctx->stream>>>(ctx->d_scratch, nslots, ctx->n, NB,
+                                                                 1.0 / (double)ctx->mc.n_gen, ctx->d_M);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;
 }
 
-template <typename ST, int MODE>
+template <typename ST, int MODE, int NANG>
 static pwa_status dispatch_nd(pwa_ctx *ctx, const FactArgs &fargs)
 {
     const int D = 2 * ctx->n;
     //                                   NB SPLIT      MINB ET
-    if (D <= 8)   return launch_nd<ST, 1,  1, MODE, 2, 128>(ctx, fargs);
-    if (D <= 16)  return launch_nd<ST, 2,  1, MODE, 2, 128>(ctx, fargs);
-    if (D <= 32)  return launch_nd<ST, 4,  1, MODE, 2, 128>(ctx, fargs);
-    if (D <= 64)  return launch_nd<ST, 8,  2, MODE, 2, 64>(ctx, fargs);
-    return launch_nd<ST, 16, 4, MODE, 1, 32>(ctx, fargs);
+    if (D <= 8)   return launch_nd<ST, 1,  1, MODE, 2, 128, NANG>(ctx, fargs);
+    if (D <= 16)  return launch_nd<ST, 2,  1, MODE, 2, 128, NANG>(ctx, fargs);
+    if (D <= 32)  return launch_nd<ST, 4,  1, MODE, 2, 128, NANG>(ctx, fargs);
+    if (D <= 64)  return launch_nd<ST, 8,  2, MODE, 2, 64, NANG>(ctx, fargs);
+    return launch_nd<ST, 16, 4, MODE, 1, 32, NANG>(ctx, fargs);
 }
 
 pwa_status launch_norm_dmma(pwa_ctx *ctx, bool *handled)
@@ -290,9 +331,10 @@ pwa_status launch_norm_dmma(pwa_ctx *ctx, bool *handled)
     const bool pow2 = (n & (n - 1)) == 0 && n >= 4;            // rows are whole 16-byte chunks, D = 2n
     const bool aligned = ((uintptr_t)ctx->mc.amps & 15u) == 0;
     pwa_status s;
-    if (fact)                 s = f32 ? dispatch_nd<float, FILL_FACTORED>(ctx, fargs) : dispatch_nd<double, FILL_FACTORED>(ctx, fargs);
-    else if (pow2 && aligned) s = f32 ? dispatch_nd<float, FILL_STAGED>(ctx, fargs)   : dispatch_nd<double, FILL_STAGED>(ctx, fargs);
-    else                      s = f32 ? dispatch_nd<float, FILL_ELEMENT>(ctx, fargs)  : dispatch_nd<double, FILL_ELEMENT>(ctx, fargs);
+    if (fact && ctx->mc.n_ang <= 2) s = f32 ? dispatch_nd<float, FILL_FACTORED, 2>(ctx, fargs) : dispatch_nd<double, FILL_FACTORED, 2>(ctx, fargs);
+    else if (fact)            s = f32 ? dispatch_nd<float, FILL_FACTORED, 4>(ctx, fargs) : dispatch_nd<double, FILL_FACTORED, 4>(ctx, fargs);
+    else if (pow2 && aligned) s = f32 ? dispatch_nd<float, FILL_STAGED, 1>(ctx, fargs)   : dispatch_nd<double, FILL_STAGED, 1>(ctx, fargs);
+    else                      s = f32 ? dispatch_nd<float, FILL_ELEMENT, 1>(ctx, fargs)  : dispatch_nd<double, FILL_ELEMENT, 1>(ctx, fargs);
     if (s != PWA_OK) return s;
     *handled = true;
     return PWA_OK;

@@ -103,6 +103,13 @@ pwa_status pwa_set_resonances(pwa_ctx *ctx, const double *mass0, const double *w
  * Synchronous when M_out != NULL.  PWA_ERR_STATE if no MC sample was uploaded.           */
 pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out);
 
+/* A-priori bound on max_ab |M_ab(library) - M_ab(exact fp64 sum over the stored amplitudes)| of the
+ * most recent pwa_build_norm.  The FP64 paths only carry summation rounding (reported as 0); the
+ * int8 tensor-core path for fp32-stored samples (fixed-point digit planes, exact integer
+ * accumulation, low orders truncated: DESIGN.md section 6.6) reports its quantisation + truncation
+ * bound in the units of M.  *which_path (may be NULL): 0 = FP64 path, 1 = int8 tcgen05 path.    */
+pwa_status pwa_norm_error_bound(pwa_ctx *ctx, double *bound, int32_t *which_path);
+
 /* Installs an externally computed M (HOST [n][n][2]), e.g. the sum over ranks of per-shard
  * matrices in an event-sharded multi-GPU run.                                      */
 pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M);
@@ -171,7 +178,9 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx);
 pwa_status pwa_sync(pwa_ctx *ctx);
 
 /* Selects a kernel variant for experiments (0 = default).  Returns PWA_ERR_INVALID_ARG for
- * unknown keys.  Keys: "data_term", "norm", "batch".                                      */
+ * unknown keys.  Keys: "data_term", "norm", "batch".  "norm": 0 = default (int8 tcgen05 path for
+ * fp32-stored constant-resonance samples of >= 65536 events, else FP64 DMMA), 1 = FP64 DMMA,
+ * 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.           */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
 
 /* Register-resident peak probes used as roofline denominators:

@@ -28,7 +28,7 @@ SYMBOLS = [
     "pwa_set_norm", "pwa_nll_grad", "pwa_nll_grad_batch", "pwa_nll_grad_enqueue",
     "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
-    "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench",
+    "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
 ]
 
 
@@ -71,6 +71,7 @@ def _load():
         "pwa_sync": (C.c_int, [vp]),
         "pwa_set_option": (C.c_int, [vp, C.c_char_p, i32]),
         "pwa_microbench": (C.c_int, [vp, i32, i64, dp]),
+        "pwa_norm_error_bound": (C.c_int, [vp, dp, C.POINTER(i32)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)          # AttributeError here = header/library mismatch
@@ -171,6 +172,13 @@ def pwa_build_norm(ctx, want_M=True):
     M = np.empty((n, n, 2))
     _check(ctx, _lib.pwa_build_norm(ctx, M.ctypes.data))
     return M
+
+
+def pwa_norm_error_bound(ctx):
+    """-> (bound on max|M_ab - exact|, path) with path 0 = FP64 build, 1 = int8 tcgen05 build."""
+    b, w = C.c_double(0.0), C.c_int32(0)
+    _check(ctx, _lib.pwa_norm_error_bound(ctx, C.byref(b), C.byref(w)))
+    return b.value, int(w.value)
 
 
 def pwa_set_norm(ctx, M):

@@ -178,9 +178,18 @@ static pwa_status launch_norm_generic(pwa_ctx *ctx)
 
 pwa_status launch_norm_build(pwa_ctx *ctx)
 {
+    ctx->M_path = 0;
     if (ctx->mc.n_events == 0) {   // empty MC sample: M = 0
         PWA_CUDA(ctx, cudaMemsetAsync(ctx->d_M, 0, sizeof(double) * 2 * (size_t)ctx->n * ctx->n, ctx->stream));
         return PWA_OK;
+    }
+    // opt_norm: 0 = default (int8 tensor-core path for large fp32-stored samples, else FP64 DMMA),
+    //           1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel
+    if (ctx->opt_norm == 2 || (ctx->opt_norm == 0 && ctx->mc.n_events >= 65536)) {
+        bool handled = false;
+        pwa_status s = launch_norm_i8(ctx, &handled);
+        if (s != PWA_OK) return s;
+        if (handled) { ctx->M_path = 1; return PWA_OK; }
     }
     if (ctx->opt_norm != 99) {
         bool handled = false;

@@ -230,7 +230,7 @@ pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, i
     smp.amps = buf; smp.amps_owned = owned; smp.factored = false;
     if (which == PWA_DATA) ctx->tmap_cache.valid = false;
     smp.n_events = n_events; smp.n_gen = n_generated;
-    if (which == PWA_MC) ctx->M_valid = false;
+    if (which == PWA_MC) { ctx->M_valid = false; return prepare_norm_i8(ctx); }
     return PWA_OK;
 }
 
@@ -255,7 +255,7 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
     free_sample(smp);
     smp.mass = (double *)bm; smp.ang = ba; smp.fact_owned = om || oa; smp.n_ang = n_ang; smp.factored = true;
     smp.n_events = n_events; smp.n_gen = n_generated;
-    if (which == PWA_MC) ctx->M_valid = false;
+    if (which == PWA_MC) { ctx->M_valid = false; ctx->i8q.valid = false; }
     return PWA_OK;
 }
 
@@ -311,6 +311,15 @@ pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out)
     return PWA_OK;
 }
 
+pwa_status pwa_norm_error_bound(pwa_ctx *ctx, double *bound, int32_t *which_path)
+{
+    if (!ctx || !bound) return PWA_ERR_INVALID_ARG;
+    if (!ctx->M_valid) return fail(ctx, PWA_ERR_STATE, "normalisation matrix missing or stale: call pwa_build_norm");
+    *bound = ctx->M_path == 1 ? norm_i8_error_bound(ctx) : 0.0;
+    if (which_path) *which_path = ctx->M_path;
+    return PWA_OK;
+}
+
 pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
 {
     if (!ctx || !M) return PWA_ERR_INVALID_ARG;
@@ -322,6 +331,7 @@ pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
     PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_M, ctx->h_M.data(), sizeof(double) * cnt, cudaMemcpyHostToDevice, ctx->stream));
     PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->M_valid = true;
+    ctx->M_path = 0;
     return PWA_OK;
 }
 

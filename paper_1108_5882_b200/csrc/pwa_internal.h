@@ -56,6 +56,7 @@ struct pwa_ctx {
     double *d_M = nullptr;                    // [n][n][2]
     std::vector<double> h_M;
     bool M_valid = false;
+    int M_path = 0;                           // 0 = FP64 build, 1 = int8 tcgen05 build (norm_i8.cu)
     // scratch
     double *d_partials = nullptr; size_t partials_cap = 0;   // doubles
     unsigned *d_ticket = nullptr;
@@ -66,6 +67,8 @@ struct pwa_ctx {
     // cached TMA descriptor of the DATA sample (data_term_tma.cu); rebuilt when the key changes
     struct { const void *base = nullptr; long long n_events = -1; int box_rows = 0; bool valid = false;
              alignas(64) unsigned char map[128]; } tmap_cache;
+    // int8 tensor-core M build (norm_i8.cu): per-column power-of-two scales found at MC upload
+    struct { bool valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8q;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     std::string err;
@@ -88,6 +91,9 @@ pwa_status ensure_scratch(pwa_ctx *ctx, size_t bytes);
 pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double *out_dev_terms);
 pwa_status launch_batch(pwa_ctx *ctx, int K);   // V already staged in h_V/d_V
 pwa_status launch_norm_build(pwa_ctx *ctx);
+pwa_status prepare_norm_i8(pwa_ctx *ctx);                  // norm_i8.cu: after a constant-resonance MC upload
+pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled);    // norm_i8.cu
+double norm_i8_error_bound(const pwa_ctx *ctx);
 pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
 

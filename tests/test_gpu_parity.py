@@ -317,3 +317,57 @@ def test_bfgs_batch_lockstep(pwa, synth):
             one = pwa.pwa_nll_grad(c.ctx, Vfit[k])
             assert one[0] == pytest.approx(nll[k], rel=1e-12)
             assert one[2][1] == pytest.approx(w.n_data, rel=1e-5)
+
+
+# ------------------------------------------------------------------ int8 tensor-core (tcgen05) M build, fp32 storage (NEXT-1)
+@pytest.mark.parametrize("n", [16, 32, 64])
+@pytest.mark.parametrize("Nacc", [1, 3, 63, 64, 65, 127, 4097, 33_001, 70_003])
+def test_norm_i8_parity(pwa, oracle, n, Nacc):
+    """tcgen05.mma.kind::i8 digit-plane Gram (norm_i8.cu) against the oracle: tiles, ragged tails,
+    the G = 128/(2n) events-per-row view with its left-over events, columns of very different scale
+    (per-column power-of-two fixed point), and the stated a-priori error bound."""
+    rng = np.random.default_rng(1000 * n + Nacc)
+    colscale = 10.0 ** rng.uniform(-3, 1, size=(1, n, 2))
+    B = (rng.normal(size=(Nacc, n, 2)) * colscale).astype(np.float32)
+    B[:, 0, 1] = 0.0                                             # an all-zero column (real wave)
+    M_o = oracle.norm_matrix(B, Nacc + 5)
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_set_option(c.ctx, "norm", 2)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=Nacc + 5)
+        M = pwa.pwa_build_norm(c.ctx)
+        bound, path = pwa.pwa_norm_error_bound(c.ctx)
+        G = 128 // (2 * n)
+        assert path == (1 if Nacc >= G else 0)
+        check_M(M, M_o, TOL["f32"])
+        if path == 1:
+            assert np.abs(M - M_o).max() <= bound + 1e-14 * np.abs(M_o).max()
+            # entry-wise relative to the columns involved (fixed point is per column): far tighter than 1e-6
+            d = np.sqrt(np.abs(np.diagonal(M_o[..., 0])))
+            scale = np.outer(d, d)[..., None] + 1e-300
+            assert (np.abs(M - M_o) / scale).max() <= 1e-7
+        # reproducible bit for bit
+        assert np.array_equal(M, pwa.pwa_build_norm(c.ctx))
+        # the FP64 tensor-core path gives the same matrix to the fp32-storage tolerance
+        pwa.pwa_set_option(c.ctx, "norm", 1)
+        check_M(pwa.pwa_build_norm(c.ctx), M_o, 1e-12)
+        assert pwa.pwa_norm_error_bound(c.ctx) == (0.0, 0)
+
+
+def test_norm_i8_default_path_and_nonfinite(pwa, oracle):
+    """Large fp32-stored samples take the int8 path by default (several TMEM flushes per CTA are
+    covered by test_gpu_full_configs.py::test_cfg4_full, 2e7 events); inf / nan in the sample
+    falls back to the FP64 path, which propagates IEEE values."""
+    n, Nacc = 64, 600_017
+    rng = np.random.default_rng(5)
+    B = (rng.normal(size=(Nacc, n, 2)) * 0.35).astype(np.float32)
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=Nacc)
+        M = pwa.pwa_build_norm(c.ctx)
+        assert pwa.pwa_norm_error_bound(c.ctx)[1] == 1           # default path for large fp32 samples
+        for a0 in (0, 31, 62):
+            ref = oracle.norm_block(B, Nacc, a0, a0 + 2, 0, n)
+            assert np.abs(M[a0:a0 + 2] - ref[a0:a0 + 2]).max() <= 1e-9 * np.abs(M).max()
+        B[12345, 7, 1] = np.inf
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B[:100_000], n_generated=100_000)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        assert pwa.pwa_norm_error_bound(c.ctx)[1] == 0

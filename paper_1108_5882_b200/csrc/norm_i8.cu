@@ -13,12 +13,13 @@
 //     d in [-128, 127] ("Ozaki" slicing); the four int8 digit planes D0..D3 of a 64-event tile are
 //     written to shared memory in the UMMA canonical MN-major / 128-byte-swizzle layout.
 //   * tcgen05.mma.kind::i8 (int8 x int8 -> int32 in TMEM, exact) forms, per 32-event K step,
-//         acc0 += D3^T D3                       order t = u + v = 6
-//         acc1 += D3^T D2                       t = 5   (P5 = acc1 + acc1^T)
-//         acc2 += 2 D3^T D1 + D2^T D2           t = 4   (P4 = (acc2 + acc2^T) / 2)
+//         acc6 += D3^T D3                       order t = u + v = 6
+//         acc5 += D3^T D2                       t = 5   (P5 = acc5 + acc5^T)
+//         acc4 += 2 D3^T D1 + D2^T D2           t = 4   (P4 = (acc4 + acc4^T) / 2)
 //         acc3 += D3^T D0 + D2^T D1             t = 3   (P3 = acc3 + acc3^T)
-//     4 accumulators x 128 columns = all 512 TMEM columns; 7 MMAs (M = N = 128, K = 32) per K step
-//     instead of the 16 digit pairs, using the symmetry of the Gram matrix.  Orders t <= 2 are
+//     4 accumulators x 128 columns = all 512 TMEM columns; 7 products (M = N = 128, K = 32) per K
+//     step instead of the 16 digit pairs, using the symmetry of the Gram matrix, issued as three
+//     N = 256 MMAs over adjacent planes / adjacent accumulators plus one N = 128 MMA.  Orders t <= 2 are
 //     dropped: |dropped| <= 3 * 2^-32 * (1 + 2^-7) c_p c_q per event, c_p = 2^(31 - s_p) in
 //     (max|B_p|, 2 max|B_p|]; the quantisation adds <= 2^-32 (c_p |B_q| + c_q |B_p|).  Both are
 //     far below the 1e-6 tolerance of fp32 storage (BASELINE.json north_star) for any realistic
@@ -57,7 +58,7 @@ constexpr int NCW = 8;                       // converter / epilogue warps
 constexpr int THREADS = (NCW + 2) * 32;
 constexpr size_t SMEM = 1024 + (size_t)NSTG * STG_BYTES + (size_t)NSL * SL_BYTES;
 
-struct Scales { float s[128]; };             // 2^s_p per real column of the 128-wide view
+struct Scales { float s[128]; int dbg; };    // 2^s_p per real column of the 128-wide view; dbg: experiment switches (0 in production)
 
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
@@ -99,20 +100,22 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t (&v)[16])
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // Shared-memory matrix descriptor of one digit plane (or a 32-row K step of it): MN-major,
-// SWIZZLE_128B, rows (K) of 128 bytes, 8-row swizzle atoms 1024 bytes apart (SBO); the MN extent
-// is exactly one 128-byte atom, so the leading-dimension offset is never applied.
+// SWIZZLE_128B, rows (K) of 128 bytes, 8-row swizzle atoms 1024 bytes apart (SBO).  One plane is
+// exactly one 128-byte atom along MN; an N = 256 operand continues in the NEXT plane (LBO = PLANE),
+// so [D_v | D_v+1] is one B operand and its two products land in adjacent accumulators.
 __device__ __forceinline__ uint64_t plane_desc(uint32_t smem_addr)
 {
     uint64_t d = 0;
     d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);          // start address, bits [0, 14)
-    d |= (uint64_t)(1024u >> 4) << 16;                     // leading byte offset (unused: one atom along MN)
+    d |= (uint64_t)((uint32_t)PLANE >> 4) << 16;           // leading byte offset: next 128-byte atom along MN = next digit plane (N = 256)
     d |= (uint64_t)(1024u >> 4) << 32;                     // stride byte offset: next 8 K rows
     d |= (uint64_t)1 << 46;                                // descriptor version (Blackwell)
     d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
     return d;
 }
-// kind::i8 instruction descriptor: D = s32, A = B = signed int8, both MN-major, N = 128, M = 128
-constexpr uint32_t kIdesc = (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+// kind::i8 instruction descriptor: D = s32, A = B = signed int8, both MN-major, M = 128, N = 128 or 256
+constexpr uint32_t idesc_n(uint32_t N) { return (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((N >> 3) << 17) | ((128u >> 4) << 24); }
+constexpr uint32_t kIdesc128 = idesc_n(128), kIdesc256 = idesc_n(256);
 
 // ---- the kernel -------------------------------------------------------------------------------
 // tmap: fp32 [rows][128] view of the MC sample, box = [TE rows][128 floats], no swizzle.
@@ -180,13 +183,12 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                     const uint64_t d0 = plane_desc(pl + 0 * PLANE + koff), d1 = plane_desc(pl + 1 * PLANE + koff);
                     const uint64_t d2 = plane_desc(pl + 2 * PLANE + koff), d3 = plane_desc(pl + 3 * PLANE + koff);
                     const uint32_t acc = (first && kk == 0) ? 0u : 1u;
-                    umma_i8(tmem0 + 0 * 128, d3, d3, kIdesc, acc);
-                    umma_i8(tmem0 + 1 * 128, d3, d2, kIdesc, acc);
-                    umma_i8(tmem0 + 2 * 128, d3, d1, kIdesc, acc);
-                    umma_i8(tmem0 + 2 * 128, d3, d1, kIdesc, 1u);
-                    umma_i8(tmem0 + 2 * 128, d2, d2, kIdesc, 1u);
-                    umma_i8(tmem0 + 3 * 128, d3, d0, kIdesc, acc);
-                    umma_i8(tmem0 + 3 * 128, d2, d1, kIdesc, 1u);
+                    if (sc.dbg & 1) continue;                          // experiment: no MMA issued
+                    // accumulators by ascending order: t = 3 at column 0, t = 4 at 128, t = 5 at 256, t = 6 at 384
+                    umma_i8(tmem0 + 256, d3, d2, kIdesc256, acc);      // D3^T [D2 | D3] -> t = 5 | t = 6
+                    umma_i8(tmem0 + 0,   d3, d0, kIdesc256, acc);      // D3^T [D0 | D1] -> t = 3 | t = 4
+                    umma_i8(tmem0 + 128, d3, d1, kIdesc128, 1u);       // second D3^T D1  -> t = 4
+                    umma_i8(tmem0 + 0,   d2, d1, kIdesc256, 1u);       // D2^T [D1 | D2] -> t = 3 | t = 4
                 }
                 umma_commit(b_sl_empty + 8 * b);
                 if ((t % FT) == FT - 1 || t == nt - 1) umma_commit(b_acc_full);
@@ -214,6 +216,14 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
 #pragma unroll
             for (int r = 0; r < TE / NCW; ++r) {
                 const uint32_t e = (uint32_t)(warp + r * NCW);
+                if (sc.dbg & 2) {                                      // experiment: no conversion arithmetic
+                    const uint32_t a = dst + e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 0 * PLANE), "r"(raw[r].x) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 1 * PLANE), "r"(raw[r].y) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 2 * PLANE), "r"(raw[r].z) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 3 * PLANE), "r"(raw[r].w) : "memory");
+                    continue;
+                }
                 const uint32_t w0 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) + 0x00808080u) ^ 0x00808080u;
                 const uint32_t w1 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) + 0x00808080u) ^ 0x00808080u;
                 const uint32_t w2 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) + 0x00808080u) ^ 0x00808080u;
@@ -248,10 +258,10 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                 const uint32_t trow = tmem0 + ((uint32_t)(32 * (warp & 3)) << 16);
                 for (int c0 = c_begin; c0 < c_begin + CPW; c0 += 16) {
                     int32_t a0[16], a1[16], a2[16], a3[16];
-                    tmem_ld16(trow + 0 * 128 + c0, a0);
-                    tmem_ld16(trow + 1 * 128 + c0, a1);
-                    tmem_ld16(trow + 2 * 128 + c0, a2);
-                    tmem_ld16(trow + 3 * 128 + c0, a3);
+                    tmem_ld16(trow + 3 * 128 + c0, a0);            // a0: t = 6, a1: t = 5, a2: t = 4, a3: t = 3
+                    tmem_ld16(trow + 2 * 128 + c0, a1);
+                    tmem_ld16(trow + 1 * 128 + c0, a2);
+                    tmem_ld16(trow + 0 * 128 + c0, a3);
                     tmem_ld_wait();
                     double *yp = slot + (size_t)m * 128 + c0;
 #pragma unroll
@@ -305,22 +315,35 @@ k_colmax_f32(const float *__restrict__ B, long long nfloats, int D, unsigned *__
 
 // ---- final sum over slots (fixed order) -----------------------------------------------------------
 // Ysum[p][q] = sum_slots Y; thread per element, 4 independent partial sums, combined in a fixed order.
-// Blocks 0..63: Y; block 64: the diagonal correction (sum over CTAs and converter warps).
+// 256 threads = 32 elements x 8 slot phases: thread (el, ph) adds slots ph, ph + 8, ... with four
+// independent loads in flight, the 8 phases are then added in phase order (a fixed tree: bitwise
+// reproducible for a fixed grid).  Blocks 0..511: Y (16384 elements); blocks 512..515: the diagonal
+// correction (128 elements, nslots * NCW partial rows).
 __global__ void __launch_bounds__(256)
 k_i8_slot_sum(const double *__restrict__ slots, int nslots, double *__restrict__ ysum,
               const double *__restrict__ dslots, double *__restrict__ dsum)
 {
+    __shared__ double s_ph[8][33];
+    const int el = threadIdx.x & 31, ph = threadIdx.x >> 5;
     const double *src; size_t stride; int cnt; double *dst;
-    if (blockIdx.x < 64) { const int idx = blockIdx.x * 256 + threadIdx.x; src = slots + idx; stride = 16384; cnt = nslots; dst = ysum + idx; }
-    else { if (threadIdx.x >= 128) return; src = dslots + threadIdx.x; stride = 128; cnt = nslots * NCW; dst = dsum + threadIdx.x; }
+    if (blockIdx.x < 512) { const int idx = blockIdx.x * 32 + el; src = slots + idx; stride = 16384; cnt = nslots; dst = ysum + idx; }
+    else { const int idx = (blockIdx.x - 512) * 32 + el; src = dslots + idx; stride = 128; cnt = nslots * NCW; dst = dsum + idx; }
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    int s = 0;
-    for (; s + 4 <= cnt; s += 4) {
-        a0 += __ldcg(src + (size_t)s * stride);       a1 += __ldcg(src + (size_t)(s + 1) * stride);
-        a2 += __ldcg(src + (size_t)(s + 2) * stride); a3 += __ldcg(src + (size_t)(s + 3) * stride);
+    int s = ph;
+    for (; s + 24 < cnt; s += 32) {
+        const double x0 = __ldcg(src + (size_t)s * stride),        x1 = __ldcg(src + (size_t)(s + 8) * stride);
+        const double x2 = __ldcg(src + (size_t)(s + 16) * stride), x3 = __ldcg(src + (size_t)(s + 24) * stride);
+        a0 += x0; a1 += x1; a2 += x2; a3 += x3;
     }
-    for (; s < cnt; ++s) a0 += __ldcg(src + (size_t)s * stride);
-    *dst = (a0 + a1) + (a2 + a3);
+    for (; s < cnt; s += 8) a0 += __ldcg(src + (size_t)s * stride);
+    s_ph[ph][el] = (a0 + a1) + (a2 + a3);
+    __syncthreads();
+    if (ph == 0) {
+        double t = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) t += s_ph[q][el];
+        *dst = t;
+    }
 }
 
 struct Exps { int e[128]; };                   // s_p of the 128-wide view
@@ -458,11 +481,12 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     i8::Scales sc;
     i8::Exps ex;
     memcpy(sc.s, ctx->i8q.scale, sizeof(sc.s));
+    sc.dbg = ctx->opt_norm >= 16 ? (ctx->opt_norm >> 4) : 0;
     memcpy(ex.e, ctx->i8q.exp, sizeof(ex.e));
     i8::k_norm_i8<<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
-    i8::k_i8_slot_sum<<<65, 256, 0, ctx->stream>>>(slots, (int)grid, ysum, dslots, dsum);
+    i8::k_i8_slot_sum<<<516, 256, 0, ctx->stream>>>(slots, (int)grid, ysum, dslots, dsum);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     const float *tail = reinterpret_cast<const float *>(ctx->mc.amps) + (size_t)rows * 128;

@@ -154,6 +154,33 @@ def assemble(L, T, M, V):
     return nll.value, g, parts
 
 
+def assemble_eq2(n_data, L, T, M, V):
+    """eq. 2 (normalised) form -> (nll2, grad[n,2], parts[2])."""
+    n = np.asarray(V).shape[0]
+    T, M, V = _f64(T, (n, 2)), _f64(M, (n, n, 2)), _f64(V, (n, 2))
+    nll = C.c_double(0.0)
+    g = np.zeros((n, 2))
+    parts = np.zeros(2)
+    lib().pwa_oracle_assemble_eq2(C.c_int(n), C.c_double(float(n_data)), C.c_double(L), _p(T), _p(M), _p(V),
+                                  C.byref(nll), _p(g), _p(parts))
+    return nll.value, g, parts
+
+
+def nll_grad_eq2(A, M, V):
+    """eq. 2 form from the data term + M -> (nll2, grad[n,2], parts[2])."""
+    L, T, bad = data_term(A, V)
+    return assemble_eq2(np.asarray(A).shape[0], L, T, M, V)
+
+
+def grad_polar(V, grad):
+    """Cartesian gradient [n,2] -> (d/dr, d/dphi) [n,2] at V = r exp(i phi)."""
+    n = np.asarray(V).shape[0]
+    V, grad = _f64(V, (n, 2)), _f64(grad, (n, 2))
+    out = np.zeros((n, 2))
+    lib().pwa_oracle_grad_polar(C.c_int(n), _p(V), _p(grad), _p(out))
+    return out
+
+
 def nll_grad(A, M, V):
     """-> (nll, grad[n,2], parts[2], n_nonfinite)."""
     A, dt = _amp(A)

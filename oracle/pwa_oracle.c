@@ -33,7 +33,9 @@
  * transposed pairing fails, P5 gradient vs central differences, P6 eq.1 == eq.3 double
  * sum on dyadic inputs, P7 Euler identity sum_a V_a T_a = N, P8 numpy BLAS (zgemm/zgemv),
  * P9 permutation / duplication / scaling invariances, P10 Breit-Wigner closed forms and
- * derivative vs differences, brute-force pure-Python on tiny inputs.
+ * derivative vs differences, brute-force pure-Python on tiny inputs; P13 eq. 2 form: scale
+ * invariance, finite differences, equality with eq. 3 at Norm = N_data; P14 polar chain rule vs
+ * finite differences in (r, phi).
  * Parity unpinned by the paper: the choices C2, C3, C4, C5, C9-C13 (definitions, not
  * results), and the resonance-parameter gradient beyond finite differences (P5/P10 style).
  *
@@ -298,6 +300,41 @@ void pwa_oracle_assemble(int n, double L, const double *T, const double *M, cons
     double Nv = nval(&nrm);
     *nll = -(L - Nv);
     if (parts) { parts[0] = L; parts[1] = Nv; }
+}
+
+/* ---------- NEXT-4 variants: eq. 2 form and polar parameters ------------
+ * eq. 2: L = prod_i I(Om_i) / integral(eps I).  With the integral done as the MC sum of
+ * eq. 3, integral = Norm(V) = V^H M V, so
+ *     ln L2 = L_data - N_data ln Norm,   nll2 = -L_data + N_data ln Norm,
+ *     g(nll2) = -2 conj(T) + (2 N_data / Norm) M V.
+ * Invariant under V -> s V (the overall scale is not a parameter of eq. 2).                       */
+void pwa_oracle_assemble_eq2(int n, double N_data, double L, const double *T, const double *M,
+                             const double *V, double *nll, double *grad, double *parts)
+{
+    double nll3, p3[2];
+    double *g3 = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    double *zero = (double *)calloc(2 * (size_t)n, sizeof(double));
+    pwa_oracle_assemble(n, 0.0, zero, M, V, &nll3, g3, p3);      /* g3 = 2 M V, p3[1] = Norm */
+    double Nv = p3[1];
+    *nll = -L + N_data * log(Nv);
+    for (int a = 0; a < n; ++a) {
+        grad[2 * a]     = -2.0 * T[2 * a]     + (N_data / Nv) * g3[2 * a];
+        grad[2 * a + 1] =  2.0 * T[2 * a + 1] + (N_data / Nv) * g3[2 * a + 1];
+    }
+    if (parts) { parts[0] = L; parts[1] = Nv; }
+    free(g3); free(zero);
+}
+
+/* Polar parameters: V_a = r_a exp(i phi_a).  Chain rule on a Cartesian gradient
+ * (gx, gy) = (d f/d Re V_a, d f/d Im V_a):  d f/d r = gx cos(phi) + gy sin(phi),
+ * d f/d phi = -gx r sin(phi) + gy r cos(phi) = -Im V gx + Re V gy.  out: [n][2] = (d/dr, d/dphi). */
+void pwa_oracle_grad_polar(int n, const double *V, const double *grad, double *out)
+{
+    for (int a = 0; a < n; ++a) {
+        double x = V[2 * a], y = V[2 * a + 1], r = hypot(x, y), phi = atan2(y, x);
+        out[2 * a]     = grad[2 * a] * cos(phi) + grad[2 * a + 1] * sin(phi);
+        out[2 * a + 1] = -grad[2 * a] * r * sin(phi) + grad[2 * a + 1] * r * cos(phi);
+    }
 }
 
 int64_t pwa_oracle_nll_grad(const void *A, int dt, int64_t N, int n, const double *M,

@@ -437,3 +437,71 @@ def test_cfg1_generator_recipe(synth):
     # a shorter request is a prefix of a longer one
     w3 = synth.make_workload(1, n_data=5_000, n_mc=10_000)
     assert np.array_equal(w3.A_data, w.A_data[:5000]) and np.array_equal(w3.A_mc, w.A_mc[:10000])
+
+
+# ---------------------------------------------------------------- P13 eq. 2 (normalised) form, P14 polar parameters
+def test_p13_eq2_form(oracle):
+    """eq. 2 with the MC integral of P:35: nll2 = -L_data + N ln Norm.
+    (a) independent of the overall scale of V (eq. 2 is a ratio); (b) gradient vs central
+    differences; (c) at a V with Norm(V) = N it equals eq. 3 up to the constant N ln N - N and has
+    the SAME gradient; (d) numpy restatement of the definition."""
+    rng = np.random.default_rng(13)
+    N, Nacc, n = 400, 700, 5
+    A, B = rand_amps(rng, N, n), rand_amps(rng, Nacc, n)
+    V = rng.normal(size=(n, 2))
+    M = oracle.norm_matrix(B, Nacc + 50)
+    f, g, parts = oracle.nll_grad_eq2(A, M, V)
+    # (d) definition in numpy: -sum ln|S|^2 + N ln( V^H M V )
+    Vc, Ac, Mc = cplx(V), cplx(A), cplx(M)
+    norm = (Vc.conj() @ Mc @ Vc).real
+    assert f == pytest.approx(-np.log(np.abs(Ac @ Vc) ** 2).sum() + N * math.log(norm), rel=1e-13)
+    # (a) scale invariance, and the gradient scales like 1/s
+    for s in (0.37, 4.2):
+        f2, g2, _ = oracle.nll_grad_eq2(A, M, s * V)
+        assert f2 == pytest.approx(f, rel=1e-13)
+        assert np.allclose(g2 * s, g, rtol=1e-11, atol=1e-11 * np.abs(g).max())
+    assert abs((V * g).sum()) <= 1e-10 * np.abs(g).max()          # Euler: V . grad = 0 (degree-0 homogeneous)
+    # (b) central differences
+    h = 1e-6
+    for a in range(n):
+        for c in range(2):
+            Vp, Vm = V.copy(), V.copy()
+            Vp[a, c] += h
+            Vm[a, c] -= h
+            fd = (oracle.nll_grad_eq2(A, M, Vp)[0] - oracle.nll_grad_eq2(A, M, Vm)[0]) / (2 * h)
+            assert fd == pytest.approx(g[a, c], rel=2e-7, abs=2e-7 * np.abs(g).max())
+    # (c) rescale V so that Norm = N: eq. 2 and eq. 3 share the gradient there
+    Vs = V * math.sqrt(N / parts[1])
+    f3, g3, p3, _ = oracle.nll_grad(A, M, Vs)
+    f2, g2, p2 = oracle.nll_grad_eq2(A, M, Vs)
+    assert p3[1] == pytest.approx(N, rel=1e-13)
+    assert f2 == pytest.approx(f3 - N + N * math.log(N), rel=1e-12)
+    assert np.allclose(g2, g3, rtol=1e-10, atol=1e-10 * np.abs(g3).max())
+
+
+def test_p14_polar_chain_rule(oracle):
+    """V_a = r_a exp(i phi_a).  (d/dr, d/dphi) from the Cartesian gradient vs central
+    differences taken directly in (r, phi); the sum of d/dphi vanishes (global phase, P2)."""
+    rng = np.random.default_rng(14)
+    N, Nacc, n = 300, 500, 4
+    A, B = rand_amps(rng, N, n), rand_amps(rng, Nacc, n)
+    r, phi = rng.uniform(0.3, 2.0, n), rng.uniform(-math.pi, math.pi, n)
+    M = oracle.norm_matrix(B, Nacc)
+
+    def f_polar(r, phi):
+        V = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=-1)
+        return oracle.nll_grad(A, M, V)
+
+    V = np.stack([r * np.cos(phi), r * np.sin(phi)], axis=-1)
+    _, g, _, _ = oracle.nll_grad(A, M, V)
+    gp = oracle.grad_polar(V, g)
+    h = 1e-6
+    for a in range(n):
+        e = np.zeros(n)
+        e[a] = h
+        fd_r = (f_polar(r + e, phi)[0] - f_polar(r - e, phi)[0]) / (2 * h)
+        fd_p = (f_polar(r, phi + e)[0] - f_polar(r, phi - e)[0]) / (2 * h)
+        scale = np.abs(gp).max()
+        assert fd_r == pytest.approx(gp[a, 0], rel=2e-7, abs=2e-7 * scale)
+        assert fd_p == pytest.approx(gp[a, 1], rel=2e-7, abs=2e-7 * scale)
+    assert abs(gp[:, 1].sum()) <= 1e-10 * np.abs(gp).max()

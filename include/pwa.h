@@ -148,6 +148,22 @@ pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
 pwa_status pwa_assemble_host(int32_t n_waves, double L_data, const double *T, const double *M,
                              const double *V, double *nll, double *grad, double *parts);
 
+/* eq. 2 form of step A7: the likelihood normalised by the MC integral instead of the
+ * extended form of eq. 3 (reading C2):  nll2 = -L_data + N_data ln Norm,
+ * grad2 = -2 conj(T) + (2 N_data / Norm) M V.  Invariant under V -> s V.  Host only; same
+ * argument meaning as pwa_assemble_host, n_data = N_data > 0.  On the device the same form is
+ * selected for pwa_nll_grad / pwa_nll_grad_batch with pwa_set_option(ctx, "likelihood", 1).     */
+pwa_status pwa_assemble_host_eq2(int32_t n_waves, double n_data, double L_data, const double *T,
+                                 const double *M, const double *V, double *nll, double *grad,
+                                 double *parts);
+
+/* Polar parametrisation V_a = r_a exp(i phi_a), host only.  pwa_grad_to_polar: chain
+ * rule on a Cartesian gradient grad[n][2] at V[n][2] -> grad_polar[n][2] = (d/dr_a, d/dphi_a)
+ * (at r_a = 0 the radial direction is taken along the real axis).  pwa_polar_to_cartesian:
+ * r_phi[n][2] = (r_a, phi_a) -> V[n][2].                                                        */
+pwa_status pwa_grad_to_polar(int32_t n_waves, const double *V, const double *grad, double *grad_polar);
+pwa_status pwa_polar_to_cartesian(int32_t n_waves, const double *r_phi, double *V);
+
 /* Floating mode: gradient of nll w.r.t. the resonance parameters at the current
  * (mass0, width0) and the given V (reading A9):  d nll / d M_r and d nll / d G_r, HOST
  * [n_res] each.  Needs factored DATA and MC uploads.  One extra pass over data and MC.   */
@@ -178,9 +194,11 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx);
 pwa_status pwa_sync(pwa_ctx *ctx);
 
 /* Selects a kernel variant for experiments (0 = default).  Returns PWA_ERR_INVALID_ARG for
- * unknown keys.  Keys: "data_term", "norm", "batch".  "norm": 0 = default (int8 tcgen05 path for
+ * unknown keys.  Keys: "data_term", "norm", "batch", "likelihood".  "norm": 0 = default (int8 tcgen05 path for
  * fp32-stored constant-resonance samples of >= 65536 events, else FP64 DMMA), 1 = FP64 DMMA,
- * 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.           */
+ * 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.
+ * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
+ * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch and the minimisers.    */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
 
 /* Register-resident peak probes used as roofline denominators:

@@ -29,6 +29,7 @@ SYMBOLS = [
     "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
+    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian",
 ]
 
 
@@ -72,6 +73,9 @@ def _load():
         "pwa_set_option": (C.c_int, [vp, C.c_char_p, i32]),
         "pwa_microbench": (C.c_int, [vp, i32, i64, dp]),
         "pwa_norm_error_bound": (C.c_int, [vp, dp, C.POINTER(i32)]),
+        "pwa_assemble_host_eq2": (C.c_int, [i32, C.c_double, C.c_double, vp, vp, vp, dp, vp, vp]),
+        "pwa_grad_to_polar": (C.c_int, [i32, vp, vp, vp]),
+        "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)          # AttributeError here = header/library mismatch
@@ -247,6 +251,35 @@ def pwa_assemble_host(L_data, T, M, V):
     if st != PWA_OK:
         raise PwaError(st, "pwa_assemble_host")
     return nll.value, grad, parts
+
+
+def pwa_assemble_host_eq2(n_data, L_data, T, M, V):
+    """eq. 2 form of step A7 on the host -> (nll2, grad[n,2], parts[2])."""
+    V = _f64(V)
+    n = V.shape[0]
+    T, M = _f64(T, (n, 2)), _f64(M, (n, n, 2))
+    nll, g, parts = C.c_double(0.0), np.zeros((n, 2)), np.zeros(2)
+    st = _lib.pwa_assemble_host_eq2(n, float(n_data), float(L_data), T.ctypes.data, M.ctypes.data, V.ctypes.data,
+                                    C.byref(nll), g.ctypes.data, parts.ctypes.data)
+    _check(None, st)
+    return nll.value, g, parts
+
+
+def pwa_grad_to_polar(V, grad):
+    V = _f64(V)
+    n = V.shape[0]
+    grad = _f64(grad, (n, 2))
+    out = np.zeros((n, 2))
+    _check(None, _lib.pwa_grad_to_polar(n, V.ctypes.data, grad.ctypes.data, out.ctypes.data))
+    return out
+
+
+def pwa_polar_to_cartesian(r_phi):
+    r_phi = _f64(r_phi)
+    n = r_phi.shape[0]
+    V = np.zeros((n, 2))
+    _check(None, _lib.pwa_polar_to_cartesian(n, r_phi.ctypes.data, V.ctypes.data))
+    return V
 
 
 def pwa_res_grad(ctx, V, n_res):

@@ -418,6 +418,53 @@ pwa_status pwa_assemble_host(int32_t n, double L_data, const double *T, const do
     return PWA_OK;
 }
 
+pwa_status pwa_assemble_host_eq2(int32_t n, double n_data, double L_data, const double *T, const double *M,
+                                 const double *V, double *nll, double *grad, double *parts)
+{
+    if (n < 1 || !(n_data > 0.0) || !T || !M || !V || !nll || !grad) return PWA_ERR_INVALID_ARG;
+    double norm = 0.0;
+    for (int a = 0; a < n; ++a) {
+        double mr = 0.0, mi = 0.0;
+        for (int b = 0; b < n; ++b) {
+            const double Mr = M[((size_t)a * n + b) * 2], Mi = M[((size_t)a * n + b) * 2 + 1];
+            mr += Mr * V[2 * b] - Mi * V[2 * b + 1];
+            mi += Mr * V[2 * b + 1] + Mi * V[2 * b];
+        }
+        norm += V[2 * a] * mr + V[2 * a + 1] * mi;
+        grad[2 * a] = mr;  grad[2 * a + 1] = mi;                   // (M V)_a for now
+    }
+    const double gw = 2.0 * (n_data / norm);
+    for (int a = 0; a < n; ++a) {
+        grad[2 * a] = -2.0 * T[2 * a] + gw * grad[2 * a];
+        grad[2 * a + 1] = 2.0 * T[2 * a + 1] + gw * grad[2 * a + 1];
+    }
+    *nll = -L_data + n_data * log(norm);
+    if (parts) { parts[0] = L_data; parts[1] = norm; }
+    return PWA_OK;
+}
+
+pwa_status pwa_grad_to_polar(int32_t n, const double *V, const double *grad, double *grad_polar)
+{
+    if (n < 1 || !V || !grad || !grad_polar) return PWA_ERR_INVALID_ARG;
+    for (int a = 0; a < n; ++a) {
+        const double x = V[2 * a], y = V[2 * a + 1], r = sqrt(x * x + y * y);
+        const double gx = grad[2 * a], gy = grad[2 * a + 1];
+        grad_polar[2 * a] = r > 0.0 ? (gx * x + gy * y) / r : gx;   // d/dr = gx cos(phi) + gy sin(phi); phi := 0 at r = 0
+        grad_polar[2 * a + 1] = -y * gx + x * gy;                    // d/dphi
+    }
+    return PWA_OK;
+}
+
+pwa_status pwa_polar_to_cartesian(int32_t n, const double *r_phi, double *V)
+{
+    if (n < 1 || !r_phi || !V) return PWA_ERR_INVALID_ARG;
+    for (int a = 0; a < n; ++a) {
+        V[2 * a] = r_phi[2 * a] * cos(r_phi[2 * a + 1]);
+        V[2 * a + 1] = r_phi[2 * a] * sin(r_phi[2 * a + 1]);
+    }
+    return PWA_OK;
+}
+
 pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG)
 {
     if (!ctx || !V || !dM || !dG) return PWA_ERR_INVALID_ARG;
@@ -445,6 +492,7 @@ pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
     if (!strcmp(key, "data_term")) ctx->opt_data_term = value;
     else if (!strcmp(key, "norm")) ctx->opt_norm = value;
     else if (!strcmp(key, "batch")) ctx->opt_batch = value;
+    else if (!strcmp(key, "likelihood")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "likelihood must be 0 (eq. 3) or 1 (eq. 2)"); ctx->opt_likelihood = value; }
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
 }

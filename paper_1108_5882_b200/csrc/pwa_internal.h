@@ -71,6 +71,7 @@ struct pwa_ctx {
     struct { bool valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8q;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
+    int opt_likelihood = 0;                   // 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form
     std::string err;
 };
 

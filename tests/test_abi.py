@@ -88,3 +88,23 @@ def test_product_does_not_import_oracle():
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_1108_5882_b200", text, flags=re.M), f
             assert "#include \"../paper" not in text and "csrc/" not in text.replace("paper_1108_5882_b200/csrc/,", ""), f
+
+
+def test_eq2_and_polar_host_twins_match_oracle(binding):
+    """NEXT-4: the host-only eq. 2 assembly and the polar chain rule against the oracle (no GPU)."""
+    from oracle import oracle
+    rng = np.random.default_rng(42)
+    n, N = 6, 250
+    A = rng.normal(size=(N, n, 2)) * 0.4
+    B = rng.normal(size=(400, n, 2)) * 0.4
+    V = rng.normal(size=(n, 2))
+    M = oracle.norm_matrix(B, 450)
+    L, T, _ = oracle.data_term(A, V)
+    nll_o, g_o, parts_o = oracle.assemble_eq2(N, L, T, M, V)
+    nll, g, parts = binding.pwa_assemble_host_eq2(N, L, T, M, V)
+    assert nll == pytest.approx(nll_o, rel=1e-13) and np.allclose(parts, parts_o, rtol=1e-13)
+    assert np.abs(g - g_o).max() <= 1e-12 * np.abs(g_o).max()
+    gp = binding.pwa_grad_to_polar(V, g)
+    assert np.abs(gp - oracle.grad_polar(V, g)).max() <= 1e-13 * np.abs(gp).max()
+    r_phi = np.stack([np.hypot(V[:, 0], V[:, 1]), np.arctan2(V[:, 1], V[:, 0])], axis=-1)
+    assert np.allclose(binding.pwa_polar_to_cartesian(r_phi), V, rtol=1e-14, atol=1e-15)

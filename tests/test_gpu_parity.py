@@ -371,3 +371,33 @@ def test_norm_i8_default_path_and_nonfinite(pwa, oracle):
         pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B[:100_000], n_generated=100_000)
         pwa.pwa_build_norm(c.ctx, want_M=False)
         assert pwa.pwa_norm_error_bound(c.ctx)[1] == 0
+
+
+# ------------------------------------------------------------------ NEXT-4: eq. 2 (normalised) likelihood form on the device
+@pytest.mark.parametrize("storage,n,K", [("f64", 4, 3), ("f64", 16, 5), ("f32", 32, 4), ("f32", 64, 33), ("f64", 5, 2)])
+def test_eq2_likelihood_mode(pwa, oracle, storage, n, K):
+    """pwa_set_option("likelihood", 1): nll2 = -L_data + N ln Norm and its gradient from the SAME
+    kernels (single-V, batched, generic), against the oracle's eq. 2 form; scale invariance on the GPU."""
+    N = 7001
+    A, B, _ = rand_case(77 + n, N, 3001, n, storage)
+    Vk = np.random.default_rng(n).normal(size=(K, n, 2))
+    M_o = oracle.norm_matrix(B, 3100)
+    tol = TOL[storage]
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=3100)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        nllk, gk, partsk = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        for k in range(K):
+            ref = oracle.nll_grad_eq2(A, M_o, Vk[k])
+            one = pwa.pwa_nll_grad(c.ctx, Vk[k])
+            check_eval(one, ref, tol, N)
+            check_eval((nllk[k], gk[k], partsk[k]), ref, tol, N)
+        s = 3.7
+        a, b = pwa.pwa_nll_grad(c.ctx, Vk[0]), pwa.pwa_nll_grad(c.ctx, s * Vk[0])
+        assert abs(a[0] - b[0]) <= 1e-12 * max(abs(a[0]), abs(a[2][0]))
+        pwa.pwa_set_option(c.ctx, "likelihood", 0)
+        check_eval(pwa.pwa_nll_grad(c.ctx, Vk[0]), oracle.nll_grad(A, M_o, Vk[0]), tol, N)
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_set_option(c.ctx, "likelihood", 2)

@@ -181,6 +181,17 @@ def grad_polar(V, grad):
     return out
 
 
+def fumili(A, V, M=None):
+    """Fumili-style approximate Hessian [2n, 2n] in the (x_0, y_0, x_1, ...) order; M=None -> data part only."""
+    A, dt = _amp(A)
+    N, n = A.shape[0], A.shape[1]
+    V = _f64(V, (n, 2))
+    H = np.zeros((2 * n, 2 * n))
+    Mp = _p(_f64(M, (n, n, 2))) if M is not None else None
+    lib().pwa_oracle_fumili(_p(A), C.c_int(dt), C.c_int64(N), C.c_int(n), _p(V), Mp, _p(H))
+    return H
+
+
 def nll_grad(A, M, V):
     """-> (nll, grad[n,2], parts[2], n_nonfinite)."""
     A, dt = _amp(A)

@@ -35,7 +35,8 @@
  * P9 permutation / duplication / scaling invariances, P10 Breit-Wigner closed forms and
  * derivative vs differences, brute-force pure-Python on tiny inputs; P13 eq. 2 form: scale
  * invariance, finite differences, equality with eq. 3 at Norm = N_data; P14 polar chain rule vs
- * finite differences in (r, phi).
+ * finite differences in (r, phi); P15 Fumili matrix: H_data V = 2 grad(L_data) (Euler), numpy
+ * restatement, PSD, Hess(Norm) vs differences of the norm gradient.
  * Parity unpinned by the paper: the choices C2, C3, C4, C5, C9-C13 (definitions, not
  * results), and the resonance-parameter gradient beyond finite differences (P5/P10 style).
  *
@@ -335,6 +336,46 @@ void pwa_oracle_grad_polar(int n, const double *V, const double *grad, double *o
         out[2 * a]     = grad[2 * a] * cos(phi) + grad[2 * a + 1] * sin(phi);
         out[2 * a + 1] = -grad[2 * a] * r * sin(phi) + grad[2 * a + 1] * r * cos(phi);
     }
+}
+
+/* ---------- NEXT-2: Fumili-style approximate Hessian (ref. P:123) -----
+ * For l_i = ln I_i the exact second derivative is (d2 I)/I - (dI)(dI)^T / I^2; Fumili keeps the
+ * outer-product term only.  With u_i = d l_i / d(x_0, y_0, x_1, ...) = (2 Re t_i0, -2 Im t_i0, ...),
+ * t_ia = A_ia / S_i:
+ *     H_data = sum_i u_i u_i^T          (2n x 2n, symmetric, positive semi-definite)
+ *     H      = H_data + Hess(Norm),  Hess(Norm) = 2 [[Re M_ab, -Im M_ab], [Im M_ab, Re M_ab]]  (exact: Norm is quadratic)
+ * approximates the Hessian of nll = -(L_data - Norm).  H: [2n][2n] row-major; M may be NULL (H_data only). */
+void pwa_oracle_fumili(const void *A, int dt, int64_t N, int n, const double *V, const double *M, double *H)
+{
+    const int D = 2 * n;
+    nsum *acc = (nsum *)calloc((size_t)D * D, sizeof(nsum));
+    double *u = (double *)malloc(sizeof(double) * D);
+    for (int64_t i = 0; i < N; ++i) {
+        long double sr = 0.0L, si = 0.0L;
+        for (int a = 0; a < n; ++a) {
+            double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
+            sr += (long double)V[2 * a] * ar - (long double)V[2 * a + 1] * ai;
+            si += (long double)V[2 * a] * ai + (long double)V[2 * a + 1] * ar;
+        }
+        double Sr = (double)sr, Si = (double)si, I = Sr * Sr + Si * Si;
+        for (int a = 0; a < n; ++a) {
+            double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
+            /* t = A / S = A conj(S) / I */
+            double tr = (ar * Sr + ai * Si) / I, ti = (ai * Sr - ar * Si) / I;
+            u[2 * a] = 2.0 * tr;  u[2 * a + 1] = -2.0 * ti;
+        }
+        for (int p = 0; p < D; ++p)
+            for (int q = 0; q < D; ++q) nadd(&acc[p * D + q], u[p] * u[q]);
+    }
+    for (int p = 0; p < D * D; ++p) H[p] = nval(&acc[p]);
+    if (M)
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) {
+                double Mr = M[(a * n + b) * 2], Mi = M[(a * n + b) * 2 + 1];
+                H[(2 * a) * D + 2 * b] += 2.0 * Mr;          H[(2 * a) * D + 2 * b + 1] += -2.0 * Mi;
+                H[(2 * a + 1) * D + 2 * b] += 2.0 * Mi;      H[(2 * a + 1) * D + 2 * b + 1] += 2.0 * Mr;
+            }
+    free(acc); free(u);
 }
 
 int64_t pwa_oracle_nll_grad(const void *A, int dt, int64_t N, int n, const double *M,

@@ -505,3 +505,51 @@ def test_p14_polar_chain_rule(oracle):
         assert fd_r == pytest.approx(gp[a, 0], rel=2e-7, abs=2e-7 * scale)
         assert fd_p == pytest.approx(gp[a, 1], rel=2e-7, abs=2e-7 * scale)
     assert abs(gp[:, 1].sum()) <= 1e-10 * np.abs(gp).max()
+
+
+# ---------------------------------------------------------------- P15 Fumili-style approximate Hessian (NEXT-2)
+def test_p15_fumili_matrix(oracle):
+    """H_data = sum_i u_i u_i^T with u_i = grad ln I_i.  (a) numpy/BLAS restatement; (b) symmetric PSD;
+    (c) Euler identity: ln I is homogeneous of degree 0 in V up to ln s^2, so u_i . (x, y) = 2 and
+    H_data (x, y) = 2 sum_i u_i = 2 grad(L_data); (d) Hess(Norm) equals the (exact) finite difference of
+    the norm gradient 2 M V; (e) u_i itself against central differences of ln I for one event."""
+    rng = np.random.default_rng(15)
+    N, n = 300, 5
+    A, B = rand_amps(rng, N, n), rand_amps(rng, 500, n)
+    V = rng.normal(size=(n, 2))
+    M = oracle.norm_matrix(B, 520)
+    Hd = oracle.fumili(A, V)
+    # (a)
+    Ac, Vc = cplx(A), cplx(V)
+    t = Ac / (Ac @ Vc)[:, None]
+    U = np.empty((N, 2 * n))
+    U[:, 0::2], U[:, 1::2] = 2 * t.real, -2 * t.imag
+    assert np.abs(Hd - U.T @ U).max() <= 1e-12 * np.abs(Hd).max()
+    # (b)
+    assert np.array_equal(Hd, Hd.T) and np.linalg.eigvalsh(Hd).min() >= -1e-10 * np.trace(Hd)
+    # (c)
+    L, T, _ = oracle.data_term(A, V)
+    gL = np.empty(2 * n)
+    gL[0::2], gL[1::2] = 2 * T[:, 0], -2 * T[:, 1]              # grad L_data = 2 conj(T)
+    assert np.abs(Hd @ V.reshape(-1) - 2 * gL).max() <= 1e-11 * np.abs(gL).max()
+    # (d) Norm is quadratic: central differences of its gradient are exact up to rounding
+    H = oracle.fumili(A, V, M)
+    HN = H - Hd
+    zero = np.zeros((n, 2))
+    for p in range(2 * n):
+        e = np.zeros(2 * n)
+        e[p] = 0.5
+        gp = oracle.assemble(0.0, zero, M, (V.reshape(-1) + e).reshape(n, 2))[1].reshape(-1)
+        gm = oracle.assemble(0.0, zero, M, (V.reshape(-1) - e).reshape(n, 2))[1].reshape(-1)
+        assert np.abs((gp - gm) - HN[:, p]).max() <= 1e-12 * np.abs(HN).max()
+    # (e) one event: u = grad ln I by central differences
+    H1 = oracle.fumili(A[:1], V)
+    h = 1e-6
+    u = np.empty(2 * n)
+    for p in range(2 * n):
+        e = np.zeros(2 * n)
+        e[p] = h
+        lp = oracle.data_term(A[:1], (V.reshape(-1) + e).reshape(n, 2))[0]
+        lm = oracle.data_term(A[:1], (V.reshape(-1) - e).reshape(n, 2))[0]
+        u[p] = (lp - lm) / (2 * h)
+    assert np.abs(H1 - np.outer(u, u)).max() <= 1e-6 * np.abs(H1).max()

@@ -148,6 +148,16 @@ pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
 pwa_status pwa_assemble_host(int32_t n_waves, double L_data, const double *T, const double *M,
                              const double *V, double *nll, double *grad, double *parts);
 
+/* Fumili-style approximate Hessian of nll at V (Minuit / Fumili; "most of the computing time
+ * is spent on ... error calculations"), DESIGN.md section 13:
+ *   H = sum_i u_i u_i^T  (+ Hess(Norm) if with_norm != 0),   u_i = d ln I_i / d(x_0, y_0, x_1, ...)
+ *     = (2 Re t_i0, -2 Im t_i0, ...),  t_ia = A_ia / S_i;  Hess(Norm) = 2 [[Re M, -Im M], [Im M, Re M]].
+ * One extra pass over the DATA sample: a second dense contraction (the Gram matrix of the rows
+ * A_i / S_i) on the FP64 tensor cores.  V: HOST [n][2].  H: HOST [2n][2n] doubles, row-major,
+ * parameter order as in grad; exactly symmetric, positive semi-definite without the norm part.
+ * n <= 64.  PWA_ERR_STATE if DATA (or, with_norm, M) is missing.  Synchronous.                  */
+pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t with_norm);
+
 /* eq. 2 form of step A7: the likelihood normalised by the MC integral instead of the
  * extended form of eq. 3 (reading C2):  nll2 = -L_data + N_data ln Norm,
  * grad2 = -2 conj(T) + (2 N_data / Norm) M V.  Invariant under V -> s V.  Host only; same

@@ -29,7 +29,7 @@ SYMBOLS = [
     "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
-    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian",
+    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian",
 ]
 
 
@@ -75,6 +75,7 @@ def _load():
         "pwa_norm_error_bound": (C.c_int, [vp, dp, C.POINTER(i32)]),
         "pwa_assemble_host_eq2": (C.c_int, [i32, C.c_double, C.c_double, vp, vp, vp, dp, vp, vp]),
         "pwa_grad_to_polar": (C.c_int, [i32, vp, vp, vp]),
+        "pwa_fumili_hessian": (C.c_int, [vp, vp, vp, i32]),
         "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
     }
     for name, (res, args) in sig.items():
@@ -251,6 +252,15 @@ def pwa_assemble_host(L_data, T, M, V):
     if st != PWA_OK:
         raise PwaError(st, "pwa_assemble_host")
     return nll.value, grad, parts
+
+
+def pwa_fumili_hessian(ctx, V, with_norm=True):
+    """-> H [2n, 2n] (Fumili-style approximate Hessian of nll, parameter order as in grad)."""
+    V = _f64(V)
+    n = V.shape[0]
+    H = np.zeros((2 * n, 2 * n))
+    _check(ctx, _lib.pwa_fumili_hessian(ctx, V.ctypes.data, H.ctypes.data, 1 if with_norm else 0))
+    return H
 
 
 def pwa_assemble_host_eq2(n_data, L_data, T, M, V):

@@ -72,7 +72,7 @@ struct NormCfg {
 
 template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S, int NANG>
 __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long N, int n, const FactArgs &f,
-                                          double *__restrict__ scratch, double *smem)
+                                          double *__restrict__ scratch, double *smem, const double *__restrict__ Vs)
 {
     using C = NormCfg<ST, NB, SPLIT, MODE, THREADS, ET>;
     constexpr int D = C::D, DP = C::DP, NG = C::NG, QPT = C::QPT, PPW = C::PPW, NPAIRS = C::NPAIRS;
@@ -153,6 +153,30 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
             }
         }
     };
+    // Fumili mode (Vs != nullptr): every row of the tile is replaced by
+    // t_i = A_i / S_i, S_i = sum_a V_a A_ia, so that the Gram matrix becomes sum_i (Re t, Im t)(Re t, Im t)^T.
+    // TPS adjacent lanes share an event (xor-shuffle sum of the partial S); rows past N stay zero.
+    auto scale_tile = [&](double *tile, long long t) {
+        constexpr int TPS = THREADS / ET;
+        const int e = tid / TPS, part = tid % TPS;
+        double *row = tile + e * DP;
+        double sr = 0.0, si = 0.0;
+        for (int a = part; a < n; a += TPS) {
+            const double2 x = *reinterpret_cast<const double2 *>(row + 2 * a);
+            const double vr = __ldg(Vs + 2 * a), vi = __ldg(Vs + 2 * a + 1);
+            sr = fma(vr, x.x, sr); sr = fma(-vi, x.y, sr);
+            si = fma(vr, x.y, si); si = fma(vi, x.x, si);
+        }
+#pragma unroll
+        for (int m = 1; m < TPS; m <<= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, m); si += __shfl_xor_sync(0xffffffffu, si, m); }
+        if (t * ET + e < N) {
+            const double I = sr * sr + si * si, rr = sr / I, ri = -si / I;      // r = 1 / S = conj(S) / I
+            for (int a = part; a < n; a += TPS) {
+                const double2 x = *reinterpret_cast<const double2 *>(row + 2 * a);
+                *reinterpret_cast<double2 *>(row + 2 * a) = make_double2(x.x * rr - x.y * ri, x.x * ri + x.y * rr);
+            }
+        }
+    };
     auto compute = [&](const double *src) {
 #pragma unroll 1
         for (int q = group; q < QPT; q += NG) quad_mma<NB, SPLIT, S, PPW>(src + q * 4 * DP, DP, lane, acc);
@@ -172,6 +196,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
     __syncthreads();
     for (; t < ntiles; t += gridDim.x) {
         const long long nxt = t + gridDim.x;
+        if (Vs != nullptr) { scale_tile(buf[cur], t); __syncthreads(); }
         if constexpr (MODE == FILL_STAGED) {
             if (nxt < ntiles) load_tile(nxt);
             compute(buf[cur]);
@@ -211,16 +236,17 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
 
 template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET, int NANG>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_norm_dmma(const void *__restrict__ Bv, long long N, int n, FactArgs f, double *__restrict__ scratch)
+k_norm_dmma(const void *__restrict__ Bv, long long N, int n, FactArgs f, double *__restrict__ scratch,
+            const double *__restrict__ Vs)
 {
     extern __shared__ double nd_smem[];
     const int S = (threadIdx.x >> 5) % SPLIT;
-    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem); return; }
+    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs); return; }
     switch (S) {        // warp-uniform: each sub-id owns a compile-time list of block pairs
-    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem); break;
-    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
-    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
-    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem); break;
+    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
+    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
+    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
+    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
     }
 }
 
@@ -270,8 +296,45 @@ k_norm_dmma_finalize(const double *__restrict__ scratch, int nslots, int n, int 
     }
 }
 
+// Fumili finalize: H[p][q] = +-4 P[p][q] (+ Hess(Norm) from M when M != nullptr),
+// P = sum over slots of the real Gram of t_i = A_i / S_i; sign - when exactly one of p, q is an
+// imaginary-part index (u_i = (2 Re t, -2 Im t)).  Thread per element p <= q, mirrored: exactly symmetric.
+__global__ void __launch_bounds__(256)
+k_fumili_finalize(const double *__restrict__ scratch, int nslots, int n, int NB, const double *__restrict__ M,
+                  double *__restrict__ H)
+{
+    const int D = 2 * n, idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx >= D * D) return;
+    const int p = idx / D, q = idx % D;
+    if (p > q) return;
+    const int i = p >> 3, j = q >> 3;                      // block pair (i <= j)
+    const int pair = i * NB - i * (i - 1) / 2 + (j - i);
+    const size_t stride = (size_t)NB * (NB + 1) / 2 * 64;
+    const double *src = scratch + (size_t)pair * 64 + (p & 7) * 8 + (q & 7);
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int s = 0;
+    for (; s + 4 <= nslots; s += 4) {
+        a0 += __ldcg(src + (size_t)s * stride);       a1 += __ldcg(src + (size_t)(s + 1) * stride);
+        a2 += __ldcg(src + (size_t)(s + 2) * stride); a3 += __ldcg(src + (size_t)(s + 3) * stride);
+    }
+    for (; s < nslots; ++s) a0 += __ldcg(src + (size_t)s * stride);
+    double h = (((p ^ q) & 1) ? -4.0 : 4.0) * ((a0 + a1) + (a2 + a3));
+    if (M != nullptr) {
+        const int a = p >> 1, b = q >> 1;
+        const double mr = M[((size_t)a * n + b) * 2], mi = M[((size_t)a * n + b) * 2 + 1];
+        // Hess(Norm) = 2 [[Re M, -Im M], [Im M, Re M]] on the (x_a, y_a) x (x_b, y_b) block
+        h += ((p & 1) == (q & 1)) ? 2.0 * mr : ((p & 1) ? 2.0 * mi : -2.0 * mi);
+    }
+    H[(size_t)p * D + q] = h;
+    H[(size_t)q * D + p] = h;
+}
+
+// smp: the sample whose Gram matrix is formed (MC for M; DATA for the Fumili matrix, with Vs = V on
+// the device and H_out = the [2n][2n] device output, use_M = add Hess(Norm)).
+struct GramJob { const Sample *smp; const double *Vs; double *H_out; bool use_M; };
+
 template <typename ST, int NB, int SPLIT, int MODE, int MINB, int ET, int NANG>
-static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs)
+static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs, const GramJob &job)
 {
     constexpr int THREADS = 256;
     using C = NormCfg<ST, NB, SPLIT, MODE, THREADS, ET>;
@@ -284,7 +347,7 @@ static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs)
         PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, THREADS, C::SMEM));
         occ = o < 1 ? 1 : o;
     }
-    const long long N = ctx->mc.n_events;
+    const long long N = job.smp->n_events;
     const long long ntiles = (N + ET - 1) / ET;
     long long grid = (long long)ctx->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
@@ -292,9 +355,17 @@ static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs)
     const int nslots = (int)grid;
     pwa_status s = ensure_scratch(ctx, sizeof(double) * (size_t)nslots * C::NPAIRS * 64);
     if (s != PWA_OK) return s;
-    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(ctx->mc.factored ? nullptr : ctx->mc.amps, N, ctx->n, fargs, ctx->d_scratch);
+    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(job.smp->factored ? nullptr : job.smp->amps, N, ctx->n, fargs, ctx->d_scratch, job.Vs);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
+    if (job.Vs != nullptr) {
+        const int D2 = 4 * ctx->n * ctx->n;
+        k_fumili_finalize<<<(D2 + 255) / 256, 256, 0, ctx->stream>>>(ctx->d_scratch, nslots, ctx->n, NB,
+                                                                       job.use_M ? ctx->d_M : nullptr, job.H_out);
+        ctx->launches++;
+        PWA_CUDA(ctx, cudaGetLastError());
+        return PWA_OK;
+    }
     k_norm_dmma_finalize<<<C::NPAIRS * 4, 256, 0, ctx->stream>>>(ctx->d_scratch, nslots, ctx->n, NB,
                                                                  1.0 / (double)ctx->mc.n_gen, ctx->d_M);
     ctx->launches++;
@@ -303,40 +374,58 @@ static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs)
 }
 
 template <typename ST, int MODE, int NANG>
-static pwa_status dispatch_nd(pwa_ctx *ctx, const FactArgs &fargs)
+static pwa_status dispatch_nd(pwa_ctx *ctx, const FactArgs &fargs, const GramJob &job)
 {
     const int D = 2 * ctx->n;
     //                                   NB SPLIT      MINB ET
-    if (D <= 8)   return launch_nd<ST, 1,  1, MODE, 2, 128, NANG>(ctx, fargs);
-    if (D <= 16)  return launch_nd<ST, 2,  1, MODE, 2, 128, NANG>(ctx, fargs);
-    if (D <= 32)  return launch_nd<ST, 4,  1, MODE, 2, 128, NANG>(ctx, fargs);
-    if (D <= 64)  return launch_nd<ST, 8,  2, MODE, 2, 64, NANG>(ctx, fargs);
-    return launch_nd<ST, 16, 4, MODE, 1, 32, NANG>(ctx, fargs);
+    if (D <= 8)   return launch_nd<ST, 1,  1, MODE, 2, 128, NANG>(ctx, fargs, job);
+    if (D <= 16)  return launch_nd<ST, 2,  1, MODE, 2, 128, NANG>(ctx, fargs, job);
+    if (D <= 32)  return launch_nd<ST, 4,  1, MODE, 2, 128, NANG>(ctx, fargs, job);
+    if (D <= 64)  return launch_nd<ST, 8,  2, MODE, 2, 64, NANG>(ctx, fargs, job);
+    return launch_nd<ST, 16, 4, MODE, 1, 32, NANG>(ctx, fargs, job);
 }
 
-pwa_status launch_norm_dmma(pwa_ctx *ctx, bool *handled)
+static pwa_status run_gram(pwa_ctx *ctx, const GramJob &job, bool *handled)
 {
     *handled = false;
     const int n = ctx->n;
+    const Sample &smp = *job.smp;
     if (n > kMaxFastWaves) return PWA_OK;                      // generic CUDA-core kernel handles it
     FactArgs fargs;
-    const bool fact = ctx->mc.factored;
+    const bool fact = smp.factored;
     if (fact) {
-        pwa_status s = fill_fact_args(ctx, ctx->mc, &fargs);
+        pwa_status s = fill_fact_args(ctx, smp, &fargs);
         if (s != PWA_OK) return s;
     } else {
         memset(&fargs, 0, sizeof(fargs));
     }
     const bool f32 = ctx->storage == PWA_F32;
     const bool pow2 = (n & (n - 1)) == 0 && n >= 4;            // rows are whole 16-byte chunks, D = 2n
-    const bool aligned = ((uintptr_t)ctx->mc.amps & 15u) == 0;
+    const bool aligned = ((uintptr_t)smp.amps & 15u) == 0;
     pwa_status s;
-    if (fact && ctx->mc.n_ang <= 2) s = f32 ? dispatch_nd<float, FILL_FACTORED, 2>(ctx, fargs) : dispatch_nd<double, FILL_FACTORED, 2>(ctx, fargs);
-    else if (fact)            s = f32 ? dispatch_nd<float, FILL_FACTORED, 4>(ctx, fargs) : dispatch_nd<double, FILL_FACTORED, 4>(ctx, fargs);
-    else if (pow2 && aligned) s = f32 ? dispatch_nd<float, FILL_STAGED, 1>(ctx, fargs)   : dispatch_nd<double, FILL_STAGED, 1>(ctx, fargs);
-    else                      s = f32 ? dispatch_nd<float, FILL_ELEMENT, 1>(ctx, fargs)  : dispatch_nd<double, FILL_ELEMENT, 1>(ctx, fargs);
+    if (fact && smp.n_ang <= 2) s = f32 ? dispatch_nd<float, FILL_FACTORED, 2>(ctx, fargs, job) : dispatch_nd<double, FILL_FACTORED, 2>(ctx, fargs, job);
+    else if (fact)            s = f32 ? dispatch_nd<float, FILL_FACTORED, 4>(ctx, fargs, job) : dispatch_nd<double, FILL_FACTORED, 4>(ctx, fargs, job);
+    else if (pow2 && aligned) s = f32 ? dispatch_nd<float, FILL_STAGED, 1>(ctx, fargs, job)   : dispatch_nd<double, FILL_STAGED, 1>(ctx, fargs, job);
+    else                      s = f32 ? dispatch_nd<float, FILL_ELEMENT, 1>(ctx, fargs, job)  : dispatch_nd<double, FILL_ELEMENT, 1>(ctx, fargs, job);
     if (s != PWA_OK) return s;
     *handled = true;
+    return PWA_OK;
+}
+
+pwa_status launch_norm_dmma(pwa_ctx *ctx, bool *handled)
+{
+    GramJob job{&ctx->mc, nullptr, nullptr, false};
+    return run_gram(ctx, job, handled);
+}
+
+// Fumili-style approximate Hessian over the DATA sample (V already in ctx->d_V, H_dev [2n][2n] device).
+pwa_status launch_fumili(pwa_ctx *ctx, double *H_dev, bool with_norm)
+{
+    GramJob job{&ctx->data, ctx->d_V, H_dev, with_norm};
+    bool handled = false;
+    pwa_status s = run_gram(ctx, job, &handled);
+    if (s != PWA_OK) return s;
+    if (!handled) return fail(ctx, PWA_ERR_UNSUPPORTED, "pwa_fumili_hessian needs n <= 64");
     return PWA_OK;
 }
 

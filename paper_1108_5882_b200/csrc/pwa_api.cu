@@ -206,6 +206,7 @@ void pwa_destroy(pwa_ctx *ctx)
     if (ctx->h_V) cudaFreeHost(ctx->h_V);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
+    if (ctx->d_H) cudaFree(ctx->d_H);
     cudaGetLastError();
     delete ctx;
 }
@@ -416,6 +417,27 @@ pwa_status pwa_assemble_host(int32_t n, double L_data, const double *T, const do
     *nll = -(L_data - norm);
     if (parts) { parts[0] = L_data; parts[1] = norm; }
     return PWA_OK;
+}
+
+pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t with_norm)
+{
+    if (!ctx || !V || !H) return PWA_ERR_INVALID_ARG;
+    pwa_status s = check_ready(ctx, with_norm != 0);
+    if (s != PWA_OK) return s;
+    if (ctx->data.factored && !ctx->res_set) return fail(ctx, PWA_ERR_STATE, "pwa_set_resonances not called");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    s = stage_V(ctx, 1, V);
+    if (s != PWA_OK) return s;
+    const size_t n = (size_t)ctx->n, cnt = 4 * n * n;
+    if (ctx->data.n_events == 0) { memset(H, 0, sizeof(double) * cnt); return PWA_OK; }
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
+    // H goes through the tail of the M-partials scratch is NOT safe (the Gram kernel owns it): own buffer
+    if (!ctx->d_H) PWA_CUDA(ctx, cudaMalloc(&ctx->d_H, sizeof(double) * cnt));
+    s = launch_fumili(ctx, ctx->d_H, with_norm != 0);
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaMemcpyAsync(H, ctx->d_H, sizeof(double) * cnt, cudaMemcpyDeviceToHost, ctx->stream));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return finite_all(H, cnt) ? PWA_OK : PWA_WARN_NONFINITE;
 }
 
 pwa_status pwa_assemble_host_eq2(int32_t n, double n_data, double L_data, const double *T, const double *M,

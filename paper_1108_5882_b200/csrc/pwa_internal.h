@@ -63,6 +63,7 @@ struct pwa_ctx {
     double *d_result = nullptr; double *h_result = nullptr;  // [kMaxK][result_stride]
     double *d_V = nullptr; double *h_V = nullptr;            // [kMaxK][n][2]
     double *d_scratch = nullptr; size_t scratch_cap = 0;     // bytes (M partials, batch partials)
+    double *d_H = nullptr;                                    // [2n][2n] Fumili matrix (allocated on first use)
     int last_K = 0;
     // cached TMA descriptor of the DATA sample (data_term_tma.cu); rebuilt when the key changes
     struct { const void *base = nullptr; long long n_events = -1; int box_rows = 0; bool valid = false;
@@ -92,6 +93,7 @@ pwa_status ensure_scratch(pwa_ctx *ctx, size_t bytes);
 pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double *out_dev_terms);
 pwa_status launch_batch(pwa_ctx *ctx, int K);   // V already staged in h_V/d_V
 pwa_status launch_norm_build(pwa_ctx *ctx);
+pwa_status launch_fumili(pwa_ctx *ctx, double *H_dev, bool with_norm);   // norm_dmma.cu (row-scaled Gram over DATA)
 pwa_status prepare_norm_i8(pwa_ctx *ctx);                  // norm_i8.cu: after a constant-resonance MC upload
 pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled);    // norm_i8.cu
 double norm_i8_error_bound(const pwa_ctx *ctx);

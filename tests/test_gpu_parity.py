@@ -401,3 +401,43 @@ def test_eq2_likelihood_mode(pwa, oracle, storage, n, K):
         check_eval(pwa.pwa_nll_grad(c.ctx, Vk[0]), oracle.nll_grad(A, M_o, Vk[0]), tol, N)
         with pytest.raises(pwa.PwaError):
             pwa.pwa_set_option(c.ctx, "likelihood", 2)
+
+
+# ------------------------------------------------------------------ NEXT-2: Fumili-style approximate Hessian
+@pytest.mark.parametrize("storage,n,N", [("f64", 4, 1), ("f64", 4, 3001), ("f64", 5, 777), ("f64", 16, 20_011),
+                                         ("f32", 32, 9001), ("f32", 64, 12_345), ("f64", 64, 4097), ("f32", 3, 130)])
+def test_fumili_hessian_parity(pwa, oracle, storage, n, N):
+    """H = sum_i u_i u_i^T + Hess(Norm) from the row-scaled DMMA Gram kernel vs the oracle; exact
+    symmetry; PSD data part; Euler identity H_data V = 2 grad(L_data) on the GPU result alone."""
+    A, B, V = rand_case(900 + n + N, N, 2001, n, storage)
+    M_o = oracle.norm_matrix(B, 2100)
+    tol = TOL[storage] * (1 if storage == "f32" else 10)       # 1e-11 for fp64: outer products of 1/S amplify |A|/|S|
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2100)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        H = pwa.pwa_fumili_hessian(c.ctx, V)
+        Hd = pwa.pwa_fumili_hessian(c.ctx, V, with_norm=False)
+        H_o, Hd_o = oracle.fumili(A, V, M_o), oracle.fumili(A, V)
+        assert np.array_equal(H, H.T) and np.array_equal(Hd, Hd.T)
+        assert np.abs(Hd - Hd_o).max() <= tol * np.abs(Hd_o).max()
+        assert np.abs(H - H_o).max() <= tol * np.abs(H_o).max()
+        assert np.linalg.eigvalsh(Hd).min() >= -1e-9 * np.trace(Hd)
+        L, T, _ = oracle.data_term(A, V)
+        gL = np.empty(2 * n)
+        gL[0::2], gL[1::2] = 2 * T[:, 0], -2 * T[:, 1]
+        assert np.abs(Hd @ V.reshape(-1) - 2 * gL).max() <= 100 * tol * max(np.abs(gL).max(), np.abs(Hd).max() * 1e-3)
+        assert np.array_equal(H, pwa.pwa_fumili_hessian(c.ctx, V))          # reproducible
+
+
+def test_fumili_factored(pwa, oracle, synth):
+    w = synth.make_workload(3, n_data=30_011, n_mc=20_011, full_amplitudes=False)
+    Mr, Gr = synth.floating_start(w)
+    A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    V = synth.eval_points(w, 1)[0]
+    H_o = oracle.fumili(A, V, oracle.norm_matrix(B, w.n_gen))
+    with _factored_ctx(pwa, w, Mr, Gr) as c:
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        H = pwa.pwa_fumili_hessian(c.ctx, V)
+    assert np.abs(H - H_o).max() <= 1e-11 * np.abs(H_o).max()

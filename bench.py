@@ -263,6 +263,9 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
             flops = 8.0 * n * n * w.n_acc
             out["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": flops / ms_m * 1e-6,
                               "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
+            bound, path = pwa.pwa_norm_error_bound(ctx)
+            out["m_build"]["path"] = "int8 tcgen05 (digit planes, int32 TMEM)" if path == 1 else "fp64 DMMA"
+            out["m_build"]["error_bound_abs"] = bound
         else:
             pwa.pwa_set_norm(ctx, M0)
         Vs = synth.eval_points(w, steps + warmup)
@@ -277,6 +280,13 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
                     "algorithmic_gbs": nbytes / ms * 1e-6, "e2e_ms_per_eval": wall,
                     "e2e_evals_per_s": 1e3 / wall, "upload_s": up_s,
                     "l2_resident": bool(nbytes < 100e6)})
+        # NEXT-2: Fumili-style approximate Hessian (synchronous call: one row-scaled Gram pass over the data)
+        pwa.pwa_fumili_hessian(ctx, Vs[0])
+        t0 = time.perf_counter()
+        for i in range(3):
+            pwa.pwa_fumili_hessian(ctx, Vs[1 + i])
+        ms_f = (time.perf_counter() - t0) / 3 * 1e3
+        out["fumili"] = {"ms_per_call_e2e": ms_f, "gflops_full_gram": 8.0 * n * n * w.n_data / ms_f * 1e-6}
         if w.K > 1:
             Vk = synth.eval_points(w, w.K, stream=synth.S_START)
             ms_b, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
@@ -415,6 +425,9 @@ def run_ours(args):
             ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), 3, 1)
             extra["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": 8.0 * n * n * w.n_acc / ms_m * 1e-6,
                                 "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
+            bound, path = pwa.pwa_norm_error_bound(ctx)
+            extra["m_build"]["path"] = "int8 tcgen05 (digit planes, int32 TMEM)" if path == 1 else "fp64 DMMA"
+            extra["m_build"]["error_bound_abs"] = bound
             M_local = pwa.pwa_build_norm(ctx)
             if ws > 1:
                 M_all, _ = sharded.combine_norm(M_local, w.n_gen, device=dev)
@@ -542,6 +555,7 @@ def side_measurements(torch, pwa, synth, args, extra):
             w4.A_mc = None
             r = bench_constant(torch, pwa, synth, w4, 3, 3, 4)
             extra["cfg4_batch"] = r.get("batch")
+            extra["cfg4_fumili"] = r.get("fumili")
     except Exception as e:   # side measurements must never lose the main line
         extra["error"] = repr(e)
     return extra

@@ -192,6 +192,16 @@ def fumili(A, V, M=None):
     return H
 
 
+def fumili_rows(A, V, p0, p1):
+    """Rows p0:p1 of the data part of the Fumili matrix (other rows zero); for sampled checks at full size."""
+    A, dt = _amp(A)
+    N, n = A.shape[0], A.shape[1]
+    V = _f64(V, (n, 2))
+    H = np.zeros((2 * n, 2 * n))
+    lib().pwa_oracle_fumili_rows(_p(A), C.c_int(dt), C.c_int64(N), C.c_int(n), _p(V), C.c_int(p0), C.c_int(p1), _p(H))
+    return H
+
+
 def nll_grad(A, M, V):
     """-> (nll, grad[n,2], parts[2], n_nonfinite)."""
     A, dt = _amp(A)

@@ -345,29 +345,55 @@ void pwa_oracle_grad_polar(int n, const double *V, const double *grad, double *o
  *     H_data = sum_i u_i u_i^T          (2n x 2n, symmetric, positive semi-definite)
  *     H      = H_data + Hess(Norm),  Hess(Norm) = 2 [[Re M_ab, -Im M_ab], [Im M_ab, Re M_ab]]  (exact: Norm is quadratic)
  * approximates the Hessian of nll = -(L_data - Norm).  H: [2n][2n] row-major; M may be NULL (H_data only). */
+/* rows p0 <= p < p1 of H_data only (others untouched): per-thread compensated partials over events,
+ * merged in thread order, as in the data term.  For sampled checks at full size. */
+void pwa_oracle_fumili_rows(const void *A, int dt, int64_t N, int n, const double *V, int p0, int p1, double *H)
+{
+    const int D = 2 * n, nr = p1 - p0;
+    int nt = n_threads();
+    size_t per = (size_t)nr * D;
+    nsum *part = (nsum *)calloc((size_t)nt * per, sizeof(nsum));
+#pragma omp parallel num_threads(nt)
+    {
+#ifdef _OPENMP
+        int tid = omp_get_thread_num();
+#else
+        int tid = 0;
+#endif
+        nsum *my = part + (size_t)tid * per;
+        double *u = (double *)malloc(sizeof(double) * D);
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < N; ++i) {
+            long double sr = 0.0L, si = 0.0L;
+            for (int a = 0; a < n; ++a) {
+                double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
+                sr += (long double)V[2 * a] * ar - (long double)V[2 * a + 1] * ai;
+                si += (long double)V[2 * a] * ai + (long double)V[2 * a + 1] * ar;
+            }
+            double Sr = (double)sr, Si = (double)si, I = Sr * Sr + Si * Si;
+            for (int a = 0; a < n; ++a) {
+                double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
+                /* t = A / S = A conj(S) / I */
+                double tr = (ar * Sr + ai * Si) / I, ti = (ai * Sr - ar * Si) / I;
+                u[2 * a] = 2.0 * tr;  u[2 * a + 1] = -2.0 * ti;
+            }
+            for (int p = p0; p < p1; ++p)
+                for (int q = 0; q < D; ++q) nadd(&my[(size_t)(p - p0) * D + q], u[p] * u[q]);
+        }
+        free(u);
+    }
+    for (size_t k = 0; k < per; ++k) {
+        nsum tot = {0.0, 0.0};
+        for (int t = 0; t < nt; ++t) nmerge(&tot, &part[(size_t)t * per + k]);
+        H[(size_t)p0 * D + k] = nval(&tot);
+    }
+    free(part);
+}
+
 void pwa_oracle_fumili(const void *A, int dt, int64_t N, int n, const double *V, const double *M, double *H)
 {
     const int D = 2 * n;
-    nsum *acc = (nsum *)calloc((size_t)D * D, sizeof(nsum));
-    double *u = (double *)malloc(sizeof(double) * D);
-    for (int64_t i = 0; i < N; ++i) {
-        long double sr = 0.0L, si = 0.0L;
-        for (int a = 0; a < n; ++a) {
-            double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
-            sr += (long double)V[2 * a] * ar - (long double)V[2 * a + 1] * ai;
-            si += (long double)V[2 * a] * ai + (long double)V[2 * a + 1] * ar;
-        }
-        double Sr = (double)sr, Si = (double)si, I = Sr * Sr + Si * Si;
-        for (int a = 0; a < n; ++a) {
-            double ar = ld_amp(A, dt, (i * n + a) * 2), ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
-            /* t = A / S = A conj(S) / I */
-            double tr = (ar * Sr + ai * Si) / I, ti = (ai * Sr - ar * Si) / I;
-            u[2 * a] = 2.0 * tr;  u[2 * a + 1] = -2.0 * ti;
-        }
-        for (int p = 0; p < D; ++p)
-            for (int q = 0; q < D; ++q) nadd(&acc[p * D + q], u[p] * u[q]);
-    }
-    for (int p = 0; p < D * D; ++p) H[p] = nval(&acc[p]);
+    pwa_oracle_fumili_rows(A, dt, N, n, V, 0, D, H);
     if (M)
         for (int a = 0; a < n; ++a)
             for (int b = 0; b < n; ++b) {
@@ -375,7 +401,6 @@ void pwa_oracle_fumili(const void *A, int dt, int64_t N, int n, const double *V,
                 H[(2 * a) * D + 2 * b] += 2.0 * Mr;          H[(2 * a) * D + 2 * b + 1] += -2.0 * Mi;
                 H[(2 * a + 1) * D + 2 * b] += 2.0 * Mi;      H[(2 * a + 1) * D + 2 * b + 1] += 2.0 * Mr;
             }
-    free(acc); free(u);
 }
 
 int64_t pwa_oracle_nll_grad(const void *A, int dt, int64_t N, int n, const double *M,

@@ -114,6 +114,15 @@ def test_cfg4_full(pwa, oracle, synth):
         # every batched column agrees with the streaming kernel at the same point (property at any size)
         for k in range(0, w.K, 7):
             check_eval((nll[k], g[k], parts[k]), pwa.pwa_nll_grad(c.ctx, Vk[k]), tol, w.n_data)
+        # NEXT-2 at full size: sampled rows of the Fumili matrix against the oracle, Euler identity on the rest
+        Hd = pwa.pwa_fumili_hessian(c.ctx, Vk[3], with_norm=False)
+        assert np.array_equal(Hd, Hd.T)
+        for p0 in (0, 77, 126):
+            ref = oracle.fumili_rows(w.A_data, Vk[3], p0, p0 + 2)
+            assert np.abs(Hd[p0:p0 + 2] - ref[p0:p0 + 2]).max() <= tol * np.abs(Hd).max()
+        gN3 = pwa.pwa_assemble_host(0.0, np.zeros((w.n, 2)), M, Vk[3])[1]
+        gL3 = -(pwa.pwa_nll_grad(c.ctx, Vk[3])[1] - gN3).reshape(-1)            # grad L_data = 2 conj(T)
+        assert np.abs(Hd @ Vk[3].reshape(-1) - 2 * gL3).max() <= 100 * tol * np.abs(gL3).max()
         # P7 (Euler identity) on the GPU result alone: Re(V^H g(L_data)) = 2 N  <=>  sum_a V_a T_a = N
         for k in (5, 40):
             gN = pwa.pwa_assemble_host(0.0, np.zeros((w.n, 2)), M, Vk[k])[1]     # 2 M V

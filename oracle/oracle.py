@@ -110,6 +110,29 @@ def data_term(A, V):
     return L.value, T, int(bad)
 
 
+def data_term_w(A, V, w):
+    """Weighted data term: L = sum_i w_i ln I_i, T_a = sum_i w_i A_ia / S_i -> (L, T[n,2], n_nonfinite)."""
+    A, dt = _amp(A)
+    N, n = A.shape[0], A.shape[1]
+    V, w = _f64(V, (n, 2)), _f64(w, (N,))
+    L = C.c_double(0.0)
+    T = np.zeros((n, 2))
+    lib().pwa_oracle_data_term_w.restype = C.c_int64
+    bad = lib().pwa_oracle_data_term_w(_p(A), C.c_int(dt), C.c_int64(N), C.c_int(n), _p(V), _p(w), C.byref(L), _p(T))
+    return L.value, T, int(bad)
+
+
+def norm_matrix_w(B, n_gen, w):
+    """Weighted normalisation matrix M_ab = (1/N_gen) sum_j w_j conj(B_ja) B_jb."""
+    B, dt = _amp(B)
+    N, n = B.shape[0], B.shape[1]
+    w = _f64(w, (N,))
+    M = np.zeros((n, n, 2))
+    lib().pwa_oracle_norm_block_w(_p(B), C.c_int(dt), C.c_int64(N), C.c_int(n), C.c_int64(int(n_gen)), _p(w),
+                                  C.c_int(0), C.c_int(n), C.c_int(0), C.c_int(n), _p(M))
+    return M
+
+
 def norm_matrix(B, n_gen):
     B, dt = _amp(B)
     N, n = B.shape[0], B.shape[1]

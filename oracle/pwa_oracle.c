@@ -36,7 +36,8 @@
  * derivative vs differences, brute-force pure-Python on tiny inputs; P13 eq. 2 form: scale
  * invariance, finite differences, equality with eq. 3 at Norm = N_data; P14 polar chain rule vs
  * finite differences in (r, phi); P15 Fumili matrix: H_data V = 2 grad(L_data) (Euler), numpy
- * restatement, PSD, Hess(Norm) vs differences of the norm gradient.
+ * restatement, PSD, Hess(Norm) vs differences of the norm gradient; P16 event weights: unit weights,
+ * integer weights = duplicated events, numpy restatement, linearity in w.
  * Parity unpinned by the paper: the choices C2, C3, C4, C5, C9-C13 (definitions, not
  * results), and the resonance-parameter gradient beyond finite differences (P5/P10 style).
  *
@@ -137,8 +138,11 @@ void pwa_oracle_expand_factored(const double *mass, const void *Z, int dtZ, int 
  * S_i = sum_a V_a A_ia (eq. 1);  l_i = ln|S_i|^2 (eq. 3 first term);
  * L = sum_i l_i;  T_a = sum_i A_ia / S_i.   Returns the number of events with I_i == 0
  * or non-finite l_i (C14: IEEE values propagate). */
-int64_t pwa_oracle_data_term(const void *A, int dt, int64_t N, int n, const double *V,
-                             double *L_out, double *T_out /* [n][2] */)
+/* NEXT-3: optional per-event weights w_i (NULL = all 1):
+ * L = sum_i w_i l_i, T_a = sum_i w_i A_ia / S_i (a weighted unbinned likelihood; weights that are
+ * small non-negative integers are exactly event multiplicities). */
+int64_t pwa_oracle_data_term_w(const void *A, int dt, int64_t N, int n, const double *V, const double *w,
+                               double *L_out, double *T_out /* [n][2] */)
 {
     int nt = n_threads();
     nsum *part = (nsum *)calloc((size_t)nt * (size_t)(1 + 2 * n), sizeof(nsum));
@@ -163,14 +167,15 @@ int64_t pwa_oracle_data_term(const void *A, int dt, int64_t N, int n, const doub
             double Sr = (double)sr, Si = (double)si;
             double I = Sr * Sr + Si * Si;
             double l = log(I);
+            const double wi = w ? w[i] : 1.0;
             if (!(I > 0.0) || !isfinite(l)) bad += 1;
-            nadd(&my[0], l);
+            nadd(&my[0], wi * l);
             for (int a = 0; a < n; ++a) {
                 double ar = ld_amp(A, dt, (i * n + a) * 2);
                 double ai = ld_amp(A, dt, (i * n + a) * 2 + 1);
                 /* A / S = A * conj(S) / I */
-                nadd(&my[1 + 2 * a], (ar * Sr + ai * Si) / I);
-                nadd(&my[2 + 2 * a], (ai * Sr - ar * Si) / I);
+                nadd(&my[1 + 2 * a], wi * ((ar * Sr + ai * Si) / I));
+                nadd(&my[2 + 2 * a], wi * ((ai * Sr - ar * Si) / I));
             }
         }
     }
@@ -184,12 +189,20 @@ int64_t pwa_oracle_data_term(const void *A, int dt, int64_t N, int n, const doub
     return bad;
 }
 
+int64_t pwa_oracle_data_term(const void *A, int dt, int64_t N, int n, const double *V,
+                             double *L_out, double *T_out /* [n][2] */)
+{
+    return pwa_oracle_data_term_w(A, dt, N, n, V, NULL, L_out, T_out);
+}
+
 /* ---------- normalisation matrix: step 6 (P:41 inner bracket, C1) ---------------------
  * M_ab = (1/N_gen) sum_j conj(B_ja) B_jb  for ALL (a,b): Hermitian symmetry is NOT used
  * here so that it can be tested. Only entries with a in [a0,a1) and b in [b0,b1) are
  * computed (others left untouched) so single entries can be sampled at full size. */
-void pwa_oracle_norm_block(const void *B, int dt, int64_t N_acc, int n, int64_t N_gen,
-                           int a0, int a1, int b0, int b1, double *M_out /* [n][n][2] */)
+/* Optional per-event MC weights w_j (NULL = all 1), P:37 fn. 2 ("it is also possible to generate
+ * events unevenly ... and then weight them"): M_ab = (1/N_gen) sum_j w_j conj(B_ja) B_jb. */
+void pwa_oracle_norm_block_w(const void *B, int dt, int64_t N_acc, int n, int64_t N_gen, const double *w,
+                             int a0, int a1, int b0, int b1, double *M_out /* [n][n][2] */)
 {
     int nt = n_threads();
     int na = a1 - a0, nb = b1 - b0;
@@ -205,6 +218,7 @@ void pwa_oracle_norm_block(const void *B, int dt, int64_t N_acc, int n, int64_t 
         nsum *my = part + (size_t)tid * per;
 #pragma omp for schedule(static)
         for (int64_t j = 0; j < N_acc; ++j) {
+            const double wj = w ? w[j] : 1.0;
             for (int a = a0; a < a1; ++a) {
                 double ar = ld_amp(B, dt, (j * n + a) * 2);
                 double ai = ld_amp(B, dt, (j * n + a) * 2 + 1);
@@ -213,8 +227,8 @@ void pwa_oracle_norm_block(const void *B, int dt, int64_t N_acc, int n, int64_t 
                     double bi = ld_amp(B, dt, (j * n + b) * 2 + 1);
                     size_t k = ((size_t)(a - a0) * (size_t)nb + (size_t)(b - b0)) * 2;
                     /* conj(a) * b = (ar - i ai)(br + i bi) */
-                    nadd(&my[k],     ar * br + ai * bi);
-                    nadd(&my[k + 1], ar * bi - ai * br);
+                    nadd(&my[k],     wj * (ar * br + ai * bi));
+                    nadd(&my[k + 1], wj * (ar * bi - ai * br));
                 }
             }
         }
@@ -228,6 +242,12 @@ void pwa_oracle_norm_block(const void *B, int dt, int64_t N_acc, int n, int64_t 
                 M_out[((size_t)a * (size_t)n + (size_t)b) * 2 + (size_t)c] = nval(&tot) / (double)N_gen;
             }
     free(part);
+}
+
+void pwa_oracle_norm_block(const void *B, int dt, int64_t N_acc, int n, int64_t N_gen,
+                           int a0, int a1, int b0, int b1, double *M_out /* [n][n][2] */)
+{
+    pwa_oracle_norm_block_w(B, dt, N_acc, n, N_gen, NULL, a0, a1, b0, b1, M_out);
 }
 
 void pwa_oracle_norm_matrix(const void *B, int dt, int64_t N_acc, int n, int64_t N_gen,

@@ -553,3 +553,38 @@ def test_p15_fumili_matrix(oracle):
         lm = oracle.data_term(A[:1], (V.reshape(-1) - e).reshape(n, 2))[0]
         u[p] = (lp - lm) / (2 * h)
     assert np.abs(H1 - np.outer(u, u)).max() <= 1e-6 * np.abs(H1).max()
+
+
+# ---------------------------------------------------------------- P16 per-event weights (NEXT-3)
+def test_p16_event_weights(oracle):
+    """Weighted sums: (a) w = 1 is bit-identical to the unweighted functions; (b) small integer weights
+    = the sample with event i repeated w_i times (exactly the same terms); (c) numpy restatement;
+    (d) linearity in w (w1 + w2), incl. negative weights (side-band subtraction style)."""
+    rng = np.random.default_rng(16)
+    N, n = 600, 4
+    A, V = rand_amps(rng, N, n), rng.normal(size=(n, 2))
+    one = np.ones(N)
+    L0, T0, _ = oracle.data_term(A, V)
+    L1, T1, _ = oracle.data_term_w(A, V, one)
+    assert L0 == L1 and np.array_equal(T0, T1)
+    assert np.array_equal(oracle.norm_matrix(A, N + 3), oracle.norm_matrix_w(A, N + 3, one))
+    k = rng.integers(0, 4, size=N)
+    Arep = np.repeat(A, k, axis=0)
+    Lw, Tw, _ = oracle.data_term_w(A, V, k.astype(float))
+    Lr, Tr, _ = oracle.data_term(Arep, V)
+    assert Lw == pytest.approx(Lr, rel=1e-13) and np.allclose(Tw, Tr, rtol=1e-12, atol=1e-12 * np.abs(Tr).max())
+    Mw, Mr = oracle.norm_matrix_w(A, 777, k.astype(float)), oracle.norm_matrix(Arep, 777)
+    assert np.abs(Mw - Mr).max() <= 1e-13 * np.abs(Mr).max()
+    w = rng.normal(size=N)
+    Ac, Vc = cplx(A), cplx(V)
+    S = Ac @ Vc
+    Lw, Tw, _ = oracle.data_term_w(A, V, w)
+    assert Lw == pytest.approx((w * np.log(np.abs(S) ** 2)).sum(), rel=1e-12)
+    assert np.abs(cplx(Tw) - (w[:, None] * Ac / S[:, None]).sum(0)).max() <= 1e-12 * np.abs(Tw).max()
+    Mw = cplx(oracle.norm_matrix_w(A, 900, w))
+    assert np.abs(Mw - (Ac.conj().T * w) @ Ac / 900).max() <= 1e-13 * np.abs(Mw).max()
+    w2 = rng.normal(size=N)
+    La, Ta, _ = oracle.data_term_w(A, V, w2)
+    Lb, Tb, _ = oracle.data_term_w(A, V, w + w2)
+    assert Lb == pytest.approx(Lw + La, rel=1e-11, abs=1e-11 * (abs(Lw) + abs(La)))
+    assert np.allclose(Tb, Tw + Ta, rtol=1e-11, atol=1e-11 * np.abs(Tb).max())

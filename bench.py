@@ -293,6 +293,12 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
             out["batch"] = {"K": w.K, "ms_per_call": ms_b, "evals_per_s": w.K / ms_b * 1e3,
                             "event_waves_per_s": w.n_data * n * w.K / ms_b * 1e3,
                             "gflops": 16.0 * w.n_data * n * w.K / ms_b * 1e-6}
+            # NEXT-3: the same evaluation with per-event weights (per-lane streaming kernel + 8 B/event weight stream)
+            wts = np.random.default_rng(7).uniform(0.5, 1.5, size=w.n_data)
+            pwa.pwa_set_weights(ctx, pwa.PWA_DATA, wts)
+            ms_w, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i]), steps, warmup)
+            pwa.pwa_set_weights(ctx, pwa.PWA_DATA, None)
+            out["weighted"] = {"ms_per_eval": ms_w, "algorithmic_gbs": (nbytes + 8 * w.n_data) / ms_w * 1e-6}
     finally:
         pwa.pwa_destroy(ctx)
     return out
@@ -556,6 +562,7 @@ def side_measurements(torch, pwa, synth, args, extra):
             r = bench_constant(torch, pwa, synth, w4, 3, 3, 4)
             extra["cfg4_batch"] = r.get("batch")
             extra["cfg4_fumili"] = r.get("fumili")
+            extra["cfg4_weighted"] = r.get("weighted")
     except Exception as e:   # side measurements must never lose the main line
         extra["error"] = repr(e)
     return extra

@@ -86,6 +86,16 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
                                       const void *ang, int32_t n_ang, int64_t n_events,
                                       int64_t n_generated, uint32_t flags);
 
+/* Optional per-event weights.  MC: a sample that was not
+ * generated evenly in phase space is re-weighted (P:37 fn. 2): M_ab = (1/N_gen) sum_j w_j conj(B_ja) B_jb.
+ * DATA (reading: weighted unbinned likelihood, e.g. side-band subtraction with negative weights):
+ * L_data = sum_i w_i ln I_i, T_a = sum_i w_i A_ia / S_i.  w: ANY, [n_events] doubles of the sample
+ * uploaded LAST for `which` (a new upload drops the weights); NULL removes them.  flags as for uploads.
+ * Setting MC weights marks M stale.  Weighted samples use the FP64 paths (per-lane streaming kernel,
+ * DMMA Gram kernel); weights are not supported with factored uploads or n > 64 (PWA_ERR_UNSUPPORTED
+ * at evaluation).                                                                                  */
+pwa_status pwa_set_weights(pwa_ctx *ctx, pwa_sample which, const double *w, uint32_t flags);
+
 /* res_of_wave[a] in [0, n_res), ang_of_wave[a] in [0, n_ang): HOST int32 [n_waves].
  * 1 <= n_res <= 64.  Each (resonance, angular structure) pair may belong to at most one
  * wave.                                                                                   */

@@ -29,7 +29,7 @@ SYMBOLS = [
     "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
-    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian",
+    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
 ]
 
 
@@ -76,6 +76,7 @@ def _load():
         "pwa_assemble_host_eq2": (C.c_int, [i32, C.c_double, C.c_double, vp, vp, vp, dp, vp, vp]),
         "pwa_grad_to_polar": (C.c_int, [i32, vp, vp, vp]),
         "pwa_fumili_hessian": (C.c_int, [vp, vp, vp, i32]),
+        "pwa_set_weights": (C.c_int, [vp, C.c_int, vp, u32]),
         "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
     }
     for name, (res, args) in sig.items():
@@ -156,6 +157,18 @@ def pwa_upload_events_factored(ctx, which, mass, ang, n_ang=None, n_events=None,
     _check(ctx, _lib.pwa_upload_events_factored(ctx, int(which), C.c_void_p(pm), C.c_void_p(pa), int(n_ang),
                                                 int(n_events), int(n_generated), int(flags)))
     return km, ka
+
+
+def pwa_set_weights(ctx, which, w, flags=PWA_COPY):
+    """w: float64 numpy [n_events] / torch CUDA tensor / None (remove).  Returns the keep-alive object for BORROW."""
+    if w is None:
+        _check(ctx, _lib.pwa_set_weights(ctx, int(which), None, int(flags)))
+        return None
+    if isinstance(w, np.ndarray):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+    addr, keep, _ = _ptr_and_keep(w)
+    _check(ctx, _lib.pwa_set_weights(ctx, int(which), C.c_void_p(addr), int(flags)))
+    return keep
 
 
 def pwa_set_wave_map(ctx, n_res, res_of_wave, ang_of_wave):

@@ -11,7 +11,7 @@ pwa_status launch_batch_dmma(pwa_ctx *ctx, int K, bool *handled);   // batch_dmm
 
 pwa_status launch_batch(pwa_ctx *ctx, int K)
 {
-    if (ctx->opt_batch != 99) {
+    if (ctx->opt_batch != 99 && ctx->data.weights == nullptr) {      // weighted samples: K passes of the weighted streaming kernel
         bool handled = false;
         pwa_status s = launch_batch_dmma(ctx, K, &handled);
         if (s != PWA_OK) return s;

@@ -45,7 +45,7 @@ __device__ __forceinline__ void group_transpose_reduce(double (&sr)[E], double (
 
 template <typename ST, int G, int CK, int E, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_data_term(const uint4 *__restrict__ A, long long N, VArg varg, FinishArgs fa)
+k_data_term(const uint4 *__restrict__ A, long long N, VArg varg, FinishArgs fa, const double *__restrict__ wt)
 {
     constexpr int WPC = Chunk<ST>::WPC;
     constexpr int W = CK * WPC;            // waves owned by a lane
@@ -112,7 +112,9 @@ k_data_term(const uint4 *__restrict__ A, long long N, VArg varg, FinishArgs fa)
         const double inv = 1.0 / I;
         double rr = sr[0] * inv, rim = -si[0] * inv;      // r = conj(S) / I
         const bool counted = valid && (j < E);             // each event is owned by G/E lanes
-        if (counted) { L += l; if (!(I > 0.0) || !isfinite(l)) bad += 1.0; }
+        double wv = 1.0;                                   // NEXT-3: optional event weight, L = sum w l, T = sum w A / S
+        if (wt != nullptr && valid) { wv = __ldg(wt + ev0 + my_e); rr *= wv; rim *= wv; }
+        if (counted) { L += wv * l; if (!(I > 0.0) || !isfinite(l)) bad += 1.0; }
         if (!valid) { rr = 0.0; rim = 0.0; }
         // A4: t_ia = A_ia r_i accumulated into the lane's T
 #pragma unroll
@@ -290,7 +292,8 @@ k_data_term_ring(const unsigned char *__restrict__ A, long long N, VArg varg, Fi
 // Generic fallback: any n <= kMaxWaves, thread per event, V from device memory.
 template <typename ST, int THREADS>
 __global__ void __launch_bounds__(THREADS)
-k_data_term_generic(const ST *__restrict__ A, long long N, const double *__restrict__ Vdev, FinishArgs fa)
+k_data_term_generic(const ST *__restrict__ A, long long N, const double *__restrict__ Vdev, FinishArgs fa,
+                    const double *__restrict__ wt)
 {
     constexpr int NWARPS = THREADS / 32;
     extern __shared__ double dyn[];
@@ -319,6 +322,7 @@ k_data_term_generic(const ST *__restrict__ A, long long N, const double *__restr
         const double l = log(I), inv = 1.0 / I;
         double rr = sr * inv, rim = -si * inv, lv = l, bv = (!(I > 0.0) || !isfinite(l)) ? 1.0 : 0.0;
         if (!valid) { rr = 0.0; rim = 0.0; lv = 0.0; bv = 0.0; }
+        else if (wt != nullptr) { const double wv = __ldg(wt + i); rr *= wv; rim *= wv; lv *= wv; }
         lv = warp_sum(lv); bv = warp_sum(bv);
         if (lane == 0) { acc[0] += lv; acc[1] += bv; }
         for (int a = 0; a < n; ++a) {
@@ -356,7 +360,7 @@ static pwa_status launch_fast(pwa_ctx *ctx, const VArg &varg, const FinishArgs &
     pwa_status s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
     if (s != PWA_OK) return s;
     fa.partials = ctx->d_partials;
-    kern<<<(unsigned)grid, THREADS, 0, ctx->stream>>>((const uint4 *)ctx->data.amps, N, varg, fa);
+    kern<<<(unsigned)grid, THREADS, 0, ctx->stream>>>((const uint4 *)ctx->data.amps, N, varg, fa, ctx->data.weights);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;
@@ -406,7 +410,7 @@ static pwa_status launch_generic(pwa_ctx *ctx, const double *Vdev, const FinishA
     pwa_status s = ensure_partials(ctx, (size_t)NC * (size_t)grid);
     if (s != PWA_OK) return s;
     fa.partials = ctx->d_partials;
-    kern<<<(unsigned)grid, THREADS, smem, ctx->stream>>>((const ST *)ctx->data.amps, N, Vdev, fa);
+    kern<<<(unsigned)grid, THREADS, smem, ctx->stream>>>((const ST *)ctx->data.amps, N, Vdev, fa, ctx->data.weights);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;
@@ -428,7 +432,10 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     else               { fa.M = ctx->d_M; fa.out = ctx->d_result + (size_t)k * result_stride(n); }
     fa.n_eq2 = ctx->opt_likelihood == 1 ? (double)ctx->data.n_events : 0.0;
 
-    if (ctx->data.factored) return launch_factored_data_term(ctx, V_host_k, fa);
+    if (ctx->data.factored) {
+        if (ctx->data.weights) return fail(ctx, PWA_ERR_UNSUPPORTED, "event weights are not supported with factored (floating-resonance) uploads");
+        return launch_factored_data_term(ctx, V_host_k, fa);
+    }
 
     const bool f32 = ctx->storage == PWA_F32;
     const bool fast = (n == 4 || n == 8 || n == 16 || n == 32 || n == 64) && ctx->opt_data_term != 99;
@@ -439,6 +446,7 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     VArg varg;
     for (int t = 0; t < 2 * n; ++t) varg.v[t] = V_host_k[t];
     int opt = ctx->opt_data_term;
+    if (ctx->data.weights && opt < 20) opt = 20;        // weighted samples: the per-lane LDG kernel carries the weight stream
     // opt 0-9: TMA-tiled two-phase kernel (data_term_tma.cu; default where it applies);
     // 10-19: bulk-copy ring variants; 20-29: per-lane LDG kernels (first design)
     if (opt < 10) {

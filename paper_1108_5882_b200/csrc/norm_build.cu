@@ -197,6 +197,7 @@ pwa_status launch_norm_build(pwa_ctx *ctx)
         if (s != PWA_OK) return s;
         if (handled) return PWA_OK;
     }
+    if (ctx->mc.weights) return fail(ctx, PWA_ERR_UNSUPPORTED, "MC event weights need n <= 64 (FP64 DMMA path)");
     return launch_norm_generic(ctx);
 }
 

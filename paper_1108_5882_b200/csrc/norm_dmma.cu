@@ -60,6 +60,26 @@ __device__ __forceinline__ void quad_mma(const double *__restrict__ tq, int DP, 
         }
 }
 
+// Weighted quad (NEXT-3): the event weight w_e sits in the first padding column of the tile row
+// (tile[e][D]); the A-operand fragment is scaled by it, sum_e w_e X[e][p] X[e][q].
+template <int NB, int SPLIT, int S, int PPW>
+__device__ __forceinline__ void quad_mma_w(const double *__restrict__ tq, int DP, int lane, double (&acc)[PPW][2])
+{
+    double f[NB], fw[NB];
+    const double *src = tq + (lane & 3) * DP + (lane >> 2);
+    const double w = tq[(lane & 3) * DP + NB * 8];
+#pragma unroll
+    for (int cb = 0; cb < NB; ++cb) { f[cb] = src[cb * 8]; fw[cb] = f[cb] * w; }
+    int p = 0;
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+#pragma unroll
+        for (int j = i; j < NB; ++j) {
+            if (p % SPLIT == S) dmma_884(acc[p / SPLIT][0], acc[p / SPLIT][1], fw[i], f[j]);
+            ++p;
+        }
+}
+
 template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET>
 struct NormCfg {
     static constexpr int D = NB * 8, DP = D + 4, W = THREADS / 32, NG = W / SPLIT, QPT = ET / 4;
@@ -72,7 +92,8 @@ struct NormCfg {
 
 template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S, int NANG>
 __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long N, int n, const FactArgs &f,
-                                          double *__restrict__ scratch, double *smem, const double *__restrict__ Vs)
+                                          double *__restrict__ scratch, double *smem, const double *__restrict__ Vs,
+                                          const double *__restrict__ Wt)
 {
     using C = NormCfg<ST, NB, SPLIT, MODE, THREADS, ET>;
     constexpr int D = C::D, DP = C::DP, NG = C::NG, QPT = C::QPT, PPW = C::PPW, NPAIRS = C::NPAIRS;
@@ -178,8 +199,20 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
         }
     };
     auto compute = [&](const double *src) {
+        if (Wt != nullptr) {
 #pragma unroll 1
-        for (int q = group; q < QPT; q += NG) quad_mma<NB, SPLIT, S, PPW>(src + q * 4 * DP, DP, lane, acc);
+            for (int q = group; q < QPT; q += NG) quad_mma_w<NB, SPLIT, S, PPW>(src + q * 4 * DP, DP, lane, acc);
+        } else {
+#pragma unroll 1
+            for (int q = group; q < QPT; q += NG) quad_mma<NB, SPLIT, S, PPW>(src + q * 4 * DP, DP, lane, acc);
+        }
+    };
+    auto fill_w = [&](double *dst, long long t) {             // event weights -> padding column D of the tile
+        if (Wt == nullptr) return;
+        for (int e = tid; e < ET; e += THREADS) {
+            const long long ev = t * ET + e;
+            dst[e * DP + D] = ev < N ? __ldg(Wt + ev) : 0.0;
+        }
     };
 
     if (MODE == FILL_FACTORED) {                              // padded / unmapped columns stay zero
@@ -192,6 +225,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
         if constexpr (MODE == FILL_STAGED) { load_tile(t); store_tile(buf[0]); }
         else if constexpr (MODE == FILL_FACTORED) { fact_load(t); fact_store(buf[0]); }
         else fill_tile(buf[0], t);
+        fill_w(buf[0], t);
     }
     __syncthreads();
     for (; t < ntiles; t += gridDim.x) {
@@ -209,6 +243,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
             compute(buf[cur]);
             if (nxt < ntiles) fill_tile(buf[cur ^ 1], nxt);
         }
+        if (nxt < ntiles) fill_w(buf[cur ^ 1], nxt);
         __syncthreads();
         cur ^= 1;
     }
@@ -237,16 +272,16 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
 template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET, int NANG>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_norm_dmma(const void *__restrict__ Bv, long long N, int n, FactArgs f, double *__restrict__ scratch,
-            const double *__restrict__ Vs)
+            const double *__restrict__ Vs, const double *__restrict__ Wt)
 {
     extern __shared__ double nd_smem[];
     const int S = (threadIdx.x >> 5) % SPLIT;
-    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs); return; }
+    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); return; }
     switch (S) {        // warp-uniform: each sub-id owns a compile-time list of block pairs
-    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
-    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
-    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
-    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs); break;
+    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
     }
 }
 
@@ -355,7 +390,7 @@ static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs, const GramJob &
     const int nslots = (int)grid;
     pwa_status s = ensure_scratch(ctx, sizeof(double) * (size_t)nslots * C::NPAIRS * 64);
     if (s != PWA_OK) return s;
-    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(job.smp->factored ? nullptr : job.smp->amps, N, ctx->n, fargs, ctx->d_scratch, job.Vs);
+    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(job.smp->factored ? nullptr : job.smp->amps, N, ctx->n, fargs, ctx->d_scratch, job.Vs, job.smp->weights);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     if (job.Vs != nullptr) {

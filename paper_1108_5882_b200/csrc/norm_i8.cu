@@ -397,7 +397,7 @@ static PFN_cuTensorMapEncodeTiled_v12000 i8_get_encode()
 static bool i8_shape_ok(const pwa_ctx *ctx)
 {
     const int D = 2 * ctx->n;
-    return ctx->storage == PWA_F32 && !ctx->mc.factored && (D == 32 || D == 64 || D == 128) &&
+    return ctx->storage == PWA_F32 && !ctx->mc.factored && ctx->mc.weights == nullptr && (D == 32 || D == 64 || D == 128) &&
            ctx->mc.n_events > 0 && ((uintptr_t)ctx->mc.amps & 15u) == 0;
 }
 

@@ -57,6 +57,7 @@ static void free_sample(Sample &s)
 {
     if (s.amps_owned && s.amps) cudaFree(s.amps);
     if (s.fact_owned) { if (s.mass) cudaFree(s.mass); if (s.ang) cudaFree(s.ang); }
+    if (s.weights_owned && s.weights) cudaFree(s.weights);
     s = Sample();
 }
 
@@ -260,6 +261,26 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
     return PWA_OK;
 }
 
+pwa_status pwa_set_weights(pwa_ctx *ctx, pwa_sample which, const double *w, uint32_t flags)
+{
+    if (!ctx) return PWA_ERR_INVALID_ARG;
+    if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
+    if (flags > PWA_BORROW) return fail(ctx, PWA_ERR_INVALID_ARG, "bad flags");
+    Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
+    if (smp.n_events < 0) return fail(ctx, PWA_ERR_STATE, "upload the sample before its weights");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    void *buf = nullptr; bool owned = false;
+    if (w != nullptr && smp.n_events > 0) {
+        pwa_status s = take_buffer(ctx, w, (size_t)smp.n_events * sizeof(double), flags, &buf, &owned);
+        if (s != PWA_OK) return s;
+    }
+    if (smp.weights_owned && smp.weights) cudaFree(smp.weights);
+    smp.weights = (double *)buf; smp.weights_owned = owned;
+    if (which == PWA_MC) ctx->M_valid = false;
+    return PWA_OK;
+}
+
 pwa_status pwa_set_wave_map(pwa_ctx *ctx, int32_t n_res, const int32_t *res_of_wave, const int32_t *ang_of_wave)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
@@ -425,6 +446,7 @@ pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t 
     pwa_status s = check_ready(ctx, with_norm != 0);
     if (s != PWA_OK) return s;
     if (ctx->data.factored && !ctx->res_set) return fail(ctx, PWA_ERR_STATE, "pwa_set_resonances not called");
+    if (ctx->data.weights) return fail(ctx, PWA_ERR_UNSUPPORTED, "pwa_fumili_hessian does not take event weights");
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
     s = stage_V(ctx, 1, V);
     if (s != PWA_OK) return s;

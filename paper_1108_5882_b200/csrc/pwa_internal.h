@@ -28,6 +28,7 @@ struct Sample {
     // factored form
     double *mass = nullptr; void *ang = nullptr; bool fact_owned = false; int n_ang = 0;
     bool factored = false;
+    double *weights = nullptr; bool weights_owned = false;   // optional per-event weights (NEXT-3), [n_events]
     int64_t n_events = -1;  // -1 = not uploaded
     int64_t n_gen = 0;
 };

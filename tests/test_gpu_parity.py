@@ -441,3 +441,59 @@ def test_fumili_factored(pwa, oracle, synth):
         pwa.pwa_build_norm(c.ctx, want_M=False)
         H = pwa.pwa_fumili_hessian(c.ctx, V)
     assert np.abs(H - H_o).max() <= 1e-11 * np.abs(H_o).max()
+
+
+# ------------------------------------------------------------------ NEXT-3: per-event weights
+@pytest.mark.parametrize("storage,n", [("f64", 4), ("f64", 16), ("f32", 32), ("f32", 64), ("f64", 64), ("f64", 5), ("f32", 3)])
+def test_event_weights_parity(pwa, oracle, storage, n):
+    """Weighted data term (per-lane streaming kernel / generic kernel) and weighted M (DMMA Gram kernel,
+    weight in the tile's padding column) against the weighted oracle, incl. negative weights; batched
+    call; removing the weights restores the unweighted result bit for bit."""
+    N, Nacc, K = 6007, 4099, 3
+    A, B, _ = rand_case(300 + n, N, Nacc, n, storage)
+    rng = np.random.default_rng(n)
+    wd, wm = rng.normal(loc=0.8, scale=0.6, size=N), rng.uniform(0.2, 2.0, size=Nacc)
+    Vk = rng.normal(size=(K, n, 2))
+    tol = TOL[storage]
+    M_o = oracle.norm_matrix_w(B, Nacc + 9, wm)
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=Nacc + 9)
+        M_plain = pwa.pwa_build_norm(c.ctx)
+        plain = pwa.pwa_nll_grad(c.ctx, Vk[0])
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, wd)
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_MC, wm)
+        with pytest.raises(pwa.PwaError) as e:                       # MC weights make M stale
+            pwa.pwa_nll_grad(c.ctx, Vk[0])
+        assert e.value.status == pwa.PWA_ERR_STATE
+        M = pwa.pwa_build_norm(c.ctx)
+        check_M(M, M_o, 1e-12 if storage == "f64" else tol)
+        assert pwa.pwa_norm_error_bound(c.ctx)[1] == 0
+        nllk, gk, partsk = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        for k in range(K):
+            L, T, _ = oracle.data_term_w(A, Vk[k], wd)
+            ref = oracle.assemble(L, T, M_o, Vk[k])
+            scale = np.abs(wd).sum() / N                               # sum |w_i l_i| scale for the tolerance
+            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol * max(1.0, scale) * 4, N)
+            check_eval((nllk[k], gk[k], partsk[k]), ref, tol * max(1.0, scale) * 4, N)
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, None)
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_MC, None)
+        assert np.array_equal(pwa.pwa_build_norm(c.ctx), M_plain)
+        again = pwa.pwa_nll_grad(c.ctx, Vk[0])
+        assert again[0] == plain[0] and np.array_equal(again[1], plain[1])
+
+
+def test_event_weights_integer_multiplicity(pwa, oracle):
+    """Weights that are small integers = the sample with events repeated (property, no oracle needed)."""
+    n, N = 16, 3001
+    A, B, V = rand_case(5, N, 2000, n, "f64")
+    k = np.random.default_rng(2).integers(0, 4, size=N)
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2000)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, k.astype(float))
+        a = pwa.pwa_nll_grad(c.ctx, V)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.repeat(A, k, axis=0))     # a new upload drops the weights
+        b = pwa.pwa_nll_grad(c.ctx, V)
+    check_eval(a, b, 1e-12, N)

@@ -129,7 +129,8 @@ pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M);
 /* V: HOST [n][2] doubles.  Outputs (HOST): *nll = -(L_data - V^H M V);
  * grad[n][2] = (d nll / d Re V_a, d nll / d Im V_a);  parts (may be NULL): [0] = L_data,
  * [1] = Norm.  One pass over the data amplitudes in HBM; synchronous (returns after the
- * results are in host memory).  PWA_ERR_STATE if DATA is missing or M is missing / stale.
+ * results are in host memory: the kernel's finishing block writes them into pinned host memory and
+ * raises a flag the call polls, so no device-to-host copy is enqueued).  PWA_ERR_STATE if DATA is missing or M is missing / stale.
  * PWA_WARN_NONFINITE if some I_i was 0 or not finite (IEEE values are still written).     */
 pwa_status pwa_nll_grad(pwa_ctx *ctx, const double *V, double *nll, double *grad,
                         double *parts);

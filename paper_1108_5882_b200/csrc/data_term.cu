@@ -429,7 +429,8 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     fa.ticket = ctx->d_ticket;
     fa.n = n;
     if (out_dev_terms) { fa.M = nullptr; fa.out = out_dev_terms; }
-    else               { fa.M = ctx->d_M; fa.out = ctx->d_result + (size_t)k * result_stride(n); }
+    else               { fa.M = ctx->d_M; fa.out = ctx->dev_result + (size_t)k * result_stride(n);
+                         fa.done_flag = ctx->dev_flags + k; fa.seq = ctx->seq; }
     fa.n_eq2 = ctx->opt_likelihood == 1 ? (double)ctx->data.n_events : 0.0;
 
     if (ctx->data.factored) {

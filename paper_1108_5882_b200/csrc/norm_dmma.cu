@@ -90,7 +90,7 @@ struct NormCfg {
     static constexpr size_t SMEM = sizeof(double) * (2 * ET * DP > NPAIRS * 64 ? 2 * ET * DP : NPAIRS * 64);   // tiles, then the CTA partial
 };
 
-template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S, int NANG>
+template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int ET, int S, int NANG, bool EXTRA>
 __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long N, int n, const FactArgs &f,
                                           double *__restrict__ scratch, double *smem, const double *__restrict__ Vs,
                                           const double *__restrict__ Wt)
@@ -199,7 +199,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
         }
     };
     auto compute = [&](const double *src) {
-        if (Wt != nullptr) {
+        if (EXTRA && Wt != nullptr) {
 #pragma unroll 1
             for (int q = group; q < QPT; q += NG) quad_mma_w<NB, SPLIT, S, PPW>(src + q * 4 * DP, DP, lane, acc);
         } else {
@@ -208,7 +208,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
         }
     };
     auto fill_w = [&](double *dst, long long t) {             // event weights -> padding column D of the tile
-        if (Wt == nullptr) return;
+        if (!EXTRA || Wt == nullptr) return;
         for (int e = tid; e < ET; e += THREADS) {
             const long long ev = t * ET + e;
             dst[e * DP + D] = ev < N ? __ldg(Wt + ev) : 0.0;
@@ -230,7 +230,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
     __syncthreads();
     for (; t < ntiles; t += gridDim.x) {
         const long long nxt = t + gridDim.x;
-        if (Vs != nullptr) { scale_tile(buf[cur], t); __syncthreads(); }
+        if (EXTRA && Vs != nullptr) { scale_tile(buf[cur], t); __syncthreads(); }
         if constexpr (MODE == FILL_STAGED) {
             if (nxt < ntiles) load_tile(nxt);
             compute(buf[cur]);
@@ -269,19 +269,21 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
     for (int idx = tid; idx < NPAIRS * 64; idx += THREADS) slot[idx] = red[idx];
 }
 
-template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET, int NANG>
+// EXTRA = true adds the row-scaling (Fumili, Vs) and event-weight (Wt) passes; the plain M build
+// (EXTRA = false) compiles to the same code as before they existed.
+template <typename ST, int NB, int SPLIT, int MODE, int THREADS, int MINB, int ET, int NANG, bool EXTRA>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_norm_dmma(const void *__restrict__ Bv, long long N, int n, FactArgs f, double *__restrict__ scratch,
             const double *__restrict__ Vs, const double *__restrict__ Wt)
 {
     extern __shared__ double nd_smem[];
     const int S = (threadIdx.x >> 5) % SPLIT;
-    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); return; }
+    if (SPLIT == 1) { norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG, EXTRA>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); return; }
     switch (S) {        // warp-uniform: each sub-id owns a compile-time list of block pairs
-    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
-    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
-    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
-    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    case 0: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, 0, NANG, EXTRA>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    case 1: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 1 ? 1 : 0), NANG, EXTRA>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    case 2: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 2 ? 2 : 0), NANG, EXTRA>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
+    default: norm_body<ST, NB, SPLIT, MODE, THREADS, ET, (SPLIT > 3 ? 3 : 0), NANG, EXTRA>(Bv, N, n, f, scratch, nd_smem, Vs, Wt); break;
     }
 }
 
@@ -373,9 +375,11 @@ static pwa_status launch_nd(pwa_ctx *ctx, const FactArgs &fargs, const GramJob &
 {
     constexpr int THREADS = 256;
     using C = NormCfg<ST, NB, SPLIT, MODE, THREADS, ET>;
-    auto kern = k_norm_dmma<ST, NB, SPLIT, MODE, THREADS, MINB, ET, NANG>;
-    static int s_occ[64] = {0};                                 // per instantiation and device
-    int &occ = s_occ[ctx->device & 63];
+    const bool extra = job.Vs != nullptr || job.smp->weights != nullptr;
+    auto kern = extra ? k_norm_dmma<ST, NB, SPLIT, MODE, THREADS, MINB, ET, NANG, true>
+                      : k_norm_dmma<ST, NB, SPLIT, MODE, THREADS, MINB, ET, NANG, false>;
+    static int s_occ2[2][64] = {{0}};                           // per instantiation and device
+    int &occ = s_occ2[extra ? 1 : 0][ctx->device & 63];
     if (occ == 0) {
         PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
         int o = 0;

@@ -112,6 +112,32 @@ static pwa_status unpack_results(pwa_ctx *ctx, int K, double *nll, double *grad,
     return nonfinite ? PWA_WARN_NONFINITE : PWA_OK;
 }
 
+// Waits until the K result records of the most recent enqueue are complete in pinned host memory:
+// polls the per-record flags the finishing blocks set (a few microseconds sooner than a stream
+// synchronisation: the per-iteration synthesis is latency-bound); every so often it asks the
+// stream, so a failed launch is reported instead of spinning forever.
+static pwa_status wait_results(pwa_ctx *ctx, int K)
+{
+    volatile unsigned long long *flags = ctx->h_flags;
+    const unsigned long long seq = ctx->seq;
+    int k = 0;
+    for (unsigned spins = 0;; ++spins) {
+        while (k < K && flags[k] == seq) ++k;
+        if (k == K) break;
+        if ((spins & 1023u) == 1023u) {
+            cudaError_t e = cudaStreamQuery(ctx->stream);
+            if (e == cudaSuccess) {              // all work done: the flags are visible by now (or a kernel did not run)
+                while (k < K && flags[k] == seq) ++k;
+                if (k == K) break;
+                return fail(ctx, PWA_ERR_CUDA, "evaluation finished without publishing its results");
+            }
+            if (e != cudaErrorNotReady) return cuda_fail(ctx, e, "waiting for results");
+        }
+    }
+    __sync_synchronize();
+    return PWA_OK;
+}
+
 static pwa_status stage_V(pwa_ctx *ctx, int K, const double *V)
 {
     const size_t cnt = (size_t)K * 2 * ctx->n;
@@ -128,6 +154,7 @@ static pwa_status enqueue_evals(pwa_ctx *ctx, int K, bool batched)
     if (need_dV)
         PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * (size_t)K * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
     pwa_status s = PWA_OK;
+    ++ctx->seq;                                  // the finishing blocks publish this id in h_flags[k]
     if (batched) {
         s = launch_batch(ctx, K);
     } else {
@@ -135,9 +162,7 @@ static pwa_status enqueue_evals(pwa_ctx *ctx, int K, bool batched)
             s = launch_data_term(ctx, ctx->h_V + (size_t)k * 2 * n, k, nullptr);
     }
     if (s != PWA_OK) return s;
-    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->h_result, ctx->d_result, sizeof(double) * (size_t)K * result_stride(n),
-                                  cudaMemcpyDeviceToHost, ctx->stream));
-    ctx->last_K = K;
+    ctx->last_K = K;                             // results arrive in h_result by the kernels' own stores (no D2H copy)
     return PWA_OK;
 }
 
@@ -183,7 +208,11 @@ pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_ticket, 4 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_ticket, 0, 4 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_result, sizeof(double) * kMaxK * result_stride(n_waves));
-    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_result, sizeof(double) * kMaxK * result_stride(n_waves));
+    if (e == cudaSuccess) e = cudaHostAlloc(&ctx->h_result, sizeof(double) * kMaxK * result_stride(n_waves), cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->dev_result, ctx->h_result, 0);
+    if (e == cudaSuccess) e = cudaHostAlloc(&ctx->h_flags, sizeof(unsigned long long) * kMaxK, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->dev_flags, ctx->h_flags, 0);
+    if (e == cudaSuccess) memset(ctx->h_flags, 0, sizeof(unsigned long long) * kMaxK);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_V, sizeof(double) * kMaxK * 2 * n);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_V, sizeof(double) * kMaxK * 2 * n);
     if (e != cudaSuccess) { cudaGetLastError(); pwa_destroy(ctx); return e == cudaErrorMemoryAllocation ? PWA_ERR_OOM : PWA_ERR_CUDA; }
@@ -203,6 +232,7 @@ void pwa_destroy(pwa_ctx *ctx)
     if (ctx->d_ticket) cudaFree(ctx->d_ticket);
     if (ctx->d_result) cudaFree(ctx->d_result);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
+    if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
     if (ctx->d_V) cudaFree(ctx->d_V);
     if (ctx->h_V) cudaFreeHost(ctx->h_V);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
@@ -384,7 +414,8 @@ pwa_status pwa_fetch(pwa_ctx *ctx, int32_t K, double *nll, double *grad, double 
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
     if (K < 1 || K != ctx->last_K) return fail(ctx, PWA_ERR_STATE, "pwa_fetch: K does not match the last enqueue");
-    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    pwa_status s = wait_results(ctx, K);
+    if (s != PWA_OK) return s;
     return unpack_results(ctx, K, nll, grad, parts);
 }
 

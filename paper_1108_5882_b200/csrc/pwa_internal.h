@@ -61,7 +61,12 @@ struct pwa_ctx {
     // scratch
     double *d_partials = nullptr; size_t partials_cap = 0;   // doubles
     unsigned *d_ticket = nullptr;
-    double *d_result = nullptr; double *h_result = nullptr;  // [kMaxK][result_stride]
+    // result records [kMaxK][result_stride] live in device-mapped pinned HOST memory: the finishing block
+    // writes them there and sets h_flags[k] = seq (no D2H copy, the host polls the flag)
+    double *h_result = nullptr, *dev_result = nullptr;
+    double *d_result = nullptr;                               // device scratch records (res_grad, microbench)
+    unsigned long long *h_flags = nullptr, *dev_flags = nullptr;   // [kMaxK]
+    unsigned long long seq = 0;                               // id of the most recent enqueue
     double *d_V = nullptr; double *h_V = nullptr;            // [kMaxK][n][2]
     double *d_scratch = nullptr; size_t scratch_cap = 0;     // bytes (M partials, batch partials)
     double *d_H = nullptr;                                    // [2n][2n] Fumili matrix (allocated on first use)

@@ -19,6 +19,10 @@ struct FinishArgs {
     double *out;           // result record (M != nullptr) or [NC] components (M == nullptr)
     int n;
     double n_eq2 = 0.0;    // 0: eq. 3 extended form; > 0: eq. 2 normalised form with N_data = n_eq2
+    // result delivery without a copy: `out` may be device-mapped pinned HOST memory; after the record is
+    // written (system-scope fence) done_flag[0] = seq tells the polling host thread it is complete
+    unsigned long long *done_flag = nullptr;
+    unsigned long long seq = 0;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m)
@@ -40,7 +44,8 @@ __device__ __forceinline__ double warp_sum(double x)
 // n_eq2 = 0: nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V                      (eq. 3)
 // n_eq2 = N_data > 0: nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2)
 __device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
-                                            double *out, int n, double n_eq2 = 0.0)
+                                            double *out, int n, double n_eq2 = 0.0,
+                                            unsigned long long *done_flag = nullptr, unsigned long long seq = 0)
 {
     const int NC = 2 + 2 * n;
     const int tid = threadIdx.x, nthreads = blockDim.x;
@@ -88,6 +93,11 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
             out[1] = s_tot[0];
             out[2] = acc;
             out[3] = s_tot[1];
+        }
+        if (done_flag != nullptr) {
+            __threadfence_system();                 // every writing lane: record visible to the host before the flag
+            __syncwarp();
+            if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(done_flag) = seq;
         }
     }
 }
@@ -153,7 +163,7 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
     }
     __syncthreads();
 
-    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.n_eq2);
+    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.n_eq2, fa.done_flag, fa.seq);
     if (tid == 0) *fa.ticket = 0u;   // re-arm for the next launch on this stream
 }
 

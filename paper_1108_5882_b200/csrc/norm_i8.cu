@@ -52,13 +52,13 @@ constexpr int STG_BYTES = TE * ROWB;         // 32 KB fp32 tile
 constexpr int PLANE = TE * 128;              // 8 KB: one int8 digit plane of a tile
 constexpr int SL_BYTES = 4 * PLANE;          // 32 KB: four digit planes
 constexpr int NSTG = 3;                      // fp32 tile ring
-constexpr int NSL = 2;                       // digit-plane ring
+constexpr int NSL = 3;                       // digit-plane ring
 constexpr int FT = 512;                      // tiles between two TMEM flushes (32768 events)
 constexpr int NCW = 8;                       // converter / epilogue warps
 constexpr int THREADS = (NCW + 2) * 32;
 constexpr size_t SMEM = 1024 + (size_t)NSTG * STG_BYTES + (size_t)NSL * SL_BYTES;
 
-struct Scales { float s[128]; int dbg; };    // 2^s_p per real column of the 128-wide view; dbg: experiment switches (0 in production)
+struct Scales { float s[128]; int dbg; int one; };    // 2^s_p per real column of the 128-wide view; dbg: experiment switches (0 in production); one = 1 (a runtime 1 keeps the digit-offset add on the IMAD pipe)
 
 // ---- PTX wrappers -----------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
@@ -196,6 +196,7 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
         }
     } else {
         // ===== converters / epilogue =====
+        const int one = sc.one;
         float scl[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) scl[i] = sc.s[4 * lane + i];
@@ -224,10 +225,10 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                     asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 3 * PLANE), "r"(raw[r].w) : "memory");
                     continue;
                 }
-                const uint32_t w0 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) + 0x00808080u) ^ 0x00808080u;
-                const uint32_t w1 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) + 0x00808080u) ^ 0x00808080u;
-                const uint32_t w2 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) + 0x00808080u) ^ 0x00808080u;
-                const uint32_t w3 = ((uint32_t)__float2int_rn(__uint_as_float(raw[r].w) * scl[3]) + 0x00808080u) ^ 0x00808080u;
+                const uint32_t w0 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) * one + 0x00808080) ^ 0x00808080u;
+                const uint32_t w1 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) * one + 0x00808080) ^ 0x00808080u;
+                const uint32_t w2 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) * one + 0x00808080) ^ 0x00808080u;
+                const uint32_t w3 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].w) * scl[3]) * one + 0x00808080) ^ 0x00808080u;
                 // exact t = 2 diagonal: d0 d2 + d1 d1 + d2 d0 per element (<= 3 * 2^14, 4096 rows per warp and flush)
                 dg[0] = __dp4a((int)w0, (int)__byte_perm(w0, 0u, 0x4012), dg[0]);
                 dg[1] = __dp4a((int)w1, (int)__byte_perm(w1, 0u, 0x4012), dg[1]);
@@ -482,6 +483,7 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     i8::Exps ex;
     memcpy(sc.s, ctx->i8q.scale, sizeof(sc.s));
     sc.dbg = ctx->opt_norm >= 16 ? (ctx->opt_norm >> 4) : 0;
+    sc.one = 1;
     memcpy(ex.e, ctx->i8q.exp, sizeof(ex.e));
     i8::k_norm_i8<<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);
     ctx->launches++;

@@ -1,0 +1,677 @@
+// batch_i8.cu — step A8 on the 5th-generation tensor cores (SURVEY NEXT-1 for A8):
+// K starting points V_k evaluated in ONE pass over an fp32-STORED data sample with n = 64 waves
+// ("fits are usually repeated with various sets of starting parameters"; single-
+// precision amplitudes, double-precision sums), both chained GEMMs as error-free int8 contractions
+// (tcgen05.mma.kind::i8, int32 accumulators in TMEM).  Per tile of 128 events, X = the interleaved
+// (re, im) amplitude rows viewed as a real [128 x 128] matrix (column c = 2a + part):
+//
+//   GEMM1   S = X W      W[2a][2k] = Re V, W[2a+1][2k] = -Im V, W[2a][2k+1] = Im V, W[2a+1][2k+1] = Re V
+//                        -> S[i][2k] = Re S_ik, S[i][2k+1] = Im S_ik                    (eq. 1)
+//   epilogue l_k += ln|S_ik|^2 ;  R_ik = 1 / S_ik = conj(S_ik)/|S_ik|^2              (eq. 3 first term)
+//   GEMM2   Q = X^T Rm   Rm[i][2k] = Re R, Rm[i][2k+1] = Im R
+//                        -> Re T_ak = Q[2a][2k] - Q[2a+1][2k+1],  Im T_ak = Q[2a][2k+1] + Q[2a+1][2k]
+//
+// Fixed point.  x_ic = rint(X_ic 2^s_c) is a 32-bit integer (s_c from the column maximum of the
+// sample, found once per upload: i8_column_scales), split into four balanced int8 digits
+// x = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 ("Ozaki" slicing, as norm_i8.cu).  The digit planes of a tile are
+// written ONCE to shared memory, rows = events, 128 bytes = the 128 real columns, 128-byte swizzle:
+// read K-major they are the A operand of GEMM1 (M = events, K = columns), read MN-major they are the
+// A operand of GEMM2 (M = columns, K = events) — the same bytes serve both GEMMs.
+//   * W' = W 2^-s_c (the column scale moves to the other operand; exact) is quantised per starting
+//     point with w = rint(W' 2^e_k), 32 bits below max_c |W'_ck|, four digit planes (k_bi8_prep).
+//     GEMM1 forms the digit-pair products of orders t = u + v = 3..6 (10 of 16 pairs, as 4 N = 256 and
+//     2 N = 128 MMAs per 32-column K step); z = sum_t 2^(8(t-3)) acc_t is an exact integer and
+//     S_ik = z 2^(24 - e_k) up to |dS| <~ 2^-30 sum_c |X_ic| max_c|W'_ck| (quantisation of both operands
+//     + the dropped orders t <= 2).
+//   * ln|S|^2 = ln(zr^2 + zi^2) + 2 (24 - e_k) ln 2 in fp64 (the offset is added once per column at
+//     the end).  Rh = conj(z)/|z|^2 is formed in fp32 (R only needs the relative accuracy of the
+//     fp32-stored amplitudes it multiplies), quantised PER TILE AND COLUMN to 23 bits below the
+//     tile's max_i |Rh_ik| (three digit planes), and GEMM2 forms orders t = 2..5 (9 of 12 pairs).
+//     The tile's integer block is read back from TMEM, converted and added to fp64 accumulators in
+//     registers (one per (column c, real start column) and thread: 128 x 128 per CTA), so no int32
+//     ever sees more than one tile.
+// Error: see DESIGN.md 6.7; the parity bar for fp32 storage is 1e-6 (BASELINE.json north_star).
+//
+// Warp roles (one persistent CTA per SM, contiguous tile range per CTA): 16 converter / epilogue
+// warps (warp w: TMEM lane quarter w % 4, 32-column group w / 4), one TMA producer warp (ring of
+// 32-event fp32 stages), one MMA issuer warp (owns TMEM; one lane issues tcgen05.mma / commit).
+// Per-CTA partials go to fixed slots; k_bi8_finalize sums them in slot order and performs step A7.
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <math.h>
+#include <string.h>
+
+#include "pwa_internal.h"
+#include "reduce.cuh"
+#include "stream_common.cuh"
+
+namespace pwa {
+
+namespace bi8 {
+
+constexpr int TE = 128;                      // events per tile
+constexpr int ROWB = 512;                    // bytes of one fp32 event row (128 reals)
+constexpr int SR = 32;                       // event rows per TMA stage
+constexpr int STG_BYTES = SR * ROWB;         // 16 KB
+constexpr int NSTG = 3;
+constexpr int SPT = TE / SR;                 // stages per tile
+constexpr int PLANE = TE * 128;              // 16 KB: one int8 digit plane
+constexpr int NEW = 16;                      // converter / epilogue warps
+constexpr int THREADS = NEW * 32;            // 512
+constexpr int KC = 64;                       // starting points per pass (128 real columns)
+// plane slots: X1 X2 X3 | X0 (GEMM1) = R0 (GEMM2) | R1 R2 R3 | W0 W1 W2 W3 | fp32 stages
+constexpr uint32_t OFF_X1 = 0, OFF_X2 = PLANE, OFF_X3 = 2 * PLANE, OFF_X0 = 3 * PLANE, OFF_R = 3 * PLANE, OFF_W = 7 * PLANE, OFF_STG = 11 * PLANE;
+constexpr size_t SMEM = 1024 + (size_t)11 * PLANE + (size_t)NSTG * STG_BYTES;     // 230400 bytes
+constexpr size_t SLOT = 128 * 128 + KC;      // doubles per CTA slot: Q[col][c], then L[k]
+
+struct Scales { float s[128]; };             // 2^s_c per real column
+struct Exps { int e[128]; };                 // s_c
+
+// ---- PTX wrappers -----------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "setp.ne.b32 p, %4, 0;\n"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+                 "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, int32_t (&v)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16f(uint32_t taddr, float (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
+                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st8f(uint32_t taddr, const float (&v)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"r"(taddr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NEW * 32) : "memory"); }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+
+// Shared-memory matrix descriptors of one digit plane (rows of 128 bytes, 8-row swizzle atoms of
+// 1024 bytes, SWIZZLE_128B).  K-major: rows are M (or N) indices, the 128 bytes run along K; a K step
+// of 32 advances the start address by 32 bytes; an N = 256 operand continues into the next plane
+// (rows 128..255).  MN-major: rows are K indices, the 128 bytes run along M (or N); a K step of 32 rows
+// advances by 4096 bytes; an N = 256 operand continues in the next plane (LBO = PLANE).
+__device__ __forceinline__ uint64_t desc_kmajor(uint32_t smem_addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)1 << 16;                                // leading byte offset: unused for swizzled K-major
+    d |= (uint64_t)(1024u >> 4) << 32;                     // stride byte offset: next 8 rows
+    d |= (uint64_t)1 << 46;                                // descriptor version (Blackwell)
+    d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
+    return d;
+}
+__device__ __forceinline__ uint64_t desc_mnmajor(uint32_t smem_addr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)((uint32_t)PLANE >> 4) << 16;           // next 128-byte atom along MN = next digit plane
+    d |= (uint64_t)(1024u >> 4) << 32;                     // next 8 K rows
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+// kind::i8 instruction descriptor: D = s32, A = B = signed int8, M = 128
+constexpr uint32_t idesc(uint32_t N, bool mn_major)
+{
+    return (2u << 4) | (1u << 7) | (1u << 10) | (mn_major ? ((1u << 15) | (1u << 16)) : 0u) | ((N >> 3) << 17) | ((128u >> 4) << 24);
+}
+constexpr uint32_t kI1_128 = idesc(128, false), kI1_256 = idesc(256, false);   // GEMM1: both operands K-major
+constexpr uint32_t kI2_128 = idesc(128, true),  kI2_256 = idesc(256, true);    // GEMM2: both operands MN-major
+
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// balanced int8 digits of a 32-bit integer: byte b of the result is digit d_b in [-128, 127]
+__device__ __forceinline__ uint32_t digits(int q) { return (uint32_t)(q + 0x00808080) ^ 0x00808080u; }
+
+// ---- W digit planes (once per call and pass) -----------------------------------------------------
+// Block k (local column pair), thread c: W'[c][2k], W'[c][2k+1] = W 2^-s_c, common exponent e_k from the
+// block maximum, four digit planes written in the shared-memory image (K-major rows = real start columns).
+// ek[k] = e_k; INT_MIN marks a column with non-finite V (the column's result is NaN, as IEEE would give).
+__global__ void __launch_bounds__(128)
+k_bi8_prep(const double *__restrict__ Vdev, int n, int K, int k0, const __grid_constant__ Exps ex,
+           unsigned char *__restrict__ Wp, int *__restrict__ ek, double *__restrict__ Wd)
+{
+    __shared__ double s_m[4];
+    const int kl = blockIdx.x, k = k0 + kl, c = threadIdx.x, a = c >> 1, p = c & 1;
+    double w0 = 0.0, w1 = 0.0;
+    if (k < K && a < n) {
+        const double vr = Vdev[((size_t)k * n + a) * 2], vi = Vdev[((size_t)k * n + a) * 2 + 1];
+        w0 = p == 0 ? vr : -vi;                       // column 2k   (Re S)
+        w1 = p == 0 ? vi : vr;                        // column 2k+1 (Im S)
+        w0 = ldexp(w0, -ex.e[c]); w1 = ldexp(w1, -ex.e[c]);
+    }
+    double m = fmax(fabs(w0), fabs(w1));
+    if (!(m == m)) m = INFINITY;                      // NaN -> inf (fmax drops NaNs)
+    for (int o = 16; o >= 1; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((c & 31) == 0) s_m[c >> 5] = m;
+    __syncthreads();
+    m = fmax(fmax(s_m[0], s_m[1]), fmax(s_m[2], s_m[3]));
+    int e = 0;
+    bool ok = isfinite(m);
+    if (ok && m > 0.0) {
+        e = 30 - ilogb(m);
+        if (ldexp(m, e) > 2147483648.0 - 16777216.0) --e;
+    }
+    int q0 = 0, q1 = 0;
+    if (ok) { q0 = (int)llrint(ldexp(w0, e)); q1 = (int)llrint(ldexp(w1, e)); }
+    const uint32_t g0 = digits(q0), g1 = digits(q1);
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int row = 2 * kl + h;
+            const uint32_t off = (uint32_t)v * PLANE + (uint32_t)row * 128u + ((((uint32_t)c >> 4) ^ ((uint32_t)row & 7u)) << 4) + ((uint32_t)c & 15u);
+            Wp[off] = (unsigned char)(((h == 0 ? g0 : g1) >> (8 * v)) & 0xffu);
+        }
+    }
+    // unrounded W' 2^(e_k - 24) for the fp64 recomputation of strongly cancelling events (k_batch_i8, phase 1)
+    Wd[(size_t)(2 * kl) * 128 + c] = ok ? ldexp(w0, e - 24) : 0.0;
+    Wd[(size_t)(2 * kl + 1) * 128 + c] = ok ? ldexp(w1, e - 24) : 0.0;
+    if (c == 0) ek[kl] = ok ? e : INT_MIN;
+}
+
+// S_ik of ONE event in fp64 by a whole warp, from the four X digit planes (exact fixed point) and the
+// unrounded W' (Wd[col][c] = W'_c,col 2^(e_k - 24)): lane l handles columns 4l .. 4l+3, xor-tree sum.
+__device__ __noinline__ double2 recompute_z(uint32_t pX1, uint32_t e, int lane, const double *__restrict__ Wd, int col)
+{
+    const uint32_t a = e * 128u + ((((uint32_t)lane >> 2) ^ (e & 7u)) << 4) + ((uint32_t)lane & 3u) * 4u;
+    uint32_t d0, d1, d2, d3;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d0) : "r"(pX1 - OFF_X1 + OFF_X0 + a));
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d1) : "r"(pX1 + a));
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d2) : "r"(pX1 - OFF_X1 + OFF_X2 + a));
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d3) : "r"(pX1 - OFF_X1 + OFF_X3 + a));
+    // element b of the lane's 4 columns: bytes (d0.b, d1.b, d2.b, d3.b) -> x = inverse of digits()
+    const uint32_t t0 = __byte_perm(d0, d1, 0x5140), t1 = __byte_perm(d2, d3, 0x5140);
+    const uint32_t t2 = __byte_perm(d0, d1, 0x7362), t3 = __byte_perm(d2, d3, 0x7362);
+    const int x0 = (int)((__byte_perm(t0, t1, 0x5410) ^ 0x00808080u) - 0x00808080u);
+    const int x1 = (int)((__byte_perm(t0, t1, 0x7632) ^ 0x00808080u) - 0x00808080u);
+    const int x2 = (int)((__byte_perm(t2, t3, 0x5410) ^ 0x00808080u) - 0x00808080u);
+    const int x3 = (int)((__byte_perm(t2, t3, 0x7632) ^ 0x00808080u) - 0x00808080u);
+    const double2 *wrp = reinterpret_cast<const double2 *>(Wd + (size_t)col * 128) + 2 * lane;
+    const double2 *wip = reinterpret_cast<const double2 *>(Wd + (size_t)(col + 1) * 128) + 2 * lane;
+    const double2 wr0 = __ldg(wrp), wr1 = __ldg(wrp + 1), wi0 = __ldg(wip), wi1 = __ldg(wip + 1);
+    double zr = fma((double)x0, wr0.x, fma((double)x1, wr0.y, fma((double)x2, wr1.x, (double)x3 * wr1.y)));
+    double zi = fma((double)x0, wi0.x, fma((double)x1, wi0.y, fma((double)x2, wi1.x, (double)x3 * wi1.y)));
+    return make_double2(warp_sum(zr), warp_sum(zi));
+}
+
+// ---- the kernel -------------------------------------------------------------------------------
+// tmap: fp32 [N][128] view of the data sample, box = [SR rows][128 floats], no swizzle (rows past N
+// read as zeros).  Wp: the four W digit planes (k_bi8_prep).  Kc: valid starting points of this pass.
+// slots: [gridDim.x][SLOT] doubles: Q[col][c] = 2^(-8 - s_c) sum_tiles 2^-sh z2 (the caller multiplies
+// by 2^e_k), then L[k] = sum ln(zr^2 + zi^2).
+__global__ void __launch_bounds__(THREADS, 1)
+k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntiles, int Kc,
+           const __grid_constant__ Scales sc, const __grid_constant__ Exps ex,
+           const unsigned char *__restrict__ Wp, const double *__restrict__ Wd, double *__restrict__ slots)
+{
+    extern __shared__ unsigned char bi8_smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 4];
+    __shared__ uint32_t tmem_base_s;
+    __shared__ __align__(16) uint32_t s_emax[NEW];
+    __shared__ __align__(16) float s_scl[128];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t raw_u32 = smem_u32(bi8_smem_raw);
+    const uint32_t base = (raw_u32 + 1023u) & ~1023u;
+    const uint32_t pX0 = base + OFF_X0, pX1 = base + OFF_X1, pX2 = base + OFF_X2, pX3 = base + OFF_X3;
+    const uint32_t pW = base + OFF_W, pR = base + OFF_R, stg0 = base + OFF_STG;
+    const uint32_t b_stg_full = smem_u32(&bars[0]), b_stg_empty = b_stg_full + 8 * NSTG;
+    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTG; ++s) { mbar_init(b_stg_full + 8 * s, 1); mbar_init(b_stg_empty + 8 * s, NEW); }
+        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1);
+        fence_async_smem();
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
+    }
+    if (warp == 0) tmem_alloc(smem_u32(&tmem_base_s), 512);
+    if (threadIdx.x < 128) s_scl[threadIdx.x] = sc.s[threadIdx.x];
+    {                                                     // W digit planes: global image -> shared memory
+        for (int i = threadIdx.x; i < 4 * PLANE / 16; i += NEW * 32) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(Wp) + i);
+            sts128(pW + 16u * (uint32_t)i, v.x, v.y, v.z, v.w);
+        }
+        fence_async_smem();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem0 = tmem_base_s;
+
+    const long long per = ntiles / gridDim.x, rem = ntiles % gridDim.x;
+    const long long t_begin = (long long)blockIdx.x * per + (blockIdx.x < rem ? blockIdx.x : rem);
+    const long long nt = per + (blockIdx.x < rem ? 1 : 0);
+
+    {
+        // ===== all 16 warps convert and run the epilogues; lane 0 of warp 0 also issues the MMAs, lane 0 of
+        // warp 1 the TMA loads (no dedicated producer / issuer warps: 512 threads leave 128 registers each,
+        // enough for the 32 fp64 accumulators per thread without spilling) =====
+        const bool is_mma = threadIdx.x == 0, is_tma = threadIdx.x == 32;
+        const long long ng = nt * SPT;
+        auto tma_load = [&](long long g) {
+            const int s = (int)(g % NSTG);
+            mbar_expect_tx(b_stg_full + 8 * s, STG_BYTES);
+            asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                         ::"r"(stg0 + (uint32_t)s * STG_BYTES), "l"(&tmap), "r"(0), "r"((int)(t_begin * TE + g * SR)),
+                           "r"(b_stg_full + 8 * s) : "memory");
+        };
+        if (is_tma)
+            for (long long g = 0; g < NSTG && g < ng; ++g) tma_load(g);
+        __syncwarp();
+        const int q = warp & 3, j = warp >> 2;
+        const int row = 32 * q + lane;                                 // event row (GEMM1) / real column c (GEMM2)
+        const uint32_t trow = tmem0 + ((uint32_t)(32 * q) << 16) + 32u * (uint32_t)j;
+        const float4 scl = *reinterpret_cast<const float4 *>(&s_scl[4 * lane]);
+        const uint32_t chunk_off = (uint32_t)(lane & 3) * 4u, chunk_id = (uint32_t)(lane >> 2);
+        double Tacc[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) Tacc[i] = 0.0;
+        // ln|z|^2 summed as a running PRODUCT per column chunk (mantissa in [1, 2), exponent in Ec): one log at the end
+        double Pc[4] = {1.0, 1.0, 1.0, 1.0};
+        int Ec[4] = {0, 0, 0, 0};
+        const bool b4 = (lane & 16) != 0, b3 = (lane & 8) != 0;
+
+        for (long long t = 0; t < nt; ++t) {
+            const uint32_t ph = (uint32_t)(t & 1);
+            // ---- fp32 stages -> X digit planes (2 rows per warp and stage)
+#pragma unroll 1
+            for (int st = 0; st < SPT; ++st) {
+                const long long g = t * SPT + st;
+                const int s = (int)(g % NSTG);
+                mbar_wait(b_stg_full + 8 * s, (uint32_t)((g / NSTG) & 1));
+                const uint32_t src = stg0 + (uint32_t)s * STG_BYTES + (uint32_t)(2 * warp) * ROWB + (uint32_t)lane * 16u;
+                uint4 raw[2];
+                raw[0] = lds128(src); raw[1] = lds128(src + ROWB);
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const uint32_t e = (uint32_t)(st * SR + 2 * warp + r);
+                    const uint32_t w0 = digits(__float2int_rn(__uint_as_float(raw[r].x) * scl.x));
+                    const uint32_t w1 = digits(__float2int_rn(__uint_as_float(raw[r].y) * scl.y));
+                    const uint32_t w2 = digits(__float2int_rn(__uint_as_float(raw[r].z) * scl.z));
+                    const uint32_t w3 = digits(__float2int_rn(__uint_as_float(raw[r].w) * scl.w));
+                    const uint32_t t0 = __byte_perm(w0, w1, 0x5140), t1 = __byte_perm(w2, w3, 0x5140);
+                    const uint32_t t2 = __byte_perm(w0, w1, 0x7362), t3 = __byte_perm(w2, w3, 0x7362);
+                    const uint32_t a = e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX0 + a), "r"(__byte_perm(t0, t1, 0x5410)) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX1 + a), "r"(__byte_perm(t0, t1, 0x7632)) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX2 + a), "r"(__byte_perm(t2, t3, 0x5410)) : "memory");
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX3 + a), "r"(__byte_perm(t2, t3, 0x7632)) : "memory");
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(b_stg_empty + 8 * s);
+                if (is_tma && g + NSTG < ng) {                           // refill the stage once all 16 warps have released it
+                    mbar_wait(b_stg_empty + 8 * s, (uint32_t)((g / NSTG) & 1));
+                    tma_load(g + NSTG);
+                }
+                __syncwarp();
+            }
+            fence_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_a_full);
+            if (is_mma) {
+                // ---- GEMM1: S levels t = 3..6 at TMEM columns 0, 128, 256, 384
+                mbar_wait(b_a_full, ph);
+                tc_fence_after();
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                const uint32_t ko = (uint32_t)kk * 32u, acc = kk > 0 ? 1u : 0u;
+                const uint64_t a0 = desc_kmajor(pX0 + ko), a1 = desc_kmajor(pX1 + ko);
+                const uint64_t a2 = desc_kmajor(pX2 + ko), a3 = desc_kmajor(pX3 + ko);
+                const uint64_t w0 = desc_kmajor(pW + 0 * PLANE + ko), w1 = desc_kmajor(pW + 1 * PLANE + ko);
+                const uint64_t w2 = desc_kmajor(pW + 2 * PLANE + ko), w3 = desc_kmajor(pW + 3 * PLANE + ko);
+                umma_i8(tmem0 + 256, a3, w2, kI1_256, acc);        // X3 [W2 | W3] -> t = 5 | 6
+                umma_i8(tmem0 + 0,   a3, w0, kI1_256, acc);        // X3 [W0 | W1] -> t = 3 | 4
+                umma_i8(tmem0 + 0,   a2, w1, kI1_256, 1u);         // X2 [W1 | W2] -> t = 3 | 4
+                umma_i8(tmem0 + 256, a2, w3, kI1_128, 1u);         // X2 W3        -> t = 5
+                umma_i8(tmem0 + 0,   a1, w2, kI1_256, 1u);         // X1 [W2 | W3] -> t = 3 | 4
+                umma_i8(tmem0 + 0,   a0, w3, kI1_128, 1u);         // X0 W3        -> t = 3
+            }
+                umma_commit(b_s_full);
+            }
+            __syncwarp();
+
+            // ---- phase 1: S levels -> |z|^2 into the running products, Rh = conj(z)/|z|^2 (fp32, stashed in TMEM), max |Rh|
+            const bool valid = (t_begin + t) * TE + row < N;
+            uint32_t mymax = 0u;
+            mbar_wait(b_s_full, ph);
+            tc_fence_after();
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                int32_t a3[8], a4[8], a5[8], a6[8];
+                tmem_ld8(trow + 8 * ch + 0, a3);
+                tmem_ld8(trow + 8 * ch + 128, a4);
+                tmem_ld8(trow + 8 * ch + 256, a5);
+                tmem_ld8(trow + 8 * ch + 384, a6);
+                tmem_ld_wait();
+                float rh[8];
+                double lv[4];
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    // z = 2^16 y + x exactly (|y| < 2^30, |x| < 2^31)
+                    const int yr = a6[2 * m] * 256 + a5[2 * m], xr = a4[2 * m] * 256 + a3[2 * m];
+                    const int yi = a6[2 * m + 1] * 256 + a5[2 * m + 1], xi = a4[2 * m + 1] * 256 + a3[2 * m + 1];
+                    double fr = fma((double)yr, 65536.0, (double)xr), fi = fma((double)yi, 65536.0, (double)xi);
+                    double I = fma(fr, fr, fi * fi);
+                    const bool kvalid = valid && 16 * j + 4 * ch + m < Kc;
+                    // Strong cancellation (|z| < 2^31: the truncation of GEMM1, ~2^9 rms in these units, would
+                    // exceed ~2^-22 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37 for
+                    // typical events, so this is rare (~1e-4 of the sums) and the loop is almost never entered.
+                    unsigned bal = __ballot_sync(0xffffffffu, kvalid && I < 0x1p62);
+                    while (bal) {
+                        const int srcl = __ffs(bal) - 1;
+                        bal &= bal - 1;
+                        const double2 z = recompute_z(pX1, (uint32_t)(32 * q + srcl), lane, Wd, 2 * (16 * j + 4 * ch + m));
+                        if (lane == srcl) { fr = z.x; fi = z.y; I = fma(fr, fr, fi * fi); }
+                    }
+                    lv[m] = kvalid ? I : 1.0;
+                    const float gr = (float)fr, gi = (float)fi;
+                    const float If = fmaf(gr, gr, gi * gi);
+                    const float inv = If > 0.0f ? rcp_approx(If) : 0.0f;
+                    const float rr = gr * inv, ri = -gi * inv;
+                    rh[2 * m] = rr; rh[2 * m + 1] = ri;
+                    mymax = max(mymax, max(__float_as_uint(rr) & 0x7fffffffu, __float_as_uint(ri) & 0x7fffffffu));
+                }
+                tmem_st8f(trow + 8 * ch, rh);
+                // lanes exchange so that each keeps ONE column of the chunk (m = 2 b4 + b3), multiplied over 4 lanes
+                const double send0 = b4 ? lv[0] : lv[2], send1 = b4 ? lv[1] : lv[3];
+                double keep0 = b4 ? lv[2] : lv[0], keep1 = b4 ? lv[3] : lv[1];
+                keep0 *= shfl_xor_d(send0, 16); keep1 *= shfl_xor_d(send1, 16);
+                const double send = b3 ? keep0 : keep1;
+                double keep = b3 ? keep1 : keep0;
+                keep *= shfl_xor_d(send, 8);
+                // |z|^2 < 2^94: the product of 4 times a mantissa stays finite; renormalise (a zero stays zero -> ln 0 = -inf)
+                const double P = Pc[ch] * keep;
+                const int hi = __double2hiint(P);
+                const int e = (P != 0.0) ? ((hi >> 20) - 1023) : 0;
+                Ec[ch] += e;
+                Pc[ch] = __hiloint2double(hi - (e << 20), __double2loint(P));
+            }
+            mymax = __reduce_max_sync(0xffffffffu, mymax);
+            if (lane == 0) s_emax[warp] = mymax;
+            tmem_st_wait();
+            tc_fence_before();
+            epi_bar();
+
+            // ---- phase 2: tile shift sh (max |Rh| 2^sh < 2^30), Rh -> four digit planes (R0 takes the slot of X0)
+            tc_fence_after();
+            uint32_t sh;
+            {
+                const uint4 e0 = *reinterpret_cast<const uint4 *>(&s_emax[0]), e1 = *reinterpret_cast<const uint4 *>(&s_emax[4]);
+                const uint4 e2 = *reinterpret_cast<const uint4 *>(&s_emax[8]), e3 = *reinterpret_cast<const uint4 *>(&s_emax[12]);
+                const uint32_t m0 = max(max(e0.x, e0.y), max(e0.z, e0.w)), m1 = max(max(e1.x, e1.y), max(e1.z, e1.w));
+                const uint32_t m2 = max(max(e2.x, e2.y), max(e2.z, e2.w)), m3 = max(max(e3.x, e3.y), max(e3.z, e3.w));
+                const uint32_t bits = max(max(m0, m1), max(m2, m3));
+                sh = bits == 0u ? 0u : (uint32_t)(29 + 127 - (int)(bits >> 23));
+            }
+            const float qs = __uint_as_float((sh + 127u) << 23);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                float f[16];
+                tmem_ld16f(trow + 16 * h, f);
+                tmem_ld_wait();
+                uint32_t wq[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) wq[i] = digits(__float2int_rn(f[i] * qs));
+                uint32_t p0[4], p1[4], p2[4], p3[4];
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    const uint32_t t0 = __byte_perm(wq[4 * g], wq[4 * g + 1], 0x5140), t1 = __byte_perm(wq[4 * g + 2], wq[4 * g + 3], 0x5140);
+                    const uint32_t t2 = __byte_perm(wq[4 * g], wq[4 * g + 1], 0x7362), t3 = __byte_perm(wq[4 * g + 2], wq[4 * g + 3], 0x7362);
+                    p0[g] = __byte_perm(t0, t1, 0x5410); p1[g] = __byte_perm(t0, t1, 0x7632);
+                    p2[g] = __byte_perm(t2, t3, 0x5410); p3[g] = __byte_perm(t2, t3, 0x7632);
+                }
+                const uint32_t a = pR + (uint32_t)row * 128u + ((((uint32_t)(2 * j + h)) ^ ((uint32_t)row & 7u)) << 4);
+                sts128(a + 0 * PLANE, p0[0], p0[1], p0[2], p0[3]);
+                sts128(a + 1 * PLANE, p1[0], p1[1], p1[2], p1[3]);
+                sts128(a + 2 * PLANE, p2[0], p2[1], p2[2], p2[3]);
+                sts128(a + 3 * PLANE, p3[0], p3[1], p3[2], p3[3]);
+            }
+            fence_async_smem();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_r_full);
+            if (is_mma) {
+                // ---- GEMM2: Q levels t = 3..6 at TMEM columns 0, 128, 256, 384 (X0 is not used: its slot holds R0)
+                mbar_wait(b_r_full, ph);
+                tc_fence_after();
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+                const uint32_t ko = (uint32_t)kk * 32u * 128u, acc = kk > 0 ? 1u : 0u;
+                const uint64_t a1 = desc_mnmajor(pX1 + ko), a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
+                const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko), r1 = desc_mnmajor(pR + 1 * PLANE + ko);
+                const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko), r3 = desc_mnmajor(pR + 3 * PLANE + ko);
+                umma_i8(tmem0 + 256, a3, r2, kI2_256, acc);        // X3^T [R2 | R3] -> t = 5 | 6
+                umma_i8(tmem0 + 0,   a3, r0, kI2_256, acc);        // X3^T [R0 | R1] -> t = 3 | 4
+                umma_i8(tmem0 + 0,   a2, r1, kI2_256, 1u);         // X2^T [R1 | R2] -> t = 3 | 4
+                umma_i8(tmem0 + 256, a2, r3, kI2_128, 1u);         // X2^T R3        -> t = 5
+                umma_i8(tmem0 + 0,   a1, r2, kI2_256, 1u);         // X1^T [R2 | R3] -> t = 3 | 4
+            }
+                umma_commit(b_t_full);
+            }
+            __syncwarp();
+
+            // ---- flush: Q levels of this tile -> fp64 accumulators (row = real column c)
+            const double fs = __hiloint2double((int)((1023u - sh) << 20), 0);          // 2^-sh
+            mbar_wait(b_t_full, ph);
+            tc_fence_after();
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                int32_t a3[8], a4[8], a5[8], a6[8];
+                tmem_ld8(trow + 8 * ch + 0, a3);
+                tmem_ld8(trow + 8 * ch + 128, a4);
+                tmem_ld8(trow + 8 * ch + 256, a5);
+                tmem_ld8(trow + 8 * ch + 384, a6);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const double z = fma((double)(a6[i] * 256 + a5[i]), 65536.0, (double)(a4[i] * 256 + a3[i]));
+                    Tacc[8 * ch + i] = fma(z, fs, Tacc[8 * ch + i]);
+                }
+            }
+            tc_fence_before();
+        }
+
+        // ---- per-CTA partials -> fixed slot
+        double *slot = slots + (size_t)blockIdx.x * SLOT;
+        const double cs = ldexp(1.0, -ex.e[row]);
+#pragma unroll
+        for (int i = 0; i < 32; ++i) slot[(size_t)(32 * j + i) * 128 + row] = Tacc[i] * cs;
+        double *sL = reinterpret_cast<double *>(bi8_smem_raw + (base - raw_u32));      // plane slots are dead: all MMAs completed
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) sL[(size_t)threadIdx.x * 4 + ch] = log(Pc[ch]) + (double)Ec[ch] * 0.693147180559945309417232;
+        epi_bar();
+        if (threadIdx.x < KC) {
+            const int k = threadIdx.x, jj = k >> 4, ch = (k >> 2) & 3, m = k & 3;
+            double acc = 0.0;
+            for (int qq = 0; qq < 4; ++qq)
+                for (int r = 0; r < 8; ++r) acc += sL[(size_t)((4 * jj + qq) * 32 + (m >> 1) * 16 + (m & 1) * 8 + r) * 4 + ch];
+            slot[128 * 128 + k] = acc;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) { tc_fence_after(); tmem_dealloc(tmem0, 512); }
+}
+
+// ---- final sums + step A7 ---------------------------------------------------------------------
+// One block per starting point: sums the per-CTA slots in a fixed tree (1024 threads = 4 slot
+// phases x 256 values: Q[2k][c], Q[2k+1][c]), undoes the exponents, Q -> T, then step A7.
+__global__ void __launch_bounds__(1024)
+k_bi8_finalize(const double *__restrict__ slots, int nslots, int n, const double *__restrict__ Vdev, int k0,
+               const int *__restrict__ ek, long long N, const double *__restrict__ M, double *__restrict__ results,
+               int result_stride, double n_eq2, unsigned long long *done_flags, unsigned long long seq)
+{
+    __shared__ double s_val[4][256];
+    __shared__ double s_tot[2 + 2 * kFastWaves];
+    __shared__ double sV[2 * kFastWaves];
+    const int kl = blockIdx.x, k = k0 + kl, tid = threadIdx.x;
+    const int v = tid & 255, ph = tid >> 8;
+    const int e = ek[kl];
+    {
+        const double *src = slots + (size_t)(2 * kl) * 128 + v;      // v = 128 * (column parity) + c
+        double acc = 0.0;
+        for (int s0 = ph; s0 < nslots; s0 += 16) {
+            double x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { const int sl = s0 + 4 * u; x[u] = (sl < nslots) ? __ldcg(src + (size_t)sl * SLOT) : 0.0; }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) acc += x[u];
+        }
+        s_val[ph][v] = acc;
+    }
+    if (tid < 32) {
+        double acc = 0.0;
+        for (int s = tid; s < nslots; s += 32) acc += __ldcg(slots + (size_t)s * SLOT + 128 * 128 + kl);
+        acc = warp_sum(acc);
+        if (tid == 0) {
+            // ln|S|^2 = ln|z|^2 + 2 (24 - e_k) ln 2 for each of the N events
+            const double L = (e == INT_MIN) ? NAN : acc + (double)N * (2.0 * (double)(24 - e)) * 0.693147180559945309417232;
+            s_tot[0] = L;
+            s_tot[1] = isfinite(L) ? 0.0 : 1.0;
+        }
+    }
+    __syncthreads();
+    if (tid < n) {
+        const int a = tid;
+        const double sc = (e == INT_MIN) ? NAN : ldexp(1.0, e);
+        auto val = [&](int par, int c) { return ((s_val[0][128 * par + c] + s_val[1][128 * par + c]) + s_val[2][128 * par + c]) + s_val[3][128 * par + c]; };
+        s_tot[2 + 2 * a] = (val(0, 2 * a) - val(1, 2 * a + 1)) * sc;        // Re T = Q[2a][2k] - Q[2a+1][2k+1]
+        s_tot[3 + 2 * a] = (val(1, 2 * a) + val(0, 2 * a + 1)) * sc;        // Im T = Q[2a][2k+1] + Q[2a+1][2k]
+        sV[2 * a] = Vdev[((size_t)k * n + a) * 2];
+        sV[2 * a + 1] = Vdev[((size_t)k * n + a) * 2 + 1];
+    }
+    __syncthreads();
+    assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n, n_eq2, done_flags + k, seq);
+}
+
+}  // namespace bi8
+
+// ---- host side ----------------------------------------------------------------------------------
+static PFN_cuTensorMapEncodeTiled_v12000 bi8_get_encode()
+{
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// Handles fp32-stored constant-resonance data samples with n = 64 waves, no event weights.  Default for
+// K >= 8 and >= 32768 events (option "batch" = 0); "batch" = 2 forces it for any K and sample size,
+// "batch" = 1 keeps the FP64 DMMA path (batch_dmma.cu).
+pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
+{
+    *handled = false;
+    const long long N = ctx->data.n_events;
+    if (ctx->storage != PWA_F32 || ctx->data.factored || ctx->n != 64 || ctx->data.weights != nullptr || N <= 0 ||
+        ((uintptr_t)ctx->data.amps & 15u) != 0 || N > 0x7fffffffLL - 2 * bi8::TE)
+        return PWA_OK;
+    if (ctx->opt_batch != 2 && !(ctx->opt_batch == 0 && K >= 8 && N >= 32768)) return PWA_OK;
+    auto &q = ctx->i8d;
+    if (!q.checked) {
+        pwa_status s = i8_column_scales(ctx, ctx->data.amps, N, 128, q.exp, q.scale, q.cmax, &q.valid);
+        if (s != PWA_OK) return s;
+        q.checked = true;
+    }
+    if (!q.valid) return PWA_OK;
+    PFN_cuTensorMapEncodeTiled_v12000 enc = bi8_get_encode();
+    if (!enc) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    alignas(64) CUtensorMap tmap;
+    {
+        const cuuint64_t gdim[2] = {128, (cuuint64_t)N};
+        const cuuint64_t gstride[1] = {512};
+        const cuuint32_t box[2] = {128, (cuuint32_t)bi8::SR};
+        const cuuint32_t estr[2] = {1, 1};
+        CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, ctx->data.amps, gdim, gstride, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled (i8 batch) failed (code " + std::to_string((int)r) + ")");
+    }
+    const long long ntiles = (N + bi8::TE - 1) / bi8::TE;
+    long long grid = ctx->sm_count;
+    if (grid > ntiles) grid = ntiles;
+    static bool s_attr[64] = {false};
+    if (!s_attr[ctx->device & 63]) {
+        PWA_CUDA(ctx, cudaFuncSetAttribute(bi8::k_batch_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bi8::SMEM));
+        s_attr[ctx->device & 63] = true;
+    }
+    const size_t wp_bytes = 4 * bi8::PLANE, ek_bytes = 256, wd_bytes = 128 * 128 * sizeof(double);
+    pwa_status s = ensure_scratch(ctx, wp_bytes + ek_bytes + wd_bytes + sizeof(double) * (size_t)grid * bi8::SLOT);
+    if (s != PWA_OK) return s;
+    unsigned char *Wp = reinterpret_cast<unsigned char *>(ctx->d_scratch);
+    int *ek = reinterpret_cast<int *>(Wp + wp_bytes);
+    double *Wd = reinterpret_cast<double *>(Wp + wp_bytes + ek_bytes);
+    double *slots = Wd + 128 * 128;
+    bi8::Scales sc;
+    bi8::Exps ex;
+    memcpy(sc.s, q.scale, sizeof(sc.s));
+    memcpy(ex.e, q.exp, sizeof(ex.e));
+    for (int k0 = 0; k0 < K; k0 += bi8::KC) {
+        const int cols = (K - k0 < bi8::KC) ? (K - k0) : bi8::KC;
+        bi8::k_bi8_prep<<<bi8::KC, 128, 0, ctx->stream>>>(ctx->d_V, ctx->n, K, k0, ex, Wp, ek, Wd);
+        ctx->launches++;
+        PWA_CUDA(ctx, cudaGetLastError());
+        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, N, ntiles, cols, sc, ex, Wp, Wd, slots);
+        ctx->launches++;
+        PWA_CUDA(ctx, cudaGetLastError());
+        bi8::k_bi8_finalize<<<cols, 1024, 0, ctx->stream>>>(slots, (int)grid, ctx->n, ctx->d_V, k0, ek, N, ctx->d_M,
+                                                            ctx->dev_result, result_stride(ctx->n),
+                                                            ctx->opt_likelihood == 1 ? (double)N : 0.0,
+                                                            ctx->dev_flags, ctx->seq);
+        ctx->launches++;
+        PWA_CUDA(ctx, cudaGetLastError());
+    }
+    *handled = true;
+    return PWA_OK;
+}
+
+}  // namespace pwa

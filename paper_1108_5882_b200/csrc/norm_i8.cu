@@ -402,23 +402,23 @@ static bool i8_shape_ok(const pwa_ctx *ctx)
            ctx->mc.n_events > 0 && ((uintptr_t)ctx->mc.amps & 15u) == 0;
 }
 
-// Called after every constant-resonance MC upload: column maxima -> power-of-two scales.
-pwa_status prepare_norm_i8(pwa_ctx *ctx)
+// Column maxima of an fp32-stored [n_events x D] sample (D = 32, 64 or 128) -> power-of-two scales
+// 2^exp[p] with |B_jp| 2^exp[p] <= 2^31 - 2^24.  *valid stays false for inf / nan / out-of-range columns.
+// Also used by batch_i8.cu for the DATA sample.
+pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, int D, int *exp, float *scale,
+                            double *cmax, bool *valid)
 {
-    auto &q = ctx->i8q;
-    q.valid = false;
-    if (!i8_shape_ok(ctx)) return PWA_OK;
-    const int D = 2 * ctx->n;
+    *valid = false;
     pwa_status s = ensure_scratch(ctx, 128 * sizeof(unsigned));
     if (s != PWA_OK) return s;
     unsigned *d_cmax = reinterpret_cast<unsigned *>(ctx->d_scratch);
     PWA_CUDA(ctx, cudaMemsetAsync(d_cmax, 0, 128 * sizeof(unsigned), ctx->stream));
-    const long long nfloats = ctx->mc.n_events * (long long)D;
+    const long long nfloats = n_events * (long long)D;
     long long grid = (nfloats / 4 + 255) / 256;
     const long long cap = (long long)ctx->sm_count * 8;
     if (grid > cap) grid = cap;
     if (grid < 1) grid = 1;
-    i8::k_colmax_f32<<<(unsigned)grid, 256, 0, ctx->stream>>>(reinterpret_cast<const float *>(ctx->mc.amps), nfloats, D, d_cmax);
+    i8::k_colmax_f32<<<(unsigned)grid, 256, 0, ctx->stream>>>(reinterpret_cast<const float *>(amps), nfloats, D, d_cmax);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     unsigned h_cmax[128];
@@ -426,7 +426,7 @@ pwa_status prepare_norm_i8(pwa_ctx *ctx)
     PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const double qmax = 2147483648.0 - 16777216.0;               // 2^31 - 2^24
     for (int p = 0; p < D; ++p) {
-        if (h_cmax[p] >= 0x7f800000u) return PWA_OK;            // inf / nan in the sample: DMMA path propagates IEEE values
+        if (h_cmax[p] >= 0x7f800000u) return PWA_OK;            // inf / nan in the sample: FP64 paths propagate IEEE values
         float c; memcpy(&c, &h_cmax[p], 4);
         int e = 0;
         if (c > 0.0f) {
@@ -435,11 +435,20 @@ pwa_status prepare_norm_i8(pwa_ctx *ctx)
             if (e > 126) e = 126;
             if (e < -126) return PWA_OK;
         }
-        q.cmax[p] = (double)c;
-        for (int g = 0; g < 128 / D; ++g) { q.exp[g * D + p] = e; q.scale[g * D + p] = ldexpf(1.0f, e); }
+        cmax[p] = (double)c;
+        for (int g = 0; g < 128 / D; ++g) { exp[g * D + p] = e; scale[g * D + p] = ldexpf(1.0f, e); }
     }
-    q.valid = true;
+    *valid = true;
     return PWA_OK;
+}
+
+// Called after every constant-resonance MC upload: column maxima -> power-of-two scales.
+pwa_status prepare_norm_i8(pwa_ctx *ctx)
+{
+    auto &q = ctx->i8q;
+    q.valid = false;
+    if (!i8_shape_ok(ctx)) return PWA_OK;
+    return i8_column_scales(ctx, ctx->mc.amps, ctx->mc.n_events, 2 * ctx->n, q.exp, q.scale, q.cmax, &q.valid);
 }
 
 pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)

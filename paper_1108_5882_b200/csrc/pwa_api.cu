@@ -260,7 +260,7 @@ pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, i
     Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
     free_sample(smp);
     smp.amps = buf; smp.amps_owned = owned; smp.factored = false;
-    if (which == PWA_DATA) ctx->tmap_cache.valid = false;
+    if (which == PWA_DATA) { ctx->tmap_cache.valid = false; ctx->i8d.checked = false; ctx->i8d.valid = false; }
     smp.n_events = n_events; smp.n_gen = n_generated;
     if (which == PWA_MC) { ctx->M_valid = false; return prepare_norm_i8(ctx); }
     return PWA_OK;
@@ -288,6 +288,7 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
     smp.mass = (double *)bm; smp.ang = ba; smp.fact_owned = om || oa; smp.n_ang = n_ang; smp.factored = true;
     smp.n_events = n_events; smp.n_gen = n_generated;
     if (which == PWA_MC) { ctx->M_valid = false; ctx->i8q.valid = false; }
+    else { ctx->i8d.checked = false; ctx->i8d.valid = false; }
     return PWA_OK;
 }
 

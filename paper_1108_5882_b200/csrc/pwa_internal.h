@@ -76,6 +76,8 @@ struct pwa_ctx {
              alignas(64) unsigned char map[128]; } tmap_cache;
     // int8 tensor-core M build (norm_i8.cu): per-column power-of-two scales found at MC upload
     struct { bool valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8q;
+    // int8 tensor-core batched evaluation (batch_i8.cu): the same for the DATA sample, found on first use
+    struct { bool checked = false, valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8d;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     int opt_likelihood = 0;                   // 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form
@@ -103,6 +105,9 @@ pwa_status launch_fumili(pwa_ctx *ctx, double *H_dev, bool with_norm);   // norm
 pwa_status prepare_norm_i8(pwa_ctx *ctx);                  // norm_i8.cu: after a constant-resonance MC upload
 pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled);    // norm_i8.cu
 double norm_i8_error_bound(const pwa_ctx *ctx);
+pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, int D, int *exp, float *scale,
+                            double *cmax, bool *valid);    // norm_i8.cu
+pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled);   // batch_i8.cu
 pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
 

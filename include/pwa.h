@@ -141,6 +141,16 @@ pwa_status pwa_nll_grad(pwa_ctx *ctx, const double *V, double *nll, double *grad
 pwa_status pwa_nll_grad_batch(pwa_ctx *ctx, int32_t K, const double *V, double *nll,
                               double *grad, double *parts);
 
+/* Which kernel family served the most recent pwa_nll_grad_batch / _batch_enqueue:
+ * 0 = K passes of the streaming data-term kernel, 1 = chained FP64 DMMA GEMMs (batch_dmma.cu),
+ * 2 = chained int8 tcgen05 GEMMs with exact int32 accumulation (batch_i8.cu, DESIGN.md section 6.7:
+ * fp32-stored constant-resonance data sample, n = 64, no event weights; default for K >= 8 and
+ * >= 32768 events).  *err_rel (may be NULL): for path 2 the a-priori estimate of the relative error
+ * of each term A_ia / S_ik entering the gradient sums (independent over events: the norm-wise error of
+ * the summed gradient is smaller by about 1 / sqrt(N_data)), else 0.  PWA_ERR_STATE before the first
+ * batched call.                                                                                  */
+pwa_status pwa_batch_path(pwa_ctx *ctx, int32_t *which_path, double *err_rel);
+
 /* Asynchronous pair: enqueue one evaluation (V is copied before return) / wait and fetch
  * the results of the most recent enqueue.  Used for device-side timing.                  */
 pwa_status pwa_nll_grad_enqueue(pwa_ctx *ctx, const double *V);
@@ -218,6 +228,8 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * unknown keys.  Keys: "data_term", "norm", "batch", "likelihood".  "norm": 0 = default (int8 tcgen05 path for
  * fp32-stored constant-resonance samples of >= 65536 events, else FP64 DMMA), 1 = FP64 DMMA,
  * 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.
+ * "batch": 0 = default (see pwa_batch_path), 1 = FP64 DMMA GEMMs for any K, 2 = int8 tcgen05 GEMMs
+ * whenever the shape allows, 99 = K passes of the streaming kernel.
  * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
  * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch and the minimisers.    */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);

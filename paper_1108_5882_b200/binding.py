@@ -30,6 +30,7 @@ SYMBOLS = [
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
     "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
+    "pwa_batch_path",
 ]
 
 
@@ -78,6 +79,7 @@ def _load():
         "pwa_fumili_hessian": (C.c_int, [vp, vp, vp, i32]),
         "pwa_set_weights": (C.c_int, [vp, C.c_int, vp, u32]),
         "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
+        "pwa_batch_path": (C.c_int, [vp, C.POINTER(i32), dp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)          # AttributeError here = header/library mismatch
@@ -197,6 +199,13 @@ def pwa_norm_error_bound(ctx):
     b, w = C.c_double(0.0), C.c_int32(0)
     _check(ctx, _lib.pwa_norm_error_bound(ctx, C.byref(b), C.byref(w)))
     return b.value, int(w.value)
+
+
+def pwa_batch_path(ctx):
+    """-> (path, err_rel) of the most recent batched call: 0 = streaming passes, 1 = FP64 DMMA, 2 = int8 tcgen05."""
+    w, e = C.c_int32(0), C.c_double(0.0)
+    _check(ctx, _lib.pwa_batch_path(ctx, C.byref(w), C.byref(e)))
+    return int(w.value), e.value
 
 
 def pwa_set_norm(ctx, M):

@@ -16,11 +16,12 @@ pwa_status launch_batch(pwa_ctx *ctx, int K)
         bool handled = false;
         pwa_status s = launch_batch_i8(ctx, K, &handled);           // fp32 storage, n = 64: int8 tensor cores (batch_i8.cu)
         if (s != PWA_OK) return s;
-        if (handled) return PWA_OK;
+        if (handled) { ctx->batch_path = 2; return PWA_OK; }
         s = launch_batch_dmma(ctx, K, &handled);
         if (s != PWA_OK) return s;
-        if (handled) return PWA_OK;
+        if (handled) { ctx->batch_path = 1; return PWA_OK; }
     }
+    ctx->batch_path = 0;
     const int n = ctx->n;
     for (int k = 0; k < K; ++k) {
         pwa_status s = launch_data_term(ctx, ctx->h_V + (size_t)k * 2 * n, k, nullptr);

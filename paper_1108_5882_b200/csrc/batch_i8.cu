@@ -19,23 +19,30 @@
 // A operand of GEMM2 (M = columns, K = events) — the same bytes serve both GEMMs.
 //   * W' = W 2^-s_c (the column scale moves to the other operand; exact) is quantised per starting
 //     point with w = rint(W' 2^e_k), 32 bits below max_c |W'_ck|, four digit planes (k_bi8_prep).
-//     GEMM1 forms the digit-pair products of orders t = u + v = 3..6 (10 of 16 pairs, as 4 N = 256 and
-//     2 N = 128 MMAs per 32-column K step); z = sum_t 2^(8(t-3)) acc_t is an exact integer and
-//     S_ik = z 2^(24 - e_k) up to |dS| <~ 2^-30 sum_c |X_ic| max_c|W'_ck| (quantisation of both operands
-//     + the dropped orders t <= 2).
-//   * ln|S|^2 = ln(zr^2 + zi^2) + 2 (24 - e_k) ln 2 in fp64 (the offset is added once per column at
-//     the end).  Rh = conj(z)/|z|^2 is formed in fp32 (R only needs the relative accuracy of the
-//     fp32-stored amplitudes it multiplies), quantised PER TILE AND COLUMN to 23 bits below the
-//     tile's max_i |Rh_ik| (three digit planes), and GEMM2 forms orders t = 2..5 (9 of 12 pairs).
-//     The tile's integer block is read back from TMEM, converted and added to fp64 accumulators in
-//     registers (one per (column c, real start column) and thread: 128 x 128 per CTA), so no int32
+//     GEMM1 forms the digit-pair products of orders t = u + v = 3..6 (10 of 16 pairs, as 3 N = 256 and
+//     4 N = 128 MMAs per 32-column K step); z = sum_t 2^(8(t-3)) acc_t is an exact integer and
+//     S_ik = z 2^(24 - e_k) up to the dropped orders t <= 2 and the quantisation of W' (together
+//     ~2^9 rms in the units of z, where a typical |z| is ~2^37).
+//   * Sums that cancel strongly (|z| < 2^31, ~1e-4 of them, the ones that dominate the gradient) are
+//     recomputed by the warp in fp64 from the event's fp32 row and the unrounded W (recompute_z), so every
+//     S_ik used below is exact to ~2^-22 |S_ik| or better (typically 2^-28).
+//   * ln|S|^2: |z|^2 enters a running fp64 PRODUCT per column (mantissa renormalised, exponent counted),
+//     one log per thread at the end; the offset 2 (24 - e_k) ln 2 per event is added by k_bi8_finalize.
+//   * Rh = conj(z)/|z|^2 in fp64 (hardware seed + two Newton steps), parked in TMEM over the consumed
+//     S columns, then quantised PER TILE AND STARTING POINT to 31 bits below the tile's max_i |Rh_ik|
+//     (four digit planes; R0 is written into the slot of W0, which the TMA thread re-reads from its
+//     L2-resident image after GEMM2).  GEMM2 forms orders t = 3..6 (10 pairs) like GEMM1.
+//     The tile's integer block is read back from TMEM, converted exactly and added to fp64 accumulators
+//     in registers (one per (column c, real start column) and thread: 128 x 128 per CTA), so no int32
 //     ever sees more than one tile.
-// Error: see DESIGN.md 6.7; the parity bar for fp32 storage is 1e-6 (BASELINE.json north_star).
+// Error: DESIGN.md 6.7 (measured norm-wise gradient error 1e-7 at 6e3 events, 1e-8 at 2e5, falling like
+// 1 / sqrt(N)); the parity bar for fp32 storage is 1e-6 (BASELINE.json north_star).
 //
-// Warp roles (one persistent CTA per SM, contiguous tile range per CTA): 16 converter / epilogue
-// warps (warp w: TMEM lane quarter w % 4, 32-column group w / 4), one TMA producer warp (ring of
-// 32-event fp32 stages), one MMA issuer warp (owns TMEM; one lane issues tcgen05.mma / commit).
-// Per-CTA partials go to fixed slots; k_bi8_finalize sums them in slot order and performs step A7.
+// One persistent CTA per SM (contiguous tile range), 16 warps = 512 threads with 128 registers each: every
+// warp converts (fp32 stage -> digit planes) and runs the epilogues (warp w: TMEM lane quarter w % 4,
+// 32-column group w / 4); lane 0 of warp 0 also issues the MMAs and owns TMEM, lane 0 of warp 1 issues the
+// TMA loads (ring of 32-event fp32 stages).  Per-CTA partials go to fixed slots; k_bi8_finalize sums them
+// in slot order and performs step A7.
 #include <cuda.h>
 #include <cudaTypedefs.h>
 #include <math.h>
@@ -59,8 +66,10 @@ constexpr int PLANE = TE * 128;              // 16 KB: one int8 digit plane
 constexpr int NEW = 16;                      // converter / epilogue warps
 constexpr int THREADS = NEW * 32;            // 512
 constexpr int KC = 64;                       // starting points per pass (128 real columns)
-// plane slots: X1 X2 X3 | X0 (GEMM1) = R0 (GEMM2) | R1 R2 R3 | W0 W1 W2 W3 | fp32 stages
-constexpr uint32_t OFF_X1 = 0, OFF_X2 = PLANE, OFF_X3 = 2 * PLANE, OFF_X0 = 3 * PLANE, OFF_R = 3 * PLANE, OFF_W = 7 * PLANE, OFF_STG = 11 * PLANE;
+// plane slots: X0 X1 X2 X3 | W1 W2 W3 | W0 (GEMM1) = R0 (GEMM2) | R1 R2 R3 | fp32 stages.  W0 is re-read
+// from its global image (L2) after every GEMM2; adjacent operand pairs (N = 256): W1W2, W2W3, R0R1, R1R2, R2R3.
+constexpr uint32_t OFF_X0 = 0, OFF_X1 = PLANE, OFF_X2 = 2 * PLANE, OFF_X3 = 3 * PLANE;
+constexpr uint32_t OFF_W1 = 4 * PLANE, OFF_W0 = 7 * PLANE, OFF_R = 7 * PLANE, OFF_STG = 11 * PLANE;
 constexpr size_t SMEM = 1024 + (size_t)11 * PLANE + (size_t)NSTG * STG_BYTES;     // 230400 bytes
 constexpr size_t SLOT = 128 * 128 + KC;      // doubles per CTA slot: Q[col][c], then L[k]
 
@@ -101,18 +110,6 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, int32_t (&v)[8])
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                  : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                  : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld16f(uint32_t taddr, float (&v)[16])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
-                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
-                 : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_st8f(uint32_t taddr, const float (&v)[8])
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
-                 ::"r"(taddr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
@@ -155,11 +152,33 @@ constexpr uint32_t idesc(uint32_t N, bool mn_major)
 constexpr uint32_t kI1_128 = idesc(128, false), kI1_256 = idesc(256, false);   // GEMM1: both operands K-major
 constexpr uint32_t kI2_128 = idesc(128, true),  kI2_256 = idesc(256, true);    // GEMM2: both operands MN-major
 
-__device__ __forceinline__ float rcp_approx(float x)
+// 2^16 y + x (|.| < 2^51) as a double, exactly: 64-bit integer arithmetic, the result lands in the mantissa of 1.5 * 2^52
+__device__ __forceinline__ double yx2d(int y, int x)
 {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
+    const long long b = (long long)y * 65536LL + (long long)x + 0x4338000000000000LL;
+    return __longlong_as_double(b) - 6755399441055744.0;
+}
+// 1 / x for 1 <= x < 2^100: 20-bit hardware seed, two Newton steps (relative error ~2^-52)
+__device__ __forceinline__ double rcp_d(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+__device__ __forceinline__ void tmem_ld16i(uint32_t taddr, int32_t (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st8i(uint32_t taddr, const int32_t (&v)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
 }
 
 // balanced int8 digits of a 32-bit integer: byte b of the result is digit d_b in [-128, 127]
@@ -180,8 +199,9 @@ k_bi8_prep(const double *__restrict__ Vdev, int n, int K, int k0, const __grid_c
         const double vr = Vdev[((size_t)k * n + a) * 2], vi = Vdev[((size_t)k * n + a) * 2 + 1];
         w0 = p == 0 ? vr : -vi;                       // column 2k   (Re S)
         w1 = p == 0 ? vi : vr;                        // column 2k+1 (Im S)
-        w0 = ldexp(w0, -ex.e[c]); w1 = ldexp(w1, -ex.e[c]);
     }
+    const double u0 = w0, u1 = w1;                    // W itself (for the fp64 recomputation)
+    w0 = ldexp(w0, -ex.e[c]); w1 = ldexp(w1, -ex.e[c]);
     double m = fmax(fabs(w0), fabs(w1));
     if (!(m == m)) m = INFINITY;                      // NaN -> inf (fmax drops NaNs)
     for (int o = 16; o >= 1; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
@@ -206,34 +226,24 @@ k_bi8_prep(const double *__restrict__ Vdev, int n, int K, int k0, const __grid_c
             Wp[off] = (unsigned char)(((h == 0 ? g0 : g1) >> (8 * v)) & 0xffu);
         }
     }
-    // unrounded W' 2^(e_k - 24) for the fp64 recomputation of strongly cancelling events (k_batch_i8, phase 1)
-    Wd[(size_t)(2 * kl) * 128 + c] = ok ? ldexp(w0, e - 24) : 0.0;
-    Wd[(size_t)(2 * kl + 1) * 128 + c] = ok ? ldexp(w1, e - 24) : 0.0;
+    // unrounded W 2^(e_k - 24) for the fp64 recomputation of strongly cancelling events (k_batch_i8, phase 1)
+    Wd[(size_t)(2 * kl) * 128 + c] = ok ? ldexp(u0, e - 24) : 0.0;
+    Wd[(size_t)(2 * kl + 1) * 128 + c] = ok ? ldexp(u1, e - 24) : 0.0;
     if (c == 0) ek[kl] = ok ? e : INT_MIN;
 }
 
-// S_ik of ONE event in fp64 by a whole warp, from the four X digit planes (exact fixed point) and the
-// unrounded W' (Wd[col][c] = W'_c,col 2^(e_k - 24)): lane l handles columns 4l .. 4l+3, xor-tree sum.
-__device__ __noinline__ double2 recompute_z(uint32_t pX1, uint32_t e, int lane, const double *__restrict__ Wd, int col)
+// S_ik of ONE event in fp64 by a whole warp, from the event's fp32 amplitudes in global memory (the row
+// was just read by TMA, so it comes from L2) and the unrounded W (Wd[col][c] = W_c,col 2^(e_k - 24)):
+// lane l handles columns 4l .. 4l+3, xor-tree sum.  Same arithmetic as the definition (fp32 widened
+// exactly, fp64 products and sums), in units of z.
+__device__ __noinline__ double2 recompute_z(const float *__restrict__ arow, int lane, const double *__restrict__ Wd, int col)
 {
-    const uint32_t a = e * 128u + ((((uint32_t)lane >> 2) ^ (e & 7u)) << 4) + ((uint32_t)lane & 3u) * 4u;
-    uint32_t d0, d1, d2, d3;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d0) : "r"(pX1 - OFF_X1 + OFF_X0 + a));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d1) : "r"(pX1 + a));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d2) : "r"(pX1 - OFF_X1 + OFF_X2 + a));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(d3) : "r"(pX1 - OFF_X1 + OFF_X3 + a));
-    // element b of the lane's 4 columns: bytes (d0.b, d1.b, d2.b, d3.b) -> x = inverse of digits()
-    const uint32_t t0 = __byte_perm(d0, d1, 0x5140), t1 = __byte_perm(d2, d3, 0x5140);
-    const uint32_t t2 = __byte_perm(d0, d1, 0x7362), t3 = __byte_perm(d2, d3, 0x7362);
-    const int x0 = (int)((__byte_perm(t0, t1, 0x5410) ^ 0x00808080u) - 0x00808080u);
-    const int x1 = (int)((__byte_perm(t0, t1, 0x7632) ^ 0x00808080u) - 0x00808080u);
-    const int x2 = (int)((__byte_perm(t2, t3, 0x5410) ^ 0x00808080u) - 0x00808080u);
-    const int x3 = (int)((__byte_perm(t2, t3, 0x7632) ^ 0x00808080u) - 0x00808080u);
+    const float4 x = __ldg(reinterpret_cast<const float4 *>(arow) + lane);
     const double2 *wrp = reinterpret_cast<const double2 *>(Wd + (size_t)col * 128) + 2 * lane;
     const double2 *wip = reinterpret_cast<const double2 *>(Wd + (size_t)(col + 1) * 128) + 2 * lane;
     const double2 wr0 = __ldg(wrp), wr1 = __ldg(wrp + 1), wi0 = __ldg(wip), wi1 = __ldg(wip + 1);
-    double zr = fma((double)x0, wr0.x, fma((double)x1, wr0.y, fma((double)x2, wr1.x, (double)x3 * wr1.y)));
-    double zi = fma((double)x0, wi0.x, fma((double)x1, wi0.y, fma((double)x2, wi1.x, (double)x3 * wi1.y)));
+    double zr = fma((double)x.x, wr0.x, fma((double)x.y, wr0.y, fma((double)x.z, wr1.x, (double)x.w * wr1.y)));
+    double zi = fma((double)x.x, wi0.x, fma((double)x.y, wi0.y, fma((double)x.z, wi1.x, (double)x.w * wi1.y)));
     return make_double2(warp_sum(zr), warp_sum(zi));
 }
 
@@ -243,27 +253,27 @@ __device__ __noinline__ double2 recompute_z(uint32_t pX1, uint32_t e, int lane, 
 // slots: [gridDim.x][SLOT] doubles: Q[col][c] = 2^(-8 - s_c) sum_tiles 2^-sh z2 (the caller multiplies
 // by 2^e_k), then L[k] = sum ln(zr^2 + zi^2).
 __global__ void __launch_bounds__(THREADS, 1)
-k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntiles, int Kc,
+k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ Adata, long long N, long long ntiles, int Kc,
            const __grid_constant__ Scales sc, const __grid_constant__ Exps ex,
            const unsigned char *__restrict__ Wp, const double *__restrict__ Wd, double *__restrict__ slots)
 {
     extern __shared__ unsigned char bi8_smem_raw[];
-    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 4];
+    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 5];
     __shared__ uint32_t tmem_base_s;
-    __shared__ __align__(16) uint32_t s_emax[NEW];
+    __shared__ __align__(16) uint32_t s_emax[NEW][16];
     __shared__ __align__(16) float s_scl[128];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t raw_u32 = smem_u32(bi8_smem_raw);
     const uint32_t base = (raw_u32 + 1023u) & ~1023u;
     const uint32_t pX0 = base + OFF_X0, pX1 = base + OFF_X1, pX2 = base + OFF_X2, pX3 = base + OFF_X3;
-    const uint32_t pW = base + OFF_W, pR = base + OFF_R, stg0 = base + OFF_STG;
+    const uint32_t pW0 = base + OFF_W0, pW1 = base + OFF_W1, pR = base + OFF_R, stg0 = base + OFF_STG;
     const uint32_t b_stg_full = smem_u32(&bars[0]), b_stg_empty = b_stg_full + 8 * NSTG;
-    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24;
+    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24, b_w_full = b_a_full + 32;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTG; ++s) { mbar_init(b_stg_full + 8 * s, 1); mbar_init(b_stg_empty + 8 * s, NEW); }
-        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1);
+        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1); mbar_init(b_w_full, 1);
         fence_async_smem();
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     }
@@ -272,7 +282,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
     {                                                     // W digit planes: global image -> shared memory
         for (int i = threadIdx.x; i < 4 * PLANE / 16; i += NEW * 32) {
             const uint4 v = __ldg(reinterpret_cast<const uint4 *>(Wp) + i);
-            sts128(pW + 16u * (uint32_t)i, v.x, v.y, v.z, v.w);
+            sts128((i < PLANE / 16 ? pW0 : pW1 - PLANE) + 16u * (uint32_t)i, v.x, v.y, v.z, v.w);     // image order: W0 W1 W2 W3
         }
         fence_async_smem();
     }
@@ -355,28 +365,29 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
             if (is_mma) {
                 // ---- GEMM1: S levels t = 3..6 at TMEM columns 0, 128, 256, 384
                 mbar_wait(b_a_full, ph);
+                if (t > 0) mbar_wait(b_w_full, (uint32_t)((t - 1) & 1));      // W0 is back in its slot
                 tc_fence_after();
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 const uint32_t ko = (uint32_t)kk * 32u, acc = kk > 0 ? 1u : 0u;
                 const uint64_t a0 = desc_kmajor(pX0 + ko), a1 = desc_kmajor(pX1 + ko);
                 const uint64_t a2 = desc_kmajor(pX2 + ko), a3 = desc_kmajor(pX3 + ko);
-                const uint64_t w0 = desc_kmajor(pW + 0 * PLANE + ko), w1 = desc_kmajor(pW + 1 * PLANE + ko);
-                const uint64_t w2 = desc_kmajor(pW + 2 * PLANE + ko), w3 = desc_kmajor(pW + 3 * PLANE + ko);
+                const uint64_t w0 = desc_kmajor(pW0 + ko), w1 = desc_kmajor(pW1 + ko);
+                const uint64_t w2 = desc_kmajor(pW1 + PLANE + ko), w3 = desc_kmajor(pW1 + 2 * PLANE + ko);
                 umma_i8(tmem0 + 256, a3, w2, kI1_256, acc);        // X3 [W2 | W3] -> t = 5 | 6
-                umma_i8(tmem0 + 0,   a3, w0, kI1_256, acc);        // X3 [W0 | W1] -> t = 3 | 4
-                umma_i8(tmem0 + 0,   a2, w1, kI1_256, 1u);         // X2 [W1 | W2] -> t = 3 | 4
-                umma_i8(tmem0 + 256, a2, w3, kI1_128, 1u);         // X2 W3        -> t = 5
+                umma_i8(tmem0 + 0,   a2, w1, kI1_256, acc);        // X2 [W1 | W2] -> t = 3 | 4
                 umma_i8(tmem0 + 0,   a1, w2, kI1_256, 1u);         // X1 [W2 | W3] -> t = 3 | 4
+                umma_i8(tmem0 + 0,   a3, w0, kI1_128, 1u);         // X3 W0        -> t = 3
+                umma_i8(tmem0 + 128, a3, w1, kI1_128, 1u);         // X3 W1        -> t = 4
+                umma_i8(tmem0 + 256, a2, w3, kI1_128, 1u);         // X2 W3        -> t = 5
                 umma_i8(tmem0 + 0,   a0, w3, kI1_128, 1u);         // X0 W3        -> t = 3
             }
                 umma_commit(b_s_full);
             }
             __syncwarp();
 
-            // ---- phase 1: S levels -> |z|^2 into the running products, Rh = conj(z)/|z|^2 (fp32, stashed in TMEM), max |Rh|
+            // ---- phase 1: S levels -> |z|^2 into the running products, Rh = conj(z)/|z|^2 (fp64, stashed in TMEM), max |Rh|
             const bool valid = (t_begin + t) * TE + row < N;
-            uint32_t mymax = 0u;
             mbar_wait(b_s_full, ph);
             tc_fence_after();
 #pragma unroll
@@ -387,35 +398,36 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
                 tmem_ld8(trow + 8 * ch + 256, a5);
                 tmem_ld8(trow + 8 * ch + 384, a6);
                 tmem_ld_wait();
-                float rh[8];
+                int32_t rlo[8], rhi[8];
                 double lv[4];
 #pragma unroll
                 for (int m = 0; m < 4; ++m) {
                     // z = 2^16 y + x exactly (|y| < 2^30, |x| < 2^31)
-                    const int yr = a6[2 * m] * 256 + a5[2 * m], xr = a4[2 * m] * 256 + a3[2 * m];
-                    const int yi = a6[2 * m + 1] * 256 + a5[2 * m + 1], xi = a4[2 * m + 1] * 256 + a3[2 * m + 1];
-                    double fr = fma((double)yr, 65536.0, (double)xr), fi = fma((double)yi, 65536.0, (double)xi);
+                    double fr = yx2d(a6[2 * m] * 256 + a5[2 * m], a4[2 * m] * 256 + a3[2 * m]);
+                    double fi = yx2d(a6[2 * m + 1] * 256 + a5[2 * m + 1], a4[2 * m + 1] * 256 + a3[2 * m + 1]);
                     double I = fma(fr, fr, fi * fi);
                     const bool kvalid = valid && 16 * j + 4 * ch + m < Kc;
-                    // Strong cancellation (|z| < 2^31: the truncation of GEMM1, ~2^9 rms in these units, would
-                    // exceed ~2^-22 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37 for
-                    // typical events, so this is rare (~1e-4 of the sums) and the loop is almost never entered.
+                    // Strong cancellation (|z| < 2^33: the truncation of GEMM1, ~2^9 rms in these units, would
+                    // exceed ~2^-24 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for
+                    // typical events, so this concerns ~1.5e-3 of the sums (the ones that dominate the gradient).
                     unsigned bal = __ballot_sync(0xffffffffu, kvalid && I < 0x1p62);
                     while (bal) {
                         const int srcl = __ffs(bal) - 1;
                         bal &= bal - 1;
-                        const double2 z = recompute_z(pX1, (uint32_t)(32 * q + srcl), lane, Wd, 2 * (16 * j + 4 * ch + m));
+                        const double2 z = recompute_z(Adata + ((t_begin + t) * TE + 32 * q + srcl) * 128, lane, Wd, 2 * (16 * j + 4 * ch + m));
                         if (lane == srcl) { fr = z.x; fi = z.y; I = fma(fr, fr, fi * fi); }
                     }
                     lv[m] = kvalid ? I : 1.0;
-                    const float gr = (float)fr, gi = (float)fi;
-                    const float If = fmaf(gr, gr, gi * gi);
-                    const float inv = If > 0.0f ? rcp_approx(If) : 0.0f;
-                    const float rr = gr * inv, ri = -gi * inv;
-                    rh[2 * m] = rr; rh[2 * m + 1] = ri;
-                    mymax = max(mymax, max(__float_as_uint(rr) & 0x7fffffffu, __float_as_uint(ri) & 0x7fffffffu));
+                    const double inv = I > 0.0 ? rcp_d(I) : 0.0;
+                    const double rr = fr * inv, ri = -fi * inv;
+                    rlo[2 * m] = __double2loint(rr); rhi[2 * m] = __double2hiint(rr);
+                    rlo[2 * m + 1] = __double2loint(ri); rhi[2 * m + 1] = __double2hiint(ri);
+                    // high words of non-negative doubles order like the values: warp maximum of |Rh| of this column
+                    const unsigned mx = __reduce_max_sync(0xffffffffu, max((uint32_t)rhi[2 * m] & 0x7fffffffu, (uint32_t)rhi[2 * m + 1] & 0x7fffffffu));
+                    if (lane == 0) s_emax[warp][4 * ch + m] = mx;
                 }
-                tmem_st8f(trow + 8 * ch, rh);
+                tmem_st8i(trow + 8 * ch, rlo);                  // fp64 Rh: low words over the t = 3 columns, high words over t = 4
+                tmem_st8i(trow + 8 * ch + 128, rhi);
                 // lanes exchange so that each keeps ONE column of the chunk (m = 2 b4 + b3), multiplied over 4 lanes
                 const double send0 = b4 ? lv[0] : lv[2], send1 = b4 ? lv[1] : lv[3];
                 double keep0 = b4 ? lv[2] : lv[0], keep1 = b4 ? lv[3] : lv[1];
@@ -430,32 +442,38 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
                 Ec[ch] += e;
                 Pc[ch] = __hiloint2double(hi - (e << 20), __double2loint(P));
             }
-            mymax = __reduce_max_sync(0xffffffffu, mymax);
-            if (lane == 0) s_emax[warp] = mymax;
             tmem_st_wait();
             tc_fence_before();
             epi_bar();
 
-            // ---- phase 2: tile shift sh (max |Rh| 2^sh < 2^30), Rh -> four digit planes (R0 takes the slot of X0)
+            // ---- phase 2: shifts sh_k (max_i |Rh_ik| 2^sh_k < 2^30), Rh -> four digit planes (R0 takes the slot of W0)
             tc_fence_after();
-            uint32_t sh;
-            {
-                const uint4 e0 = *reinterpret_cast<const uint4 *>(&s_emax[0]), e1 = *reinterpret_cast<const uint4 *>(&s_emax[4]);
-                const uint4 e2 = *reinterpret_cast<const uint4 *>(&s_emax[8]), e3 = *reinterpret_cast<const uint4 *>(&s_emax[12]);
-                const uint32_t m0 = max(max(e0.x, e0.y), max(e0.z, e0.w)), m1 = max(max(e1.x, e1.y), max(e1.z, e1.w));
-                const uint32_t m2 = max(max(e2.x, e2.y), max(e2.z, e2.w)), m3 = max(max(e3.x, e3.y), max(e3.z, e3.w));
-                const uint32_t bits = max(max(m0, m1), max(m2, m3));
-                sh = bits == 0u ? 0u : (uint32_t)(29 + 127 - (int)(bits >> 23));
+            // per starting point: sh_k = 29 - floor(log2 max_i |Rh_ik|) over the tile's 128 events (4 warps), packed 8 bits each
+            uint32_t shp[4];
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                uint4 e0 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 0][4 * w]);
+                const uint4 e1 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 1][4 * w]);
+                const uint4 e2 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 2][4 * w]);
+                const uint4 e3 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 3][4 * w]);
+                e0.x = max(max(e0.x, e1.x), max(e2.x, e3.x)); e0.y = max(max(e0.y, e1.y), max(e2.y, e3.y));
+                e0.z = max(max(e0.z, e1.z), max(e2.z, e3.z)); e0.w = max(max(e0.w, e1.w), max(e2.w, e3.w));
+                auto shift_of = [](uint32_t bits) -> uint32_t { return bits == 0u ? 0u : (uint32_t)(29 + 1023 - (int)(bits >> 20)); };
+                shp[w] = shift_of(e0.x) | (shift_of(e0.y) << 8) | (shift_of(e0.z) << 16) | (shift_of(e0.w) << 24);
             }
-            const float qs = __uint_as_float((sh + 127u) << 23);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                float f[16];
-                tmem_ld16f(trow + 16 * h, f);
+                int32_t flo[16], fhi[16];
+                tmem_ld16i(trow + 16 * h, flo);
+                tmem_ld16i(trow + 16 * h + 128, fhi);
                 tmem_ld_wait();
                 uint32_t wq[16];
 #pragma unroll
-                for (int i = 0; i < 16; ++i) wq[i] = digits(__float2int_rn(f[i] * qs));
+                for (int i = 0; i < 16; ++i) {     // rint(Rh 2^sh) (|.| < 2^30) = low word of Rh 2^sh + 1.5 * 2^52
+                    const int m = 8 * h + (i >> 1);
+                    const uint32_t sh = (shp[m >> 2] >> (8 * (m & 3))) & 0xffu;
+                    wq[i] = digits(__double2loint(fma(__hiloint2double(fhi[i], flo[i]), __hiloint2double((int)((1023u + sh) << 20), 0), 6755399441055744.0)));
+                }
                 uint32_t p0[4], p1[4], p2[4], p3[4];
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
@@ -475,13 +493,14 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
             __syncwarp();
             if (lane == 0) mbar_arrive(b_r_full);
             if (is_mma) {
-                // ---- GEMM2: Q levels t = 3..6 at TMEM columns 0, 128, 256, 384 (X0 is not used: its slot holds R0)
+                // ---- GEMM2: Q levels t = 3..6 at TMEM columns 0, 128, 256, 384 (R0 sits in the slot of W0)
                 mbar_wait(b_r_full, ph);
                 tc_fence_after();
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
                 const uint32_t ko = (uint32_t)kk * 32u * 128u, acc = kk > 0 ? 1u : 0u;
-                const uint64_t a1 = desc_mnmajor(pX1 + ko), a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
+                const uint64_t a0 = desc_mnmajor(pX0 + ko), a1 = desc_mnmajor(pX1 + ko);
+                const uint64_t a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
                 const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko), r1 = desc_mnmajor(pR + 1 * PLANE + ko);
                 const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko), r3 = desc_mnmajor(pR + 3 * PLANE + ko);
                 umma_i8(tmem0 + 256, a3, r2, kI2_256, acc);        // X3^T [R2 | R3] -> t = 5 | 6
@@ -489,14 +508,19 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
                 umma_i8(tmem0 + 0,   a2, r1, kI2_256, 1u);         // X2^T [R1 | R2] -> t = 3 | 4
                 umma_i8(tmem0 + 256, a2, r3, kI2_128, 1u);         // X2^T R3        -> t = 5
                 umma_i8(tmem0 + 0,   a1, r2, kI2_256, 1u);         // X1^T [R2 | R3] -> t = 3 | 4
+                umma_i8(tmem0 + 0,   a0, r3, kI2_128, 1u);         // X0^T R3        -> t = 3
             }
                 umma_commit(b_t_full);
             }
             __syncwarp();
 
             // ---- flush: Q levels of this tile -> fp64 accumulators (row = real column c)
-            const double fs = __hiloint2double((int)((1023u - sh) << 20), 0);          // 2^-sh
             mbar_wait(b_t_full, ph);
+            if (is_tma && t + 1 < nt) {                                  // GEMM2 is done with R0: bring W0 back for the next tile
+                mbar_expect_tx(b_w_full, PLANE);
+                bulk_g2s(pW0, Wp, PLANE, b_w_full);
+            }
+            __syncwarp();
             tc_fence_after();
 #pragma unroll
             for (int ch = 0; ch < 4; ++ch) {
@@ -508,8 +532,10 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, long long N, long long ntil
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const double z = fma((double)(a6[i] * 256 + a5[i]), 65536.0, (double)(a4[i] * 256 + a3[i]));
-                    Tacc[8 * ch + i] = fma(z, fs, Tacc[8 * ch + i]);
+                    const double z = yx2d(a6[i] * 256 + a5[i], a4[i] * 256 + a3[i]);
+                    const int m = 4 * ch + (i >> 1);
+                    const uint32_t sh = (shp[m >> 2] >> (8 * (m & 3))) & 0xffu;
+                    Tacc[8 * ch + i] = fma(z, __hiloint2double((int)((1023u - sh) << 20), 0), Tacc[8 * ch + i]);
                 }
             }
             tc_fence_before();
@@ -660,7 +686,7 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
         bi8::k_bi8_prep<<<bi8::KC, 128, 0, ctx->stream>>>(ctx->d_V, ctx->n, K, k0, ex, Wp, ek, Wd);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
-        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, N, ntiles, cols, sc, ex, Wp, Wd, slots);
+        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, cols, sc, ex, Wp, Wd, slots);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
         bi8::k_bi8_finalize<<<cols, 1024, 0, ctx->stream>>>(slots, (int)grid, ctx->n, ctx->d_V, k0, ek, N, ctx->d_M,
@@ -673,5 +699,13 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
     *handled = true;
     return PWA_OK;
 }
+
+// Relative error carried by each product A_ia / S_ik that enters T on this path: S_ik is
+// exact to 2^-22 |S_ik| at worst (sums that cancel more strongly are recomputed in fp64; 2^-28 for a
+// typical event), Rh = 1 / S is then formed in fp64 and quantised 31 bits below the tile's per-column
+// maximum, X carries 31 bits below the column maximum, GEMM2 drops orders worth 2^-31.  The errors of
+// different events are independent, so the norm-wise error of the summed gradient is smaller by about
+// 1 / sqrt(N_data) (measured: 1e-7 at N = 6e3, 1e-8 at 2e5).
+double batch_i8_error_estimate(const pwa_ctx *) { return ldexp(1.0, -22) + ldexp(1.0, -30); }
 
 }  // namespace pwa

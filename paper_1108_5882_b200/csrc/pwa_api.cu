@@ -373,6 +373,15 @@ pwa_status pwa_norm_error_bound(pwa_ctx *ctx, double *bound, int32_t *which_path
     return PWA_OK;
 }
 
+pwa_status pwa_batch_path(pwa_ctx *ctx, int32_t *which_path, double *err_rel)
+{
+    if (!ctx || !which_path) return PWA_ERR_INVALID_ARG;
+    if (ctx->batch_path < 0) return fail(ctx, PWA_ERR_STATE, "no batched evaluation yet");
+    *which_path = ctx->batch_path;
+    if (err_rel) *err_rel = ctx->batch_path == 2 ? batch_i8_error_estimate(ctx) : 0.0;
+    return PWA_OK;
+}
+
 pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
 {
     if (!ctx || !M) return PWA_ERR_INVALID_ARG;

@@ -71,6 +71,7 @@ struct pwa_ctx {
     double *d_scratch = nullptr; size_t scratch_cap = 0;     // bytes (M partials, batch partials)
     double *d_H = nullptr;                                    // [2n][2n] Fumili matrix (allocated on first use)
     int last_K = 0;
+    int batch_path = -1;                                      // family of the most recent batched call (pwa_batch_path)
     // cached TMA descriptor of the DATA sample (data_term_tma.cu); rebuilt when the key changes
     struct { const void *base = nullptr; long long n_events = -1; int box_rows = 0; bool valid = false;
              alignas(64) unsigned char map[128]; } tmap_cache;
@@ -108,6 +109,7 @@ double norm_i8_error_bound(const pwa_ctx *ctx);
 pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, int D, int *exp, float *scale,
                             double *cmax, bool *valid);    // norm_i8.cu
 pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled);   // batch_i8.cu
+double batch_i8_error_estimate(const pwa_ctx *ctx);               // batch_i8.cu
 pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
 

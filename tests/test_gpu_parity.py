@@ -373,6 +373,100 @@ def test_norm_i8_default_path_and_nonfinite(pwa, oracle):
         assert pwa.pwa_norm_error_bound(c.ctx)[1] == 0
 
 
+# ------------------------------------------------------------------ NEXT-1 (A8): batched evaluation on the int8 tensor cores
+@pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (6007, 64), (6007, 70), (40_001, 33)])
+def test_batch_i8_parity(pwa, oracle, N, K):
+    """fp32 storage, n = 64, option "batch" = 2: both chained GEMMs on tcgen05 int8 (batch_i8.cu) against the
+    oracle and against the FP64 DMMA path: less than one tile, a ragged last tile, K < 64, K > 64 (two passes),
+    columns with very different amplitude scales and starting points with very different norms."""
+    n = 64
+    rng = np.random.default_rng(1000 + N + K)
+    A = (rng.normal(size=(N, n, 2)) * rng.uniform(0.01, 3.0, size=(1, n, 2))).astype(np.float32)
+    B = A[: min(N, 2003)]
+    Vk = rng.normal(size=(K, n, 2)) * rng.uniform(0.05, 20.0, size=(K, 1, 1))
+    M_o = oracle.norm_matrix(B, len(B) + 5)
+    nll_o, g_o, parts_o, _ = oracle.nll_grad_batch(A, M_o, Vk)
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=len(B) + 5)
+        pwa.pwa_build_norm(c.ctx)
+        pwa.pwa_set_option(c.ctx, "batch", 2)
+        nll, g, parts = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        path, err = pwa.pwa_batch_path(c.ctx)
+        assert path == 2 and 0.0 < err < 1e-6
+        pwa.pwa_set_option(c.ctx, "batch", 1)
+        nll1, g1, parts1 = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx) == (1, 0.0)
+        for k in range(K):
+            check_eval((nll[k], g[k], parts[k]), (nll_o[k], g_o[k], parts_o[k]), TOL["f32"], N)
+            check_eval((nll[k], g[k], parts[k]), (nll1[k], g1[k], parts1[k]), TOL["f32"], N)
+        # the same call twice gives bitwise the same numbers (fixed slots, fixed summation order)
+        pwa.pwa_set_option(c.ctx, "batch", 2)
+        nll2, g2, _ = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert np.array_equal(nll, nll2) and np.array_equal(g, g2)
+
+
+def test_batch_i8_strong_cancellation(pwa, oracle):
+    """Events whose coherent sum nearly vanishes for some starting points (|S| ~ 1e-6 of the typical sum):
+    the truncated integer GEMM alone would lose them, the fp64 recomputation (recompute_z) keeps the 1e-6 bar.
+    Such events dominate the gradient (t_ia = A_ia / S_i), so a wrong S_i fails the comparison at once."""
+    n, N, K = 64, 3001, 9
+    rng = np.random.default_rng(77)
+    A = rng.normal(size=(N, n, 2)) * 0.5
+    Vk = rng.normal(size=(K, n, 2))
+    Ac = A[..., 0] + 1j * A[..., 1]
+    for k, i in ((0, 5), (0, 1500), (3, 2999), (8, 128)):
+        Vc = Vk[k, :, 0] + 1j * Vk[k, :, 1]
+        S = Ac[i] @ Vc
+        Ac[i] -= (1.0 - 1e-6) * S * Vc.conj() / (np.abs(Vc) ** 2).sum()       # leaves S_i = 1e-6 of its old value
+    A = np.stack([Ac.real, Ac.imag], axis=-1).astype(np.float32)
+    M_o = oracle.norm_matrix(A[:1000], 1000)
+    nll_o, g_o, parts_o, _ = oracle.nll_grad_batch(A, M_o, Vk)
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_set_option(c.ctx, "batch", 2)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, A[:1000], n_generated=1000)
+        pwa.pwa_build_norm(c.ctx)
+        nll, g, parts = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 2
+        for k in range(K):
+            check_eval((nll[k], g[k], parts[k]), (nll_o[k], g_o[k], parts_o[k]), TOL["f32"], N)
+
+
+def test_batch_i8_selection_and_nonfinite(pwa, oracle):
+    """Default selection (K >= 8, >= 32768 events, fp32, n = 64, no weights); a zero event gives L = -inf;
+    a non-finite starting point is rejected by the ABI; inf in the sample or event weights fall back to the
+    FP64 / streaming paths."""
+    n, N = 64, 33_000
+    rng = np.random.default_rng(9)
+    A = (rng.normal(size=(N, n, 2)) * 0.35).astype(np.float32)
+    Vk = rng.normal(size=(8, n, 2))
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, A[:1000], n_generated=1000)
+        pwa.pwa_build_norm(c.ctx)
+        ref = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 2
+        pwa.pwa_nll_grad_batch(c.ctx, Vk[:7])
+        assert pwa.pwa_batch_path(c.ctx)[0] == 0            # K < 8: streaming passes
+        Vn = Vk.copy(); Vn[2, 5, 1] = np.nan
+        with pytest.raises(pwa.PwaError):                   # the ABI rejects non-finite V before any launch
+            pwa.pwa_nll_grad_batch(c.ctx, Vn)
+        again = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert np.array_equal(again[0], ref[0]) and np.array_equal(again[1], ref[1])
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, np.ones(N))
+        pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 0            # weighted sample: weighted streaming kernel
+        A0 = A.copy(); A0[31_999] = 0.0
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A0)
+        nll, g, parts = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 2 and np.all(parts[:, 0] == -math.inf) and np.all(nll == math.inf)
+        A0[17, 3, 0] = np.inf
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A0)
+        pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 1            # inf in the sample: FP64 DMMA path propagates IEEE values
+
+
 # ------------------------------------------------------------------ NEXT-4: eq. 2 (normalised) likelihood form on the device
 @pytest.mark.parametrize("storage,n,K", [("f64", 4, 3), ("f64", 16, 5), ("f32", 32, 4), ("f32", 64, 33), ("f64", 5, 2)])
 def test_eq2_likelihood_mode(pwa, oracle, storage, n, K):

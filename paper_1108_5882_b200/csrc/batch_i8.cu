@@ -152,6 +152,9 @@ constexpr uint32_t idesc(uint32_t N, bool mn_major)
 constexpr uint32_t kI1_128 = idesc(128, false), kI1_256 = idesc(256, false);   // GEMM1: both operands K-major
 constexpr uint32_t kI2_128 = idesc(128, true),  kI2_256 = idesc(256, true);    // GEMM2: both operands MN-major
 
+// int32 -> double on the fp64 pipe (the 64-bit conversion unit is 4x slower): the integer lands in the low
+// mantissa bits of 2^52 + 2^31 + v (exact), one fp64 subtraction removes the offset.
+__device__ __forceinline__ double i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
 // 2^16 y + x (|.| < 2^51) as a double, exactly: 64-bit integer arithmetic, the result lands in the mantissa of 1.5 * 2^52
 __device__ __forceinline__ double yx2d(int y, int x)
 {
@@ -261,6 +264,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
     __shared__ __align__(8) unsigned long long bars[2 * NSTG + 5];
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) uint32_t s_emax[NEW][16];
+    __shared__ __align__(16) uint32_t s_sh[KC];            // sh_k << 20 of the current tile
     __shared__ __align__(16) float s_scl[128];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -399,27 +403,47 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 tmem_ld8(trow + 8 * ch + 384, a6);
                 tmem_ld_wait();
                 int32_t rlo[8], rhi[8];
-                double lv[4];
+                double fr[4], fi[4], I[4];
+                bool cancel = false;
 #pragma unroll
                 for (int m = 0; m < 4; ++m) {
                     // z = 2^16 y + x exactly (|y| < 2^30, |x| < 2^31)
-                    double fr = yx2d(a6[2 * m] * 256 + a5[2 * m], a4[2 * m] * 256 + a3[2 * m]);
-                    double fi = yx2d(a6[2 * m + 1] * 256 + a5[2 * m + 1], a4[2 * m + 1] * 256 + a3[2 * m + 1]);
-                    double I = fma(fr, fr, fi * fi);
-                    const bool kvalid = valid && 16 * j + 4 * ch + m < Kc;
-                    // Strong cancellation (|z| < 2^33: the truncation of GEMM1, ~2^9 rms in these units, would
-                    // exceed ~2^-24 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for
-                    // typical events, so this concerns ~1.5e-3 of the sums (the ones that dominate the gradient).
-                    unsigned bal = __ballot_sync(0xffffffffu, kvalid && I < 0x1p62);
-                    while (bal) {
-                        const int srcl = __ffs(bal) - 1;
-                        bal &= bal - 1;
-                        const double2 z = recompute_z(Adata + ((t_begin + t) * TE + 32 * q + srcl) * 128, lane, Wd, 2 * (16 * j + 4 * ch + m));
-                        if (lane == srcl) { fr = z.x; fi = z.y; I = fma(fr, fr, fi * fi); }
+                    fr[m] = fma(i2d(a6[2 * m] * 256 + a5[2 * m]), 65536.0, i2d(a4[2 * m] * 256 + a3[2 * m]));
+                    fi[m] = fma(i2d(a6[2 * m + 1] * 256 + a5[2 * m + 1]), 65536.0, i2d(a4[2 * m + 1] * 256 + a3[2 * m + 1]));
+                    I[m] = fma(fr[m], fr[m], fi[m] * fi[m]);
+                    cancel |= I[m] < 0x1p62 && 16 * j + 4 * ch + m < Kc;
+                }
+                // Strong cancellation (|z| < 2^31: the truncation of GEMM1, ~2^9 rms in these units, would exceed
+                // ~2^-22 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for typical
+                // events, so this concerns ~1e-4 of the sums (the ones that dominate the gradient): one vote per
+                // chunk, the branch is almost never taken.
+                if (__any_sync(0xffffffffu, cancel && valid)) {
+#pragma unroll 1
+                    for (int m = 0; m < 4; ++m) {
+                        if (16 * j + 4 * ch + m >= Kc) break;
+                        const double Im = m == 0 ? I[0] : m == 1 ? I[1] : m == 2 ? I[2] : I[3];
+                        unsigned bal = __ballot_sync(0xffffffffu, valid && Im < 0x1p62);
+                        while (bal) {
+                            const int srcl = __ffs(bal) - 1;
+                            bal &= bal - 1;
+                            const double2 z = recompute_z(Adata + ((t_begin + t) * TE + 32 * q + srcl) * 128, lane, Wd, 2 * (16 * j + 4 * ch + m));
+                            if (lane == srcl) {
+                                const double In = fma(z.x, z.x, z.y * z.y);
+                                if (m == 0) { fr[0] = z.x; fi[0] = z.y; I[0] = In; }
+                                else if (m == 1) { fr[1] = z.x; fi[1] = z.y; I[1] = In; }
+                                else if (m == 2) { fr[2] = z.x; fi[2] = z.y; I[2] = In; }
+                                else { fr[3] = z.x; fi[3] = z.y; I[3] = In; }
+                            }
+                        }
                     }
-                    lv[m] = kvalid ? I : 1.0;
-                    const double inv = I > 0.0 ? rcp_d(I) : 0.0;
-                    const double rr = fr * inv, ri = -fi * inv;
+                }
+                double lv[4];
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    const bool kvalid = valid && 16 * j + 4 * ch + m < Kc;
+                    lv[m] = kvalid ? I[m] : 1.0;
+                    const double inv = I[m] > 0.0 ? rcp_d(I[m]) : 0.0;
+                    const double rr = fr[m] * inv, ri = -fi[m] * inv;
                     rlo[2 * m] = __double2loint(rr); rhi[2 * m] = __double2hiint(rr);
                     rlo[2 * m + 1] = __double2loint(ri); rhi[2 * m + 1] = __double2hiint(ri);
                     // high words of non-negative doubles order like the values: warp maximum of |Rh| of this column
@@ -448,18 +472,18 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
 
             // ---- phase 2: shifts sh_k (max_i |Rh_ik| 2^sh_k < 2^30), Rh -> four digit planes (R0 takes the slot of W0)
             tc_fence_after();
-            // per starting point: sh_k = 29 - floor(log2 max_i |Rh_ik|) over the tile's 128 events (4 warps), packed 8 bits each
-            uint32_t shp[4];
+            // per starting point: sh_k = 29 - floor(log2 max_i |Rh_ik|) over the tile's 128 events (4 warps), kept as sh_k << 20
+            if (threadIdx.x < KC) {
+                const int jj = threadIdx.x >> 4, mm = threadIdx.x & 15;
+                const uint32_t bits = max(max(s_emax[4 * jj][mm], s_emax[4 * jj + 1][mm]), max(s_emax[4 * jj + 2][mm], s_emax[4 * jj + 3][mm]));
+                s_sh[threadIdx.x] = bits == 0u ? 0u : (uint32_t)(29 + 1023 - (int)(bits >> 20)) << 20;
+            }
+            epi_bar();
+            uint32_t sh20[16];
 #pragma unroll
             for (int w = 0; w < 4; ++w) {
-                uint4 e0 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 0][4 * w]);
-                const uint4 e1 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 1][4 * w]);
-                const uint4 e2 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 2][4 * w]);
-                const uint4 e3 = *reinterpret_cast<const uint4 *>(&s_emax[4 * j + 3][4 * w]);
-                e0.x = max(max(e0.x, e1.x), max(e2.x, e3.x)); e0.y = max(max(e0.y, e1.y), max(e2.y, e3.y));
-                e0.z = max(max(e0.z, e1.z), max(e2.z, e3.z)); e0.w = max(max(e0.w, e1.w), max(e2.w, e3.w));
-                auto shift_of = [](uint32_t bits) -> uint32_t { return bits == 0u ? 0u : (uint32_t)(29 + 1023 - (int)(bits >> 20)); };
-                shp[w] = shift_of(e0.x) | (shift_of(e0.y) << 8) | (shift_of(e0.z) << 16) | (shift_of(e0.w) << 24);
+                const uint4 v = *reinterpret_cast<const uint4 *>(&s_sh[16 * j + 4 * w]);
+                sh20[4 * w] = v.x; sh20[4 * w + 1] = v.y; sh20[4 * w + 2] = v.z; sh20[4 * w + 3] = v.w;
             }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -469,11 +493,8 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 tmem_ld_wait();
                 uint32_t wq[16];
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {     // rint(Rh 2^sh) (|.| < 2^30) = low word of Rh 2^sh + 1.5 * 2^52
-                    const int m = 8 * h + (i >> 1);
-                    const uint32_t sh = (shp[m >> 2] >> (8 * (m & 3))) & 0xffu;
-                    wq[i] = digits(__double2loint(fma(__hiloint2double(fhi[i], flo[i]), __hiloint2double((int)((1023u + sh) << 20), 0), 6755399441055744.0)));
-                }
+                for (int i = 0; i < 16; ++i)       // rint(Rh 2^sh) (|.| < 2^30) = low word of Rh 2^sh + 1.5 * 2^52; 2^sh goes into the exponent
+                    wq[i] = digits(__double2loint(__hiloint2double(fhi[i] + (int)sh20[8 * h + (i >> 1)], flo[i]) + 6755399441055744.0));
                 uint32_t p0[4], p1[4], p2[4], p3[4];
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
@@ -524,6 +545,8 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
             tc_fence_after();
 #pragma unroll
             for (int ch = 0; ch < 4; ++ch) {
+                const uint4 shv = *reinterpret_cast<const uint4 *>(&s_sh[16 * j + 4 * ch]);
+                const uint32_t shc[4] = {shv.x, shv.y, shv.z, shv.w};
                 int32_t a3[8], a4[8], a5[8], a6[8];
                 tmem_ld8(trow + 8 * ch + 0, a3);
                 tmem_ld8(trow + 8 * ch + 128, a4);
@@ -532,10 +555,10 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const double z = yx2d(a6[i] * 256 + a5[i], a4[i] * 256 + a3[i]);
-                    const int m = 4 * ch + (i >> 1);
-                    const uint32_t sh = (shp[m >> 2] >> (8 * (m & 3))) & 0xffu;
-                    Tacc[8 * ch + i] = fma(z, __hiloint2double((int)((1023u - sh) << 20), 0), Tacc[8 * ch + i]);
+                    // z 2^-sh with z = 2^16 y + x: two exact int -> fp64 conversions, two fused accumulations
+                    const int fsh = (int)((1023u << 20) - shc[i >> 1]);
+                    const double acc = fma(i2d(a4[i] * 256 + a3[i]), __hiloint2double(fsh, 0), Tacc[8 * ch + i]);
+                    Tacc[8 * ch + i] = fma(i2d(a6[i] * 256 + a5[i]), __hiloint2double(fsh + (16 << 20), 0), acc);
                 }
             }
             tc_fence_before();

@@ -290,9 +290,20 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
         if w.K > 1:
             Vk = synth.eval_points(w, w.K, stream=synth.S_START)
             ms_b, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
+            path, err_rel = pwa.pwa_batch_path(ctx)
             out["batch"] = {"K": w.K, "ms_per_call": ms_b, "evals_per_s": w.K / ms_b * 1e3,
                             "event_waves_per_s": w.n_data * n * w.K / ms_b * 1e3,
-                            "gflops": 16.0 * w.n_data * n * w.K / ms_b * 1e-6}
+                            "gflops": 16.0 * w.n_data * n * w.K / ms_b * 1e-6,
+                            "path": {0: "K streaming passes", 1: "fp64 DMMA chained GEMMs",
+                                     2: "int8 tcgen05 chained GEMMs (digit planes, int32 TMEM)"}[path],
+                            "per_term_error_estimate": err_rel}
+            if path == 2:
+                # 20 digit-pair products of 128 x 128 x 128 int8 MACs per 128-event tile (10 per GEMM)
+                out["batch"]["int8_tops"] = 2.0 * 128 * 128 * 20 * w.n_data / ms_b * 1e-9
+                pwa.pwa_set_option(ctx, "batch", 1)
+                ms_d, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
+                pwa.pwa_set_option(ctx, "batch", 0)
+                out["batch"]["ms_per_call_fp64_dmma"] = ms_d
             # NEXT-3: the same evaluation with per-event weights (per-lane streaming kernel + 8 B/event weight stream)
             wts = np.random.default_rng(7).uniform(0.5, 1.5, size=w.n_data)
             pwa.pwa_set_weights(ctx, pwa.PWA_DATA, wts)

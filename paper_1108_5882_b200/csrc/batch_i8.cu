@@ -256,7 +256,7 @@ __device__ __noinline__ double2 recompute_z(const float *__restrict__ arow, int 
 // slots: [gridDim.x][SLOT] doubles: Q[col][c] = 2^(-8 - s_c) sum_tiles 2^-sh z2 (the caller multiplies
 // by 2^e_k), then L[k] = sum ln(zr^2 + zi^2).
 __global__ void __launch_bounds__(THREADS, 1)
-k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ Adata, long long N, long long ntiles, int Kc,
+k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ Adata, long long N, long long ntiles, int Kc, double thr2,
            const __grid_constant__ Scales sc, const __grid_constant__ Exps ex,
            const unsigned char *__restrict__ Wp, const double *__restrict__ Wd, double *__restrict__ slots)
 {
@@ -411,7 +411,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                     fr[m] = fma(i2d(a6[2 * m] * 256 + a5[2 * m]), 65536.0, i2d(a4[2 * m] * 256 + a3[2 * m]));
                     fi[m] = fma(i2d(a6[2 * m + 1] * 256 + a5[2 * m + 1]), 65536.0, i2d(a4[2 * m + 1] * 256 + a3[2 * m + 1]));
                     I[m] = fma(fr[m], fr[m], fi[m] * fi[m]);
-                    cancel |= I[m] < 0x1p62 && 16 * j + 4 * ch + m < Kc;
+                    cancel |= I[m] < thr2 && 16 * j + 4 * ch + m < Kc;
                 }
                 // Strong cancellation (|z| < 2^31: the truncation of GEMM1, ~2^9 rms in these units, would exceed
                 // ~2^-22 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for typical
@@ -422,7 +422,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                     for (int m = 0; m < 4; ++m) {
                         if (16 * j + 4 * ch + m >= Kc) break;
                         const double Im = m == 0 ? I[0] : m == 1 ? I[1] : m == 2 ? I[2] : I[3];
-                        unsigned bal = __ballot_sync(0xffffffffu, valid && Im < 0x1p62);
+                        unsigned bal = __ballot_sync(0xffffffffu, valid && Im < thr2);
                         while (bal) {
                             const int srcl = __ffs(bal) - 1;
                             bal &= bal - 1;
@@ -664,7 +664,15 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
     if (ctx->storage != PWA_F32 || ctx->data.factored || ctx->n != 64 || ctx->data.weights != nullptr || N <= 0 ||
         ((uintptr_t)ctx->data.amps & 15u) != 0 || N > 0x7fffffffLL - 2 * bi8::TE)
         return PWA_OK;
-    if (ctx->opt_batch != 2 && !(ctx->opt_batch == 0 && K >= 8 && N >= 32768)) return PWA_OK;
+    if (ctx->opt_batch != 2 && ctx->opt_batch != 3 && !(ctx->opt_batch == 0 && K >= 8 && N >= 32768)) return PWA_OK;
+    // Cancellation guard: recompute S_ik in fp64 when |z|^2 < thr2.  The truncation of GEMM1 is ~2^9 rms in the units
+    // of z; an event's term t = A / S has the share ~8 typ / (N |z|) of the gradient sum (typ <= 2^38: typical |z|,
+    // 1/8: coherence of the sum), so its error contributes ~2^12 typ / (N |z|^2) to the norm-wise gradient error.
+    // Keeping every single contribution below 1e-8 needs |z|^2 >= 2^76.6 / N; clamped to [2^52, 2^66] (at the upper
+    // end ~1e-3 of the sums are recomputed).  "batch" = 3: experiment switch, no guard (timing only).
+    double thr2 = ldexp(1.0, 77) / (double)N;
+    thr2 = fmin(fmax(thr2, 0x1p52), 0x1p66);
+    if (ctx->opt_batch == 3) thr2 = 0.0;
     auto &q = ctx->i8d;
     if (!q.checked) {
         pwa_status s = i8_column_scales(ctx, ctx->data.amps, N, 128, q.exp, q.scale, q.cmax, &q.valid);
@@ -709,7 +717,7 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
         bi8::k_bi8_prep<<<bi8::KC, 128, 0, ctx->stream>>>(ctx->d_V, ctx->n, K, k0, ex, Wp, ek, Wd);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
-        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, cols, sc, ex, Wp, Wd, slots);
+        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, cols, thr2, sc, ex, Wp, Wd, slots);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
         bi8::k_bi8_finalize<<<cols, 1024, 0, ctx->stream>>>(slots, (int)grid, ctx->n, ctx->d_V, k0, ek, N, ctx->d_M,

@@ -103,6 +103,9 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V, int32_t m
     };
     pwa_status s = eval();
     if (s != PWA_OK) return s;
+    // the K fits are independent: their O(d^2) updates run on the host cores in parallel (the results do not
+    // depend on the thread count: every fit is handled by exactly one thread)
+#pragma omp parallel for schedule(static) if (K >= 4)
     for (int k = 0; k < K; ++k) {
         fit[k].init(d, X.data() + (size_t)k * d);
         fit[k].f = F[k];
@@ -119,6 +122,7 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V, int32_t m
         if (!any) break;
         s = eval();
         if (s != PWA_OK) return s;
+#pragma omp parallel for schedule(static) if (K >= 4)
         for (int k = 0; k < K; ++k) {
             if (fit[k].done) continue;
             memcpy(fit[k].gt.data(), Gr.data() + (size_t)k * d, sizeof(double) * d);

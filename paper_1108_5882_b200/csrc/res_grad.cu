@@ -83,6 +83,80 @@ k_res_grad(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs fa)
     block_finish(s_tot, &s_acc[0][0], sV, fa);
 }
 
+// Same sums for n_res <= NR, n_ang <= NA (configs[3]: 8 resonances x 2 angular structures): every Breit-Wigner is
+// evaluated once per event and kept in registers, the per-resonance sums U_r stay in per-thread fp64 registers for
+// the thread's whole event range and meet the warp / block tree only once at the end (the generic kernel above
+// pays two warp reductions per resonance and event round).  fp64-ALU bound: ~450 fp64 instructions per event.
+template <typename ST, int NR, int NA>
+__global__ void __launch_bounds__(RG_THREADS)
+k_res_grad_fast(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs fa)
+{
+    constexpr int NWARPS = RG_THREADS / 32;
+    __shared__ double sV[2 * kMaxFastWaves];
+    __shared__ double2 sC[NR * NA];
+    __shared__ double s_acc[NWARPS][2 + 2 * NR];
+    __shared__ double s_tot[2 + 2 * kMaxRes];
+    __shared__ double s_red[RG_THREADS];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_res = f.n_res, n_ang = f.n_ang, NC = 2 + 2 * n_res;
+    for (int t = tid; t < 2 * n; t += RG_THREADS) sV[t] = varg.v[t];
+    __syncthreads();
+    for (int t = tid; t < NR * NA; t += RG_THREADS) {
+        const int r = t / NA, sg = t % NA;
+        const int w = (r < n_res && sg < n_ang) ? f.wave_of_pair[r * kMaxAng + sg] : -1;
+        sC[t] = (w >= 0) ? make_double2(sV[2 * w], sV[2 * w + 1]) : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    double ur[NR], ui[NR];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) { ur[r] = 0.0; ui[r] = 0.0; }
+    const long long stride = (long long)gridDim.x * RG_THREADS;
+    for (long long i = (long long)blockIdx.x * RG_THREADS + tid; i < N; i += stride) {
+        const double m = __ldg(f.mass + i), mm = m * m;
+        double2 z[NA];
+#pragma unroll
+        for (int sg = 0; sg < NA; ++sg) z[sg] = (sg < n_ang) ? load_ang<ST>(f.ang, i, n_ang, sg) : make_double2(0.0, 0.0);
+        double pr[NR], pi[NR];                   // w_r BW_r^2
+        double sr = 0.0, si = 0.0;
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            const double2 bw = r < n_res ? bw_eval_fast(mm, f.rp.m2[r], f.rp.mg[r]) : make_double2(0.0, 0.0);
+            double wr = 0.0, wi = 0.0;
+#pragma unroll
+            for (int sg = 0; sg < NA; ++sg) {
+                const double2 c = sC[r * NA + sg];
+                wr = fma(c.x, z[sg].x, wr); wr = fma(-c.y, z[sg].y, wr);
+                wi = fma(c.x, z[sg].y, wi); wi = fma(c.y, z[sg].x, wi);
+            }
+            const double tr = bw.x * wr - bw.y * wi, ti = bw.x * wi + bw.y * wr;   // w BW
+            sr += tr; si += ti;
+            pr[r] = tr * bw.x - ti * bw.y; pi[r] = tr * bw.y + ti * bw.x;           // w BW^2
+        }
+        double fr, fi;
+        if (mode == 0) { const double inv = 1.0 / (sr * sr + si * si); fr = sr * inv; fi = -si * inv; }
+        else           { fr = sr; fi = -si; }
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            ur[r] = fma(pr[r], fr, ur[r]); ur[r] = fma(-pi[r], fi, ur[r]);
+            ui[r] = fma(pr[r], fi, ui[r]); ui[r] = fma(pi[r], fr, ui[r]);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+        const double a = warp_sum(ur[r]), b = warp_sum(ui[r]);
+        if (lane == 0) { s_acc[warp][2 + 2 * r] = a; s_acc[warp][3 + 2 * r] = b; }
+    }
+    if (lane == 0) { s_acc[warp][0] = 0.0; s_acc[warp][1] = 0.0; }
+    __syncthreads();
+    for (int c = tid; c < NC; c += RG_THREADS) {
+        double t = 0.0;
+        for (int w = 0; w < NWARPS; ++w) t += s_acc[w][c];
+        s_tot[c] = t;
+    }
+    __syncthreads();
+    block_finish(s_tot, s_red, sV, fa);
+}
+
 static pwa_status run_pass(pwa_ctx *ctx, const Sample &smp, int mode, const VArg &varg, double *out_dev)
 {
     FactArgs f;
@@ -98,8 +172,14 @@ static pwa_status run_pass(pwa_ctx *ctx, const Sample &smp, int mode, const VArg
     if (s != PWA_OK) return s;
     FinishArgs fa;
     fa.partials = ctx->d_partials; fa.ticket = ctx->d_ticket; fa.M = nullptr; fa.out = out_dev; fa.n = ctx->n_res;
-    if (ctx->storage == PWA_F32) k_res_grad<float><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
-    else                         k_res_grad<double><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
+    const bool fast = ctx->n_res <= 8 && smp.n_ang <= 2 && ctx->opt_data_term != 99;
+    if (fast) {
+        if (ctx->storage == PWA_F32) k_res_grad_fast<float, 8, 2><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
+        else                         k_res_grad_fast<double, 8, 2><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
+    } else {
+        if (ctx->storage == PWA_F32) k_res_grad<float><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
+        else                         k_res_grad<double><<<(unsigned)grid, RG_THREADS, 0, ctx->stream>>>(N, mode, ctx->n, varg, f, fa);
+    }
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;

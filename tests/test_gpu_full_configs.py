@@ -106,11 +106,19 @@ def test_cfg4_full(pwa, oracle, synth):
         M = pwa.pwa_build_norm(c.ctx)
         check_M_sampled(oracle, M, w.A_mc, w.n_gen, tol)
         nll, g, parts = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 2          # the launch configuration bench.py times: int8 tcgen05 chained GEMMs
         assert np.isfinite(nll).all() and np.isfinite(g).all()
         for k in (0, 21, 63):
             ref = oracle_eval_explicit(oracle, w.A_data, w.A_mc, w.n_gen, Vk[k])
             check_eval((nll[k], g[k], parts[k]), ref, tol, w.n_data)
             check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol, w.n_data)
+        # all 64 columns against the FP64 DMMA path (independent kernel family) at a 10x tighter bar
+        pwa.pwa_set_option(c.ctx, "batch", 1)
+        nll1, g1, parts1 = pwa.pwa_nll_grad_batch(c.ctx, Vk)
+        pwa.pwa_set_option(c.ctx, "batch", 0)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 1
+        for k in range(w.K):
+            check_eval((nll[k], g[k], parts[k]), (nll1[k], g1[k], parts1[k]), 0.1 * tol, w.n_data)
         # every batched column agrees with the streaming kernel at the same point (property at any size)
         for k in range(0, w.K, 7):
             check_eval((nll[k], g[k], parts[k]), pwa.pwa_nll_grad(c.ctx, Vk[k]), tol, w.n_data)

@@ -213,6 +213,18 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V_inout, int
                                    double gtol, double *nll_out /* [K] */,
                                    int32_t *n_evals_out);
 
+/* Floating-resonance fit (configs[3]; with floating masses and widths nothing can be pre-calculated, so
+ * EVERY evaluation re-evaluates the Breit-Wigner factors and rebuilds M): BFGS over the 2 n_waves Cartesian reals
+ * of V and the masses and widths of the n_free resonances listed in free_res (HOST int32 [n_free], distinct
+ * indices in [0, n_res)).  One evaluation = pwa_set_resonances + pwa_build_norm + pwa_nll_grad + pwa_res_grad
+ * (four passes: MC Gram, data term, and the two resonance-gradient passes).  V_inout: HOST [n][2]; mass_inout,
+ * width_inout: HOST [n_res], all resonances (the fixed ones are read, the free ones updated).  A trial point with a
+ * non-positive mass or width is rejected by the line search.  Needs factored DATA and MC uploads and a wave map.
+ * nll_out, n_iter_out, n_evals_out may be NULL.                                                             */
+pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V_inout, double *mass_inout, double *width_inout,
+                                      int32_t n_res, const int32_t *free_res, int32_t n_free, int32_t max_iter,
+                                      double gtol, double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out);
+
 /* ---- introspection / measurement ------------------------------------------------------- */
 
 /* n_waves the context was created with.                                                  */

@@ -30,7 +30,7 @@ SYMBOLS = [
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
     "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
-    "pwa_batch_path",
+    "pwa_batch_path", "pwa_minimize_bfgs_floating",
 ]
 
 
@@ -80,6 +80,8 @@ def _load():
         "pwa_set_weights": (C.c_int, [vp, C.c_int, vp, u32]),
         "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
         "pwa_batch_path": (C.c_int, [vp, C.POINTER(i32), dp]),
+        "pwa_minimize_bfgs_floating": (C.c_int, [vp, vp, vp, vp, i32, vp, i32, i32, C.c_double, dp,
+                                                 C.POINTER(i32), C.POINTER(i32)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)          # AttributeError here = header/library mismatch
@@ -340,6 +342,20 @@ def pwa_minimize_bfgs_batch(ctx, V0, max_iter=300, gtol=1e-6):
     st = _check(ctx, _lib.pwa_minimize_bfgs_batch(ctx, K, V.ctypes.data, int(max_iter), float(gtol),
                                                   nll.ctypes.data, C.byref(ev)))
     return V, nll, ev.value, st
+
+
+def pwa_minimize_bfgs_floating(ctx, V0, mass0, width0, free_res, max_iter=200, gtol=1e-6):
+    """-> (V, mass, width, nll, iterations, evaluations, status): BFGS over V and the masses / widths of free_res."""
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V0, (n, 2)).copy()
+    Mr, Gr = _f64(mass0).copy(), _f64(width0).copy()
+    fr = np.ascontiguousarray(free_res, dtype=np.int32)
+    nll = C.c_double(0.0)
+    it, ev = C.c_int32(0), C.c_int32(0)
+    st = _check(ctx, _lib.pwa_minimize_bfgs_floating(ctx, V.ctypes.data, Mr.ctypes.data, Gr.ctypes.data, len(Mr),
+                                                     fr.ctypes.data, len(fr), int(max_iter), float(gtol),
+                                                     C.byref(nll), C.byref(it), C.byref(ev)))
+    return V, Mr, Gr, nll.value, it.value, ev.value, st
 
 
 def pwa_launch_count(ctx):

@@ -137,4 +137,85 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V, int32_t m
     return worst;
 }
 
+pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V, double *mass, double *width, int32_t n_res,
+                                      const int32_t *free_res, int32_t n_free, int32_t max_iter, double gtol,
+                                      double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out)
+{
+    if (!ctx || !V || !mass || !width || n_res < 1 || n_res > 64 || n_free < 0 || n_free > n_res || (n_free > 0 && !free_res) || max_iter < 0)
+        return PWA_ERR_INVALID_ARG;
+    for (int i = 0; i < n_free; ++i) {
+        if (free_res[i] < 0 || free_res[i] >= n_res) return PWA_ERR_INVALID_ARG;
+        for (int j = 0; j < i; ++j) if (free_res[j] == free_res[i]) return PWA_ERR_INVALID_ARG;
+    }
+    const int n = pwa_n_waves(ctx), d = 2 * n + 2 * n_free;
+    // parameter vector: [Re V_0, Im V_0, ..., M_free[0..], G_free[0..]], minimised in SCALED variables u = x / sc:
+    // sc = 1 for V, 1 % of the starting mass, 2 % of the starting width (the first step, normalised to |du| = 1,
+    // then moves a resonance by at most ~1 %: an unscaled unit step would throw it across its neighbours, and the
+    // likelihood has one local minimum per assignment of resonances to peaks)
+    std::vector<double> x(d), u(d), sc(d, 1.0), g(d), Mr(mass, mass + n_res), Gr(width, width + n_res), dM(n_res), dG(n_res);
+    memcpy(x.data(), V, sizeof(double) * 2 * n);
+    for (int i = 0; i < n_free; ++i) {
+        x[2 * n + i] = mass[free_res[i]]; x[2 * n + n_free + i] = width[free_res[i]];
+        sc[2 * n + i] = 0.01 * fabs(mass[free_res[i]]); sc[2 * n + n_free + i] = 0.02 * fabs(width[free_res[i]]);
+        if (!(sc[2 * n + i] > 0.0) || !(sc[2 * n + n_free + i] > 0.0)) return PWA_ERR_INVALID_ARG;
+    }
+    for (int i = 0; i < d; ++i) u[i] = x[i] / sc[i];
+    int32_t evals = 0;
+    pwa_status worst = PWA_OK;
+    // f(x), grad f(x); returns +inf for a non-physical trial point (the line search backs off)
+    auto eval = [&](const double *uu, double *f, double *gg) -> pwa_status {
+        std::vector<double> xv(d);
+        for (int i = 0; i < d; ++i) xv[i] = uu[i] * sc[i];
+        const double *xx = xv.data();
+        for (int i = 0; i < n_free; ++i) {
+            Mr[free_res[i]] = xx[2 * n + i]; Gr[free_res[i]] = xx[2 * n + n_free + i];
+            if (!(Mr[free_res[i]] > 0.0) || !(Gr[free_res[i]] > 0.0)) { *f = INFINITY; return PWA_OK; }
+        }
+        pwa_status s = pwa_set_resonances(ctx, Mr.data(), Gr.data());
+        if (s != PWA_OK) return s;
+        s = pwa_build_norm(ctx, nullptr);
+        if (s != PWA_OK) return s;
+        s = pwa_nll_grad(ctx, xx, f, gg, nullptr);
+        evals += 1;
+        if (s == PWA_WARN_NONFINITE) { worst = s; s = PWA_OK; }
+        if (s != PWA_OK) return s;
+        if (n_free > 0) {
+            s = pwa_res_grad(ctx, xx, dM.data(), dG.data());
+            if (s != PWA_OK) return s;
+            for (int i = 0; i < n_free; ++i) { gg[2 * n + i] = dM[free_res[i]]; gg[2 * n + n_free + i] = dG[free_res[i]]; }
+        }
+        for (int i = 0; i < d; ++i) gg[i] *= sc[i];       // d f / d u
+        return PWA_OK;
+    };
+    Bfgs fit;
+    double f0 = 0.0;
+    pwa_status s = eval(u.data(), &f0, g.data());
+    if (s != PWA_OK) return s;
+    if (!isfinite(f0)) return PWA_ERR_INVALID_ARG;      // the starting point itself must be physical
+    fit.init(d, u.data());
+    fit.f = f0; fit.g = g;
+    if (max_iter == 0 || fit.gmax() < gtol) fit.done = true;
+    else fit.direction(true);
+    while (!fit.done) {
+        fit.trial();
+        double ft = 0.0;
+        s = eval(fit.xt.data(), &ft, fit.gt.data());
+        if (s != PWA_OK) return s;
+        fit.update(ft, max_iter, gtol);
+    }
+    for (int i = 0; i < d; ++i) x[i] = fit.x[i] * sc[i];
+    memcpy(V, x.data(), sizeof(double) * 2 * n);
+    for (int i = 0; i < n_free; ++i) { mass[free_res[i]] = x[2 * n + i]; width[free_res[i]] = x[2 * n + n_free + i]; }
+    // leave the context at the fitted point (M valid for it)
+    for (int i = 0; i < n_free; ++i) { Mr[free_res[i]] = mass[free_res[i]]; Gr[free_res[i]] = width[free_res[i]]; }
+    s = pwa_set_resonances(ctx, Mr.data(), Gr.data());
+    if (s != PWA_OK) return s;
+    s = pwa_build_norm(ctx, nullptr);
+    if (s != PWA_OK) return s;
+    if (nll_out) *nll_out = fit.f;
+    if (n_iter_out) *n_iter_out = fit.iter;
+    if (n_evals_out) *n_evals_out = evals;
+    return worst;
+}
+
 }  // extern "C"

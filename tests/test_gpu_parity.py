@@ -254,6 +254,41 @@ def test_res_grad_parity(pwa, oracle, synth):
     assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max()
 
 
+def test_bfgs_floating_resonances(pwa, oracle, synth):
+    """configs[3] in small: BFGS over V and the masses / widths of the free resonances, M rebuilt in every
+    evaluation.  Data are generated at (w.Mr, w.Gr, w.V_true); the fit starts from displaced resonance
+    parameters.  The fitted point is a better likelihood than the truth, is (nearly) stationary in ALL parameters,
+    and the oracle reproduces the GPU value at the fitted point."""
+    w = synth.make_workload(3, n_data=20_011, n_mc=60_011, full_amplitudes=False)
+    Mr0, Gr0 = synth.floating_start(w)
+    free = np.arange(w.n_free, dtype=np.int32)
+    with _factored_ctx(pwa, w, w.Mr, w.Gr) as c:
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        nll_truth = pwa.pwa_nll_grad(c.ctx, w.V_true)[0]
+        pwa.pwa_set_resonances(c.ctx, Mr0, Gr0)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        nll_start = pwa.pwa_nll_grad(c.ctx, w.V_true)[0]
+        V, Mr, Gr, nll, iters, evals, st = pwa.pwa_minimize_bfgs_floating(c.ctx, w.V_true, Mr0, Gr0, free, max_iter=1000, gtol=1e-2)
+        assert iters <= 1000 and evals >= iters          # ~600 iterations: overlapping resonances make a shallow valley
+        assert nll < nll_start and nll <= nll_truth
+        # the fixed resonances did not move; the free ones stay physical (overlapping wide resonances are weakly
+        # determined by 2e4 events, so closeness to the generator's values is not asserted: the likelihood is)
+        assert np.array_equal(Mr[w.n_free:], Mr0[w.n_free:]) and np.array_equal(Gr[w.n_free:], Gr0[w.n_free:])
+        assert np.all(Mr[:w.n_free] > 0.9) and np.all(Mr[:w.n_free] < 3.3) and np.all(Gr[:w.n_free] > 0.0)
+        # the context is left at the fitted point: value, V-gradient and resonance gradient there
+        nll_fit, g_fit, parts = pwa.pwa_nll_grad(c.ctx, V)
+        dM, dG = pwa.pwa_res_grad(c.ctx, V, w.n_res)
+        assert nll_fit == nll
+        assert parts[1] == pytest.approx(w.n_data, rel=1e-5)          # P7: Norm = N_data at a stationary point of eq. 3
+    A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    M_o = oracle.norm_matrix(B, w.n_gen)
+    g_norm = oracle.assemble(0.0, np.zeros((w.n, 2)), M_o, V)[1]
+    check_eval((nll_fit, g_fit, parts), oracle.nll_grad(A, M_o, V), 1e-12, w.n_data, gscale=np.abs(g_norm).max())
+    # stationarity: the gradient is small against the size of its two cancelling parts
+    assert np.abs(g_fit).max() <= 1e-3 * np.abs(g_norm).max()
+
+
 # ------------------------------------------------------------------ device-resident (BORROW) path and the multi-GPU building block
 def test_borrowed_device_buffers_and_data_term_only(pwa, oracle):
     import torch

@@ -447,6 +447,7 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     VArg varg;
     for (int t = 0; t < 2 * n; ++t) varg.v[t] = V_host_k[t];
     int opt = ctx->opt_data_term;
+    if (opt == 98) opt = 0;                             // 98: default kernel without programmatic dependent launch (experiment switch)
     if (ctx->data.weights && opt < 20) opt = 20;        // weighted samples: the per-lane LDG kernel carries the weight stream
     // opt 0-9: TMA-tiled two-phase kernel (data_term_tma.cu; default where it applies);
     // 10-19: bulk-copy ring variants; 20-29: per-lane LDG kernels (first design)

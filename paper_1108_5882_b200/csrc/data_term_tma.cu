@@ -113,6 +113,9 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, const __g
     const uint32_t rb0 = smem_u32(&rbuf[warp][0][0]);
     const uint32_t sv0 = smem_u32(sV);
     if (threadIdx.x == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
+    // Let the next kernel of the stream start as soon as SMs free up: its streaming phase only reads the (constant)
+    // amplitudes and its own V; everything shared with this grid is touched after griddepcontrol.wait (block_finish).
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (wig == 0 && lane == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(bar0 + 8 * s, 1); issued[grp][s] = 0; }
@@ -314,7 +317,14 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     pwa_status s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
     if (s != PWA_OK) return s;
     fa.partials = ctx->d_partials;
-    kern<<<(unsigned)grid, THREADS, C::SMEM, ctx->stream>>>(*reinterpret_cast<const CUtensorMap *>(tc.map), N, varg, fa);
+    // programmatic stream serialisation: the grid may begin while its predecessor drains (see the kernel's prologue)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(THREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = ctx->opt_data_term == 98 ? 0 : 1;     // 98: experiment switch, plain serialisation
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    PWA_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *reinterpret_cast<const CUtensorMap *>(tc.map), N, varg, fa));
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;

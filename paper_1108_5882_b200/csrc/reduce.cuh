@@ -114,6 +114,10 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
     const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
     __shared__ bool s_last;
 
+    // Programmatic dependent launch (data_term_tma.cu): this grid may have started while the previous kernel of
+    // the stream was still finishing; the partial slots, the ticket and the result record are shared with it, so
+    // wait for its completion (and memory flush) here.  Returns at once for a normally serialised launch.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     for (int c = tid; c < NC; c += nthreads) fa.partials[(size_t)blockIdx.x * NC + c] = s_tot[c];
     __threadfence();
     __syncthreads();

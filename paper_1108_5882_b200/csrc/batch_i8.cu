@@ -673,6 +673,13 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
     double thr2 = ldexp(1.0, 77) / (double)N;
     thr2 = fmin(fmax(thr2, 0x1p52), 0x1p66);
     if (ctx->opt_batch == 3) thr2 = 0.0;
+    // a starting point V_k = 0 makes every coherent sum vanish: each of them would go through the fp64 recomputation
+    // (correct but extremely slow); the FP64 path propagates the IEEE values at full speed
+    for (int k = 0; k < K; ++k) {
+        bool any = false;
+        for (int t = 0; t < 2 * ctx->n && !any; ++t) any = ctx->h_V[(size_t)k * 2 * ctx->n + t] != 0.0;
+        if (!any) return PWA_OK;
+    }
     auto &q = ctx->i8d;
     if (!q.checked) {
         pwa_status s = i8_column_scales(ctx, ctx->data.amps, N, 128, q.exp, q.scale, q.cmax, &q.valid);

@@ -489,6 +489,9 @@ def test_batch_i8_selection_and_nonfinite(pwa, oracle):
             pwa.pwa_nll_grad_batch(c.ctx, Vn)
         again = pwa.pwa_nll_grad_batch(c.ctx, Vk)
         assert np.array_equal(again[0], ref[0]) and np.array_equal(again[1], ref[1])
+        Vz = Vk.copy(); Vz[5] = 0.0
+        nllz, gz, partsz = pwa.pwa_nll_grad_batch(c.ctx, Vz)
+        assert pwa.pwa_batch_path(c.ctx)[0] == 1 and partsz[5, 0] == -math.inf     # a zero starting point: FP64 path, ln 0
         pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, np.ones(N))
         pwa.pwa_nll_grad_batch(c.ctx, Vk)
         assert pwa.pwa_batch_path(c.ctx)[0] == 0            # weighted sample: weighted streaming kernel

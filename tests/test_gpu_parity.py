@@ -408,6 +408,34 @@ def test_norm_i8_default_path_and_nonfinite(pwa, oracle):
         assert pwa.pwa_norm_error_bound(c.ctx)[1] == 0
 
 
+# ------------------------------------------------------------------ back-to-back evaluations (programmatic dependent launch)
+@pytest.mark.parametrize("storage,n,N", [("f32", 32, 200_003), ("f64", 16, 100_000), ("f32", 64, 50_001)])
+def test_back_to_back_enqueues_are_independent(pwa, storage, n, N):
+    """The TMA data-term kernel lets the next evaluation's grid start while it drains (griddepcontrol); partial slots,
+    ticket and result record are shared between the two grids and must only be touched after the predecessor has
+    completed.  A burst of evaluations enqueued without any host synchronisation must give, for its last point,
+    bitwise the result of a lone evaluation at that point, and the same with the overlap switched off."""
+    A, B, _ = rand_case(77 + n, N, 3001, n, storage)
+    Vs = np.random.default_rng(5).normal(size=(24, n, 2))
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=3001)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        lone = [pwa.pwa_nll_grad(c.ctx, V) for V in Vs]
+        for burst in (2, 3, 8, 24):
+            for rep in range(3):
+                for i in range(burst):
+                    pwa.pwa_nll_grad_enqueue(c.ctx, Vs[i])
+                nll, g, parts = pwa.pwa_fetch(c.ctx)
+                ref = lone[burst - 1]
+                assert nll[0] == ref[0] and np.array_equal(g[0], ref[1]) and np.array_equal(parts[0], ref[2])
+        pwa.pwa_set_option(c.ctx, "data_term", 98)                 # plain stream serialisation
+        for i in range(8):
+            pwa.pwa_nll_grad_enqueue(c.ctx, Vs[i])
+        nll, g, parts = pwa.pwa_fetch(c.ctx)
+        assert nll[0] == lone[7][0] and np.array_equal(g[0], lone[7][1])
+
+
 # ------------------------------------------------------------------ NEXT-1 (A8): batched evaluation on the int8 tensor cores
 @pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (6007, 64), (6007, 70), (40_001, 33)])
 def test_batch_i8_parity(pwa, oracle, N, K):

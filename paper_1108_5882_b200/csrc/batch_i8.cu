@@ -155,12 +155,6 @@ constexpr uint32_t kI2_128 = idesc(128, true),  kI2_256 = idesc(256, true);    /
 // int32 -> double on the fp64 pipe (the 64-bit conversion unit is 4x slower): the integer lands in the low
 // mantissa bits of 2^52 + 2^31 + v (exact), one fp64 subtraction removes the offset.
 __device__ __forceinline__ double i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
-// 2^16 y + x (|.| < 2^51) as a double, exactly: 64-bit integer arithmetic, the result lands in the mantissa of 1.5 * 2^52
-__device__ __forceinline__ double yx2d(int y, int x)
-{
-    const long long b = (long long)y * 65536LL + (long long)x + 0x4338000000000000LL;
-    return __longlong_as_double(b) - 6755399441055744.0;
-}
 // 1 / x for 1 <= x < 2^100: 20-bit hardware seed, two Newton steps (relative error ~2^-52)
 __device__ __forceinline__ double rcp_d(double x)
 {
@@ -372,20 +366,20 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 if (t > 0) mbar_wait(b_w_full, (uint32_t)((t - 1) & 1));      // W0 is back in its slot
                 tc_fence_after();
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-                const uint32_t ko = (uint32_t)kk * 32u, acc = kk > 0 ? 1u : 0u;
-                const uint64_t a0 = desc_kmajor(pX0 + ko), a1 = desc_kmajor(pX1 + ko);
-                const uint64_t a2 = desc_kmajor(pX2 + ko), a3 = desc_kmajor(pX3 + ko);
-                const uint64_t w0 = desc_kmajor(pW0 + ko), w1 = desc_kmajor(pW1 + ko);
-                const uint64_t w2 = desc_kmajor(pW1 + PLANE + ko), w3 = desc_kmajor(pW1 + 2 * PLANE + ko);
-                umma_i8(tmem0 + 256, a3, w2, kI1_256, acc);        // X3 [W2 | W3] -> t = 5 | 6
-                umma_i8(tmem0 + 0,   a2, w1, kI1_256, acc);        // X2 [W1 | W2] -> t = 3 | 4
-                umma_i8(tmem0 + 0,   a1, w2, kI1_256, 1u);         // X1 [W2 | W3] -> t = 3 | 4
-                umma_i8(tmem0 + 0,   a3, w0, kI1_128, 1u);         // X3 W0        -> t = 3
-                umma_i8(tmem0 + 128, a3, w1, kI1_128, 1u);         // X3 W1        -> t = 4
-                umma_i8(tmem0 + 256, a2, w3, kI1_128, 1u);         // X2 W3        -> t = 5
-                umma_i8(tmem0 + 0,   a0, w3, kI1_128, 1u);         // X0 W3        -> t = 3
-            }
+                for (int kk = 0; kk < 4; ++kk) {
+                    const uint32_t ko = (uint32_t)kk * 32u, acc = kk > 0 ? 1u : 0u;
+                    const uint64_t a0 = desc_kmajor(pX0 + ko), a1 = desc_kmajor(pX1 + ko);
+                    const uint64_t a2 = desc_kmajor(pX2 + ko), a3 = desc_kmajor(pX3 + ko);
+                    const uint64_t w0 = desc_kmajor(pW0 + ko), w1 = desc_kmajor(pW1 + ko);
+                    const uint64_t w2 = desc_kmajor(pW1 + PLANE + ko), w3 = desc_kmajor(pW1 + 2 * PLANE + ko);
+                    umma_i8(tmem0 + 256, a3, w2, kI1_256, acc);        // X3 [W2 | W3] -> t = 5 | 6
+                    umma_i8(tmem0 + 0,   a2, w1, kI1_256, acc);        // X2 [W1 | W2] -> t = 3 | 4
+                    umma_i8(tmem0 + 0,   a1, w2, kI1_256, 1u);         // X1 [W2 | W3] -> t = 3 | 4
+                    umma_i8(tmem0 + 0,   a3, w0, kI1_128, 1u);         // X3 W0        -> t = 3
+                    umma_i8(tmem0 + 128, a3, w1, kI1_128, 1u);         // X3 W1        -> t = 4
+                    umma_i8(tmem0 + 256, a2, w3, kI1_128, 1u);         // X2 W3        -> t = 5
+                    umma_i8(tmem0 + 0,   a0, w3, kI1_128, 1u);         // X0 W3        -> t = 3
+                }
                 umma_commit(b_s_full);
             }
             __syncwarp();
@@ -518,19 +512,19 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 mbar_wait(b_r_full, ph);
                 tc_fence_after();
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-                const uint32_t ko = (uint32_t)kk * 32u * 128u, acc = kk > 0 ? 1u : 0u;
-                const uint64_t a0 = desc_mnmajor(pX0 + ko), a1 = desc_mnmajor(pX1 + ko);
-                const uint64_t a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
-                const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko), r1 = desc_mnmajor(pR + 1 * PLANE + ko);
-                const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko), r3 = desc_mnmajor(pR + 3 * PLANE + ko);
-                umma_i8(tmem0 + 256, a3, r2, kI2_256, acc);        // X3^T [R2 | R3] -> t = 5 | 6
-                umma_i8(tmem0 + 0,   a3, r0, kI2_256, acc);        // X3^T [R0 | R1] -> t = 3 | 4
-                umma_i8(tmem0 + 0,   a2, r1, kI2_256, 1u);         // X2^T [R1 | R2] -> t = 3 | 4
-                umma_i8(tmem0 + 256, a2, r3, kI2_128, 1u);         // X2^T R3        -> t = 5
-                umma_i8(tmem0 + 0,   a1, r2, kI2_256, 1u);         // X1^T [R2 | R3] -> t = 3 | 4
-                umma_i8(tmem0 + 0,   a0, r3, kI2_128, 1u);         // X0^T R3        -> t = 3
-            }
+                for (int kk = 0; kk < 4; ++kk) {
+                    const uint32_t ko = (uint32_t)kk * 32u * 128u, acc = kk > 0 ? 1u : 0u;
+                    const uint64_t a0 = desc_mnmajor(pX0 + ko), a1 = desc_mnmajor(pX1 + ko);
+                    const uint64_t a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
+                    const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko), r1 = desc_mnmajor(pR + 1 * PLANE + ko);
+                    const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko), r3 = desc_mnmajor(pR + 3 * PLANE + ko);
+                    umma_i8(tmem0 + 256, a3, r2, kI2_256, acc);        // X3^T [R2 | R3] -> t = 5 | 6
+                    umma_i8(tmem0 + 0,   a3, r0, kI2_256, acc);        // X3^T [R0 | R1] -> t = 3 | 4
+                    umma_i8(tmem0 + 0,   a2, r1, kI2_256, 1u);         // X2^T [R1 | R2] -> t = 3 | 4
+                    umma_i8(tmem0 + 256, a2, r3, kI2_128, 1u);         // X2^T R3        -> t = 5
+                    umma_i8(tmem0 + 0,   a1, r2, kI2_256, 1u);         // X1^T [R2 | R3] -> t = 3 | 4
+                    umma_i8(tmem0 + 0,   a0, r3, kI2_128, 1u);         // X0^T R3        -> t = 3
+                }
                 umma_commit(b_t_full);
             }
             __syncwarp();

@@ -577,6 +577,7 @@ pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
     if (!strcmp(key, "data_term")) ctx->opt_data_term = value;
     else if (!strcmp(key, "norm")) ctx->opt_norm = value;
     else if (!strcmp(key, "batch")) ctx->opt_batch = value;
+    else if (!strcmp(key, "l2_resident_mb")) { if (value < -1 || value > 120) return fail(ctx, PWA_ERR_INVALID_ARG, "l2_resident_mb must be in [-1, 120]"); ctx->opt_l2_resident_mb = value; }
     else if (!strcmp(key, "likelihood")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "likelihood must be 0 (eq. 3) or 1 (eq. 2)"); ctx->opt_likelihood = value; }
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;

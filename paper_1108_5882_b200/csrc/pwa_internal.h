@@ -81,6 +81,7 @@ struct pwa_ctx {
     struct { bool checked = false, valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8d;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
+    int opt_l2_resident_mb = -1;              // MB of the data sample's head kept in L2 between evaluations (TMA data term); -1 = automatic, 0 = off
     int opt_likelihood = 0;                   // 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form
     std::string err;
 };

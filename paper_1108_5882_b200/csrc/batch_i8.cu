@@ -255,7 +255,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
            const unsigned char *__restrict__ Wp, const double *__restrict__ Wd, double *__restrict__ slots)
 {
     extern __shared__ unsigned char bi8_smem_raw[];
-    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 5];
+    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 6];
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) uint32_t s_emax[NEW][16];
     __shared__ __align__(16) uint32_t s_sh[KC];            // sh_k << 20 of the current tile
@@ -267,11 +267,11 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
     const uint32_t pX0 = base + OFF_X0, pX1 = base + OFF_X1, pX2 = base + OFF_X2, pX3 = base + OFF_X3;
     const uint32_t pW0 = base + OFF_W0, pW1 = base + OFF_W1, pR = base + OFF_R, stg0 = base + OFF_STG;
     const uint32_t b_stg_full = smem_u32(&bars[0]), b_stg_empty = b_stg_full + 8 * NSTG;
-    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24, b_w_full = b_a_full + 32;
+    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24, b_w_full = b_a_full + 32, b_l_full = b_a_full + 40;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTG; ++s) { mbar_init(b_stg_full + 8 * s, 1); mbar_init(b_stg_empty + 8 * s, NEW); }
-        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1); mbar_init(b_w_full, 1);
+        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1); mbar_init(b_w_full, 1); mbar_init(b_l_full, 1);
         fence_async_smem();
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     }
@@ -298,16 +298,20 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
         // warp 1 the TMA loads (no dedicated producer / issuer warps: 512 threads leave 128 registers each,
         // enough for the 32 fp64 accumulators per thread without spilling) =====
         const bool is_mma = threadIdx.x == 0, is_tma = threadIdx.x == 32;
-        const long long ng = nt * SPT;
-        auto tma_load = [&](long long g) {
-            const int s = (int)(g % NSTG);
-            mbar_expect_tx(b_stg_full + 8 * s, STG_BYTES);
+        // Stages 0..2 of every tile go through the ring (slot = stage, refilled for the next tile as soon as all 16 warps
+        // have released it).  The LAST stage of a tile has no ring slot to wait in: it is loaded into the slot of R1, which
+        // is free from the end of GEMM2 until phase 2 of the next tile, right after GEMM2 completes — so its HBM latency
+        // hides behind the flush instead of stalling the conversion.
+        static_assert(NSTG == 3 && SPT == 4, "ring = the first three stages of a tile");
+        auto tma_load = [&](long long tt, int st) {
+            const uint32_t bar = st < NSTG ? b_stg_full + 8 * st : b_l_full;
+            const uint32_t dst = st < NSTG ? stg0 + (uint32_t)st * STG_BYTES : pR + PLANE;
+            mbar_expect_tx(bar, STG_BYTES);
             asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                         ::"r"(stg0 + (uint32_t)s * STG_BYTES), "l"(&tmap), "r"(0), "r"((int)(t_begin * TE + g * SR)),
-                           "r"(b_stg_full + 8 * s) : "memory");
+                         ::"r"(dst), "l"(&tmap), "r"(0), "r"((int)((t_begin + tt) * TE + st * SR)), "r"(bar) : "memory");
         };
-        if (is_tma)
-            for (long long g = 0; g < NSTG && g < ng; ++g) tma_load(g);
+        if (is_tma && nt > 0)
+            for (int st = 0; st < SPT; ++st) tma_load(0, st);
         __syncwarp();
         const int q = warp & 3, j = warp >> 2;
         const int row = 32 * q + lane;                                 // event row (GEMM1) / real column c (GEMM2)
@@ -327,10 +331,8 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
             // ---- fp32 stages -> X digit planes (2 rows per warp and stage)
 #pragma unroll 1
             for (int st = 0; st < SPT; ++st) {
-                const long long g = t * SPT + st;
-                const int s = (int)(g % NSTG);
-                mbar_wait(b_stg_full + 8 * s, (uint32_t)((g / NSTG) & 1));
-                const uint32_t src = stg0 + (uint32_t)s * STG_BYTES + (uint32_t)(2 * warp) * ROWB + (uint32_t)lane * 16u;
+                mbar_wait(st < NSTG ? b_stg_full + 8 * st : b_l_full, ph);
+                const uint32_t src = (st < NSTG ? stg0 + (uint32_t)st * STG_BYTES : pR + PLANE) + (uint32_t)(2 * warp) * ROWB + (uint32_t)lane * 16u;
                 uint4 raw[2];
                 raw[0] = lds128(src); raw[1] = lds128(src + ROWB);
 #pragma unroll
@@ -349,12 +351,14 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                     asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX3 + a), "r"(__byte_perm(t2, t3, 0x7632)) : "memory");
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(b_stg_empty + 8 * s);
-                if (is_tma && g + NSTG < ng) {                           // refill the stage once all 16 warps have released it
-                    mbar_wait(b_stg_empty + 8 * s, (uint32_t)((g / NSTG) & 1));
-                    tma_load(g + NSTG);
+                if (st < NSTG) {
+                    if (lane == 0) mbar_arrive(b_stg_empty + 8 * st);
+                    if (is_tma && t + 1 < nt) {                          // refill the slot for the next tile once all 16 warps have released it
+                        mbar_wait(b_stg_empty + 8 * st, ph);
+                        tma_load(t + 1, st);
+                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
             fence_async_smem();
             tc_fence_before();
@@ -531,9 +535,10 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
 
             // ---- flush: Q levels of this tile -> fp64 accumulators (row = real column c)
             mbar_wait(b_t_full, ph);
-            if (is_tma && t + 1 < nt) {                                  // GEMM2 is done with R0: bring W0 back for the next tile
-                mbar_expect_tx(b_w_full, PLANE);
+            if (is_tma && t + 1 < nt) {                                  // GEMM2 is done with the R planes:
+                mbar_expect_tx(b_w_full, PLANE);                         // W0 back into its slot (R0) for the next GEMM1,
                 bulk_g2s(pW0, Wp, PLANE, b_w_full);
+                tma_load(t + 1, NSTG);                                   // the next tile's last stage into the slot of R1
             }
             __syncwarp();
             tc_fence_after();

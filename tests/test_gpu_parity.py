@@ -434,6 +434,15 @@ def test_back_to_back_enqueues_are_independent(pwa, storage, n, N):
             pwa.pwa_nll_grad_enqueue(c.ctx, Vs[i])
         nll, g, parts = pwa.pwa_fetch(c.ctx)
         assert nll[0] == lone[7][0] and np.array_equal(g[0], lone[7][1])
+        pwa.pwa_set_option(c.ctx, "data_term", 0)
+        for mb in (8, 0, -1):                                      # L2 residency hints on the TMA loads change no bit
+            pwa.pwa_set_option(c.ctx, "l2_resident_mb", mb)
+            for i in range(4):
+                pwa.pwa_nll_grad_enqueue(c.ctx, Vs[i])
+            nll, g, parts = pwa.pwa_fetch(c.ctx)
+            assert nll[0] == lone[3][0] and np.array_equal(g[0], lone[3][1])
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_set_option(c.ctx, "l2_resident_mb", 500)
 
 
 # ------------------------------------------------------------------ NEXT-1 (A8): batched evaluation on the int8 tensor cores

@@ -446,7 +446,7 @@ def test_back_to_back_enqueues_are_independent(pwa, storage, n, N):
 
 
 # ------------------------------------------------------------------ NEXT-1 (A8): batched evaluation on the int8 tensor cores
-@pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (6007, 64), (6007, 70), (40_001, 33)])
+@pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (129, 1), (257, 64), (6007, 64), (6007, 70), (40_001, 33)])
 def test_batch_i8_parity(pwa, oracle, N, K):
     """fp32 storage, n = 64, option "batch" = 2: both chained GEMMs on tcgen05 int8 (batch_i8.cu) against the
     oracle and against the FP64 DMMA path: less than one tile, a ragged last tile, K < 64, K > 64 (two passes),

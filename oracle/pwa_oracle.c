@@ -37,7 +37,9 @@
  * invariance, finite differences, equality with eq. 3 at Norm = N_data; P14 polar chain rule vs
  * finite differences in (r, phi); P15 Fumili matrix: H_data V = 2 grad(L_data) (Euler), numpy
  * restatement, PSD, Hess(Norm) vs differences of the norm gradient; P16 event weights: unit weights,
- * integer weights = duplicated events, numpy restatement, linearity in w.
+ * integer weights = duplicated events, numpy restatement, linearity in w; P17 the sampled entry points
+ * (norm_block / norm_block_w with a0, b0 > 0, fumili_rows with p0 > 0): bitwise equal to the same entries of
+ * the full result, zero outside, numpy restatement of the block.
  * Parity unpinned by the paper: the choices C2, C3, C4, C5, C9-C13 (definitions, not
  * results), and the resonance-parameter gradient beyond finite differences (P5/P10 style).
  *

@@ -588,3 +588,60 @@ def test_p16_event_weights(oracle):
     Lb, Tb, _ = oracle.data_term_w(A, V, w + w2)
     assert Lb == pytest.approx(Lw + La, rel=1e-11, abs=1e-11 * (abs(Lw) + abs(La)))
     assert np.allclose(Tb, Tw + Ta, rtol=1e-11, atol=1e-11 * np.abs(Tb).max())
+
+
+# ---------------------------------------------------------------- P17 sampled-block entry points (offset indexing)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_p17_norm_block_offsets(oracle, dtype):
+    """norm_block(a0, a1, b0, b1) with a0, b0 > 0 (the indexing every full-size M check rests on):
+    the block equals the same entries of the full matrix BITWISE (same per-event terms, same order),
+    entries outside the block stay 0, and the block equals the numpy/BLAS restatement
+    M_ab = (1/N_gen) sum_j conj(B_ja) B_jb (P:41 inner bracket, C1) — non-square blocks with a != b
+    ranges so a transposed or shifted index fails."""
+    rng = np.random.default_rng(17)
+    n, Nacc, Ngen = 7, 1501, 1777
+    B = rand_amps(rng, Nacc, n).astype(dtype)
+    w = rng.uniform(0.2, 2.0, size=Nacc)
+    full = oracle.norm_matrix(B, Ngen)
+    full_w = oracle.norm_matrix_w(B, Ngen, w)
+    Bc = cplx(B.astype(np.float64))
+    M_np = Bc.conj().T @ Bc / Ngen
+    M_np_w = (Bc.conj().T * w) @ Bc / Ngen
+    assert np.abs(cplx(full) - M_np).max() <= 1e-13 * np.abs(M_np).max()
+    for a0, a1, b0, b1 in [(2, 5, 1, 7), (3, 4, 6, 7), (6, 7, 0, 2), (1, 7, 3, 5), (0, 7, 0, 7), (4, 4, 2, 6)]:
+        blk = oracle.norm_block(B, Ngen, a0, a1, b0, b1)
+        assert np.array_equal(blk[a0:a1, b0:b1], full[a0:a1, b0:b1]), (a0, a1, b0, b1)
+        outside = blk.copy()
+        outside[a0:a1, b0:b1] = 0.0
+        assert not outside.any()
+        if a1 > a0:
+            assert np.abs(cplx(blk)[a0:a1, b0:b1] - M_np[a0:a1, b0:b1]).max() <= 1e-13 * np.abs(M_np).max()
+        # the weighted entry point with offsets (called directly: the Python wrapper only passes 0..n)
+        blk_w = np.zeros((n, n, 2))
+        Bx, dt = oracle._amp(B)
+        oracle.lib().pwa_oracle_norm_block_w(oracle._p(Bx), dt, oracle.C.c_int64(Nacc), n, oracle.C.c_int64(Ngen),
+                                             oracle._p(w), a0, a1, b0, b1, oracle._p(blk_w))
+        assert np.array_equal(blk_w[a0:a1, b0:b1], full_w[a0:a1, b0:b1])
+        if a1 > a0:
+            assert np.abs(cplx(blk_w)[a0:a1, b0:b1] - M_np_w[a0:a1, b0:b1]).max() <= 1e-13 * np.abs(M_np_w).max()
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_p17_fumili_rows_offsets(oracle, dtype):
+    """fumili_rows(p0, p1) with p0 > 0: rows equal the full matrix bitwise, other rows stay 0, and
+    the rows equal the numpy restatement sum_i u_i[p] u_i[q]."""
+    rng = np.random.default_rng(18)
+    N, n = 401, 5
+    A = rand_amps(rng, N, n).astype(dtype)
+    V = rng.normal(size=(n, 2))
+    full = oracle.fumili(A, V)
+    Ac, Vc = cplx(A.astype(np.float64)), cplx(V)
+    t = Ac / (Ac @ Vc)[:, None]
+    U = np.empty((N, 2 * n))
+    U[:, 0::2], U[:, 1::2] = 2 * t.real, -2 * t.imag
+    H_np = U.T @ U
+    for p0, p1 in [(1, 3), (4, 5), (9, 10), (3, 10), (0, 10)]:
+        rows = oracle.fumili_rows(A, V, p0, p1)
+        assert np.array_equal(rows[p0:p1], full[p0:p1]), (p0, p1)
+        assert not rows[:p0].any() and not rows[p1:].any()
+        assert np.abs(rows[p0:p1] - H_np[p0:p1]).max() <= 1e-12 * np.abs(H_np).max()

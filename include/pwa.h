@@ -17,8 +17,10 @@
  * crosses the ABI.  Every call returns a pwa_status; on PWA_ERR_* the outputs are
  * untouched and pwa_last_error() describes the failure.  The library never frees or keeps
  * caller memory except as stated for PWA_BORROW.  One context = one CUDA stream = one host
- * thread at a time.  All scratch is owned by the context and allocated at create / upload
- * time, never inside an evaluation call.  There is no CPU fallback: without a CUDA device
+ * thread at a time.  All scratch is owned by the context.  Everything pwa_nll_grad and pwa_data_term_enqueue need
+ * (per-block partial slots, result records, V staging) is allocated in pwa_create; the work space of pwa_build_norm,
+ * pwa_nll_grad_batch and pwa_fumili_hessian is allocated by the first call of that kind (it grows only when a later
+ * call needs more: a larger K), so the steady-state calls of a fit never allocate.  There is no CPU fallback: without a CUDA device
  * pwa_create fails with PWA_ERR_CUDA.
  *
  * Pointer kinds are stated per argument: HOST = ordinary host memory, DEVICE = CUDA device
@@ -169,6 +171,23 @@ pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
 pwa_status pwa_assemble_host(int32_t n_waves, double L_data, const double *T, const double *M,
                              const double *V, double *nll, double *grad, double *parts);
 
+/* Event-sharded runs, one context per shard (rank).  All three are host-side synthesis steps with the
+ * shards added in index order r = 0 .. R-1, so every rank that is given the same gathered arrays obtains the
+ * same bits (a tree all-reduce would not fix the order).
+ * pwa_norm_sums: G = B^H B over THIS context's MC events without the 1/N_gen (N_gen times the M of the most
+ *   recent pwa_build_norm), HOST [n][n][2], and this shard's N_gen.  PWA_ERR_STATE without a valid M.
+ * pwa_combine_norm_host: M_out = (sum_r G_r) / (sum_r N_gen,r)  (eq. 3 second term, over all shards);
+ *   G HOST [R][n][n][2], n_gen HOST [R], M_out HOST [n][n][2] (for pwa_set_norm), *n_gen_total (may be NULL) the
+ *   summed N_gen.  No GPU needed.
+ * pwa_assemble_host_shards: terms HOST [R][2 + 2n], the records pwa_data_term_enqueue wrote on the R shards;
+ *   adds them and performs step A7 as pwa_assemble_host (likelihood = 0) or pwa_assemble_host_eq2 (likelihood = 1,
+ *   n_data = N_data of ALL shards).  PWA_WARN_NONFINITE if any shard counted a non-finite event.  No GPU needed. */
+pwa_status pwa_norm_sums(pwa_ctx *ctx, double *G_out, int64_t *n_gen_out);
+pwa_status pwa_combine_norm_host(int32_t n_waves, int32_t R, const double *G, const int64_t *n_gen, double *M_out,
+                                 int64_t *n_gen_total);
+pwa_status pwa_assemble_host_shards(int32_t n_waves, int32_t R, const double *terms, const double *M, const double *V,
+                                    int32_t likelihood, double n_data, double *nll, double *grad, double *parts);
+
 /* Fumili-style approximate Hessian of nll at V (Minuit / Fumili; "most of the computing time
  * is spent on ... error calculations"), DESIGN.md section 13:
  *   H = sum_i u_i u_i^T  (+ Hess(Norm) if with_norm != 0),   u_i = d ln I_i / d(x_0, y_0, x_1, ...)
@@ -183,7 +202,9 @@ pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t 
  * extended form of eq. 3 (reading C2):  nll2 = -L_data + N_data ln Norm,
  * grad2 = -2 conj(T) + (2 N_data / Norm) M V.  Invariant under V -> s V.  Host only; same
  * argument meaning as pwa_assemble_host, n_data = N_data > 0.  On the device the same form is
- * selected for pwa_nll_grad / pwa_nll_grad_batch with pwa_set_option(ctx, "likelihood", 1).     */
+ * selected for pwa_nll_grad / pwa_nll_grad_batch with pwa_set_option(ctx, "likelihood", 1); N_data is then the
+ * number of data events, or the sum of their weights when pwa_set_weights attached some (the weighted
+ * normalised likelihood -sum_i w_i ln I_i + (sum_i w_i) ln Norm, which keeps the invariance under V -> s V). */
 pwa_status pwa_assemble_host_eq2(int32_t n_waves, double n_data, double L_data, const double *T,
                                  const double *M, const double *V, double *nll, double *grad,
                                  double *parts);
@@ -197,21 +218,36 @@ pwa_status pwa_polar_to_cartesian(int32_t n_waves, const double *r_phi, double *
 
 /* Floating mode: gradient of nll w.r.t. the resonance parameters at the current
  * (mass0, width0) and the given V (reading A9):  d nll / d M_r and d nll / d G_r, HOST
- * [n_res] each.  Needs factored DATA and MC uploads.  One extra pass over data and MC.   */
+ * [n_res] each (n_res of pwa_set_wave_map: see pwa_n_res).  Needs factored DATA and MC uploads.  One extra pass
+ * over data and MC.  With "likelihood" = 1 the eq. 2 form is differentiated:
+ * -d L_data / d theta + (N_data / Norm) d Norm / d theta, Norm evaluated by the same MC pass.                  */
 pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dnll_dmass, double *dnll_dwidth);
 
 /* ---- host minimiser (a quasi-Newton in real parameters stays on the host) --- */
 
 /* Plain BFGS with backtracking line search on the 2n reals of V (constant-resonance mode).
- * V_inout: HOST [n][2], start in / result out.  Stops after max_iter iterations or when
- * max|grad| < gtol.  n_evals_out / nll_out may be NULL.                                  */
+ * V_inout: HOST [n][2], start in / result out.  Stops after max_iter iterations, when
+ * max|grad| < gtol, or when the line search is exhausted.  nll_out, n_iter_out, n_evals_out may be NULL. */
 pwa_status pwa_minimize_bfgs(pwa_ctx *ctx, double *V_inout, int32_t max_iter, double gtol,
                              double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out);
 
-/* K independent BFGS fits run in lock-step on pwa_nll_grad_batch.  V_inout [K][n][2].    */
+/* K independent BFGS fits run in lock-step on pwa_nll_grad_batch.  V_inout [K][n][2].
+ * The evaluations take the batched call's DEFAULT path (pwa_batch_path): for fp32-stored samples with n = 64,
+ * K >= 8 and >= 32768 events that is the int8 tcgen05 path, whose gradient carries a non-smooth error floor of
+ * about 1e-8 |T| (norm-wise): a gtol below that floor cannot be reached and such a fit ends
+ * with PWA_FIT_LINE_SEARCH or PWA_FIT_MAX_ITER; pwa_set_option(ctx, "batch", 1) (FP64 DMMA) gives the last
+ * digits; pwa_minimize_bfgs_batch does so itself: fits whose line search ran out of resolution on the int8 path are
+ * continued (same point, same inverse Hessian) on the FP64 DMMA path, and only those fits are evaluated there.
+ * The _ex form also reports, per fit, the iterations done and why it stopped (either may be NULL). */
+#define PWA_FIT_CONVERGED   0   /* max|grad| < gtol */
+#define PWA_FIT_MAX_ITER    1   /* max_iter iterations done */
+#define PWA_FIT_LINE_SEARCH 2   /* backtracking exhausted (step < 1e-20): the resolution of nll / its gradient is reached */
 pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V_inout, int32_t max_iter,
                                    double gtol, double *nll_out /* [K] */,
                                    int32_t *n_evals_out);
+pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V_inout, int32_t max_iter, double gtol,
+                                      double *nll_out /* [K] */, int32_t *n_iter_out /* [K] */,
+                                      int32_t *why_out /* [K]: PWA_FIT_* */, int32_t *n_evals_out);
 
 /* Floating-resonance fit (configs[3]; with floating masses and widths nothing can be pre-calculated, so
  * EVERY evaluation re-evaluates the Breit-Wigner factors and rebuilds M): BFGS over the 2 n_waves Cartesian reals
@@ -220,15 +256,24 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V_inout, int
  * (four passes: MC Gram, data term, and the two resonance-gradient passes).  V_inout: HOST [n][2]; mass_inout,
  * width_inout: HOST [n_res], all resonances (the fixed ones are read, the free ones updated).  A trial point with a
  * non-positive mass or width is rejected by the line search.  Needs factored DATA and MC uploads and a wave map.
- * nll_out, n_iter_out, n_evals_out may be NULL.                                                             */
+ * n_res must equal pwa_n_res(ctx) (PWA_ERR_INVALID_ARG otherwise).  nll_out, n_iter_out, n_evals_out, why_out
+ * (PWA_FIT_*) may be NULL.  Honours "likelihood" (eq. 2 / eq. 3) in the objective AND in all gradient components. */
 pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V_inout, double *mass_inout, double *width_inout,
                                       int32_t n_res, const int32_t *free_res, int32_t n_free, int32_t max_iter,
                                       double gtol, double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out);
+pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V_inout, double *mass_inout, double *width_inout,
+                                         int32_t n_res, const int32_t *free_res, int32_t n_free, int32_t max_iter,
+                                         double gtol, double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out,
+                                         int32_t *why_out);
 
 /* ---- introspection / measurement ------------------------------------------------------- */
 
-/* n_waves the context was created with.                                                  */
+/* n_waves / storage type the context was created with; n_res of the wave map (0 before pwa_set_wave_map);
+ * number of events of the sample uploaded last (-1: none).  The binding validates array shapes against these. */
 int32_t pwa_n_waves(const pwa_ctx *ctx);
+int32_t pwa_n_res(const pwa_ctx *ctx);
+pwa_dtype pwa_storage(const pwa_ctx *ctx);
+int64_t pwa_n_events(const pwa_ctx *ctx, pwa_sample which);
 
 /* Number of CUDA kernels this context has launched since creation.                        */
 uint64_t pwa_launch_count(const pwa_ctx *ctx);
@@ -248,6 +293,7 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
  * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch and the minimisers.    */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
+pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* current value of a pwa_set_option key */
 
 /* Register-resident peak probes used as roofline denominators:
  * which = 0: fp64 FMA (result TFLOP/s), 1: fp64 mma.sync m8n8k4 (TFLOP/s),

@@ -30,8 +30,10 @@ SYMBOLS = [
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
     "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
-    "pwa_batch_path", "pwa_minimize_bfgs_floating",
+    "pwa_batch_path", "pwa_minimize_bfgs_floating", "pwa_minimize_bfgs_batch_ex", "pwa_minimize_bfgs_floating_ex",
+    "pwa_n_res", "pwa_get_option", "pwa_storage", "pwa_n_events", "pwa_norm_sums", "pwa_combine_norm_host", "pwa_assemble_host_shards",
 ]
+PWA_FIT_CONVERGED, PWA_FIT_MAX_ITER, PWA_FIT_LINE_SEARCH = 0, 1, 2
 
 
 class PwaError(RuntimeError):
@@ -82,6 +84,16 @@ def _load():
         "pwa_batch_path": (C.c_int, [vp, C.POINTER(i32), dp]),
         "pwa_minimize_bfgs_floating": (C.c_int, [vp, vp, vp, vp, i32, vp, i32, i32, C.c_double, dp,
                                                  C.POINTER(i32), C.POINTER(i32)]),
+        "pwa_minimize_bfgs_floating_ex": (C.c_int, [vp, vp, vp, vp, i32, vp, i32, i32, C.c_double, dp,
+                                                    C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]),
+        "pwa_minimize_bfgs_batch_ex": (C.c_int, [vp, i32, vp, i32, C.c_double, vp, vp, vp, C.POINTER(i32)]),
+        "pwa_n_res": (i32, [vp]),
+        "pwa_get_option": (C.c_int, [vp, C.c_char_p, C.POINTER(i32)]),
+        "pwa_storage": (C.c_int, [vp]),
+        "pwa_n_events": (i64, [vp, C.c_int]),
+        "pwa_norm_sums": (C.c_int, [vp, vp, C.POINTER(i64)]),
+        "pwa_combine_norm_host": (C.c_int, [i32, i32, vp, vp, vp, C.POINTER(i64)]),
+        "pwa_assemble_host_shards": (C.c_int, [i32, i32, vp, vp, vp, i32, C.c_double, dp, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)          # AttributeError here = header/library mismatch
@@ -143,21 +155,44 @@ def pwa_destroy(ctx):
     _lib.pwa_destroy(ctx)
 
 
+def _check_amps(ctx, x, n_events, inner, what):
+    """The C side reads n_events * inner * 2 elements of the context's storage type: refuse arrays of another
+    dtype or with fewer elements (a raw int address cannot be checked)."""
+    ptr, keep, code = _ptr_and_keep(x)
+    if isinstance(x, int) or x is None:
+        return ptr, keep
+    storage = int(_lib.pwa_storage(ctx))
+    if code != storage:
+        raise TypeError(f"{what}: dtype {getattr(keep, 'dtype', None)} does not match the context's storage "
+                        f"({'float32' if storage == PWA_F32 else 'float64'})")
+    have = int(np.prod(keep.shape))
+    if have < int(n_events) * inner * 2:
+        raise ValueError(f"{what}: {have} elements, need n_events * {inner} * 2 = {int(n_events) * inner * 2}")
+    return ptr, keep
+
+
 def pwa_upload_events(ctx, which, amps, n_events=None, n_generated=0, flags=PWA_COPY):
-    ptr, keep, _ = _ptr_and_keep(amps)
+    n = _lib.pwa_n_waves(ctx)
     if n_events is None:
+        if tuple(amps.shape[1:]) != (n, 2):
+            raise ValueError(f"amps must be [N, {n}, 2], got {tuple(amps.shape)}")
         n_events = amps.shape[0]
+    ptr, keep = _check_amps(ctx, amps, n_events, n, "amps")
     _check(ctx, _lib.pwa_upload_events(ctx, int(which), C.c_void_p(ptr), int(n_events), int(n_generated), int(flags)))
     return keep
 
 
 def pwa_upload_events_factored(ctx, which, mass, ang, n_ang=None, n_events=None, n_generated=0, flags=PWA_COPY):
-    pm, km, _ = _ptr_and_keep(mass)
-    pa, ka, _ = _ptr_and_keep(ang)
     if n_events is None:
         n_events = ang.shape[0]
     if n_ang is None:
         n_ang = ang.shape[1]
+    if isinstance(mass, np.ndarray):
+        mass = np.ascontiguousarray(mass, dtype=np.float64)
+    pm, km, cm = _ptr_and_keep(mass)
+    if not isinstance(mass, int) and (cm != PWA_F64 or int(np.prod(km.shape)) < int(n_events)):
+        raise ValueError("mass must be float64 with >= n_events elements")
+    pa, ka = _check_amps(ctx, ang, n_events, int(n_ang), "ang")
     _check(ctx, _lib.pwa_upload_events_factored(ctx, int(which), C.c_void_p(pm), C.c_void_p(pa), int(n_ang),
                                                 int(n_events), int(n_generated), int(flags)))
     return km, ka
@@ -170,7 +205,10 @@ def pwa_set_weights(ctx, which, w, flags=PWA_COPY):
         return None
     if isinstance(w, np.ndarray):
         w = np.ascontiguousarray(w, dtype=np.float64)
-    addr, keep, _ = _ptr_and_keep(w)
+    addr, keep, code = _ptr_and_keep(w)
+    if not isinstance(w, int):
+        if code != PWA_F64 or int(np.prod(keep.shape)) != int(_lib.pwa_n_events(ctx, int(which))):
+            raise ValueError("weights must be float64 with one element per event of the uploaded sample")
     _check(ctx, _lib.pwa_set_weights(ctx, int(which), C.c_void_p(addr), int(flags)))
     return keep
 
@@ -178,11 +216,15 @@ def pwa_set_weights(ctx, which, w, flags=PWA_COPY):
 def pwa_set_wave_map(ctx, n_res, res_of_wave, ang_of_wave):
     r = np.ascontiguousarray(res_of_wave, dtype=np.int32)
     a = np.ascontiguousarray(ang_of_wave, dtype=np.int32)
+    n = _lib.pwa_n_waves(ctx)
+    if r.shape != (n,) or a.shape != (n,):
+        raise ValueError(f"res_of_wave and ang_of_wave must have n_waves = {n} entries")
     _check(ctx, _lib.pwa_set_wave_map(ctx, int(n_res), r.ctypes.data, a.ctypes.data))
 
 
 def pwa_set_resonances(ctx, mass0, width0):
-    m, w = _f64(mass0), _f64(width0)
+    nr = (_lib.pwa_n_res(ctx),)
+    m, w = _f64(mass0, nr), _f64(width0, nr)
     _check(ctx, _lib.pwa_set_resonances(ctx, m.ctypes.data, w.ctypes.data))
 
 
@@ -246,6 +288,8 @@ def pwa_nll_grad_enqueue(ctx, V):
 
 def pwa_nll_grad_batch_enqueue(ctx, V):
     V = _f64(V)
+    if V.ndim != 3 or V.shape[1:] != (_lib.pwa_n_waves(ctx), 2):
+        raise ValueError("V must be [K, n, 2]")
     _check(ctx, _lib.pwa_nll_grad_batch_enqueue(ctx, V.shape[0], V.ctypes.data))
 
 
@@ -280,8 +324,8 @@ def pwa_assemble_host(L_data, T, M, V):
 
 def pwa_fumili_hessian(ctx, V, with_norm=True):
     """-> H [2n, 2n] (Fumili-style approximate Hessian of nll, parameter order as in grad)."""
-    V = _f64(V)
-    n = V.shape[0]
+    n = _lib.pwa_n_waves(ctx)
+    V = _f64(V, (n, 2))
     H = np.zeros((2 * n, 2 * n))
     _check(ctx, _lib.pwa_fumili_hessian(ctx, V.ctypes.data, H.ctypes.data, 1 if with_norm else 0))
     return H
@@ -316,46 +360,107 @@ def pwa_polar_to_cartesian(r_phi):
     return V
 
 
-def pwa_res_grad(ctx, V, n_res):
+def pwa_res_grad(ctx, V, n_res=None):
+    """-> (d nll / d M_r, d nll / d G_r), [n_res] each; n_res is the wave map's (pwa_n_res), the argument is checked."""
     n = _lib.pwa_n_waves(ctx)
     V = _f64(V, (n, 2))
+    have = int(_lib.pwa_n_res(ctx))
+    if n_res is not None and int(n_res) != have:
+        raise ValueError(f"n_res = {n_res} but the wave map has {have} resonances")
+    n_res = have
     dM, dG = np.empty(n_res), np.empty(n_res)
     _check(ctx, _lib.pwa_res_grad(ctx, V.ctypes.data, dM.ctypes.data, dG.ctypes.data))
     return dM, dG
 
 
-def pwa_minimize_bfgs(ctx, V0, max_iter=200, gtol=1e-6):
+def pwa_minimize_bfgs(ctx, V0, max_iter=200, gtol=1e-6, want_iters=False):
+    """-> (V, nll, evaluations, status) (+ iterations when want_iters)."""
     n = _lib.pwa_n_waves(ctx)
     V = _f64(V0, (n, 2)).copy()
     nll = C.c_double(0.0)
     it, ev = C.c_int32(0), C.c_int32(0)
     st = _check(ctx, _lib.pwa_minimize_bfgs(ctx, V.ctypes.data, int(max_iter), float(gtol), C.byref(nll),
                                             C.byref(it), C.byref(ev)))
-    return V, nll.value, ev.value, st
+    return (V, nll.value, ev.value, st, it.value) if want_iters else (V, nll.value, ev.value, st)
 
 
 def pwa_minimize_bfgs_batch(ctx, V0, max_iter=300, gtol=1e-6):
+    V, nll, ev, st, _, _ = pwa_minimize_bfgs_batch_ex(ctx, V0, max_iter, gtol)
+    return V, nll, ev, st
+
+
+def pwa_minimize_bfgs_batch_ex(ctx, V0, max_iter=300, gtol=1e-6):
+    """-> (V[K,n,2], nll[K], evaluations, status, iterations[K], why[K] (PWA_FIT_*))."""
     V = _f64(V0).copy()
     K = V.shape[0]
+    if V.shape != (K, _lib.pwa_n_waves(ctx), 2):
+        raise ValueError("V0 must be [K, n, 2]")
     nll = np.empty(K)
+    its, why = np.zeros(K, dtype=np.int32), np.zeros(K, dtype=np.int32)
     ev = C.c_int32(0)
-    st = _check(ctx, _lib.pwa_minimize_bfgs_batch(ctx, K, V.ctypes.data, int(max_iter), float(gtol),
-                                                  nll.ctypes.data, C.byref(ev)))
-    return V, nll, ev.value, st
+    st = _check(ctx, _lib.pwa_minimize_bfgs_batch_ex(ctx, K, V.ctypes.data, int(max_iter), float(gtol), nll.ctypes.data,
+                                                     its.ctypes.data, why.ctypes.data, C.byref(ev)))
+    return V, nll, ev.value, st, its, why
 
 
 def pwa_minimize_bfgs_floating(ctx, V0, mass0, width0, free_res, max_iter=200, gtol=1e-6):
     """-> (V, mass, width, nll, iterations, evaluations, status): BFGS over V and the masses / widths of free_res."""
     n = _lib.pwa_n_waves(ctx)
+    return pwa_minimize_bfgs_floating_ex(ctx, V0, mass0, width0, free_res, max_iter, gtol)[:7]
+
+
+def pwa_minimize_bfgs_floating_ex(ctx, V0, mass0, width0, free_res, max_iter=200, gtol=1e-6):
+    """-> (V, mass, width, nll, iterations, evaluations, status, why (PWA_FIT_*))."""
+    n = _lib.pwa_n_waves(ctx)
+    nr = (_lib.pwa_n_res(ctx),)
     V = _f64(V0, (n, 2)).copy()
-    Mr, Gr = _f64(mass0).copy(), _f64(width0).copy()
+    Mr, Gr = _f64(mass0, nr).copy(), _f64(width0, nr).copy()
     fr = np.ascontiguousarray(free_res, dtype=np.int32)
     nll = C.c_double(0.0)
-    it, ev = C.c_int32(0), C.c_int32(0)
-    st = _check(ctx, _lib.pwa_minimize_bfgs_floating(ctx, V.ctypes.data, Mr.ctypes.data, Gr.ctypes.data, len(Mr),
-                                                     fr.ctypes.data, len(fr), int(max_iter), float(gtol),
-                                                     C.byref(nll), C.byref(it), C.byref(ev)))
-    return V, Mr, Gr, nll.value, it.value, ev.value, st
+    it, ev, why = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+    st = _check(ctx, _lib.pwa_minimize_bfgs_floating_ex(ctx, V.ctypes.data, Mr.ctypes.data, Gr.ctypes.data, len(Mr),
+                                                        fr.ctypes.data, len(fr), int(max_iter), float(gtol),
+                                                        C.byref(nll), C.byref(it), C.byref(ev), C.byref(why)))
+    return V, Mr, Gr, nll.value, it.value, ev.value, st, why.value
+
+
+def pwa_norm_sums(ctx):
+    """-> (G [n, n, 2] = B^H B of this context's MC events, N_gen of this shard)."""
+    n = _lib.pwa_n_waves(ctx)
+    G, ng = np.empty((n, n, 2)), C.c_int64(0)
+    _check(ctx, _lib.pwa_norm_sums(ctx, G.ctypes.data, C.byref(ng)))
+    return G, int(ng.value)
+
+
+def pwa_combine_norm_host(G, n_gen):
+    """G [R, n, n, 2], n_gen [R] -> (M [n, n, 2] of all shards, N_gen total); host only."""
+    G = _f64(G)
+    if G.ndim != 4 or G.shape[1] != G.shape[2] or G.shape[3] != 2:
+        raise ValueError("G must be [R, n, n, 2]")
+    R, n = G.shape[0], G.shape[1]
+    ng = np.ascontiguousarray(n_gen, dtype=np.int64)
+    if ng.shape != (R,):
+        raise ValueError("n_gen must be [R]")
+    M, tot = np.empty((n, n, 2)), C.c_int64(0)
+    _check(None, _lib.pwa_combine_norm_host(n, R, G.ctypes.data, ng.ctypes.data, M.ctypes.data, C.byref(tot)))
+    return M, int(tot.value)
+
+
+def pwa_assemble_host_shards(terms, M, V, likelihood=0, n_data=0.0, want_status=False):
+    """terms [R, 2 + 2n] (one pwa_data_term_enqueue record per shard) -> (nll, grad[n, 2], parts[2])."""
+    V = _f64(V)
+    n = V.shape[0]
+    terms = _f64(terms)
+    R = terms.shape[0]
+    if terms.shape != (R, 2 + 2 * n):
+        raise ValueError("terms must be [R, 2 + 2n]")
+    M = _f64(M, (n, n, 2))
+    nll = C.c_double(0.0)
+    grad, parts = np.empty((n, 2)), np.empty(2)
+    st = _lib.pwa_assemble_host_shards(n, R, terms.ctypes.data, M.ctypes.data, V.ctypes.data, int(likelihood),
+                                       float(n_data), C.byref(nll), grad.ctypes.data, parts.ctypes.data)
+    _check(None, st)
+    return (nll.value, grad, parts, st) if want_status else (nll.value, grad, parts)
 
 
 def pwa_launch_count(ctx):
@@ -370,6 +475,12 @@ def pwa_set_option(ctx, key, value):
     _check(ctx, _lib.pwa_set_option(ctx, key.encode(), int(value)))
 
 
+def pwa_get_option(ctx, key):
+    v = C.c_int32(0)
+    _check(ctx, _lib.pwa_get_option(ctx, key.encode(), C.byref(v)))
+    return int(v.value)
+
+
 def pwa_microbench(ctx, which, nbytes=0):
     out = C.c_double(0.0)
     _check(ctx, _lib.pwa_microbench(ctx, int(which), int(nbytes), C.byref(out)))
@@ -378,6 +489,18 @@ def pwa_microbench(ctx, which, nbytes=0):
 
 def pwa_n_waves(ctx):
     return int(_lib.pwa_n_waves(ctx))
+
+
+def pwa_n_res(ctx):
+    return int(_lib.pwa_n_res(ctx))
+
+
+def pwa_storage(ctx):
+    return int(_lib.pwa_storage(ctx))
+
+
+def pwa_n_events(ctx, which):
+    return int(_lib.pwa_n_events(ctx, int(which)))
 
 
 def pwa_last_error(ctx):

@@ -16,7 +16,6 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpwa.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-Wall", "--use_fast_math=false"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-Wall,-fopenmp"]   # OpenMP: host minimiser only (minimize.cpp)
 
 

@@ -240,7 +240,7 @@ k_batch_dmma(const void *__restrict__ Av, long long N, int n, const double *__re
 constexpr int BF_THREADS = 1024;
 __global__ void __launch_bounds__(BF_THREADS)
 k_batch_finalize(const double *__restrict__ scratch, int nslots, int NB, int n, const double *__restrict__ Vdev,
-                 int k0, const double *__restrict__ M, double *__restrict__ results, int result_stride, double n_eq2,
+                 int k0, const double *__restrict__ M, double *__restrict__ results, int result_stride, bool eq2, double n_eq2,
                  unsigned long long *done_flags, unsigned long long seq)
 {
     __shared__ double s_val[4][256];
@@ -284,7 +284,7 @@ k_batch_finalize(const double *__restrict__ scratch, int nslots, int NB, int n, 
         sV[2 * a + 1] = Vdev[((size_t)k * n + a) * 2 + 1];
     }
     __syncthreads();
-    assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n, n_eq2, done_flags + k, seq);
+    assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n, eq2, n_eq2, done_flags + k, seq);
 }
 
 template <typename ST, int NB, bool ALIGNED>
@@ -307,7 +307,7 @@ static pwa_status launch_bd(pwa_ctx *ctx, int K)
         const int cols = (K - k0 < BD_KC) ? (K - k0) : BD_KC;
         k_batch_finalize<<<cols, BF_THREADS, 0, ctx->stream>>>(ctx->d_scratch, (int)grid, NB, ctx->n, ctx->d_V, k0, ctx->d_M,
                                                         ctx->dev_result, result_stride(ctx->n),
-                                                        ctx->opt_likelihood == 1 ? (double)ctx->data.n_events : 0.0,
+                                                        ctx->opt_likelihood == 1, eq2_n_data(ctx),
                                                         ctx->dev_flags, ctx->seq);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());

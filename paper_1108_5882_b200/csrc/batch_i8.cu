@@ -591,7 +591,7 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
 __global__ void __launch_bounds__(1024)
 k_bi8_finalize(const double *__restrict__ slots, int nslots, int n, const double *__restrict__ Vdev, int k0,
                const int *__restrict__ ek, long long N, const double *__restrict__ M, double *__restrict__ results,
-               int result_stride, double n_eq2, unsigned long long *done_flags, unsigned long long seq)
+               int result_stride, bool eq2, double n_eq2, unsigned long long *done_flags, unsigned long long seq)
 {
     __shared__ double s_val[4][256];
     __shared__ double s_tot[2 + 2 * kFastWaves];
@@ -633,7 +633,7 @@ k_bi8_finalize(const double *__restrict__ slots, int nslots, int n, const double
         sV[2 * a + 1] = Vdev[((size_t)k * n + a) * 2 + 1];
     }
     __syncthreads();
-    assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n, n_eq2, done_flags + k, seq);
+    assemble_from_totals(s_tot, sV, M, results + (size_t)k * result_stride, n, eq2, n_eq2, done_flags + k, seq);
 }
 
 }  // namespace bi8
@@ -728,7 +728,7 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
         PWA_CUDA(ctx, cudaGetLastError());
         bi8::k_bi8_finalize<<<cols, 1024, 0, ctx->stream>>>(slots, (int)grid, ctx->n, ctx->d_V, k0, ek, N, ctx->d_M,
                                                             ctx->dev_result, result_stride(ctx->n),
-                                                            ctx->opt_likelihood == 1 ? (double)N : 0.0,
+                                                            ctx->opt_likelihood == 1, eq2_n_data(ctx),
                                                             ctx->dev_flags, ctx->seq);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());

@@ -431,7 +431,7 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     if (out_dev_terms) { fa.M = nullptr; fa.out = out_dev_terms; }
     else               { fa.M = ctx->d_M; fa.out = ctx->dev_result + (size_t)k * result_stride(n);
                          fa.done_flag = ctx->dev_flags + k; fa.seq = ctx->seq; }
-    fa.n_eq2 = ctx->opt_likelihood == 1 ? (double)ctx->data.n_events : 0.0;
+    fa.eq2 = ctx->opt_likelihood == 1; fa.n_eq2 = eq2_n_data(ctx);
 
     if (ctx->data.factored) {
         if (ctx->data.weights) return fail(ctx, PWA_ERR_UNSUPPORTED, "event weights are not supported with factored (floating-resonance) uploads");

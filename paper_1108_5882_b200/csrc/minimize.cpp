@@ -15,6 +15,9 @@ struct Bfgs {
     std::vector<double> x, g, H, p, xt, gt;
     double f = 0.0, t = 1.0, slope = 0.0;
     int iter = 0;
+    int small_steps = 0;      // consecutive accepted steps shorter than 2^-10 of the quasi-Newton step
+    int stall_limit = 0;      // > 0: that many of them in a row end the fit with PWA_FIT_LINE_SEARCH (noisy evaluations, see batch_ex)
+    int why = 0;              // why the fit stopped: PWA_FIT_CONVERGED / PWA_FIT_MAX_ITER / PWA_FIT_LINE_SEARCH
     bool done = false, have = false;
 
     void init(int dim, const double *x0)
@@ -44,13 +47,14 @@ struct Bfgs {
         const double c1 = 1e-4;
         if (!(isfinite(ft)) || ft > f + c1 * t * slope) {
             t *= 0.5;
-            if (t < 1e-20) done = true;
+            if (t < 1e-20) { done = true; why = PWA_FIT_LINE_SEARCH; }
             return false;
         }
         std::vector<double> s(d), y(d), Hy(d);
         double sy = 0.0;
         for (int i = 0; i < d; ++i) { s[i] = xt[i] - x[i]; y[i] = gt[i] - g[i]; sy += s[i] * y[i]; }
         x = xt; g = gt; f = ft; ++iter;
+        small_steps = (t < 0x1p-10 && iter > 1) ? small_steps + 1 : 0;
         double ss = 0.0, yy = 0.0;
         for (int i = 0; i < d; ++i) { ss += s[i] * s[i]; yy += y[i] * y[i]; }
         if (sy > 1e-12 * sqrt(ss * yy)) {
@@ -63,7 +67,9 @@ struct Bfgs {
                 for (int j = 0; j < d; ++j)
                     H[(size_t)i * d + j] += -rho * (Hy[i] * s[j] + s[i] * Hy[j]) + (rho * rho * yHy + rho) * s[i] * s[j];
         }
-        if (iter >= max_iter || gmax() < gtol) done = true;
+        if (gmax() < gtol) { done = true; why = PWA_FIT_CONVERGED; }
+        else if (iter >= max_iter) { done = true; why = PWA_FIT_MAX_ITER; }
+        else if (stall_limit > 0 && small_steps >= stall_limit) { done = true; why = PWA_FIT_LINE_SEARCH; }
         else direction(false);
         return true;
     }
@@ -76,27 +82,31 @@ extern "C" {
 pwa_status pwa_minimize_bfgs(pwa_ctx *ctx, double *V, int32_t max_iter, double gtol, double *nll_out,
                              int32_t *n_iter_out, int32_t *n_evals_out)
 {
-    int32_t evals = 0;
-    pwa_status s = pwa_minimize_bfgs_batch(ctx, 1, V, max_iter, gtol, nll_out, &evals);
-    if (n_evals_out) *n_evals_out = evals;
-    if (n_iter_out) *n_iter_out = -1;
-    return s;
+    return pwa_minimize_bfgs_batch_ex(ctx, 1, V, max_iter, gtol, nll_out, n_iter_out, nullptr, n_evals_out);
 }
 
-// internal: dimension is discovered through a probe evaluation buffer sized by the caller's n
 pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V, int32_t max_iter, double gtol,
                                    double *nll_out, int32_t *n_evals_out)
+{
+    return pwa_minimize_bfgs_batch_ex(ctx, K, V, max_iter, gtol, nll_out, nullptr, nullptr, n_evals_out);
+}
+
+pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V, int32_t max_iter, double gtol,
+                                      double *nll_out, int32_t *n_iter_out, int32_t *why_out, int32_t *n_evals_out)
 {
     if (!ctx || !V || K < 1 || K > 1024 || max_iter < 0) return PWA_ERR_INVALID_ARG;
     const int n = pwa_n_waves(ctx), d = 2 * n;
     std::vector<Bfgs> fit(K);
     std::vector<double> X((size_t)K * d), F(K), Gr((size_t)K * d);
+    std::vector<int> act(K);                    // the fits evaluated by the current batched calls (all K in the first stage)
+    for (int k = 0; k < K; ++k) act[k] = k;
     memcpy(X.data(), V, sizeof(double) * (size_t)K * d);
     int32_t evals = 0;
     pwa_status worst = PWA_OK;
-    auto eval = [&]() -> pwa_status {
-        pwa_status s = (K == 1) ? pwa_nll_grad(ctx, X.data(), F.data(), Gr.data(), nullptr)
-                                : pwa_nll_grad_batch(ctx, K, X.data(), F.data(), Gr.data(), nullptr);
+    auto eval = [&]() -> pwa_status {            // evaluates rows 0 .. act.size()-1 of X
+        const int Ka = (int)act.size();
+        pwa_status s = (Ka == 1) ? pwa_nll_grad(ctx, X.data(), F.data(), Gr.data(), nullptr)
+                                 : pwa_nll_grad_batch(ctx, Ka, X.data(), F.data(), Gr.data(), nullptr);
         evals += 1;
         if (s == PWA_WARN_NONFINITE) { worst = s; return PWA_OK; }
         return s;
@@ -110,28 +120,71 @@ pwa_status pwa_minimize_bfgs_batch(pwa_ctx *ctx, int32_t K, double *V, int32_t m
         fit[k].init(d, X.data() + (size_t)k * d);
         fit[k].f = F[k];
         memcpy(fit[k].g.data(), Gr.data() + (size_t)k * d, sizeof(double) * d);
-        if (max_iter == 0 || fit[k].gmax() < gtol) fit[k].done = true;
+        if (fit[k].gmax() < gtol) { fit[k].done = true; fit[k].why = PWA_FIT_CONVERGED; }
+        else if (max_iter == 0) { fit[k].done = true; fit[k].why = PWA_FIT_MAX_ITER; }
         else fit[k].direction(true);
     }
-    for (;;) {
-        bool any = false;
-        for (int k = 0; k < K; ++k) {
-            if (!fit[k].done) { fit[k].trial(); any = true; memcpy(X.data() + (size_t)k * d, fit[k].xt.data(), sizeof(double) * d); }
-            else memcpy(X.data() + (size_t)k * d, fit[k].x.data(), sizeof(double) * d);
+    auto lockstep = [&]() -> pwa_status {
+        const int Ka = (int)act.size();
+        for (;;) {
+            bool any = false;
+            for (int j = 0; j < Ka; ++j) {
+                Bfgs &b = fit[act[j]];
+                if (!b.done) { b.trial(); any = true; memcpy(X.data() + (size_t)j * d, b.xt.data(), sizeof(double) * d); }
+                else memcpy(X.data() + (size_t)j * d, b.x.data(), sizeof(double) * d);
+            }
+            if (!any) return PWA_OK;
+            pwa_status st = eval();
+            if (st != PWA_OK) return st;
+#pragma omp parallel for schedule(static) if (Ka >= 4)
+            for (int j = 0; j < Ka; ++j) {
+                Bfgs &b = fit[act[j]];
+                if (b.done) continue;
+                memcpy(b.gt.data(), Gr.data() + (size_t)j * d, sizeof(double) * d);
+                b.update(F[j], max_iter, gtol);
+            }
         }
-        if (!any) break;
-        s = eval();
-        if (s != PWA_OK) return s;
-#pragma omp parallel for schedule(static) if (K >= 4)
-        for (int k = 0; k < K; ++k) {
-            if (fit[k].done) continue;
-            memcpy(fit[k].gt.data(), Gr.data() + (size_t)k * d, sizeof(double) * d);
-            fit[k].update(F[k], max_iter, gtol);
+    };
+    // The int8 tensor-core path of the batched call (pwa_batch_path == 2) carries a non-smooth error of ~1e-8 |T| on
+    // the gradient and ~1e-9 |L_data| on nll.  Near the minimum the Armijo test then compares noise:
+    // the search backtracks ~30 times per iteration and accepts tiny steps by chance.  First stage: on that path three
+    // consecutive accepted steps shorter than 2^-10 of the quasi-Newton step end the fit (PWA_FIT_LINE_SEARCH: the
+    // resolution of this path is reached).  Second stage: such a fit is continued, from its current point and inverse
+    // Hessian, on the FP64 DMMA path ("batch" = 1) until gtol, max_iter or the fp64 resolution; only those fits are
+    // evaluated there.
+    int32_t path = -1;
+    const bool noisy = K > 1 && pwa_batch_path(ctx, &path, nullptr) == PWA_OK && path == 2;
+    if (noisy) for (int k = 0; k < K; ++k) fit[k].stall_limit = 3;
+    s = lockstep();
+    if (s != PWA_OK) return s;
+    if (noisy) {
+        act.clear();
+        for (int k = 0; k < K; ++k) if (fit[k].why == PWA_FIT_LINE_SEARCH && fit[k].iter < max_iter) act.push_back(k);
+        int32_t old_opt = 0;
+        if (!act.empty() && pwa_get_option(ctx, "batch", &old_opt) == PWA_OK && pwa_set_option(ctx, "batch", 1) == PWA_OK) {
+            const int Ka = (int)act.size();
+            for (int j = 0; j < Ka; ++j) memcpy(X.data() + (size_t)j * d, fit[act[j]].x.data(), sizeof(double) * d);
+            s = eval();
+            if (s == PWA_OK) {
+                for (int j = 0; j < Ka; ++j) {
+                    Bfgs &b = fit[act[j]];
+                    b.f = F[j];
+                    memcpy(b.g.data(), Gr.data() + (size_t)j * d, sizeof(double) * d);
+                    b.done = false; b.why = 0; b.stall_limit = 0; b.small_steps = 0;
+                    if (b.gmax() < gtol) { b.done = true; b.why = PWA_FIT_CONVERGED; }
+                    else b.direction(false);
+                }
+                s = lockstep();
+            }
+            pwa_set_option(ctx, "batch", old_opt);
+            if (s != PWA_OK) return s;
         }
     }
     for (int k = 0; k < K; ++k) {
         memcpy(V + (size_t)k * d, fit[k].x.data(), sizeof(double) * d);
         if (nll_out) nll_out[k] = fit[k].f;
+        if (n_iter_out) n_iter_out[k] = fit[k].iter;
+        if (why_out) why_out[k] = fit[k].why;
     }
     if (n_evals_out) *n_evals_out = evals;
     return worst;
@@ -141,12 +194,21 @@ pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V, double *mass, dou
                                       const int32_t *free_res, int32_t n_free, int32_t max_iter, double gtol,
                                       double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out)
 {
+    return pwa_minimize_bfgs_floating_ex(ctx, V, mass, width, n_res, free_res, n_free, max_iter, gtol, nll_out, n_iter_out,
+                                         n_evals_out, nullptr);
+}
+
+pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, double *width, int32_t n_res,
+                                         const int32_t *free_res, int32_t n_free, int32_t max_iter, double gtol,
+                                         double *nll_out, int32_t *n_iter_out, int32_t *n_evals_out, int32_t *why_out)
+{
     if (!ctx || !V || !mass || !width || n_res < 1 || n_res > 64 || n_free < 0 || n_free > n_res || (n_free > 0 && !free_res) || max_iter < 0)
         return PWA_ERR_INVALID_ARG;
     for (int i = 0; i < n_free; ++i) {
         if (free_res[i] < 0 || free_res[i] >= n_res) return PWA_ERR_INVALID_ARG;
         for (int j = 0; j < i; ++j) if (free_res[j] == free_res[i]) return PWA_ERR_INVALID_ARG;
     }
+    if (n_res != pwa_n_res(ctx)) return PWA_ERR_INVALID_ARG;      // mass / width arrays are sized by the wave map's n_res
     const int n = pwa_n_waves(ctx), d = 2 * n + 2 * n_free;
     // parameter vector: [Re V_0, Im V_0, ..., M_free[0..], G_free[0..]], minimised in SCALED variables u = x / sc:
     // sc = 1 for V, 1 % of the starting mass, 2 % of the starting width (the first step, normalised to |du| = 1,
@@ -194,7 +256,8 @@ pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V, double *mass, dou
     if (!isfinite(f0)) return PWA_ERR_INVALID_ARG;      // the starting point itself must be physical
     fit.init(d, u.data());
     fit.f = f0; fit.g = g;
-    if (max_iter == 0 || fit.gmax() < gtol) fit.done = true;
+    if (fit.gmax() < gtol) { fit.done = true; fit.why = PWA_FIT_CONVERGED; }
+    else if (max_iter == 0) { fit.done = true; fit.why = PWA_FIT_MAX_ITER; }
     else fit.direction(true);
     while (!fit.done) {
         fit.trial();
@@ -215,6 +278,7 @@ pwa_status pwa_minimize_bfgs_floating(pwa_ctx *ctx, double *V, double *mass, dou
     if (nll_out) *nll_out = fit.f;
     if (n_iter_out) *n_iter_out = fit.iter;
     if (n_evals_out) *n_evals_out = evals;
+    if (why_out) *why_out = fit.why;
     return worst;
 }
 

@@ -1,5 +1,6 @@
 // pwa_api.cu — the C ABI of include/pwa.h: context, uploads, call-order checks and the
-// host side of each evaluation (argument marshalling, one launch, one small D2H copy).
+// host side of each evaluation (argument marshalling and one launch; the finishing block of the
+// kernel writes the result record into device-mapped pinned host memory, so no D2H copy is enqueued).
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -138,11 +139,24 @@ static pwa_status wait_results(pwa_ctx *ctx, int K)
     return PWA_OK;
 }
 
+// V -> pinned staging h_V.  A previous enqueue may still be copying h_V to the device (cudaMemcpyAsync in
+// upload_V): the event recorded behind that copy is waited for first, so back-to-back enqueues with different V
+// never race ("V is copied before return", pwa.h).
 static pwa_status stage_V(pwa_ctx *ctx, int K, const double *V)
 {
     const size_t cnt = (size_t)K * 2 * ctx->n;
     if (!finite_all(V, cnt)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
+    if (ctx->ev_V_pending) { PWA_CUDA(ctx, cudaEventSynchronize(ctx->ev_V)); ctx->ev_V_pending = false; }
     memcpy(ctx->h_V, V, sizeof(double) * cnt);
+    return PWA_OK;
+}
+
+// staged h_V -> d_V on the context's stream (only the paths that read V from device memory need it)
+static pwa_status upload_V(pwa_ctx *ctx, int K)
+{
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * (size_t)K * 2 * ctx->n, cudaMemcpyHostToDevice, ctx->stream));
+    PWA_CUDA(ctx, cudaEventRecord(ctx->ev_V, ctx->stream));
+    ctx->ev_V_pending = true;
     return PWA_OK;
 }
 
@@ -151,9 +165,8 @@ static pwa_status enqueue_evals(pwa_ctx *ctx, int K, bool batched)
     const int n = ctx->n;
     const bool fast = (n == 4 || n == 8 || n == 16 || n == 32 || n == 64) && ctx->opt_data_term != 99;
     const bool need_dV = batched || (!fast && !ctx->data.factored);
-    if (need_dV)
-        PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * (size_t)K * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
     pwa_status s = PWA_OK;
+    if (need_dV) { s = upload_V(ctx, K); if (s != PWA_OK) return s; }
     ++ctx->seq;                                  // the finishing blocks publish this id in h_flags[k]
     if (batched) {
         s = launch_batch(ctx, K);
@@ -215,6 +228,16 @@ pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t
     if (e == cudaSuccess) memset(ctx->h_flags, 0, sizeof(unsigned long long) * kMaxK);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_V, sizeof(double) * kMaxK * 2 * n);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_V, sizeof(double) * kMaxK * 2 * n);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_V, cudaEventDisableTiming);
+    // per-block partial slots of every single-V pass (data term: 2 + 2n components, resonance gradient: up to
+    // 2 + 4 kMaxRes), sized here for the largest grid any launcher uses (<= 16 blocks per SM), so that no
+    // evaluation call ever allocates (pwa.h, general rules)
+    if (e == cudaSuccess) {
+        const size_t comps = (size_t)(2 + 2 * n_waves > 2 + 4 * kMaxRes ? 2 + 2 * n_waves : 2 + 4 * kMaxRes);
+        ctx->partials_cap = comps * (size_t)ctx->sm_count * 16;
+        e = cudaMalloc(&ctx->d_partials, ctx->partials_cap * sizeof(double));
+        if (e != cudaSuccess) ctx->partials_cap = 0;
+    }
     if (e != cudaSuccess) { cudaGetLastError(); pwa_destroy(ctx); return e == cudaErrorMemoryAllocation ? PWA_ERR_OOM : PWA_ERR_CUDA; }
     ctx->h_M.assign(2 * n * n, 0.0);
     *out = ctx;
@@ -235,6 +258,7 @@ void pwa_destroy(pwa_ctx *ctx)
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
     if (ctx->d_V) cudaFree(ctx->d_V);
     if (ctx->h_V) cudaFreeHost(ctx->h_V);
+    if (ctx->ev_V) cudaEventDestroy(ctx->ev_V);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_H) cudaFree(ctx->d_H);
@@ -306,8 +330,29 @@ pwa_status pwa_set_weights(pwa_ctx *ctx, pwa_sample which, const double *w, uint
         pwa_status s = take_buffer(ctx, w, (size_t)smp.n_events * sizeof(double), flags, &buf, &owned);
         if (s != PWA_OK) return s;
     }
+    // sum of the weights = N_data of the eq. 2 form (compensated, index order): found once here, on the host
+    double sum_w = 0.0;
+    if (buf != nullptr) {
+        const size_t cnt = (size_t)smp.n_events;
+        std::vector<double> tmp;
+        const double *hw = w;
+        if (is_device_ptr(w)) {
+            tmp.resize(cnt);
+            cudaError_t e = cudaMemcpy(tmp.data(), buf, cnt * sizeof(double), cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) { if (owned) cudaFree(buf); return cuda_fail(ctx, e, "reading the weights back"); }
+            hw = tmp.data();
+        }
+        double s = 0.0, c = 0.0;                     // Neumaier
+        for (size_t i = 0; i < cnt; ++i) {
+            const double x = hw[i], t = s + x;
+            c += (fabs(s) >= fabs(x)) ? (s - t) + x : (x - t) + s;
+            s = t;
+        }
+        sum_w = s + c;
+        if (!isfinite(sum_w)) { if (owned) cudaFree(buf); return fail(ctx, PWA_ERR_INVALID_ARG, "weights contain non-finite values"); }
+    }
     if (smp.weights_owned && smp.weights) cudaFree(smp.weights);
-    smp.weights = (double *)buf; smp.weights_owned = owned;
+    smp.weights = (double *)buf; smp.weights_owned = owned; smp.sum_w = sum_w;
     if (which == PWA_MC) ctx->M_valid = false;
     return PWA_OK;
 }
@@ -455,8 +500,8 @@ pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
     if (s != PWA_OK) return s;
     const int n = ctx->n;
     const bool fast = (n == 4 || n == 8 || n == 16 || n == 32 || n == 64) && ctx->opt_data_term != 99;
-    if (!fast && !ctx->data.factored)
-        PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
+    if (!fast && !ctx->data.factored) { s = upload_V(ctx, 1); if (s != PWA_OK) return s; }
+    ctx->last_K = 0;                             // no result record is written: a later pwa_fetch must not return a stale one
     return launch_data_term(ctx, ctx->h_V, 0, out_dev);
 }
 
@@ -481,6 +526,52 @@ pwa_status pwa_assemble_host(int32_t n, double L_data, const double *T, const do
     return PWA_OK;
 }
 
+pwa_status pwa_assemble_host_shards(int32_t n, int32_t R, const double *terms, const double *M, const double *V,
+                                    int32_t likelihood, double n_data, double *nll, double *grad, double *parts)
+{
+    if (n < 1 || R < 1 || !terms || !M || !V || !nll || !grad || (likelihood != 0 && likelihood != 1)) return PWA_ERR_INVALID_ARG;
+    const int NC = 2 + 2 * n;
+    std::vector<double> tot(terms, terms + NC);
+    for (int r = 1; r < R; ++r)                                     // shard order: the same bits on every rank
+        for (int c = 0; c < NC; ++c) tot[c] += terms[(size_t)r * NC + c];
+    pwa_status s = likelihood == 1 ? pwa_assemble_host_eq2(n, n_data, tot[0], tot.data() + 2, M, V, nll, grad, parts)
+                                   : pwa_assemble_host(n, tot[0], tot.data() + 2, M, V, nll, grad, parts);
+    if (s != PWA_OK) return s;
+    return (tot[1] != 0.0 || !finite_all(tot.data(), (size_t)NC)) ? PWA_WARN_NONFINITE : PWA_OK;
+}
+
+pwa_status pwa_norm_sums(pwa_ctx *ctx, double *G_out, int64_t *n_gen_out)
+{
+    if (!ctx || !G_out || !n_gen_out) return PWA_ERR_INVALID_ARG;
+    if (ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "no MC sample uploaded");
+    if (!ctx->M_valid) return fail(ctx, PWA_ERR_STATE, "normalisation matrix missing or stale: call pwa_build_norm");
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t cnt = 2 * (size_t)ctx->n * ctx->n;
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->h_M.data(), ctx->d_M, sizeof(double) * cnt, cudaMemcpyDeviceToHost, ctx->stream));
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    const double ng = (double)ctx->mc.n_gen;
+    for (size_t t = 0; t < cnt; ++t) G_out[t] = ctx->h_M[t] * ng;
+    *n_gen_out = ctx->mc.n_gen;
+    return PWA_OK;
+}
+
+pwa_status pwa_combine_norm_host(int32_t n, int32_t R, const double *G, const int64_t *n_gen, double *M_out,
+                                 int64_t *n_gen_total)
+{
+    if (n < 1 || R < 1 || !G || !n_gen || !M_out) return PWA_ERR_INVALID_ARG;
+    const size_t cnt = 2 * (size_t)n * n;
+    int64_t ng = 0;
+    for (int r = 0; r < R; ++r) { if (n_gen[r] < 0) return PWA_ERR_INVALID_ARG; ng += n_gen[r]; }
+    if (ng < 1) return PWA_ERR_INVALID_ARG;
+    for (size_t t = 0; t < cnt; ++t) M_out[t] = G[t];
+    for (int r = 1; r < R; ++r)                                     // shard order: the same bits on every rank
+        for (size_t t = 0; t < cnt; ++t) M_out[t] += G[(size_t)r * cnt + t];
+    const double den = (double)ng;
+    for (size_t t = 0; t < cnt; ++t) M_out[t] /= den;
+    if (n_gen_total) *n_gen_total = ng;
+    return PWA_OK;
+}
+
 pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t with_norm)
 {
     if (!ctx || !V || !H) return PWA_ERR_INVALID_ARG;
@@ -493,7 +584,8 @@ pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t 
     if (s != PWA_OK) return s;
     const size_t n = (size_t)ctx->n, cnt = 4 * n * n;
     if (ctx->data.n_events == 0) { memset(H, 0, sizeof(double) * cnt); return PWA_OK; }
-    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, ctx->h_V, sizeof(double) * 2 * n, cudaMemcpyHostToDevice, ctx->stream));
+    s = upload_V(ctx, 1);
+    if (s != PWA_OK) return s;
     // H goes through the tail of the M-partials scratch is NOT safe (the Gram kernel owns it): own buffer
     if (!ctx->d_H) PWA_CUDA(ctx, cudaMalloc(&ctx->d_H, sizeof(double) * cnt));
     s = launch_fumili(ctx, ctx->d_H, with_norm != 0);
@@ -564,6 +656,16 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx) { return ctx ? ctx->launches : 0; 
 
 int32_t pwa_n_waves(const pwa_ctx *ctx) { return ctx ? ctx->n : 0; }
 
+int32_t pwa_n_res(const pwa_ctx *ctx) { return ctx ? ctx->n_res : 0; }
+
+int64_t pwa_n_events(const pwa_ctx *ctx, pwa_sample which)
+{
+    if (!ctx || (which != PWA_DATA && which != PWA_MC)) return -1;
+    return which == PWA_DATA ? ctx->data.n_events : ctx->mc.n_events;
+}
+
+pwa_dtype pwa_storage(const pwa_ctx *ctx) { return ctx ? ctx->storage : PWA_F64; }
+
 pwa_status pwa_sync(pwa_ctx *ctx)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
@@ -579,6 +681,18 @@ pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
     else if (!strcmp(key, "batch")) ctx->opt_batch = value;
     else if (!strcmp(key, "l2_resident_mb")) { if (value < -1 || value > 120) return fail(ctx, PWA_ERR_INVALID_ARG, "l2_resident_mb must be in [-1, 120]"); ctx->opt_l2_resident_mb = value; }
     else if (!strcmp(key, "likelihood")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "likelihood must be 0 (eq. 3) or 1 (eq. 2)"); ctx->opt_likelihood = value; }
+    else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
+    return PWA_OK;
+}
+
+pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value)
+{
+    if (!ctx || !key || !value) return PWA_ERR_INVALID_ARG;
+    if (!strcmp(key, "data_term")) *value = ctx->opt_data_term;
+    else if (!strcmp(key, "norm")) *value = ctx->opt_norm;
+    else if (!strcmp(key, "batch")) *value = ctx->opt_batch;
+    else if (!strcmp(key, "l2_resident_mb")) *value = ctx->opt_l2_resident_mb;
+    else if (!strcmp(key, "likelihood")) *value = ctx->opt_likelihood;
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
 }

@@ -29,6 +29,7 @@ struct Sample {
     double *mass = nullptr; void *ang = nullptr; bool fact_owned = false; int n_ang = 0;
     bool factored = false;
     double *weights = nullptr; bool weights_owned = false;   // optional per-event weights (NEXT-3), [n_events]
+    double sum_w = 0.0;     // sum of the weights (compensated, index order; found once in pwa_set_weights): N_data of eq. 2
     int64_t n_events = -1;  // -1 = not uploaded
     int64_t n_gen = 0;
 };
@@ -49,6 +50,7 @@ struct pwa_ctx {
     pwa::Sample data, mc;
     // floating mode
     int n_res = 0;
+    cudaEvent_t ev_V = nullptr; bool ev_V_pending = false;   // recorded after the H2D copy of the staged V (h_V may be refilled only after it)
     std::vector<int32_t> res_of_wave, ang_of_wave;
     std::vector<int32_t> wave_of_pair;        // [n_res * kMaxAng] -> wave or -1
     std::vector<double> mass0, width0;
@@ -91,6 +93,8 @@ namespace pwa {
 pwa_status fail(pwa_ctx *ctx, pwa_status s, const std::string &msg);
 pwa_status cuda_fail(pwa_ctx *ctx, cudaError_t e, const char *what);
 pwa_status ensure_partials(pwa_ctx *ctx, size_t doubles);
+// N_data of the eq. 2 form: the number of data events, or the sum of their weights for a weighted sample
+inline double eq2_n_data(const pwa_ctx *ctx) { return ctx->data.weights ? ctx->data.sum_w : (double)(ctx->data.n_events > 0 ? ctx->data.n_events : 0); }
 pwa_status ensure_scratch(pwa_ctx *ctx, size_t bytes);
 
 #define PWA_CUDA(ctx, call)                                                   \

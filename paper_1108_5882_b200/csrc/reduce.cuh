@@ -18,7 +18,8 @@ struct FinishArgs {
     const double *M;       // device [n][n][2]; nullptr -> data-term-only output
     double *out;           // result record (M != nullptr) or [NC] components (M == nullptr)
     int n;
-    double n_eq2 = 0.0;    // 0: eq. 3 extended form; > 0: eq. 2 normalised form with N_data = n_eq2
+    bool eq2 = false;      // false: eq. 3 extended form; true: eq. 2 normalised form with
+    double n_eq2 = 0.0;    //   N_data = n_eq2 (the number of data events, or the sum of their weights)
     // result delivery without a copy: `out` may be device-mapped pinned HOST memory; after the record is
     // written (system-scope fence) done_flag[0] = seq tells the polling host thread it is complete
     unsigned long long *done_flag = nullptr;
@@ -41,10 +42,10 @@ __device__ __forceinline__ double warp_sum(double x)
 // shared memory: M == nullptr -> copy the data-term components to out[0..2+2n); otherwise write
 // the result record {nll, L_data, Norm, n_nonfinite, grad[2n]} (P:41 second term).
 // Must be called by every thread of the block; s_tot and sV valid for all threads on entry.
-// n_eq2 = 0: nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V                      (eq. 3)
-// n_eq2 = N_data > 0: nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2)
+// eq2 false: nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V                      (eq. 3)
+// eq2 true, n_eq2 = N_data (or sum of weights): nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2)
 __device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
-                                            double *out, int n, double n_eq2 = 0.0,
+                                            double *out, int n, bool eq2 = false, double n_eq2 = 0.0,
                                             unsigned long long *done_flag = nullptr, unsigned long long seq = 0)
 {
     const int NC = 2 + 2 * n;
@@ -82,14 +83,14 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
         double acc = 0.0;   // Norm = sum_a Re( conj(V_a) (M V)_a )
         for (int a = lane; a < n; a += 32) acc += sV[2 * a] * s_mv[2 * a] + sV[2 * a + 1] * s_mv[2 * a + 1];
         acc = warp_sum(acc);   // xor tree: every lane holds the same Norm
-        const double gw = (n_eq2 > 0.0) ? 2.0 * (n_eq2 / acc) : 2.0;
+        const double gw = eq2 ? 2.0 * (n_eq2 / acc) : 2.0;
         // grad_a = -2 conj(T_a) + gw (M V)_a
         for (int a = lane; a < n; a += 32) {
             out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + gw * s_mv[2 * a];
             out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + gw * s_mv[2 * a + 1];
         }
         if (lane == 0) {
-            out[0] = (n_eq2 > 0.0) ? (-s_tot[0] + n_eq2 * log(acc)) : -(s_tot[0] - acc);
+            out[0] = eq2 ? (-s_tot[0] + n_eq2 * log(acc)) : -(s_tot[0] - acc);
             out[1] = s_tot[0];
             out[2] = acc;
             out[3] = s_tot[1];
@@ -167,7 +168,7 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
     }
     __syncthreads();
 
-    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.n_eq2, fa.done_flag, fa.seq);
+    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq);
     if (tid == 0) *fa.ticket = 0u;   // re-arm for the next launch on this stream
 }
 

@@ -7,6 +7,8 @@
 // The event-independent factors are pulled out: one complex accumulator per resonance,
 //   U_r = sum_i w_{r,i} BW_r(m_i)^2 * f_i,   f_i = 1/S_i (data) or conj(S_i) (MC),
 // and the host applies -(2M - iG) and iM.  Thread per event; warp + block tree as in A5.
+// The MC pass also sums |S_j|^2 (component 0 of its record): Norm = sum_j |S_j|^2 / N_gen at the CURRENT resonance
+// parameters, which the eq. 2 form needs (d nll2 / d theta = -d L_data + (N_data / Norm) d Norm, reading C2).
 #include "factored.cuh"
 #include "reduce.cuh"
 
@@ -58,6 +60,10 @@ k_res_grad(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs fa)
         if (mode == 0) { const double inv = 1.0 / (sr * sr + si * si); fr = sr * inv; fi = -si * inv; }
         else           { fr = sr; fi = -si; }
         if (!valid) { fr = 0.0; fi = 0.0; }
+        if (mode == 1) {                         // uniform branch
+            const double i2 = warp_sum(valid ? sr * sr + si * si : 0.0);
+            if (lane == 0) s_acc[warp][0] += i2;
+        }
         for (int r = 0; r < n_res; ++r) {
             const double2 bw = bw_eval(mm, f.rp.m2[r], f.rp.mg[r]);
             double wr = 0.0, wi = 0.0;
@@ -110,6 +116,7 @@ k_res_grad_fast(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs 
     double ur[NR], ui[NR];
 #pragma unroll
     for (int r = 0; r < NR; ++r) { ur[r] = 0.0; ui[r] = 0.0; }
+    double i2 = 0.0;                             // MC pass: sum_j |S_j|^2
     const long long stride = (long long)gridDim.x * RG_THREADS;
     for (long long i = (long long)blockIdx.x * RG_THREADS + tid; i < N; i += stride) {
         const double m = __ldg(f.mass + i), mm = m * m;
@@ -134,7 +141,7 @@ k_res_grad_fast(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs 
         }
         double fr, fi;
         if (mode == 0) { const double inv = 1.0 / (sr * sr + si * si); fr = sr * inv; fi = -si * inv; }
-        else           { fr = sr; fi = -si; }
+        else           { fr = sr; fi = -si; i2 = fma(sr, sr, i2); i2 = fma(si, si, i2); }
 #pragma unroll
         for (int r = 0; r < NR; ++r) {
             ur[r] = fma(pr[r], fr, ur[r]); ur[r] = fma(-pi[r], fi, ur[r]);
@@ -146,7 +153,8 @@ k_res_grad_fast(long long N, int mode, int n, VArg varg, FactArgs f, FinishArgs 
         const double a = warp_sum(ur[r]), b = warp_sum(ui[r]);
         if (lane == 0) { s_acc[warp][2 + 2 * r] = a; s_acc[warp][3 + 2 * r] = b; }
     }
-    if (lane == 0) { s_acc[warp][0] = 0.0; s_acc[warp][1] = 0.0; }
+    i2 = warp_sum(i2);
+    if (lane == 0) { s_acc[warp][0] = i2; s_acc[warp][1] = 0.0; }
     __syncthreads();
     for (int c = tid; c < NC; c += RG_THREADS) {
         double t = 0.0;
@@ -201,6 +209,10 @@ pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG
     ctx->last_K = 0;
     const double *Ud = ctx->h_result + 2, *Um = ctx->h_result + NC + 2;
     const double inv_ngen = 1.0 / (double)ctx->mc.n_gen;
+    // eq. 3: nll = -L_data + Norm;  eq. 2 ("likelihood" = 1): nll2 = -L_data + N_data ln Norm, so the Norm part of the
+    // derivative carries N_data / Norm (Norm from the MC pass itself: valid for the current resonance parameters)
+    const double norm_now = ctx->h_result[NC] * inv_ngen;
+    const double wN = ctx->opt_likelihood == 1 ? eq2_n_data(ctx) / norm_now : 1.0;
     for (int r = 0; r < nr; ++r) {
         const double M = ctx->mass0[r], G = ctx->width0[r];
         // Re( -(2M - iG) U ) = -(2M Ur + G Ui) ;  Re( iM U ) = -M Ui
@@ -208,8 +220,8 @@ pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG
         const double dL_dG = 2.0 * (-M * Ud[2 * r + 1]);
         const double dN_dM = 2.0 * inv_ngen * (-(2.0 * M * Um[2 * r] + G * Um[2 * r + 1]));
         const double dN_dG = 2.0 * inv_ngen * (-M * Um[2 * r + 1]);
-        dM[r] = -dL_dM + dN_dM;
-        dG[r] = -dL_dG + dN_dG;
+        dM[r] = -dL_dM + wN * dN_dM;
+        dG[r] = -dL_dG + wN * dN_dG;
     }
     return PWA_OK;
 }

@@ -42,7 +42,7 @@ def check_eval(res, ref, tol, N, gscale=0.0):
     norm-wise on the terms that are actually summed)."""
     nll, g, parts = res[0], res[1], res[2]
     nll_o, g_o, parts_o = ref[0], ref[1], ref[2]
-    scaleL = max(abs(parts_o[0]), 1e-2 * N, 1e-300)
+    scaleL = max(abs(parts_o[0]), 1e-300)                   # DESIGN.md C8 as written: |dL| <= tol |L_data|, |dnll| <= tol max(|nll|, |L_data|)
     assert abs(parts[0] - parts_o[0]) <= tol * scaleL, ("L_data", parts[0], parts_o[0])
     assert abs(parts[1] - parts_o[1]) <= tol * max(abs(parts_o[1]), 1e-300), ("Norm", parts[1], parts_o[1])
     assert abs(nll - nll_o) <= tol * max(abs(nll_o), scaleL), ("nll", nll, nll_o)
@@ -251,7 +251,7 @@ def test_res_grad_parity(pwa, oracle, synth):
         dM, dG = pwa.pwa_res_grad(c.ctx, V, w.n_res)
     ref = np.concatenate([-dLM + dNM, -dLG + dNG])
     got = np.concatenate([dM, dG])
-    assert np.abs(got - ref).max() <= 1e-11 * np.abs(ref).max()
+    assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
 def test_bfgs_floating_resonances(pwa, oracle, synth):
@@ -580,7 +580,7 @@ def test_fumili_hessian_parity(pwa, oracle, storage, n, N):
     symmetry; PSD data part; Euler identity H_data V = 2 grad(L_data) on the GPU result alone."""
     A, B, V = rand_case(900 + n + N, N, 2001, n, storage)
     M_o = oracle.norm_matrix(B, 2100)
-    tol = TOL[storage] * (1 if storage == "f32" else 10)       # 1e-11 for fp64: outer products of 1/S amplify |A|/|S|
+    tol = TOL[storage]                                         # measured 4e-16 .. 8e-15 for fp64 storage
     with Ctx(pwa, n, storage) as c:
         pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
         pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2100)
@@ -609,7 +609,7 @@ def test_fumili_factored(pwa, oracle, synth):
     with _factored_ctx(pwa, w, Mr, Gr) as c:
         pwa.pwa_build_norm(c.ctx, want_M=False)
         H = pwa.pwa_fumili_hessian(c.ctx, V)
-    assert np.abs(H - H_o).max() <= 1e-11 * np.abs(H_o).max()
+    assert np.abs(H - H_o).max() <= 1e-12 * np.abs(H_o).max()
 
 
 # ------------------------------------------------------------------ NEXT-3: per-event weights
@@ -642,9 +642,8 @@ def test_event_weights_parity(pwa, oracle, storage, n):
         for k in range(K):
             L, T, _ = oracle.data_term_w(A, Vk[k], wd)
             ref = oracle.assemble(L, T, M_o, Vk[k])
-            scale = np.abs(wd).sum() / N                               # sum |w_i l_i| scale for the tolerance
-            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol * max(1.0, scale) * 4, N)
-            check_eval((nllk[k], gk[k], partsk[k]), ref, tol * max(1.0, scale) * 4, N)
+            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol, N)
+            check_eval((nllk[k], gk[k], partsk[k]), ref, tol, N)
         pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, None)
         pwa.pwa_set_weights(c.ctx, pwa.PWA_MC, None)
         assert np.array_equal(pwa.pwa_build_norm(c.ctx), M_plain)
@@ -666,3 +665,180 @@ def test_event_weights_integer_multiplicity(pwa, oracle):
         pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.repeat(A, k, axis=0))     # a new upload drops the weights
         b = pwa.pwa_nll_grad(c.ctx, V)
     check_eval(a, b, 1e-12, N)
+
+
+# ------------------------------------------------------------------ eq. 2 form with event weights (N_data = sum of weights)
+@pytest.mark.parametrize("storage,n", [("f64", 16), ("f32", 64), ("f64", 5)])
+def test_eq2_with_event_weights(pwa, oracle, storage, n):
+    """nll2 = -sum_i w_i ln I_i + (sum_i w_i) ln Norm: against the oracle's eq. 2 assembly with N_data = sum w;
+    integer weights == repeated events also under eq. 2; invariance under V -> s V is kept with weights."""
+    N, K = 5003, 9
+    A, B, V = rand_case(40 + n, N, 2001, n, storage)
+    rng = np.random.default_rng(3 * n)
+    wd = rng.uniform(0.2, 2.5, size=N)
+    mult = rng.integers(0, 4, size=N)
+    Vk = rng.normal(size=(K, n, 2))
+    M_o = oracle.norm_matrix(B, 2100)
+    tol = TOL[storage]
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2100)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, wd)
+        L, T, _ = oracle.data_term_w(A, V, wd)
+        ref = oracle.assemble_eq2(float(np.sum(wd)), L, T, M_o, V)
+        check_eval(pwa.pwa_nll_grad(c.ctx, V), ref, tol, N)
+        nllk, gk, partsk = pwa.pwa_nll_grad_batch(c.ctx, Vk)            # weighted batched call (K weighted passes)
+        for k in (0, K - 1):
+            Lk, Tk, _ = oracle.data_term_w(A, Vk[k], wd)
+            check_eval((nllk[k], gk[k], partsk[k]), oracle.assemble_eq2(float(np.sum(wd)), Lk, Tk, M_o, Vk[k]), tol, N)
+        a, b = pwa.pwa_nll_grad(c.ctx, V), pwa.pwa_nll_grad(c.ctx, 2.5 * V)
+        assert abs(a[0] - b[0]) <= 1e-12 * max(abs(a[0]), abs(a[2][0]))   # scale invariance needs N_data = sum w
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, mult.astype(float))
+        wi = pwa.pwa_nll_grad(c.ctx, V)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.repeat(A, mult, axis=0))
+        rep = pwa.pwa_nll_grad(c.ctx, V)
+        check_eval(wi, rep, 1e-12 if storage == "f64" else tol, N)
+        with pytest.raises(ValueError):                                   # one weight per event of the uploaded sample
+            pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, np.ones(N))
+
+
+# ------------------------------------------------------------------ floating resonances under the eq. 2 form
+def test_res_grad_eq2_form(pwa, oracle, synth):
+    """pwa_res_grad with "likelihood" = 1 differentiates nll2 = -L_data + N ln Norm: against the oracle's pieces
+    (-dL + (N / Norm) dNorm) and against central differences of the GPU's own nll2 in (M_r, G_r)."""
+    w = synth.make_workload(3, n_data=20_011, n_mc=30_011, full_amplitudes=False)
+    Mr, Gr = synth.floating_start(w)
+    V = synth.eval_points(w, 1)[0]
+    dLM, dLG = oracle.res_grad(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 0)
+    dNM, dNG = oracle.res_grad(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 1, w.n_gen)
+    B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    norm_o = oracle.norm_explicit(B, w.n_gen, V)[0]
+    wN = w.n_data / norm_o
+    ref = np.concatenate([-dLM + wN * dNM, -dLG + wN * dNG])
+    with _factored_ctx(pwa, w, Mr, Gr) as c:
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        dM, dG = pwa.pwa_res_grad(c.ctx, V)
+        got = np.concatenate([dM, dG])
+        assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+
+        def nll2(Mx, Gx):
+            pwa.pwa_set_resonances(c.ctx, Mx, Gx)
+            pwa.pwa_build_norm(c.ctx, want_M=False)
+            return pwa.pwa_nll_grad(c.ctx, V)[0]
+        for r in (0, 3, 6):
+            h = 1e-6
+            Mp, Mm = Mr.copy(), Mr.copy(); Mp[r] += h; Mm[r] -= h
+            fd = (nll2(Mp, Gr) - nll2(Mm, Gr)) / (2 * h)
+            assert abs(fd - dM[r]) <= 1e-5 * np.abs(ref).max(), (r, fd, dM[r])
+            Gp, Gm = Gr.copy(), Gr.copy(); Gp[r] += h; Gm[r] -= h
+            fd = (nll2(Mr, Gp) - nll2(Mr, Gm)) / (2 * h)
+            assert abs(fd - dG[r]) <= 1e-5 * np.abs(ref).max(), (r, fd, dG[r])
+        with pytest.raises(ValueError):
+            pwa.pwa_res_grad(c.ctx, V, n_res=w.n_res - 1)
+
+
+def test_bfgs_floating_eq2_form(pwa, synth):
+    """The floating-resonance minimiser with "likelihood" = 1: objective and ALL gradient components are the eq. 2
+    form, so the fit descends and ends (nearly) stationary; nll2 is scale-invariant, so Norm is not driven to N."""
+    w = synth.make_workload(3, n_data=20_011, n_mc=60_011, full_amplitudes=False)
+    Mr0, Gr0 = synth.floating_start(w)
+    free = np.arange(w.n_free, dtype=np.int32)
+    with _factored_ctx(pwa, w, Mr0, Gr0) as c:
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        nll_start, g_start, _ = pwa.pwa_nll_grad(c.ctx, w.V_true)
+        V, Mr, Gr, nll, iters, evals, st, why = pwa.pwa_minimize_bfgs_floating_ex(c.ctx, w.V_true, Mr0, Gr0, free,
+                                                                                 max_iter=400, gtol=1e-2)
+        assert nll < nll_start and iters >= 5 and why in (pwa.PWA_FIT_CONVERGED, pwa.PWA_FIT_MAX_ITER, pwa.PWA_FIT_LINE_SEARCH)
+        nll_fit, g_fit, _ = pwa.pwa_nll_grad(c.ctx, V)
+        dM, dG = pwa.pwa_res_grad(c.ctx, V)
+        assert nll_fit == nll
+        assert np.abs(g_fit).max() <= 1e-2 * np.abs(g_start).max()
+        with pytest.raises(pwa.PwaError) as e:                            # mass / width arrays sized by another n_res
+            pwa._check(c.ctx, pwa._lib.pwa_minimize_bfgs_floating(c.ctx, V.ctypes.data, Mr.ctypes.data, Gr.ctypes.data,
+                                                                  w.n_res - 1, free.ctypes.data, len(free), 1, 1e-3,
+                                                                  None, None, None))
+        assert e.value.status == pwa.PWA_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------ binding / ABI argument checks and async hazards
+def test_binding_rejects_wrong_dtype_and_shape(pwa):
+    with Ctx(pwa, 4, "f64") as c:
+        with pytest.raises(TypeError):
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.ones((8, 4, 2), dtype=np.float32))
+        with pytest.raises(ValueError):
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.ones((8, 5, 2)))
+        with pytest.raises(ValueError):
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.ones((8, 4, 2)), n_events=9)
+        with pytest.raises(ValueError):
+            pwa.pwa_set_wave_map(c.ctx, 2, [0, 1, 1], [0, 0, 1])
+        pwa.pwa_set_wave_map(c.ctx, 2, [0, 0, 1, 1], [0, 1, 0, 1])
+        assert pwa.pwa_n_res(c.ctx) == 2 and pwa.pwa_storage(c.ctx) == pwa.PWA_F64
+        with pytest.raises(ValueError):
+            pwa.pwa_set_resonances(c.ctx, [1.5, 1.7, 2.0], [0.1, 0.1, 0.1])
+        with pytest.raises(ValueError):
+            pwa.pwa_fumili_hessian(c.ctx, np.ones((5, 2)))
+        assert pwa.pwa_n_events(c.ctx, pwa.PWA_DATA) == -1
+    with Ctx(pwa, 4, "f32") as c:
+        with pytest.raises(TypeError):
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, np.ones((8, 4, 2)), n_generated=8)
+
+
+def test_async_hazards(pwa):
+    """(a) two batched enqueues with different V back to back: the second must not overwrite the pinned staging of
+    the first while its H2D copy is in flight; (b) pwa_fetch after pwa_data_term_enqueue has no record to return."""
+    import torch
+    n, N, K = 16, 200_003, 40
+    A, B, _ = rand_case(12, N, 3001, n, "f64")
+    rng = np.random.default_rng(1)
+    V1, V2 = rng.normal(size=(K, n, 2)), rng.normal(size=(K, n, 2))
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=3001)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        lone1, lone2 = pwa.pwa_nll_grad_batch(c.ctx, V1), pwa.pwa_nll_grad_batch(c.ctx, V2)
+        for rep in range(5):
+            pwa.pwa_nll_grad_batch_enqueue(c.ctx, V1)
+            pwa.pwa_nll_grad_batch_enqueue(c.ctx, V2)
+            nll, g, parts = pwa.pwa_fetch(c.ctx, K)
+            assert np.array_equal(nll, lone2[0]) and np.array_equal(g, lone2[1])
+            pwa.pwa_nll_grad_batch_enqueue(c.ctx, V2)
+            pwa.pwa_nll_grad_batch_enqueue(c.ctx, V1)
+            nll, g, parts = pwa.pwa_fetch(c.ctx, K)
+            assert np.array_equal(nll, lone1[0]) and np.array_equal(g, lone1[1])
+        out = torch.zeros(2 + 2 * n, dtype=torch.float64, device="cuda")
+        pwa.pwa_nll_grad_enqueue(c.ctx, V1[0])
+        pwa.pwa_data_term_enqueue(c.ctx, V1[1], out)
+        with pytest.raises(pwa.PwaError) as e:
+            pwa.pwa_fetch(c.ctx, 1)
+        assert e.value.status == pwa.PWA_ERR_STATE
+
+
+def test_bfgs_reports_iterations_and_two_stage_batch(pwa):
+    """pwa_minimize_bfgs returns its real iteration count; the batched minimiser on the int8 path continues fits whose
+    line search ran out of resolution on the FP64 path and restores the "batch" option."""
+    n, N, K = 64, 40_000, 8
+    rng = np.random.default_rng(21)
+    A = (rng.normal(size=(N, n, 2)) * 0.35).astype(np.float32)
+    V0 = rng.normal(size=(K, n, 2))
+    with Ctx(pwa, n, "f32") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, A[:20_000], n_generated=25_000)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        V, nll, evals, st, its = pwa.pwa_minimize_bfgs(c.ctx, V0[0], max_iter=7, gtol=0.0, want_iters=True)
+        assert its == 7 and evals >= 8
+        # gtol = 0: the int8 stage cannot converge; it must detect its noise floor (three tiny accepted steps in a row),
+        # hand the fits to the FP64 stage, and that stage drives the gradient ~1e4 x lower than int8 alone reaches
+        # (measured: <= 7e-7 against 1e-4 .. 1e-3 with the int8 path alone after 8000 iterations)
+        Vf, nllf, evals, st, its, why = pwa.pwa_minimize_bfgs_batch_ex(c.ctx, V0, max_iter=3000, gtol=0.0)
+        assert pwa.pwa_get_option(c.ctx, "batch") == 0                    # option restored
+        assert pwa.pwa_batch_path(c.ctx)[0] == 1                          # the last batched calls were the FP64 stage
+        assert set(why.tolist()) <= {pwa.PWA_FIT_MAX_ITER, pwa.PWA_FIT_LINE_SEARCH}
+        assert (its > 10).all()
+        for k in range(K):
+            one = pwa.pwa_nll_grad(c.ctx, Vf[k])
+            assert one[0] == pytest.approx(nllf[k], rel=1e-12)
+            assert one[2][1] == pytest.approx(N, rel=1e-7)                # P7: Norm = N_data at a stationary point of eq. 3
+            assert np.abs(one[1]).max() < 1e-5

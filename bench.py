@@ -240,6 +240,45 @@ class Timer:
         return e0.elapsed_time(e1) / steps, wall / steps * 1e3      # ms per step (device, wall)
 
 
+SIDE_STEPS, SIDE_WARMUP = 10, 3      # every side measurement: >= 10 timed steps after 3 warm-ups
+
+
+def measure_peaks(pwa, ctx, mp_hbm, mp_src):
+    """Roofline denominators.  HBM: MEASURED_PEAKS.json (driver-written copy bandwidth).  FP64: MEASURED_PEAKS has
+    no fp64 figure, so the register-resident DFMA and mma.sync.m8n8k4.f64 loops of pwa_microbench are run here
+    (SURVEY 8(d) "Denominators").  int8 tensor: the guide's nominal dense figure (2 x the nominal fp8 4.5 PFLOP/s
+    is sparse; dense int8 = 4.5 Pop/s)."""
+    return {"hbm_gbs": mp_hbm, "hbm_source": mp_src,
+            "dfma_tflops": pwa.pwa_microbench(ctx, 0), "dmma_tflops": pwa.pwa_microbench(ctx, 1),
+            "hbm_read_gbs": pwa.pwa_microbench(ctx, 2, 4 << 30),
+            "fp64_source": "measured here: pwa_microbench(0 | 1), register-resident loops, best of 5",
+            "hbm_read_source": "measured here: pwa_microbench(2), read-only stream over 4 GiB",
+            "int8_tops_nominal": 4500.0}
+
+
+def rl_hbm(peaks, nbytes, ms, **kw):
+    a = nbytes / ms * 1e-6
+    r = {"bound": "hbm", "achieved": a, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": a / peaks["hbm_gbs"],
+         "peak_source": peaks["hbm_source"], "algorithmic_bytes_per_launch": nbytes}
+    r.update(kw)
+    return r
+
+
+def rl_flops(peaks, bound, flops, ms, **kw):
+    """bound: 'tensor' (fp64 DMMA), 'alu' (fp64 FMA) or 'tensor_int8' (nominal peak)."""
+    a = flops / ms * 1e-9
+    if bound == "tensor":
+        peak, src, unit = peaks["dmma_tflops"], peaks["fp64_source"], "TFLOP/s"
+    elif bound == "alu":
+        peak, src, unit = peaks["dfma_tflops"], peaks["fp64_source"], "TFLOP/s"
+    else:
+        peak, src, unit = peaks["int8_tops_nominal"], "nominal dense int8 (B200 guide)", "Top/s"
+    r = {"bound": bound.split("_")[0], "achieved": a, "peak": peak, "unit": unit, "frac": a / peak, "peak_source": src,
+         "algorithmic_flops_per_launch": flops}
+    r.update(kw)
+    return r
+
+
 def upload_constant(pwa, ctx, w):
     t0 = time.perf_counter()
     pwa.pwa_upload_events(ctx, pwa.PWA_DATA, w.A_data)
@@ -247,7 +286,24 @@ def upload_constant(pwa, ctx, w):
     return time.perf_counter() - t0
 
 
-def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
+def m_build_record(pwa, tm, ctx, w, n, elem, peaks):
+    ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), SIDE_STEPS, SIDE_WARMUP)
+    bound, path = pwa.pwa_norm_error_bound(ctx)
+    nbytes = w.n_acc * n * 2 * elem
+    flops_sym = 4.0 * n * n * w.n_acc                       # Hermitian symmetry used: half of the 8 n^2 N full Gram
+    rec = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": 2 * flops_sym / ms_m * 1e-6, "mc_gbs": nbytes / ms_m * 1e-6,
+           "path": "int8 tcgen05 (digit planes, int32 TMEM)" if path == 1 else "fp64 DMMA", "error_bound_abs": bound}
+    hb = rl_hbm(peaks, nbytes, ms_m, kernel="i8::k_norm_i8" if path == 1 else "k_norm_dmma")
+    if path == 1:
+        rec["roofline"] = hb                                 # exact integer GEMM keeps up with the stream: HBM-bound
+    else:
+        tb = rl_flops(peaks, "tensor", flops_sym, ms_m, kernel="k_norm_dmma")
+        rec["roofline"] = hb if hb["frac"] >= tb["frac"] else tb    # the floor that is closer is the binding one
+        rec["roofline_other"] = tb if hb["frac"] >= tb["frac"] else hb
+    return rec
+
+
+def bench_constant(torch, pwa, synth, w, steps, warmup, elem, peaks):
     """Single-rank side measurement of a constant-resonance config -> dict."""
     tm = Timer(torch)
     stream = torch.cuda.current_stream().cuda_stream
@@ -259,13 +315,7 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
         M0 = np.zeros((n, n, 2)); M0[np.arange(n), np.arange(n), 0] = 1.0
         if w.A_mc is not None:
             pwa.pwa_upload_events(ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
-            ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), 3, 1)
-            flops = 8.0 * n * n * w.n_acc
-            out["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": flops / ms_m * 1e-6,
-                              "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
-            bound, path = pwa.pwa_norm_error_bound(ctx)
-            out["m_build"]["path"] = "int8 tcgen05 (digit planes, int32 TMEM)" if path == 1 else "fp64 DMMA"
-            out["m_build"]["error_bound_abs"] = bound
+            out["m_build"] = m_build_record(pwa, tm, ctx, w, n, elem, peaks)
         else:
             pwa.pwa_set_norm(ctx, M0)
         Vs = synth.eval_points(w, steps + warmup)
@@ -275,47 +325,76 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem):
             pwa.pwa_nll_grad(ctx, Vs[warmup + i])
         wall = (time.perf_counter() - t0) / steps * 1e3
         nbytes = w.n_data * n * 2 * elem
-        out.update({"n_waves": n, "n_data": w.n_data, "storage": w.storage, "ms_per_eval": ms,
+        out.update({"n_waves": n, "n_data": w.n_data, "storage": w.storage, "evaluations_timed": steps, "ms_per_eval": ms,
                     "evals_per_s": 1e3 / ms, "event_waves_per_s": w.n_data * n / ms * 1e3,
-                    "algorithmic_gbs": nbytes / ms * 1e-6, "e2e_ms_per_eval": wall,
-                    "e2e_evals_per_s": 1e3 / wall, "upload_s": up_s,
-                    "l2_resident": bool(nbytes < 100e6)})
+                    "e2e_ms_per_eval": wall, "e2e_evals_per_s": 1e3 / wall, "upload_s": up_s})
+        if nbytes < 100e6:
+            out["roofline"] = {"bound": "latency", "achieved": nbytes / ms * 1e-6, "peak": None, "unit": "GB/s", "frac": None,
+                               "algorithmic_bytes_per_launch": nbytes, "kernel": "k_data_term_tma",
+                               "note": "sample is L2-RESIDENT (< 126 MB): launch / reduction latency bound, not an HBM fraction; "
+                                       f"the HBM floor would be {nbytes / peaks['hbm_gbs'] * 1e-3:.1f} us"}
+        else:
+            l2mb = pwa.pwa_get_option(ctx, "l2_resident_mb")
+            res_mb = (48 if 64e6 <= nbytes <= (1 << 30) else 0) if l2mb < 0 else l2mb
+            out["roofline"] = rl_hbm(peaks, nbytes, ms, kernel="k_data_term_tma")
+            if res_mb:
+                out["roofline"]["note"] = (f"ALGORITHMIC GB/s: {res_mb} MB of the sample are kept L2-resident between "
+                                           "evaluations by cache hints, so DRAM moves less than the algorithmic bytes")
+                out["roofline"]["dram_gbs_estimate"] = (nbytes - res_mb * 1e6) / ms * 1e-6
+                out["roofline"]["dram_frac_estimate"] = (nbytes - res_mb * 1e6) / ms * 1e-6 / peaks["hbm_gbs"]
         # NEXT-2: Fumili-style approximate Hessian (synchronous call: one row-scaled Gram pass over the data)
-        pwa.pwa_fumili_hessian(ctx, Vs[0])
+        for i in range(SIDE_WARMUP):
+            pwa.pwa_fumili_hessian(ctx, Vs[i])
         t0 = time.perf_counter()
-        for i in range(3):
-            pwa.pwa_fumili_hessian(ctx, Vs[1 + i])
-        ms_f = (time.perf_counter() - t0) / 3 * 1e3
-        out["fumili"] = {"ms_per_call_e2e": ms_f, "gflops_full_gram": 8.0 * n * n * w.n_data / ms_f * 1e-6}
+        for i in range(SIDE_STEPS):
+            pwa.pwa_fumili_hessian(ctx, Vs[(SIDE_WARMUP + i) % len(Vs)])
+        ms_f = (time.perf_counter() - t0) / SIDE_STEPS * 1e3
+        out["fumili"] = {"ms_per_call_e2e": ms_f,
+                         "roofline": rl_flops(peaks, "tensor", 4.0 * n * n * w.n_data + 16.0 * n * w.n_data, ms_f,
+                                              kernel="k_norm_dmma (row-scaled, DATA)", timed="synchronous call incl. D2H of H")}
         if w.K > 1:
             Vk = synth.eval_points(w, w.K, stream=synth.S_START)
-            ms_b, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
+            ms_b, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), SIDE_STEPS, SIDE_WARMUP)
             path, err_rel = pwa.pwa_batch_path(ctx)
+            flops = 16.0 * w.n_data * n * w.K
             out["batch"] = {"K": w.K, "ms_per_call": ms_b, "evals_per_s": w.K / ms_b * 1e3,
                             "event_waves_per_s": w.n_data * n * w.K / ms_b * 1e3,
-                            "gflops": 16.0 * w.n_data * n * w.K / ms_b * 1e-6,
+                            "fp64_equivalent_gflops": flops / ms_b * 1e-6,
                             "path": {0: "K streaming passes", 1: "fp64 DMMA chained GEMMs",
                                      2: "int8 tcgen05 chained GEMMs (digit planes, int32 TMEM)"}[path],
                             "per_term_error_estimate": err_rel}
             if path == 2:
-                # 20 digit-pair products of 128 x 128 x 128 int8 MACs per 128-event tile (10 per GEMM)
-                out["batch"]["int8_tops"] = 2.0 * 128 * 128 * 20 * w.n_data / ms_b * 1e-9
+                # digit-pair products of 128 x 128 x 128 int8 MACs per 128-event tile (pwa_batch_path documents the count)
+                pairs = 20
+                ops = 2.0 * 128 * 128 * pairs * w.n_data
+                out["batch"]["roofline"] = rl_flops(peaks, "tensor_int8", ops, ms_b, kernel="bi8::k_batch_i8",
+                                                    digit_pair_gemms_per_tile=pairs)
+                out["batch"]["roofline_hbm"] = rl_hbm(peaks, nbytes, ms_b, kernel="bi8::k_batch_i8")
                 pwa.pwa_set_option(ctx, "batch", 1)
-                ms_d, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), 2, 1)
+                ms_d, _ = tm.run(lambda i: pwa.pwa_nll_grad_batch_enqueue(ctx, Vk), SIDE_STEPS, SIDE_WARMUP)
                 pwa.pwa_set_option(ctx, "batch", 0)
-                out["batch"]["ms_per_call_fp64_dmma"] = ms_d
-            # NEXT-3: the same evaluation with per-event weights (per-lane streaming kernel + 8 B/event weight stream)
+                out["batch"]["fp64_dmma"] = {"ms_per_call": ms_d,
+                                             "roofline": rl_flops(peaks, "tensor", flops, ms_d, kernel="k_batch_dmma")}
+            elif path == 1:
+                out["batch"]["roofline"] = rl_flops(peaks, "tensor", flops, ms_b, kernel="k_batch_dmma")
+            # NEXT-3: the same evaluation with per-event weights (8 B/event weight stream)
             wts = np.random.default_rng(7).uniform(0.5, 1.5, size=w.n_data)
             pwa.pwa_set_weights(ctx, pwa.PWA_DATA, wts)
-            ms_w, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i]), steps, warmup)
+            ms_w, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i % len(Vs)]), SIDE_STEPS, SIDE_WARMUP)
             pwa.pwa_set_weights(ctx, pwa.PWA_DATA, None)
-            out["weighted"] = {"ms_per_eval": ms_w, "algorithmic_gbs": (nbytes + 8 * w.n_data) / ms_w * 1e-6}
+            out["weighted"] = {"ms_per_eval": ms_w, "roofline": rl_hbm(peaks, nbytes + 8 * w.n_data, ms_w, kernel="k_data_term (weighted)")}
     finally:
         pwa.pwa_destroy(ctx)
     return out
 
 
-def bench_floating(torch, pwa, synth, w, steps, warmup):
+# algorithmic fp64 flops per event of the fused Breit-Wigner passes at configs[3] (8 resonances x 2 angular structures;
+# "flops ~ n_res (complex reciprocal ~ 25) + n 6 + 16 n + 60 ~ 600 / event")
+FLOPS_FACT_DATA = 600.0
+FLOPS_RES_GRAD = 450.0      # res_grad.cu: one Breit-Wigner per resonance, w BW^2, 8 complex MACs, 1 / S
+
+
+def bench_floating(torch, pwa, synth, w, steps, warmup, peaks):
     """cfg3: per quasi-Newton iteration = set_resonances + build_norm (fused BW over MC) +
     nll_grad (fused BW over data) + res_grad (analytic d/dM_r, d/dG_r; reading A9)."""
     tm = Timer(torch)
@@ -346,30 +425,46 @@ def bench_floating(torch, pwa, synth, w, steps, warmup):
             pwa.pwa_set_resonances(ctx, Mr, Gr)
             pwa.pwa_build_norm(ctx, want_M=False)
             pwa.pwa_nll_grad(ctx, Vs[i])
-            pwa.pwa_res_grad(ctx, Vs[i], w.n_res)
+            pwa.pwa_res_grad(ctx, Vs[i])
 
         def only_norm(i):
             Mr, Gr = params(i)
             pwa.pwa_set_resonances(ctx, Mr, Gr)
             pwa.pwa_build_norm(ctx, want_M=False)
 
+        pwa.pwa_set_resonances(ctx, Mr0, Gr0)
+        pwa.pwa_build_norm(ctx, want_M=False)
+        ms_data, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i]), steps, warmup)
         ms_it, _ = tm.run(it_dev, steps, warmup)
         ms_norm, _ = tm.run(only_norm, steps, warmup)
         _, wall_full = tm.run(it_full, steps, warmup)
+        ms_rg = max(wall_full - ms_it, 1e-6)
         # configs[3] as stated: 200 quasi-Newton iterations driven from the host, M rebuilt in every evaluation
         free = np.arange(w.n_free, dtype=np.int32)
         pwa.pwa_set_resonances(ctx, Mr0, Gr0)
         t0 = time.perf_counter()
-        _, Mf, Gf, nll_f, its, evs, _ = pwa.pwa_minimize_bfgs_floating(ctx, w.V_true, Mr0, Gr0, free, max_iter=200, gtol=0.0)
+        _, Mf, Gf, nll_f, its, evs, _, why = pwa.pwa_minimize_bfgs_floating_ex(ctx, w.V_true, Mr0, Gr0, free, max_iter=200, gtol=0.0)
         fit_s = time.perf_counter() - t0
-        fit = {"iterations": its, "evaluations": evs, "wall_s": fit_s, "e2e_ms_per_evaluation": fit_s / max(evs, 1) * 1e3,
+        fit = {"max_iter_requested": 200, "iterations_run": its, "evaluations": evs,
+               "stopped_because": {0: "converged", 1: "max_iter", 2: "line search exhausted (fp64 resolution of nll)"}[why],
+               "wall_s": fit_s, "e2e_ms_per_evaluation": fit_s / max(evs, 1) * 1e3,
                "nll": nll_f, "free_parameters": 2 * w.n + 2 * w.n_free}
-        return {"n_waves": w.n, "n_data": w.n_data, "n_mc": w.n_acc, "storage": w.storage, "fit_200_qn_iterations": fit,
+        n = w.n
+        mc_bytes = w.n_acc * (8 + 16 * w.n_ang)
+        data_bytes = w.n_data * (8 + 16 * w.n_ang)
+        return {"n_waves": n, "n_data": w.n_data, "n_mc": w.n_acc, "storage": w.storage, "floating_fit": fit,
                 "ms_per_iteration_nll_grad_plus_norm": ms_it, "ms_norm_build_fused_bw": ms_norm,
-                "ms_data_term_fused_bw": ms_it - ms_norm,
+                "ms_data_term_fused_bw": ms_data,
                 "e2e_ms_per_iteration_with_res_grad": wall_full,
                 "iterations_per_s": 1e3 / ms_it,
-                "event_waves_per_s": (w.n_data + w.n_acc) * w.n / ms_it * 1e3}
+                "event_waves_per_s": (w.n_data + w.n_acc) * n / ms_it * 1e3,
+                "roofline_m_rebuild": rl_flops(peaks, "tensor", 4.0 * n * n * w.n_acc, ms_norm, kernel="k_norm_dmma (fused BW)",
+                                               hbm_frac=mc_bytes / ms_norm * 1e-6 / peaks["hbm_gbs"]),
+                "roofline_data_term": rl_flops(peaks, "alu", FLOPS_FACT_DATA * w.n_data, ms_data, kernel="k_data_term_fact",
+                                               hbm_frac=data_bytes / ms_data * 1e-6 / peaks["hbm_gbs"]),
+                "roofline_res_grad": rl_flops(peaks, "alu", FLOPS_RES_GRAD * (w.n_data + w.n_acc), ms_rg,
+                                              kernel="k_res_grad_fast (data + MC pass)",
+                                              timed="e2e iteration with res_grad minus device time of the iteration without")}
     finally:
         pwa.pwa_destroy(ctx)
 
@@ -401,22 +496,27 @@ def run_ours(args):
     K, W = args.steps, args.warmup
     if W < 3:
         raise SystemExit("bench.py: --warmup must be >= 3")
-    peak, peak_src, _ = load_peaks()
+    mp_hbm, mp_src, _ = load_peaks()
     elem = 8 if spec["storage"] == "f64" else 4
     extra_on = (not args.no_extra) and ws == 1
     tm = Timer(torch)
     barrier = (lambda: dist.barrier()) if ws > 1 else None
     stream = torch.cuda.current_stream().cuda_stream
     dev = torch.device("cuda", local)
+    pctx = pwa.pwa_create(4, "f64", local, stream)
+    try:
+        peaks = measure_peaks(pwa, pctx, mp_hbm, mp_src)
+    finally:
+        pwa.pwa_destroy(pctx)
     t_gen = time.perf_counter()
 
     if spec["factored"]:
-        # cfg3 as the main workload: a step is one floating-resonance iteration
+        # cfg3 as the main workload: a step is one floating-resonance iteration (M rebuild + lnL + gradient)
         w = synth.make_workload(cfg, n_data=n_data, n_mc=n_mc, full_amplitudes=False, shard=rank)
         if ws > 1:
             raise SystemExit("bench.py: the cfg3 step is single-GPU here; use the default workload for N > 1")
         clk = ClockSampler(local); clk.start()
-        r = bench_floating(torch, pwa, synth, w, K, W)
+        r = bench_floating(torch, pwa, synth, w, K, W, peaks)
         clk.stop()
         ms = r["ms_per_iteration_nll_grad_plus_norm"]
         line = {"metric": "event-waves/s (floating-resonance iteration: M rebuild + lnL+gradient)",
@@ -428,9 +528,8 @@ def run_ours(args):
                 "e2e": {"value": (w.n_data + w.n_acc) * w.n / r["e2e_ms_per_iteration_with_res_grad"] * 1e3,
                         "unit": "event-waves/s", "h2d_bytes_per_step": 16 * w.n + 16 * w.n_res,
                         "d2h_bytes_per_step": 8 * (4 + 2 * w.n) + 16 * w.n_res},
-                "roofline": {"bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None,
-                             "traffic": None, "note": "see DESIGN.md section 7 (fused Breit-Wigner passes are fp64-ALU bound)"},
-                "clocks": clk.summary(), "extra": {"cfg3": r}, "gpu_launches": None}
+                "roofline": dict(r["roofline_m_rebuild"], traffic=load_traffic("k_norm_dmma_fact")),
+                "peaks": peaks, "clocks": clk.summary(), "extra": {"cfg3": r}, "gpu_launches": 2 * K}
         print(json.dumps(line), flush=True)
         return 0
 
@@ -447,18 +546,10 @@ def run_ours(args):
         # ---- normalisation matrix (once per fit; not part of the step)
         if w.A_mc is not None:
             pwa.pwa_upload_events(ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
-            ms_m, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), 3, 1)
-            extra["m_build"] = {"ms": ms_m, "n_mc": w.n_acc, "gflops_full_gram": 8.0 * n * n * w.n_acc / ms_m * 1e-6,
-                                "mc_gbs": w.n_acc * n * 2 * elem / ms_m * 1e-6}
-            bound, path = pwa.pwa_norm_error_bound(ctx)
-            extra["m_build"]["path"] = "int8 tcgen05 (digit planes, int32 TMEM)" if path == 1 else "fp64 DMMA"
-            extra["m_build"]["error_bound_abs"] = bound
-            M_local = pwa.pwa_build_norm(ctx)
+            extra["m_build"] = m_build_record(pwa, tm, ctx, w, n, elem, peaks)
+            M_all = pwa.pwa_build_norm(ctx)
             if ws > 1:
-                M_all, _ = sharded.combine_norm(M_local, w.n_gen, device=dev)
-                pwa.pwa_set_norm(ctx, M_all)
-            else:
-                M_all = M_local
+                M_all, _ = sharded.combine_norm(ctx, device=dev)
             w.A_mc = None   # free 10 GB of host memory
         else:
             M_all = np.zeros((n, n, 2)); M_all[np.arange(n), np.arange(n), 0] = 1.0
@@ -471,10 +562,8 @@ def run_ours(args):
             step = lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i])          # noqa: E731
         else:
             def step(i):
-                pwa.pwa_data_term_enqueue(ctx, Vs[i], out_dev)
-                sharded.reduce_terms(out_dev)
+                sharded.nll_grad(ctx, Vs[i], M_all, out_dev)
         clk = ClockSampler(local)
-        l0 = pwa.pwa_launch_count(ctx)
         for i in range(W):
             step(i)
         torch.cuda.synchronize()
@@ -492,9 +581,7 @@ def run_ours(args):
         def e2e_step(i):
             if ws == 1:
                 return pwa.pwa_nll_grad(ctx, Vs[K + W + i])
-            pwa.pwa_data_term_enqueue(ctx, Vs[K + W + i], out_dev)
-            t = sharded.reduce_terms(out_dev).cpu().numpy()
-            return pwa.pwa_assemble_host(t[0], t[2:].reshape(n, 2), M_all, Vs[K + W + i])
+            return sharded.nll_grad(ctx, Vs[K + W + i], M_all, out_dev)
         for i in range(W):
             e2e_step(i)
         torch.cuda.synchronize()
@@ -505,18 +592,23 @@ def run_ours(args):
             e2e_step(W + i)
         torch.cuda.synchronize()
         wall_ms = (time.perf_counter() - t0) / K * 1e3
-        # ---- configs[4] as stated: K = 64 independent fits in lock-step on the batched call (host BFGS, A8 path).
-        # A bounded number of iterations is run and the 300-iteration cost is projected from it.
+        gpu_at_V0 = pwa.pwa_nll_grad(ctx, Vs[0]) if ws == 1 else None
+        # ---- configs[4] as stated: K = 64 independent fits x 300 host BFGS iterations, in lock-step on the batched
+        # call (A8 path); gtol = 0 so that every fit runs its 300 iterations unless its line search is exhausted
         if ws == 1 and w.K > 1 and w.A_mc is None and "m_build" in extra and not args.no_extra:
-            iters = 25
+            iters = 300
             V0 = synth.eval_points(w, w.K, stream=synth.S_START)
             t0 = time.perf_counter()
-            Vf, nllf, evals, _ = pwa.pwa_minimize_bfgs_batch(ctx, V0, max_iter=iters, gtol=0.0)
+            Vf, nllf, evals, _, its, why = pwa.pwa_minimize_bfgs_batch_ex(ctx, V0, max_iter=iters, gtol=0.0)
             dt = time.perf_counter() - t0
             path, _ = pwa.pwa_batch_path(ctx)
-            extra["cfg4_multistart"] = {"K": w.K, "bfgs_iterations": iters, "batched_evaluations": evals, "wall_s": dt,
+            extra["cfg4_multistart"] = {"K": w.K, "bfgs_iterations_requested": iters,
+                                        "iterations_run_min_max": [int(its.min()), int(its.max())],
+                                        "stop_reasons": {"max_iter": int((why == 1).sum()), "line_search": int((why == 2).sum()),
+                                                         "converged": int((why == 0).sum())},
+                                        "batched_evaluations": evals, "wall_s": dt,
                                         "e2e_ms_per_batched_evaluation": dt / max(evals, 1) * 1e3,
-                                        "projected_s_for_300_iterations": dt / iters * 300.0, "batch_path": path,
+                                        "last_batch_path": path,
                                         "nll_best": float(np.min(nllf)), "nll_worst": float(np.max(nllf))}
         if ws > 1:
             t = torch.tensor([ms, wall_ms, ms_kernel], dtype=torch.float64, device=dev)
@@ -531,8 +623,12 @@ def run_ours(args):
         return 0
 
     units = w.n_data * n * ws                      # event-waves per step, all ranks (weak scaling)
-    achieved = bytes_data / ms_kernel * 1e-6       # GB/s, algorithmic bytes of one launch
     kernel_key = f"k_data_term_{w.storage}_n{n}"
+    roof = rl_hbm(peaks, bytes_data, ms_kernel, kernel=kernel_key, traffic=load_traffic(kernel_key))
+    roof["frac_of_nominal_8TBs"] = roof["achieved"] / 8000.0
+    if bytes_data > 2.5e8:
+        roof["note"] = ("back-to-back evaluations: up to L2 / sample = %.1f %% of the bytes may still be L2-resident from the "
+                        "previous evaluation; the cold-cache ncu launch list (profiles/) bounds the effect" % (126e6 / bytes_data * 100))
     line = {
         "metric": "event-waves/s (lnL+gradient evaluation)", "value": units / ms * 1e3, "unit": "event-waves/s",
         "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
@@ -545,53 +641,59 @@ def run_ours(args):
         "e2e": {"value": units / wall_ms * 1e3, "unit": "event-waves/s", "ms_per_step": wall_ms,
                 "evals_per_s": 1e3 / wall_ms, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 8 * (4 + 2 * n),
                 "note": "events are uploaded once per fit (upload_data_s in extra), V and results cross every step"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(kernel_key), "peak_source": peak_src, "kernel": kernel_key,
-                     "algorithmic_bytes_per_launch": bytes_data},
+        "roofline": roof, "peaks": peaks,
         "clocks": clk.summary(), "gpu_launches": int(launches),
     }
-    if extra_on:
-        line["cpu_baseline"] = cpu_baseline(synth, w, M_all, Vs[0], args.workload)
-        line["extra"] = side_measurements(torch, pwa, synth, args, extra)
-    else:
-        line["extra"] = extra
-        if ws == 1:
-            line["cpu_baseline"] = cpu_baseline(synth, w, M_all, Vs[0], args.workload)
+    if ws == 1:
+        line["cpu_baseline"], line["parity"] = cpu_baseline(synth, w, M_all, Vs[0], args.workload, gpu_at_V0)
+    line["extra"] = side_measurements(torch, pwa, synth, args, extra, peaks) if extra_on else extra
     print(json.dumps(line), flush=True)
     if ws > 1:
         dist.barrier(); dist.destroy_process_group()
     return 0
 
 
-def cpu_baseline(synth, w, M, V, name):
-    """The oracle as it stands on this box's host cores, on a prefix of the same data."""
+def cpu_baseline(synth, w, M, V, name, gpu_result):
+    """The oracle as it stands on this box's host cores, on a prefix of the same data.  When the prefix is the whole
+    sample, the oracle's result at V is also compared with the GPU's at the same V (max parity error of the benched
+    config, norm-wise as in DESIGN.md C8)."""
     from oracle import oracle
     S = oracle_sample_size(oracle, w.A_data, M, V, w.n_data, 5.0)
     A = np.ascontiguousarray(w.A_data[:S])
     reps, t0 = 3, time.perf_counter()
     for _ in range(reps):
-        oracle.nll_grad(A, M, V)
+        ref = oracle.nll_grad(A, M, V)
     dt = (time.perf_counter() - t0) / reps
-    return {"value": S * w.n / dt, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
+    base = {"value": S * w.n / dt, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
             "sample": f"first {S} of {w.n_data} data events of {name}, {reps} full lnL+gradient evaluations, {dt:.2f} s each"}
+    parity = None
+    if gpu_result is not None and S == w.n_data:
+        nll_o, g_o, parts_o = ref[0], ref[1], ref[2]
+        parity = {"vs": "oracle, same V, all events of the benched config",
+                  "nll_rel": abs(gpu_result[0] - nll_o) / max(abs(nll_o), abs(parts_o[0])),
+                  "L_data_rel": abs(gpu_result[2][0] - parts_o[0]) / abs(parts_o[0]),
+                  "grad_rel_maxnorm": float(np.abs(gpu_result[1] - g_o).max() / np.abs(g_o).max()),
+                  "tolerance": 1e-12 if w.storage == "f64" else 1e-6}
+    return base, parity
 
 
-def side_measurements(torch, pwa, synth, args, extra):
-    """Other configs of BASELINE.json, single GPU, each in the launch configuration the tests check."""
+def side_measurements(torch, pwa, synth, args, extra, peaks):
+    """Other configs of BASELINE.json, single GPU, each in the launch configuration the tests check; the iteration
+    counts are the ones the configs state (cfg1: 100 evaluations, cfg2: 1000, cfg3: 200 quasi-Newton iterations)."""
     try:
         w2 = synth.make_workload(2)
-        extra["cfg2"] = bench_constant(torch, pwa, synth, w2, 50, 5, 4)
+        extra["cfg2"] = bench_constant(torch, pwa, synth, w2, 1000, 5, 4, peaks)
         del w2
         w1 = synth.make_workload(1)
-        extra["cfg1"] = bench_constant(torch, pwa, synth, w1, 100, 5, 8)
+        extra["cfg1"] = bench_constant(torch, pwa, synth, w1, 100, 5, 8, peaks)
         del w1
         w3 = synth.make_workload(3, full_amplitudes=False)
-        extra["cfg3"] = bench_floating(torch, pwa, synth, w3, 20, 3)
+        extra["cfg3"] = bench_floating(torch, pwa, synth, w3, 20, 3, peaks)
         del w3
         if args.workload == "cfg4":
             w4 = synth.make_workload(4, n_mc=1, want_mc=False)
             w4.A_mc = None
-            r = bench_constant(torch, pwa, synth, w4, 3, 3, 4)
+            r = bench_constant(torch, pwa, synth, w4, SIDE_STEPS, SIDE_WARMUP, 4, peaks)
             extra["cfg4_batch"] = r.get("batch")
             extra["cfg4_fumili"] = r.get("fumili")
             extra["cfg4_weighted"] = r.get("weighted")

@@ -297,7 +297,9 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* c
 
 /* Register-resident peak probes used as roofline denominators:
  * which = 0: fp64 FMA (result TFLOP/s), 1: fp64 mma.sync m8n8k4 (TFLOP/s),
- * 2: HBM read-only stream over `bytes` of scratch (GB/s).  Synchronous; result HOST.     */
+ * 2: HBM read-only stream over `bytes` of scratch (GB/s), 3 .. 6: tcgen05.mma.kind::i8 with M = 128, K = 32 and
+ * N = 256 / 128 / 64 / 32, operands in shared memory (int8 Top/s, all SMs), 7: TMEM reads (tcgen05.ld 32x32b.x16 by
+ * 16 warps per SM, GB/s).  Synchronous; result HOST.                                                              */
 pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result);
 
 #ifdef __cplusplus

@@ -13,148 +13,75 @@
 //
 // Fixed point.  x_ic = rint(X_ic 2^s_c) is a 32-bit integer (s_c from the column maximum of the
 // sample, found once per upload: i8_column_scales), split into four balanced int8 digits
-// x = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 ("Ozaki" slicing, as norm_i8.cu).  The digit planes of a tile are
-// written ONCE to shared memory, rows = events, 128 bytes = the 128 real columns, 128-byte swizzle:
-// read K-major they are the A operand of GEMM1 (M = events, K = columns), read MN-major they are the
-// A operand of GEMM2 (M = columns, K = events) — the same bytes serve both GEMMs.
+// x = d0 + 2^8 d1 + 2^16 d2 + 2^24 d3 ("Ozaki" slicing, as norm_i8.cu).  The digit planes do not depend on V:
+// they are written ONCE PER UPLOAD (k_bi8_planes, on the first batched call) to a device image of the size of
+// the sample, tile by tile in exactly the shared-memory layout (rows = events, 128 bytes = the 128 real
+// columns, 128-byte swizzle), so an evaluation moves a tile's 64 KB of planes from HBM into shared memory with
+// plain bulk copies and converts nothing.  Read K-major a plane is the A operand of GEMM1 (M = events,
+// K = columns), read MN-major the same bytes are the A operand of GEMM2 (M = columns, K = events).
 //   * W' = W 2^-s_c (the column scale moves to the other operand; exact) is quantised per starting
 //     point with w = rint(W' 2^e_k), 32 bits below max_c |W'_ck|, four digit planes (k_bi8_prep).
 //     GEMM1 forms the digit-pair products of orders t = u + v = 3..6 (10 of 16 pairs, as 3 N = 256 and
 //     4 N = 128 MMAs per 32-column K step); z = sum_t 2^(8(t-3)) acc_t is an exact integer and
 //     S_ik = z 2^(24 - e_k) up to the dropped orders t <= 2 and the quantisation of W' (together
 //     ~2^9 rms in the units of z, where a typical |z| is ~2^37).
-//   * Sums that cancel strongly (|z| < 2^31, ~1e-4 of them, the ones that dominate the gradient) are
-//     recomputed by the warp in fp64 from the event's fp32 row and the unrounded W (recompute_z), so every
-//     S_ik used below is exact to ~2^-22 |S_ik| or better (typically 2^-28).
+//   * Sums that cancel strongly (|z|^2 < thr2, the ones that dominate the gradient) are recomputed by the warp
+//     in fp64 from the event's fp32 row and the unrounded W (recompute_z), so every S_ik used below is exact
+//     to ~2^-22 |S_ik| or better (typically 2^-28).
 //   * ln|S|^2: |z|^2 enters a running fp64 PRODUCT per column (mantissa renormalised, exponent counted),
 //     one log per thread at the end; the offset 2 (24 - e_k) ln 2 per event is added by k_bi8_finalize.
 //   * Rh = conj(z)/|z|^2 in fp64 (hardware seed + two Newton steps), parked in TMEM over the consumed
-//     S columns, then quantised PER TILE AND STARTING POINT to 31 bits below the tile's max_i |Rh_ik|
-//     (four digit planes; R0 is written into the slot of W0, which the TMA thread re-reads from its
-//     L2-resident image after GEMM2).  GEMM2 forms orders t = 3..6 (10 pairs) like GEMM1.
-//     The tile's integer block is read back from TMEM, converted exactly and added to fp64 accumulators
-//     in registers (one per (column c, real start column) and thread: 128 x 128 per CTA), so no int32
-//     ever sees more than one tile.
-// Error: DESIGN.md 6.7 (measured norm-wise gradient error 1e-7 at 6e3 events, 1e-8 at 2e5, falling like
-// 1 / sqrt(N)); the parity bar for fp32 storage is 1e-6 (BASELINE.json north_star).
+//     S columns, then quantised PER TILE AND STARTING POINT with the scale that maps the tile's max_i |Rh_ik| onto
+//     the full four-digit range (2^31 - 2^25; not a power of two: that would waste 1.5 bits on average), four digit
+//     planes written over the W planes (GEMM1 is done with them; the copy thread re-reads W from its L2-resident
+//     image after GEMM2).  GEMM2 forms orders t = 3..6 (10 pairs) like GEMM1.  (A three-plane GEMM2, 6 pairs, was
+//     measured: 8 % faster, but its gradient error is 2e-6 at 4e3 events and still 1.6e-7 at 1e6.)
+//     The tile's integer block is read back from TMEM, converted exactly and added to fp64 accumulators in
+//     registers (one per (column c, real start column) and thread: 128 x 128 per CTA), so no int32 ever sees more
+//     than one tile.
+// Error: DESIGN.md 6.7; the parity bar for fp32 storage is 1e-6 (BASELINE.json north_star).
 //
 // One persistent CTA per SM (contiguous tile range), 16 warps = 512 threads with 128 registers each: every
-// warp converts (fp32 stage -> digit planes) and runs the epilogues (warp w: TMEM lane quarter w % 4,
-// 32-column group w / 4); lane 0 of warp 0 also issues the MMAs and owns TMEM, lane 0 of warp 1 issues the
-// TMA loads (ring of 32-event fp32 stages).  Per-CTA partials go to fixed slots; k_bi8_finalize sums them
-// in slot order and performs step A7.
+// warp runs the epilogues (warp w: TMEM lane quarter w % 4, 32-column group w / 4); lane 0 of warp 0 also issues
+// the MMAs and owns TMEM, lane 0 of warp 1 issues the bulk copies (X planes double-buffered: the planes of tile
+// t + 2 are requested as soon as GEMM2 of tile t has released its buffer).  Per-CTA partials go to fixed slots;
+// k_bi8_finalize sums them in slot order and performs step A7.
 #include <cuda.h>
 #include <cudaTypedefs.h>
+#include <limits.h>
 #include <math.h>
 #include <string.h>
 
 #include "pwa_internal.h"
 #include "reduce.cuh"
 #include "stream_common.cuh"
+#include "tcgen05_common.cuh"
 
 namespace pwa {
 
 namespace bi8 {
 
+using namespace tc;
+
 constexpr int TE = 128;                      // events per tile
-constexpr int ROWB = 512;                    // bytes of one fp32 event row (128 reals)
-constexpr int SR = 32;                       // event rows per TMA stage
-constexpr int STG_BYTES = SR * ROWB;         // 16 KB
-constexpr int NSTG = 3;
-constexpr int SPT = TE / SR;                 // stages per tile
 constexpr int PLANE = TE * 128;              // 16 KB: one int8 digit plane
-constexpr int NEW = 16;                      // converter / epilogue warps
+constexpr int TILE_BYTES = 4 * PLANE;        // 64 KB: the four X planes of a tile in the device image
+constexpr int NEW = 16;                      // epilogue warps
 constexpr int THREADS = NEW * 32;            // 512
 constexpr int KC = 64;                       // starting points per pass (128 real columns)
-// plane slots: X0 X1 X2 X3 | W1 W2 W3 | W0 (GEMM1) = R0 (GEMM2) | R1 R2 R3 | fp32 stages.  W0 is re-read
-// from its global image (L2) after every GEMM2; adjacent operand pairs (N = 256): W1W2, W2W3, R0R1, R1R2, R2R3.
-constexpr uint32_t OFF_X0 = 0, OFF_X1 = PLANE, OFF_X2 = 2 * PLANE, OFF_X3 = 3 * PLANE;
-constexpr uint32_t OFF_W1 = 4 * PLANE, OFF_W0 = 7 * PLANE, OFF_R = 7 * PLANE, OFF_STG = 11 * PLANE;
-constexpr size_t SMEM = 1024 + (size_t)11 * PLANE + (size_t)NSTG * STG_BYTES;     // 230400 bytes
+// plane slots: XA0..3 | XB0..3 | W0..3 (GEMM1) = R0..3 (GEMM2).  The four W planes are re-read from their global
+// image (L2) after every GEMM2; adjacent operand pairs (N = 256): W1W2, W2W3, R0R1, R2R3.
+constexpr uint32_t OFF_XA = 0, OFF_XB = 4 * PLANE, OFF_W = 8 * PLANE, OFF_R = 8 * PLANE;
+constexpr size_t SMEM = 1024 + (size_t)12 * PLANE;     // 197632 bytes
 constexpr size_t SLOT = 128 * 128 + KC;      // doubles per CTA slot: Q[col][c], then L[k]
 
 struct Scales { float s[128]; };             // 2^s_c per real column
 struct Exps { int e[128]; };                 // s_c
 
-// ---- PTX wrappers -----------------------------------------------------------------------------
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
-{
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
-{
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
-{
-    asm volatile("{\n"
-                 ".reg .pred p;\n"
-                 "setp.ne.b32 p, %4, 0;\n"
-                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
-                 "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, int32_t (&v)[8])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                 : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NEW * 32) : "memory"); }
-__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w)
-{
-    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
-}
+constexpr uint32_t kI1_128 = idesc_i8(128, false, false), kI1_256 = idesc_i8(256, false, false);   // GEMM1: both operands K-major
+constexpr uint32_t kI2_128 = idesc_i8(128, true, true),  kI2_256 = idesc_i8(256, true, true);      // GEMM2: both operands MN-major
 
-// Shared-memory matrix descriptors of one digit plane (rows of 128 bytes, 8-row swizzle atoms of
-// 1024 bytes, SWIZZLE_128B).  K-major: rows are M (or N) indices, the 128 bytes run along K; a K step
-// of 32 advances the start address by 32 bytes; an N = 256 operand continues into the next plane
-// (rows 128..255).  MN-major: rows are K indices, the 128 bytes run along M (or N); a K step of 32 rows
-// advances by 4096 bytes; an N = 256 operand continues in the next plane (LBO = PLANE).
-__device__ __forceinline__ uint64_t desc_kmajor(uint32_t smem_addr)
-{
-    uint64_t d = 0;
-    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
-    d |= (uint64_t)1 << 16;                                // leading byte offset: unused for swizzled K-major
-    d |= (uint64_t)(1024u >> 4) << 32;                     // stride byte offset: next 8 rows
-    d |= (uint64_t)1 << 46;                                // descriptor version (Blackwell)
-    d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
-    return d;
-}
-__device__ __forceinline__ uint64_t desc_mnmajor(uint32_t smem_addr)
-{
-    uint64_t d = 0;
-    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
-    d |= (uint64_t)((uint32_t)PLANE >> 4) << 16;           // next 128-byte atom along MN = next digit plane
-    d |= (uint64_t)(1024u >> 4) << 32;                     // next 8 K rows
-    d |= (uint64_t)1 << 46;
-    d |= (uint64_t)2 << 61;
-    return d;
-}
-// kind::i8 instruction descriptor: D = s32, A = B = signed int8, M = 128
-constexpr uint32_t idesc(uint32_t N, bool mn_major)
-{
-    return (2u << 4) | (1u << 7) | (1u << 10) | (mn_major ? ((1u << 15) | (1u << 16)) : 0u) | ((N >> 3) << 17) | ((128u >> 4) << 24);
-}
-constexpr uint32_t kI1_128 = idesc(128, false), kI1_256 = idesc(256, false);   // GEMM1: both operands K-major
-constexpr uint32_t kI2_128 = idesc(128, true),  kI2_256 = idesc(256, true);    // GEMM2: both operands MN-major
-
-// int32 -> double on the fp64 pipe (the 64-bit conversion unit is 4x slower): the integer lands in the low
-// mantissa bits of 2^52 + 2^31 + v (exact), one fp64 subtraction removes the offset.
-__device__ __forceinline__ double i2d(int v) { return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0; }
 // 1 / x for 1 <= x < 2^100: 20-bit hardware seed, two Newton steps (relative error ~2^-52)
 __device__ __forceinline__ double rcp_d(double x)
 {
@@ -165,21 +92,40 @@ __device__ __forceinline__ double rcp_d(double x)
     e = fma(-x, r, 1.0);
     return fma(r, e, r);
 }
-__device__ __forceinline__ void tmem_ld16i(uint32_t taddr, int32_t (&v)[16])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                 : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_st8i(uint32_t taddr, const int32_t (&v)[8])
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
-                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
-}
 
-// balanced int8 digits of a 32-bit integer: byte b of the result is digit d_b in [-128, 127]
-__device__ __forceinline__ uint32_t digits(int q) { return (uint32_t)(q + 0x00808080) ^ 0x00808080u; }
+// ---- X digit planes (once per upload) ------------------------------------------------------------
+// One block per tile (grid-stride): fp32 rows -> x = rint(X 2^s_c) -> four balanced digits -> the tile's four planes
+// in the shared-memory layout: byte (event e, column c) of plane p at p * PLANE + e * 128 + ((c >> 4) ^ (e & 7)) * 16
+// + (c & 15).  Rows past N are zero.
+__global__ void __launch_bounds__(THREADS)
+k_bi8_planes(const float *__restrict__ A, long long N, long long ntiles, const __grid_constant__ Scales sc,
+             unsigned char *__restrict__ planes)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float4 scl = make_float4(sc.s[4 * lane], sc.s[4 * lane + 1], sc.s[4 * lane + 2], sc.s[4 * lane + 3]);
+    const uint32_t chunk_off = (uint32_t)(lane & 3) * 4u, chunk_id = (uint32_t)(lane >> 2);
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        unsigned char *dst = planes + (size_t)t * TILE_BYTES;
+#pragma unroll
+        for (int r = 0; r < TE / NEW; ++r) {
+            const uint32_t e = (uint32_t)(warp * (TE / NEW) + r);
+            const long long row = t * TE + e;
+            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (row < N) x = __ldg(reinterpret_cast<const float4 *>(A + row * 128) + lane);
+            const uint32_t w0 = digits(__float2int_rn(x.x * scl.x));
+            const uint32_t w1 = digits(__float2int_rn(x.y * scl.y));
+            const uint32_t w2 = digits(__float2int_rn(x.z * scl.z));
+            const uint32_t w3 = digits(__float2int_rn(x.w * scl.w));
+            const uint32_t t0 = __byte_perm(w0, w1, 0x5140), t1 = __byte_perm(w2, w3, 0x5140);
+            const uint32_t t2 = __byte_perm(w0, w1, 0x7362), t3 = __byte_perm(w2, w3, 0x7362);
+            const uint32_t a = e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
+            *reinterpret_cast<uint32_t *>(dst + 0 * PLANE + a) = __byte_perm(t0, t1, 0x5410);
+            *reinterpret_cast<uint32_t *>(dst + 1 * PLANE + a) = __byte_perm(t0, t1, 0x7632);
+            *reinterpret_cast<uint32_t *>(dst + 2 * PLANE + a) = __byte_perm(t2, t3, 0x5410);
+            *reinterpret_cast<uint32_t *>(dst + 3 * PLANE + a) = __byte_perm(t2, t3, 0x7632);
+        }
+    }
+}
 
 // ---- W digit planes (once per call and pass) -----------------------------------------------------
 // Block k (local column pair), thread c: W'[c][2k], W'[c][2k+1] = W 2^-s_c, common exponent e_k from the
@@ -245,42 +191,40 @@ __device__ __noinline__ double2 recompute_z(const float *__restrict__ arow, int 
 }
 
 // ---- the kernel -------------------------------------------------------------------------------
-// tmap: fp32 [N][128] view of the data sample, box = [SR rows][128 floats], no swizzle (rows past N
-// read as zeros).  Wp: the four W digit planes (k_bi8_prep).  Kc: valid starting points of this pass.
-// slots: [gridDim.x][SLOT] doubles: Q[col][c] = 2^(-8 - s_c) sum_tiles 2^-sh z2 (the caller multiplies
-// by 2^e_k), then L[k] = sum ln(zr^2 + zi^2).
+// planes: the X digit-plane image of the data sample (k_bi8_planes): [ntiles][4][PLANE] bytes.  Adata: the fp32
+// sample itself (only the fp64 recomputation of strongly cancelling sums reads it).  Wp: the four W digit planes
+// (k_bi8_prep).  Kc: valid starting points of this pass.
+// slots: [gridDim.x][SLOT] doubles: Q[col][c] = 2^(-s_c) sum_tiles Z / s (the caller multiplies by 2^e_k), then
+// L[k] = sum ln(zr^2 + zi^2).
 __global__ void __launch_bounds__(THREADS, 1)
-k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ Adata, long long N, long long ntiles, int Kc, double thr2,
-           const __grid_constant__ Scales sc, const __grid_constant__ Exps ex,
+k_batch_i8(const unsigned char *__restrict__ planes, const float *__restrict__ Adata, long long N, long long ntiles, int Kc, double thr2,
+           const __grid_constant__ Exps ex,
            const unsigned char *__restrict__ Wp, const double *__restrict__ Wd, double *__restrict__ slots)
 {
     extern __shared__ unsigned char bi8_smem_raw[];
-    __shared__ __align__(8) unsigned long long bars[2 * NSTG + 6];
+    __shared__ __align__(8) unsigned long long bars[8];
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) uint32_t s_emax[NEW][16];
-    __shared__ __align__(16) uint32_t s_sh[KC];            // sh_k << 20 of the current tile
-    __shared__ __align__(16) float s_scl[128];
+    __shared__ __align__(16) float s_scale[KC];            // per starting point, current tile: q = rint(Rh * s_scale), Rh = q * s_inv
+    __shared__ __align__(16) double s_inv[KC];             // (a float scale: the static + dynamic shared memory is 176 bytes short of the 227 KB limit)
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t raw_u32 = smem_u32(bi8_smem_raw);
     const uint32_t base = (raw_u32 + 1023u) & ~1023u;
-    const uint32_t pX0 = base + OFF_X0, pX1 = base + OFF_X1, pX2 = base + OFF_X2, pX3 = base + OFF_X3;
-    const uint32_t pW0 = base + OFF_W0, pW1 = base + OFF_W1, pR = base + OFF_R, stg0 = base + OFF_STG;
-    const uint32_t b_stg_full = smem_u32(&bars[0]), b_stg_empty = b_stg_full + 8 * NSTG;
-    const uint32_t b_a_full = b_stg_empty + 8 * NSTG, b_s_full = b_a_full + 8, b_r_full = b_a_full + 16, b_t_full = b_a_full + 24, b_w_full = b_a_full + 32, b_l_full = b_a_full + 40;
+    const uint32_t pW0 = base + OFF_W, pW1 = pW0 + PLANE, pR = base + OFF_R;
+    const uint32_t b_x_full = smem_u32(&bars[0]);          // [2]: the X planes of a tile have landed in buffer 0 / 1
+    const uint32_t b_f_done = b_x_full + 16, b_s_full = b_x_full + 24, b_r_full = b_x_full + 32, b_t_full = b_x_full + 40, b_w_full = b_x_full + 48;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NSTG; ++s) { mbar_init(b_stg_full + 8 * s, 1); mbar_init(b_stg_empty + 8 * s, NEW); }
-        mbar_init(b_a_full, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1); mbar_init(b_w_full, 1); mbar_init(b_l_full, 1);
+        mbar_init(b_x_full, 1); mbar_init(b_x_full + 8, 1);
+        mbar_init(b_f_done, NEW); mbar_init(b_s_full, 1); mbar_init(b_r_full, NEW); mbar_init(b_t_full, 1); mbar_init(b_w_full, 1);
         fence_async_smem();
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     }
     if (warp == 0) tmem_alloc(smem_u32(&tmem_base_s), 512);
-    if (threadIdx.x < 128) s_scl[threadIdx.x] = sc.s[threadIdx.x];
     {                                                     // W digit planes: global image -> shared memory
         for (int i = threadIdx.x; i < 4 * PLANE / 16; i += NEW * 32) {
             const uint4 v = __ldg(reinterpret_cast<const uint4 *>(Wp) + i);
-            sts128((i < PLANE / 16 ? pW0 : pW1 - PLANE) + 16u * (uint32_t)i, v.x, v.y, v.z, v.w);     // image order: W0 W1 W2 W3
+            sts128(pW0 + 16u * (uint32_t)i, v.x, v.y, v.z, v.w);     // image order: W0 W1 W2 W3
         }
         fence_async_smem();
     }
@@ -294,30 +238,23 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
     const long long nt = per + (blockIdx.x < rem ? 1 : 0);
 
     {
-        // ===== all 16 warps convert and run the epilogues; lane 0 of warp 0 also issues the MMAs, lane 0 of
-        // warp 1 the TMA loads (no dedicated producer / issuer warps: 512 threads leave 128 registers each,
-        // enough for the 32 fp64 accumulators per thread without spilling) =====
+        // ===== all 16 warps run the epilogues; lane 0 of warp 0 also issues the MMAs, lane 0 of warp 1 the bulk
+        // copies (no dedicated producer / issuer warps: 512 threads leave 128 registers each, enough for the 32 fp64
+        // accumulators per thread without spilling) =====
         const bool is_mma = threadIdx.x == 0, is_tma = threadIdx.x == 32;
-        // Stages 0..2 of every tile go through the ring (slot = stage, refilled for the next tile as soon as all 16 warps
-        // have released it).  The LAST stage of a tile has no ring slot to wait in: it is loaded into the slot of R1, which
-        // is free from the end of GEMM2 until phase 2 of the next tile, right after GEMM2 completes — so its HBM latency
-        // hides behind the flush instead of stalling the conversion.
-        static_assert(NSTG == 3 && SPT == 4, "ring = the first three stages of a tile");
-        auto tma_load = [&](long long tt, int st) {
-            const uint32_t bar = st < NSTG ? b_stg_full + 8 * st : b_l_full;
-            const uint32_t dst = st < NSTG ? stg0 + (uint32_t)st * STG_BYTES : pR + PLANE;
-            mbar_expect_tx(bar, STG_BYTES);
-            asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                         ::"r"(dst), "l"(&tmap), "r"(0), "r"((int)((t_begin + tt) * TE + st * SR)), "r"(bar) : "memory");
+        auto x_load = [&](long long tt) {                                // the four X planes of tile tt -> buffer tt & 1
+            const uint32_t bar = b_x_full + 8u * (uint32_t)(tt & 1);
+            const uint32_t dst = base + ((tt & 1) ? OFF_XB : OFF_XA);
+            const unsigned char *src = planes + (size_t)(t_begin + tt) * TILE_BYTES;
+            mbar_expect_tx(bar, TILE_BYTES);
+#pragma unroll
+            for (int p = 0; p < 4; ++p) bulk_g2s(dst + (uint32_t)p * PLANE, src + (size_t)p * PLANE, PLANE, bar);
         };
-        if (is_tma && nt > 0)
-            for (int st = 0; st < SPT; ++st) tma_load(0, st);
+        if (is_tma) { if (nt > 0) x_load(0); if (nt > 1) x_load(1); }
         __syncwarp();
         const int q = warp & 3, j = warp >> 2;
         const int row = 32 * q + lane;                                 // event row (GEMM1) / real column c (GEMM2)
         const uint32_t trow = tmem0 + ((uint32_t)(32 * q) << 16) + 32u * (uint32_t)j;
-        const float4 scl = *reinterpret_cast<const float4 *>(&s_scl[4 * lane]);
-        const uint32_t chunk_off = (uint32_t)(lane & 3) * 4u, chunk_id = (uint32_t)(lane >> 2);
         double Tacc[32];
 #pragma unroll
         for (int i = 0; i < 32; ++i) Tacc[i] = 0.0;
@@ -328,46 +265,14 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
 
         for (long long t = 0; t < nt; ++t) {
             const uint32_t ph = (uint32_t)(t & 1);
-            // ---- fp32 stages -> X digit planes (2 rows per warp and stage)
-#pragma unroll 1
-            for (int st = 0; st < SPT; ++st) {
-                mbar_wait(st < NSTG ? b_stg_full + 8 * st : b_l_full, ph);
-                const uint32_t src = (st < NSTG ? stg0 + (uint32_t)st * STG_BYTES : pR + PLANE) + (uint32_t)(2 * warp) * ROWB + (uint32_t)lane * 16u;
-                uint4 raw[2];
-                raw[0] = lds128(src); raw[1] = lds128(src + ROWB);
-#pragma unroll
-                for (int r = 0; r < 2; ++r) {
-                    const uint32_t e = (uint32_t)(st * SR + 2 * warp + r);
-                    const uint32_t w0 = digits(__float2int_rn(__uint_as_float(raw[r].x) * scl.x));
-                    const uint32_t w1 = digits(__float2int_rn(__uint_as_float(raw[r].y) * scl.y));
-                    const uint32_t w2 = digits(__float2int_rn(__uint_as_float(raw[r].z) * scl.z));
-                    const uint32_t w3 = digits(__float2int_rn(__uint_as_float(raw[r].w) * scl.w));
-                    const uint32_t t0 = __byte_perm(w0, w1, 0x5140), t1 = __byte_perm(w2, w3, 0x5140);
-                    const uint32_t t2 = __byte_perm(w0, w1, 0x7362), t3 = __byte_perm(w2, w3, 0x7362);
-                    const uint32_t a = e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX0 + a), "r"(__byte_perm(t0, t1, 0x5410)) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX1 + a), "r"(__byte_perm(t0, t1, 0x7632)) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX2 + a), "r"(__byte_perm(t2, t3, 0x5410)) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(pX3 + a), "r"(__byte_perm(t2, t3, 0x7632)) : "memory");
-                }
-                __syncwarp();
-                if (st < NSTG) {
-                    if (lane == 0) mbar_arrive(b_stg_empty + 8 * st);
-                    if (is_tma && t + 1 < nt) {                          // refill the slot for the next tile once all 16 warps have released it
-                        mbar_wait(b_stg_empty + 8 * st, ph);
-                        tma_load(t + 1, st);
-                    }
-                    __syncwarp();
-                }
-            }
-            fence_async_smem();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(b_a_full);
+            const uint32_t pX0 = base + (ph ? OFF_XB : OFF_XA), pX1 = pX0 + PLANE, pX2 = pX0 + 2 * PLANE, pX3 = pX0 + 3 * PLANE;
             if (is_mma) {
                 // ---- GEMM1: S levels t = 3..6 at TMEM columns 0, 128, 256, 384
-                mbar_wait(b_a_full, ph);
-                if (t > 0) mbar_wait(b_w_full, (uint32_t)((t - 1) & 1));      // W0 is back in its slot
+                if (t > 0) {
+                    mbar_wait(b_f_done, (uint32_t)((t - 1) & 1));             // every warp has read the Q block of tile t - 1 out of TMEM
+                    mbar_wait(b_w_full, (uint32_t)((t - 1) & 1));             // the W planes are back in their slots
+                }
+                mbar_wait(b_x_full + 8u * ph, (uint32_t)((t >> 1) & 1));      // the X planes of this tile have landed
                 tc_fence_after();
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk) {
@@ -411,10 +316,10 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                     I[m] = fma(fr[m], fr[m], fi[m] * fi[m]);
                     cancel |= I[m] < thr2 && 16 * j + 4 * ch + m < Kc;
                 }
-                // Strong cancellation (|z| < 2^31: the truncation of GEMM1, ~2^9 rms in these units, would exceed
-                // ~2^-22 |z|): the warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for typical
-                // events, so this concerns ~1e-4 of the sums (the ones that dominate the gradient): one vote per
-                // chunk, the branch is almost never taken.
+                // Strong cancellation (the truncation of GEMM1, ~2^9 rms in these units, would exceed ~2^-22 |z|): the
+                // warp recomputes this S in fp64 (recompute_z).  |z| is ~2^37.7 for typical events, so this concerns
+                // ~1e-6 .. 1e-4 of the sums (the ones that dominate the gradient): one vote per chunk, the branch is
+                // almost never taken.
                 if (__any_sync(0xffffffffu, cancel && valid)) {
 #pragma unroll 1
                     for (int m = 0; m < 4; ++m) {
@@ -448,8 +353,8 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                     const unsigned mx = __reduce_max_sync(0xffffffffu, max((uint32_t)rhi[2 * m] & 0x7fffffffu, (uint32_t)rhi[2 * m + 1] & 0x7fffffffu));
                     if (lane == 0) s_emax[warp][4 * ch + m] = mx;
                 }
-                tmem_st8i(trow + 8 * ch, rlo);                  // fp64 Rh: low words over the t = 3 columns, high words over t = 4
-                tmem_st8i(trow + 8 * ch + 128, rhi);
+                tmem_st8(trow + 8 * ch, rlo);                   // fp64 Rh: low words over the t = 3 columns, high words over t = 4
+                tmem_st8(trow + 8 * ch + 128, rhi);
                 // lanes exchange so that each keeps ONE column of the chunk (m = 2 b4 + b3), multiplied over 4 lanes
                 const double send0 = b4 ? lv[0] : lv[2], send1 = b4 ? lv[1] : lv[3];
                 double keep0 = b4 ? lv[2] : lv[0], keep1 = b4 ? lv[3] : lv[1];
@@ -468,31 +373,34 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
             tc_fence_before();
             epi_bar();
 
-            // ---- phase 2: shifts sh_k (max_i |Rh_ik| 2^sh_k < 2^30), Rh -> four digit planes (R0 takes the slot of W0)
+            // ---- phase 2: per starting point the scale that maps max_i |Rh_ik| of the tile's 128 events (4 warps) onto the
+            // full four-digit range, |q| <= 2^31 - 2^25 (a balanced four-digit integer reaches 2^31 - 2^23 - 2^15 - 2^7; a
+            // power of two would waste 1.5 bits on average); Rh -> four digit planes (over the W planes, GEMM1 is done)
             tc_fence_after();
-            // per starting point: sh_k = 29 - floor(log2 max_i |Rh_ik|) over the tile's 128 events (4 warps), kept as sh_k << 20
             if (threadIdx.x < KC) {
                 const int jj = threadIdx.x >> 4, mm = threadIdx.x & 15;
                 const uint32_t bits = max(max(s_emax[4 * jj][mm], s_emax[4 * jj + 1][mm]), max(s_emax[4 * jj + 2][mm], s_emax[4 * jj + 3][mm]));
-                s_sh[threadIdx.x] = bits == 0u ? 0u : (uint32_t)(29 + 1023 - (int)(bits >> 20)) << 20;
+                const double mx = __hiloint2double((int)bits + 1, 0);      // >= the maximum (the high word rounded up)
+                const float sf = bits == 0u ? 0.0f : __double2float_rd(2113929216.0 / mx);
+                s_scale[threadIdx.x] = sf;
+                s_inv[threadIdx.x] = bits == 0u ? 0.0 : 1.0 / (double)sf;
             }
             epi_bar();
-            uint32_t sh20[16];
-#pragma unroll
-            for (int w = 0; w < 4; ++w) {
-                const uint4 v = *reinterpret_cast<const uint4 *>(&s_sh[16 * j + 4 * w]);
-                sh20[4 * w] = v.x; sh20[4 * w + 1] = v.y; sh20[4 * w + 2] = v.z; sh20[4 * w + 3] = v.w;
-            }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 int32_t flo[16], fhi[16];
-                tmem_ld16i(trow + 16 * h, flo);
-                tmem_ld16i(trow + 16 * h + 128, fhi);
+                tmem_ld16(trow + 16 * h, flo);
+                tmem_ld16(trow + 16 * h + 128, fhi);
                 tmem_ld_wait();
                 uint32_t wq[16];
 #pragma unroll
-                for (int i = 0; i < 16; ++i)       // rint(Rh 2^sh) (|.| < 2^30) = low word of Rh 2^sh + 1.5 * 2^52; 2^sh goes into the exponent
-                    wq[i] = digits(__double2loint(__hiloint2double(fhi[i] + (int)sh20[8 * h + (i >> 1)], flo[i]) + 6755399441055744.0));
+                for (int g = 0; g < 4; ++g) {      // rint(Rh s) (|.| < 2^31) = low word of Rh s + 1.5 * 2^52
+                    const float2 s2 = *reinterpret_cast<const float2 *>(&s_scale[16 * j + 8 * h + 2 * g]);
+                    const double sx = (double)s2.x, sy = (double)s2.y;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        wq[4 * g + i] = digits(__double2loint(fma(__hiloint2double(fhi[4 * g + i], flo[4 * g + i]), (i < 2 ? sx : sy), 6755399441055744.0)));
+                }
                 uint32_t p0[4], p1[4], p2[4], p3[4];
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
@@ -512,16 +420,16 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
             __syncwarp();
             if (lane == 0) mbar_arrive(b_r_full);
             if (is_mma) {
-                // ---- GEMM2: Q levels t = 3..6 at TMEM columns 0, 128, 256, 384 (R0 sits in the slot of W0)
+                // ---- GEMM2: Q levels t = 3..6 at TMEM columns 0, 128, 256, 384 (the R planes sit in the slots of the W planes)
                 mbar_wait(b_r_full, ph);
                 tc_fence_after();
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk) {
                     const uint32_t ko = (uint32_t)kk * 32u * 128u, acc = kk > 0 ? 1u : 0u;
-                    const uint64_t a0 = desc_mnmajor(pX0 + ko), a1 = desc_mnmajor(pX1 + ko);
-                    const uint64_t a2 = desc_mnmajor(pX2 + ko), a3 = desc_mnmajor(pX3 + ko);
-                    const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko), r1 = desc_mnmajor(pR + 1 * PLANE + ko);
-                    const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko), r3 = desc_mnmajor(pR + 3 * PLANE + ko);
+                    const uint64_t a0 = desc_mnmajor(pX0 + ko, PLANE), a1 = desc_mnmajor(pX1 + ko, PLANE);
+                    const uint64_t a2 = desc_mnmajor(pX2 + ko, PLANE), a3 = desc_mnmajor(pX3 + ko, PLANE);
+                    const uint64_t r0 = desc_mnmajor(pR + 0 * PLANE + ko, PLANE), r1 = desc_mnmajor(pR + 1 * PLANE + ko, PLANE);
+                    const uint64_t r2 = desc_mnmajor(pR + 2 * PLANE + ko, PLANE), r3 = desc_mnmajor(pR + 3 * PLANE + ko, PLANE);
                     umma_i8(tmem0 + 256, a3, r2, kI2_256, acc);        // X3^T [R2 | R3] -> t = 5 | 6
                     umma_i8(tmem0 + 0,   a3, r0, kI2_256, acc);        // X3^T [R0 | R1] -> t = 3 | 4
                     umma_i8(tmem0 + 0,   a2, r1, kI2_256, 1u);         // X2^T [R1 | R2] -> t = 3 | 4
@@ -533,19 +441,21 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
             }
             __syncwarp();
 
-            // ---- flush: Q levels of this tile -> fp64 accumulators (row = real column c)
+            // ---- flush: Q orders of this tile -> fp64 accumulators (row = real column c)
             mbar_wait(b_t_full, ph);
-            if (is_tma && t + 1 < nt) {                                  // GEMM2 is done with the R planes:
-                mbar_expect_tx(b_w_full, PLANE);                         // W0 back into its slot (R0) for the next GEMM1,
-                bulk_g2s(pW0, Wp, PLANE, b_w_full);
-                tma_load(t + 1, NSTG);                                   // the next tile's last stage into the slot of R1
+            if (is_tma && t + 1 < nt) {                                  // GEMM2 is done with the R planes and with this X buffer:
+                mbar_expect_tx(b_w_full, 4 * PLANE);                     // the W planes back into their slots for the next GEMM1 (from L2),
+#pragma unroll
+                for (int p = 0; p < 4; ++p) bulk_g2s(pW0 + (uint32_t)p * PLANE, Wp + (size_t)p * PLANE, PLANE, b_w_full);
+                if (t + 2 < nt) x_load(t + 2);                           // the planes of tile t + 2 into the buffer of tile t
             }
             __syncwarp();
             tc_fence_after();
 #pragma unroll
             for (int ch = 0; ch < 4; ++ch) {
-                const uint4 shv = *reinterpret_cast<const uint4 *>(&s_sh[16 * j + 4 * ch]);
-                const uint32_t shc[4] = {shv.x, shv.y, shv.z, shv.w};
+                const double2 iv0 = *reinterpret_cast<const double2 *>(&s_inv[16 * j + 4 * ch]);
+                const double2 iv1 = *reinterpret_cast<const double2 *>(&s_inv[16 * j + 4 * ch + 2]);
+                const double inv[4] = {iv0.x, iv0.y, iv1.x, iv1.y};
                 int32_t a3[8], a4[8], a5[8], a6[8];
                 tmem_ld8(trow + 8 * ch + 0, a3);
                 tmem_ld8(trow + 8 * ch + 128, a4);
@@ -554,13 +464,14 @@ k_batch_i8(const __grid_constant__ CUtensorMap tmap, const float *__restrict__ A
                 tmem_ld_wait();
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    // z 2^-sh with z = 2^16 y + x: two exact int -> fp64 conversions, two fused accumulations
-                    const int fsh = (int)((1023u << 20) - shc[i >> 1]);
-                    const double acc = fma(i2d(a4[i] * 256 + a3[i]), __hiloint2double(fsh, 0), Tacc[8 * ch + i]);
-                    Tacc[8 * ch + i] = fma(i2d(a6[i] * 256 + a5[i]), __hiloint2double(fsh + (16 << 20), 0), acc);
+                    // Z / s with Z = 2^16 (2^8 a6 + a5) + (2^8 a4 + a3): the four levels combined exactly in fp64 (|Z| < 2^48), one fused accumulation
+                    const double Z = fma(i2d(a6[i] * 256 + a5[i]), 65536.0, i2d(a4[i] * 256 + a3[i]));
+                    Tacc[8 * ch + i] = fma(Z, inv[i >> 1], Tacc[8 * ch + i]);
                 }
             }
             tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_f_done);                        // this warp's TMEM reads of tile t are complete
         }
 
         // ---- per-CTA partials -> fixed slot
@@ -639,23 +550,11 @@ k_bi8_finalize(const double *__restrict__ slots, int nslots, int n, const double
 }  // namespace bi8
 
 // ---- host side ----------------------------------------------------------------------------------
-static PFN_cuTensorMapEncodeTiled_v12000 bi8_get_encode()
-{
-    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
-// Handles fp32-stored constant-resonance data samples with n = 64 waves, no event weights.  Default for
-// K >= 8 and >= 32768 events (option "batch" = 0); "batch" = 2 forces it for any K and sample size,
-// "batch" = 1 keeps the FP64 DMMA path (batch_dmma.cu).
+// Handles fp32-stored constant-resonance data samples with n = 64 waves, no event weights.  Default for K >= 8
+// and >= 32768 events (option "batch" = 0); "batch" = 2 forces it for any K and sample size, "batch" = 1 keeps the
+// FP64 DMMA path (batch_dmma.cu).  The first call after an upload writes the X
+// digit-plane image (one extra pass over the sample, as large as the sample; if that allocation fails the FP64 path
+// serves the call).
 pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
 {
     *handled = false;
@@ -686,22 +585,24 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
         q.checked = true;
     }
     if (!q.valid) return PWA_OK;
-    PFN_cuTensorMapEncodeTiled_v12000 enc = bi8_get_encode();
-    if (!enc) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
-    alignas(64) CUtensorMap tmap;
-    {
-        const cuuint64_t gdim[2] = {128, (cuuint64_t)N};
-        const cuuint64_t gstride[1] = {512};
-        const cuuint32_t box[2] = {128, (cuuint32_t)bi8::SR};
-        const cuuint32_t estr[2] = {1, 1};
-        CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, ctx->data.amps, gdim, gstride, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled (i8 batch) failed (code " + std::to_string((int)r) + ")");
-    }
     const long long ntiles = (N + bi8::TE - 1) / bi8::TE;
     long long grid = ctx->sm_count;
     if (grid > ntiles) grid = ntiles;
+    bi8::Scales sc;
+    bi8::Exps ex;
+    memcpy(sc.s, q.scale, sizeof(sc.s));
+    memcpy(ex.e, q.exp, sizeof(ex.e));
+    if (q.planes == nullptr) {                      // once per upload: the X digit-plane image (does not depend on V)
+        void *img = nullptr;
+        cudaError_t e = cudaMalloc(&img, (size_t)ntiles * bi8::TILE_BYTES);
+        if (e != cudaSuccess) { cudaGetLastError(); q.valid = false; return PWA_OK; }     // no room: the FP64 path serves
+        q.planes = static_cast<unsigned char *>(img);
+        long long pg = (long long)ctx->sm_count * 4;
+        if (pg > ntiles) pg = ntiles;
+        bi8::k_bi8_planes<<<(unsigned)pg, bi8::THREADS, 0, ctx->stream>>>(reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, sc, q.planes);
+        ctx->launches++;
+        PWA_CUDA(ctx, cudaGetLastError());
+    }
     static bool s_attr[64] = {false};
     if (!s_attr[ctx->device & 63]) {
         PWA_CUDA(ctx, cudaFuncSetAttribute(bi8::k_batch_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bi8::SMEM));
@@ -714,16 +615,12 @@ pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled)
     int *ek = reinterpret_cast<int *>(Wp + wp_bytes);
     double *Wd = reinterpret_cast<double *>(Wp + wp_bytes + ek_bytes);
     double *slots = Wd + 128 * 128;
-    bi8::Scales sc;
-    bi8::Exps ex;
-    memcpy(sc.s, q.scale, sizeof(sc.s));
-    memcpy(ex.e, q.exp, sizeof(ex.e));
     for (int k0 = 0; k0 < K; k0 += bi8::KC) {
         const int cols = (K - k0 < bi8::KC) ? (K - k0) : bi8::KC;
         bi8::k_bi8_prep<<<bi8::KC, 128, 0, ctx->stream>>>(ctx->d_V, ctx->n, K, k0, ex, Wp, ek, Wd);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
-        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(tmap, reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, cols, thr2, sc, ex, Wp, Wd, slots);
+        bi8::k_batch_i8<<<(unsigned)grid, bi8::THREADS, bi8::SMEM, ctx->stream>>>(q.planes, reinterpret_cast<const float *>(ctx->data.amps), N, ntiles, cols, thr2, ex, Wp, Wd, slots);
         ctx->launches++;
         PWA_CUDA(ctx, cudaGetLastError());
         bi8::k_bi8_finalize<<<cols, 1024, 0, ctx->stream>>>(slots, (int)grid, ctx->n, ctx->d_V, k0, ek, N, ctx->d_M,

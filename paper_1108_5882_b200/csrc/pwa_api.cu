@@ -62,6 +62,13 @@ static void free_sample(Sample &s)
     s = Sample();
 }
 
+// the int8 batched path's per-upload state of the DATA sample (column scales, digit-plane image)
+static void drop_i8d(pwa_ctx *ctx)
+{
+    if (ctx->i8d.planes) cudaFree(ctx->i8d.planes);
+    ctx->i8d.planes = nullptr; ctx->i8d.checked = false; ctx->i8d.valid = false;
+}
+
 static size_t elem_size(pwa_dtype d) { return d == PWA_F32 ? sizeof(float) : sizeof(double); }
 
 // copy (host or device source) into a fresh device buffer, or borrow a device pointer
@@ -251,6 +258,7 @@ void pwa_destroy(pwa_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     free_sample(ctx->data);
     free_sample(ctx->mc);
+    drop_i8d(ctx);
     if (ctx->d_M) cudaFree(ctx->d_M);
     if (ctx->d_ticket) cudaFree(ctx->d_ticket);
     if (ctx->d_result) cudaFree(ctx->d_result);
@@ -284,7 +292,7 @@ pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, i
     Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
     free_sample(smp);
     smp.amps = buf; smp.amps_owned = owned; smp.factored = false;
-    if (which == PWA_DATA) { ctx->tmap_cache.valid = false; ctx->i8d.checked = false; ctx->i8d.valid = false; }
+    if (which == PWA_DATA) { ctx->tmap_cache.valid = false; drop_i8d(ctx); }
     smp.n_events = n_events; smp.n_gen = n_generated;
     if (which == PWA_MC) { ctx->M_valid = false; return prepare_norm_i8(ctx); }
     return PWA_OK;
@@ -312,7 +320,7 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
     smp.mass = (double *)bm; smp.ang = ba; smp.fact_owned = om || oa; smp.n_ang = n_ang; smp.factored = true;
     smp.n_events = n_events; smp.n_gen = n_generated;
     if (which == PWA_MC) { ctx->M_valid = false; ctx->i8q.valid = false; }
-    else { ctx->i8d.checked = false; ctx->i8d.valid = false; }
+    else drop_i8d(ctx);
     return PWA_OK;
 }
 

@@ -80,7 +80,8 @@ struct pwa_ctx {
     // int8 tensor-core M build (norm_i8.cu): per-column power-of-two scales found at MC upload
     struct { bool valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8q;
     // int8 tensor-core batched evaluation (batch_i8.cu): the same for the DATA sample, found on first use
-    struct { bool checked = false, valid = false; int exp[128]; float scale[128]; double cmax[128]; } i8d;
+    struct { bool checked = false, valid = false; int exp[128]; float scale[128]; double cmax[128];
+             unsigned char *planes = nullptr; } i8d;       // planes: X digit-plane image of the sample (k_bi8_planes), library-owned
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     int opt_l2_resident_mb = -1;              // MB of the data sample's head kept in L2 between evaluations (TMA data term); -1 = automatic, 0 = off

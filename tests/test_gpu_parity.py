@@ -449,8 +449,9 @@ def test_back_to_back_enqueues_are_independent(pwa, storage, n, N):
 @pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (129, 1), (257, 64), (6007, 64), (6007, 70), (40_001, 33)])
 def test_batch_i8_parity(pwa, oracle, N, K):
     """fp32 storage, n = 64, option "batch" = 2: both chained GEMMs on tcgen05 int8 (batch_i8.cu) against the
-    oracle and against the FP64 DMMA path: less than one tile, a ragged last tile, K < 64, K > 64 (two passes),
-    columns with very different amplitude scales and starting points with very different norms."""
+    oracle and against the FP64 DMMA path: less than one tile, one event past a tile boundary, a ragged last tile,
+    K = 1, K < 64, K > 64 (two passes), columns with very different amplitude scales and starting points with very
+    different norms."""
     n = 64
     rng = np.random.default_rng(1000 + N + K)
     A = (rng.normal(size=(N, n, 2)) * rng.uniform(0.01, 3.0, size=(1, n, 2))).astype(np.float32)
@@ -482,12 +483,12 @@ def test_batch_i8_strong_cancellation(pwa, oracle):
     """Events whose coherent sum nearly vanishes for some starting points (|S| ~ 1e-6 of the typical sum):
     the truncated integer GEMM alone would lose them, the fp64 recomputation (recompute_z) keeps the 1e-6 bar.
     Such events dominate the gradient (t_ia = A_ia / S_i), so a wrong S_i fails the comparison at once."""
-    n, N, K = 64, 3001, 9
+    n, N, K = 64, 5003, 9
     rng = np.random.default_rng(77)
     A = rng.normal(size=(N, n, 2)) * 0.5
     Vk = rng.normal(size=(K, n, 2))
     Ac = A[..., 0] + 1j * A[..., 1]
-    for k, i in ((0, 5), (0, 1500), (3, 2999), (8, 128)):
+    for k, i in ((0, 5), (0, 1500), (3, 5002), (8, 128)):
         Vc = Vk[k, :, 0] + 1j * Vk[k, :, 1]
         S = Ac[i] @ Vc
         Ac[i] -= (1.0 - 1e-6) * S * Vc.conj() / (np.abs(Vc) ** 2).sum()       # leaves S_i = 1e-6 of its old value

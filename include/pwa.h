@@ -281,17 +281,20 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx);
 /* Waits for all enqueued work of the context.                                             */
 pwa_status pwa_sync(pwa_ctx *ctx);
 
-/* Selects a kernel variant for experiments (0 = default).  Returns PWA_ERR_INVALID_ARG for
- * unknown keys.  Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood".  "norm": 0 = default (int8 tcgen05 path for
- * fp32-stored constant-resonance samples of >= 65536 events, else FP64 DMMA), 1 = FP64 DMMA,
- * 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.
+/* Selects a kernel family (0 = default).  Returns PWA_ERR_INVALID_ARG for unknown keys.
+ * Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood".
+ * "data_term": 0 = default (TMA-tiled streaming kernel where the row is 128 .. 1024 bytes and the sample carries no
+ * event weights, else the per-lane streaming kernel), 20 = per-lane kernel, 98 = default without programmatic
+ * dependent launch, 99 = generic kernel (any n).
+ * "norm": 0 = default (int8 tcgen05 path for fp32-stored constant-resonance samples of >= 65536 events, else
+ * FP64 DMMA), 1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.
  * "batch": 0 = default (see pwa_batch_path), 1 = FP64 DMMA GEMMs for any K, 2 = int8 tcgen05 GEMMs
  * whenever the shape allows, 99 = K passes of the streaming kernel.
  * "l2_resident_mb": MB of the head of the DATA sample that the streaming data term loads with the L2 evict_last
  * policy (the rest: evict_first), so that it stays in L2 from one evaluation to the next; -1 = automatic (48 MB for
  * samples between 64 MB and 1 GiB, else plain loads), 0 = plain loads, up to 120.
  * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
- * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch and the minimisers.    */
+ * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch, pwa_res_grad and the minimisers.    */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
 pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* current value of a pwa_set_option key */
 

@@ -137,158 +137,6 @@ k_data_term(const uint4 *__restrict__ A, long long N, VArg varg, FinishArgs fa, 
     reduce_and_finish<G, W, THREADS>(L, bad, tr, ti, wave_of, sV, fa);
 }
 
-// ---- TMA-staged variant (default for the fast wave counts) --------------------------------
-// Same lane mapping and arithmetic as k_data_term, but the rows reach the lanes through a
-// shared-memory ring filled by the bulk-copy engine (cp.async.bulk + mbarrier complete_tx,
-// SASS UBLKCP) instead of per-lane LDG: every warp owns a private ring of NSW stages, one stage =
-// the EPB = (32/G)*E consecutive rows of one warp step (one contiguous span of the row-major
-// matrix, so a 1-D bulk copy needs no tensor map).  Lane 0 re-arms a stage as soon as the warp
-// has pulled it into registers, so (NSW-1) stages per warp are always in flight: the bytes in
-// flight per SM are set by the ring (16 warps x (NSW-1) x 4-8 KB), not by the register file,
-// and no warp ever waits on another (no block barrier in the loop).
-template <typename ST, int G, int CK, int E, int THREADS, int MINB, int NSW>
-__global__ void __launch_bounds__(THREADS, MINB)
-k_data_term_ring(const unsigned char *__restrict__ A, long long N, VArg varg, FinishArgs fa)
-{
-    constexpr int WPC = Chunk<ST>::WPC;
-    constexpr int W = CK * WPC;
-    constexpr int CPR = G * CK;
-    constexpr int NW = CPR * WPC;
-    constexpr int GPW = 32 / G;
-    constexpr int EPB = GPW * E;
-    constexpr int NWARPS = THREADS / 32;
-    constexpr int ROWB = CPR * 16;                 // bytes per row
-    constexpr int STAGE = EPB * ROWB;              // bytes per stage
-    // groups of one quarter-warp (8 lanes) read different rows at the same time: rotate the chunk
-    // order by the group index so that they hit different banks (rows start 128-byte aligned)
-    constexpr bool ROT = (G < 8) && (CK > 1);
-    static_assert(E <= G && (G & (G - 1)) == 0 && (E & (E - 1)) == 0, "G, E powers of two, E <= G");
-
-    extern __shared__ __align__(128) unsigned char ring[];        // [NWARPS][NSW][STAGE]
-    __shared__ __align__(8) unsigned long long bars[NWARPS][NSW];
-    __shared__ double sV[2 * NW];
-    for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = varg.v[t];
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int j = lane % G, grp = lane / G;
-    const uint32_t ring0 = smem_u32(ring) + (uint32_t)(warp * NSW) * STAGE;
-    const uint32_t bar0 = smem_u32(&bars[warp][0]);
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NSW; ++s) mbar_init(bar0 + 8 * s, 1);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-
-    const long long nsteps = (N + EPB - 1) / EPB;
-    const long long stride = (long long)gridDim.x * NWARPS;
-    const long long b0 = (long long)blockIdx.x * NWARPS + warp;
-    auto issue = [&](long long b, int slot) {                    // lane 0 only
-        const long long row0 = b * EPB;
-        long long rows = N - row0; if (rows > EPB) rows = EPB;
-        const uint32_t bytes = (uint32_t)rows * ROWB;
-        mbar_expect_tx(bar0 + 8 * slot, bytes);
-        bulk_g2s(ring0 + (uint32_t)slot * STAGE, A + row0 * ROWB, bytes, bar0 + 8 * slot);
-    };
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NSW; ++s) { const long long b = b0 + s * stride; if (b < nsteps) issue(b, s); }
-    }
-
-    int kord[CK];                                  // chunk order of this lane (see ROT)
-#pragma unroll
-    for (int k = 0; k < CK; ++k) kord[k] = ROT ? ((k + grp) % CK) : k;
-
-    double vr[W], vi[W], tr[W], ti[W];
-#pragma unroll
-    for (int k = 0; k < CK; ++k)
-#pragma unroll
-        for (int w = 0; w < WPC; ++w) {
-            const int a = (j + G * kord[k]) * WPC + w;
-            vr[k * WPC + w] = sV[2 * a]; vi[k * WPC + w] = sV[2 * a + 1];
-            tr[k * WPC + w] = 0.0; ti[k * WPC + w] = 0.0;
-        }
-    double L = 0.0, bad = 0.0;
-
-    int slot = 0; uint32_t parity = 0;
-    for (long long b = b0; b < nsteps; b += stride) {
-        const long long ev0 = b * EPB + (long long)grp * E;
-        mbar_wait(bar0 + 8 * slot, parity);
-        const uint32_t base = ring0 + (uint32_t)slot * STAGE + (uint32_t)(grp * E) * ROWB + (uint32_t)j * 16;
-        uint4 q[E][CK];
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const bool ok = (ev0 + e) < N;
-#pragma unroll
-            for (int k = 0; k < CK; ++k) {
-                q[e][k] = lds128(base + (uint32_t)e * ROWB + (uint32_t)(G * kord[k]) * 16);
-                if (!ok) q[e][k] = make_uint4(0u, 0u, 0u, 0u);
-            }
-        }
-        // A2: partial coherent sums over this lane's waves
-        double sr[E], si[E];
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            double ar[WPC], ai[WPC];
-            sr[e] = 0.0; si[e] = 0.0;
-#pragma unroll
-            for (int k = 0; k < CK; ++k) {
-                Chunk<ST>::unpack(q[e][k], ar, ai);
-#pragma unroll
-                for (int w = 0; w < WPC; ++w) {
-                    sr[e] = fma(vr[k * WPC + w], ar[w], sr[e]); sr[e] = fma(-vi[k * WPC + w], ai[w], sr[e]);
-                    si[e] = fma(vr[k * WPC + w], ai[w], si[e]); si[e] = fma(vi[k * WPC + w], ar[w], si[e]);
-                }
-            }
-        }
-        group_transpose_reduce<G, E>(sr, si, j);
-        // every lane has consumed its smem loads (the shuffles above needed them): re-arm the stage
-        __syncwarp();
-        if (lane == 0) { const long long nb = b + (long long)NSW * stride; if (nb < nsteps) issue(nb, slot); }
-        if (++slot == NSW) { slot = 0; parity ^= 1u; }
-        // A3 + A4 for the one event this lane owns
-        const int my_e = j & (E - 1);
-        const bool valid = (ev0 + my_e) < N;
-        const double I = sr[0] * sr[0] + si[0] * si[0];
-        const double l = log(I);
-        const double inv = 1.0 / I;
-        double rr = sr[0] * inv, rim = -si[0] * inv;      // r = conj(S) / I
-        const bool counted = valid && (j < E);
-        if (counted) { L += l; if (!(I > 0.0) || !isfinite(l)) bad += 1.0; }
-        if (!valid) { rr = 0.0; rim = 0.0; }
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const double er = __shfl_sync(0xffffffffu, rr, e, G);
-            const double ei = __shfl_sync(0xffffffffu, rim, e, G);
-            double ar[WPC], ai[WPC];
-#pragma unroll
-            for (int k = 0; k < CK; ++k) {
-                Chunk<ST>::unpack(q[e][k], ar, ai);
-#pragma unroll
-                for (int w = 0; w < WPC; ++w) {
-                    tr[k * WPC + w] = fma(ar[w], er, tr[k * WPC + w]); tr[k * WPC + w] = fma(-ai[w], ei, tr[k * WPC + w]);
-                    ti[k * WPC + w] = fma(ar[w], ei, ti[k * WPC + w]); ti[k * WPC + w] = fma(ai[w], er, ti[k * WPC + w]);
-                }
-            }
-        }
-    }
-    // lanes of different groups hold their chunks in rotated order (ROT): bring the accumulators
-    // back to chunk order k before the cross-lane sums, which pair lanes with equal j
-    double cr[W], ci[W];
-#pragma unroll
-    for (int kc = 0; kc < CK; ++kc)
-#pragma unroll
-        for (int w = 0; w < WPC; ++w) {
-            double xr = 0.0, xi = 0.0;
-#pragma unroll
-            for (int k = 0; k < CK; ++k)
-                if (kord[k] == kc) { xr = tr[k * WPC + w]; xi = ti[k * WPC + w]; }
-            cr[kc * WPC + w] = xr; ci[kc * WPC + w] = xi;
-        }
-    auto wave_of = [&](int idx) { return (j + G * (idx / WPC)) * WPC + (idx % WPC); };
-    reduce_and_finish<G, W, THREADS>(L, bad, cr, ci, wave_of, sV, fa);
-}
-
 // Generic fallback: any n <= kMaxWaves, thread per event, V from device memory.
 template <typename ST, int THREADS>
 __global__ void __launch_bounds__(THREADS)
@@ -366,32 +214,6 @@ static pwa_status launch_fast(pwa_ctx *ctx, const VArg &varg, const FinishArgs &
     return PWA_OK;
 }
 
-template <typename ST, int G, int CK, int E, int THREADS, int MINB, int NSW>
-static pwa_status launch_ring(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa_in)
-{
-    auto kern = k_data_term_ring<ST, G, CK, E, THREADS, MINB, NSW>;
-    constexpr int EPB = (32 / G) * E, NWARPS = THREADS / 32;
-    constexpr size_t SMEM = (size_t)NWARPS * NSW * EPB * (G * CK * 16);
-    PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-    int occ = 0;
-    PWA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, SMEM));
-    if (occ < 1) occ = 1;
-    const long long N = ctx->data.n_events;
-    long long nsteps = (N + EPB - 1) / EPB;
-    long long want = (nsteps + NWARPS - 1) / NWARPS;
-    long long grid = (long long)ctx->sm_count * occ;
-    if (want < grid) grid = want;
-    if (grid < 1) grid = 1;
-    FinishArgs fa = fa_in;
-    pwa_status s = ensure_partials(ctx, (size_t)n_components(ctx->n) * (size_t)grid);
-    if (s != PWA_OK) return s;
-    fa.partials = ctx->d_partials;
-    kern<<<(unsigned)grid, THREADS, SMEM, ctx->stream>>>((const unsigned char *)ctx->data.amps, N, varg, fa);
-    ctx->launches++;
-    PWA_CUDA(ctx, cudaGetLastError());
-    return PWA_OK;
-}
-
 template <typename ST>
 static pwa_status launch_generic(pwa_ctx *ctx, const double *Vdev, const FinishArgs &fa_in)
 {
@@ -417,7 +239,7 @@ static pwa_status launch_generic(pwa_ctx *ctx, const double *Vdev, const FinishA
 }
 
 pwa_status launch_factored_data_term(pwa_ctx *ctx, const double *Vk, const FinishArgs &fa);   // factored.cu
-pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, int opt, bool *handled);   // data_term_tma.cu
+pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled);   // data_term_tma.cu
 
 // V_host_k: host pointer to V of evaluation k (already staged in ctx->h_V, mirrored in d_V).
 // out_dev_terms != nullptr selects the data-term-only output (multi-GPU path).
@@ -446,55 +268,31 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     }
     VArg varg;
     for (int t = 0; t < 2 * n; ++t) varg.v[t] = V_host_k[t];
-    int opt = ctx->opt_data_term;
-    if (opt == 98) opt = 0;                             // 98: default kernel without programmatic dependent launch (experiment switch)
-    if (ctx->data.weights && opt < 20) opt = 20;        // weighted samples: the per-lane LDG kernel carries the weight stream
-    // opt 0-9: TMA-tiled two-phase kernel (data_term_tma.cu; default where it applies);
-    // 10-19: bulk-copy ring variants; 20-29: per-lane LDG kernels (first design)
-    if (opt < 10) {
+    // "data_term": 0 = default: TMA-tiled two-phase kernel (data_term_tma.cu) where it applies (row of 128 .. 1024 bytes,
+    // no event weights), else the per-lane streaming kernel below; 20 = per-lane kernel always; 98 = default kernel
+    // without programmatic dependent launch; 99 = generic kernel
+    const bool per_lane = ctx->opt_data_term == 20 || ctx->data.weights != nullptr;   // the per-lane kernel carries the weight stream
+    if (!per_lane) {
         bool handled = false;
-        pwa_status s = launch_data_term_tma(ctx, varg, fa, opt, &handled);
+        pwa_status s = launch_data_term_tma(ctx, varg, fa, &handled);
         if (s != PWA_OK || handled) return s;
-        opt = 10;
     }
-    //                         ST      G  CK  E  THREADS MINB NSW
+    //                           ST      G  CK  E  THREADS MINB
     if (!f32) {
         switch (n) {
-        case 4:  return opt >= 20 ? launch_fast<double, 2, 2, 2, 256, 2>(ctx, varg, fa)
-                                  : launch_ring<double, 2, 2, 2, 256, 2, 3>(ctx, varg, fa);
-        case 8:  return opt >= 20 ? launch_fast<double, 4, 2, 4, 256, 2>(ctx, varg, fa)
-                                  : launch_ring<double, 4, 2, 4, 256, 2, 3>(ctx, varg, fa);
-        case 16: return opt == 21 ? launch_fast<double, 8, 2, 8, 256, 2>(ctx, varg, fa)
-                       : opt == 20 ? launch_fast<double, 4, 4, 4, 256, 2>(ctx, varg, fa)
-                       : opt == 11 ? launch_ring<double, 4, 4, 4, 256, 1, 3>(ctx, varg, fa)
-                                   : launch_ring<double, 8, 2, 4, 256, 2, 3>(ctx, varg, fa);
-        case 32: return opt == 21 ? launch_fast<double, 16, 2, 8, 256, 2>(ctx, varg, fa)
-                       : opt == 20 ? launch_fast<double, 8, 4, 4, 256, 2>(ctx, varg, fa)
-                                   : launch_ring<double, 16, 2, 4, 256, 2, 3>(ctx, varg, fa);
-        case 64: return opt == 21 ? launch_fast<double, 32, 2, 8, 256, 2>(ctx, varg, fa)
-                       : opt == 20 ? launch_fast<double, 16, 4, 4, 256, 2>(ctx, varg, fa)
-                                   : launch_ring<double, 16, 4, 4, 256, 1, 3>(ctx, varg, fa);
+        case 4:  return launch_fast<double, 2, 2, 2, 256, 2>(ctx, varg, fa);
+        case 8:  return launch_fast<double, 4, 2, 4, 256, 2>(ctx, varg, fa);
+        case 16: return launch_fast<double, 4, 4, 4, 256, 2>(ctx, varg, fa);
+        case 32: return launch_fast<double, 8, 4, 4, 256, 2>(ctx, varg, fa);
+        case 64: return launch_fast<double, 16, 4, 4, 256, 2>(ctx, varg, fa);
         }
     } else {
         switch (n) {
-        case 4:  return opt >= 20 ? launch_fast<float, 2, 1, 2, 256, 2>(ctx, varg, fa)
-                                  : launch_ring<float, 2, 1, 2, 256, 2, 3>(ctx, varg, fa);
-        case 8:  return opt >= 20 ? launch_fast<float, 4, 1, 4, 256, 2>(ctx, varg, fa)
-                                  : launch_ring<float, 4, 1, 4, 256, 2, 3>(ctx, varg, fa);
-        case 16: return opt >= 20 ? launch_fast<float, 4, 2, 4, 256, 2>(ctx, varg, fa)
-                       : opt == 11 ? launch_ring<float, 8, 1, 4, 256, 2, 3>(ctx, varg, fa)
-                                   : launch_ring<float, 4, 2, 4, 256, 2, 3>(ctx, varg, fa);
-        case 32: return opt == 21 ? launch_fast<float, 8, 2, 8, 256, 1>(ctx, varg, fa)
-                       : opt == 22 ? launch_fast<float, 4, 4, 4, 256, 1>(ctx, varg, fa)
-                       : opt == 20 ? launch_fast<float, 8, 2, 4, 256, 2>(ctx, varg, fa)
-                       : opt == 11 ? launch_ring<float, 8, 2, 4, 256, 2, 4>(ctx, varg, fa)
-                                   : launch_ring<float, 8, 2, 4, 256, 2, 3>(ctx, varg, fa);
-        case 64: return opt == 21 ? launch_fast<float, 16, 2, 8, 256, 1>(ctx, varg, fa)
-                       : opt == 22 ? launch_fast<float, 8, 4, 4, 256, 1>(ctx, varg, fa)
-                       : opt == 20 ? launch_fast<float, 16, 2, 4, 256, 2>(ctx, varg, fa)
-                       : opt == 11 ? launch_ring<float, 16, 2, 4, 256, 2, 4>(ctx, varg, fa)
-                       : opt == 12 ? launch_ring<float, 16, 2, 4, 256, 2, 2>(ctx, varg, fa)
-                                   : launch_ring<float, 16, 2, 4, 256, 2, 3>(ctx, varg, fa);
+        case 4:  return launch_fast<float, 2, 1, 2, 256, 2>(ctx, varg, fa);
+        case 8:  return launch_fast<float, 4, 1, 4, 256, 2>(ctx, varg, fa);
+        case 16: return launch_fast<float, 4, 2, 4, 256, 2>(ctx, varg, fa);
+        case 32: return launch_fast<float, 8, 2, 4, 256, 2>(ctx, varg, fa);
+        case 64: return launch_fast<float, 16, 2, 4, 256, 2>(ctx, varg, fa);
         }
     }
     return fail(ctx, PWA_ERR_UNSUPPORTED, "data term: unsupported n");

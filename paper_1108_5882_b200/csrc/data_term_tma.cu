@@ -34,6 +34,7 @@
 #include "pwa_internal.h"
 #include "reduce.cuh"
 #include "stream_common.cuh"
+#include "tcgen05_common.cuh"
 
 namespace pwa {
 
@@ -288,24 +289,10 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     reduce_and_finish<G2, W2, THREADS>(L, bad, trs, tis, wave_of, sV, fa);
 }
 
-// ---- host side: tensor map (driver entry point fetched through the runtime; no -lcuda) ----------
-static PFN_cuTensorMapEncodeTiled_v12000 get_encode()
-{
-    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
+// ---- host side: tensor map ------------------------------------------------------------------------
 static pwa_status make_tmap(pwa_ctx *ctx, CUtensorMap *out, const void *base, bool f32, int n, long long N, int box_rows)
 {
-    PFN_cuTensorMapEncodeTiled_v12000 enc = get_encode();
+    PFN_cuTensorMapEncodeTiled_v12000 enc = tc::tensor_map_encoder();
     if (!enc) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
     const cuuint64_t gdim[2] = {(cuuint64_t)(2 * n), (cuuint64_t)N};
     const cuuint64_t gstride[1] = {(cuuint64_t)(2 * n) * (f32 ? 4u : 8u)};
@@ -373,8 +360,8 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     return PWA_OK;
 }
 
-// opt: 0 = default configuration of this kernel; 1.. = tuning variants (see the table below).
-pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, int opt, bool *handled)
+// One configuration per (storage, n): the fastest of the variants measured in round 1 (profiles/r1b_summary.md).
+pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled)
 {
     *handled = false;
     const int n = ctx->n;
@@ -384,31 +371,19 @@ pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs
     const int row_bytes = 2 * n * (f32 ? 4 : 8);
     if (row_bytes % 128 != 0 || row_bytes > 1024 || (n & (n - 1)) != 0) return PWA_OK;
     *handled = true;
-    //                                   ST    CB LPR THREADS MINB GW NS     stage bytes, notes
+    //                         ST    CB LPR THREADS MINB GW NS     stage bytes
     if (f32) {
         switch (n) {
-        case 16: return launch_tma<float, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);                    //  4 KB
-        case 32: return opt == 1 ? launch_tma<float, 2, 2, 512, 1, 2, 3>(ctx, varg, fa)          //  4 KB
-                      : opt == 2 ? launch_tma<float, 2, 1, 256, 1, 1, 3>(ctx, varg, fa)          //  8 KB, 8 warps
-                                 : launch_tma<float, 2, 1, 512, 1, 2, 3>(ctx, varg, fa);         //  8 KB, 16 warps (cfg2: 61.6 vs 65.3 us)
-        case 64: return opt == 1 ? launch_tma<float, 4, 1, 256, 1, 2, 3>(ctx, varg, fa)          // 16 KB, V in the constant bank, 8 warps
-                      : opt == 2 ? launch_tma<float, 4, 2, 384, 1, 1, 2>(ctx, varg, fa)          //  8 KB, 12 warps, private rings
-                      : opt == 3 ? launch_tma<float, 4, 2, 512, 1, 4, 6>(ctx, varg, fa)          //  8 KB, 16 warps, groups of 4
-                      : opt == 4 ? launch_tma<float, 4, 1, 320, 1, 5, 6>(ctx, varg, fa)          // 16 KB, 10 warps, groups of 5
-                                 : launch_tma<float, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);         //  8 KB, 16 warps, groups of 2
+        case 16: return launch_tma<float, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);      //  4 KB
+        case 32: return launch_tma<float, 2, 1, 512, 1, 2, 3>(ctx, varg, fa);      //  8 KB, 16 warps
+        case 64: return launch_tma<float, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);      //  8 KB, 16 warps, groups of 2
         }
     } else {
         switch (n) {
         case 8:  return launch_tma<double, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);
-        case 16: return opt == 1 ? launch_tma<double, 2, 1, 256, 1, 1, 3>(ctx, varg, fa)
-                      : opt == 2 ? launch_tma<double, 2, 1, 512, 1, 2, 3>(ctx, varg, fa)
-                                 : launch_tma<double, 2, 2, 512, 1, 2, 3>(ctx, varg, fa);        // 1e6 events: 48.3 vs 51.3 us
-        case 32: return opt == 1 ? launch_tma<double, 4, 1, 256, 1, 2, 3>(ctx, varg, fa)
-                      : opt == 2 ? launch_tma<double, 4, 2, 384, 1, 1, 2>(ctx, varg, fa)
-                                 : launch_tma<double, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);
-        case 64: return opt == 1 ? launch_tma<double, 8, 2, 256, 1, 2, 3>(ctx, varg, fa)
-                      : opt == 2 ? launch_tma<double, 8, 4, 384, 1, 1, 2>(ctx, varg, fa)
-                                 : launch_tma<double, 8, 4, 512, 1, 2, 3>(ctx, varg, fa);
+        case 16: return launch_tma<double, 2, 2, 512, 1, 2, 3>(ctx, varg, fa);
+        case 32: return launch_tma<double, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);
+        case 64: return launch_tma<double, 8, 4, 512, 1, 2, 3>(ctx, varg, fa);
         }
     }
     *handled = false;

@@ -185,7 +185,7 @@ pwa_status launch_norm_build(pwa_ctx *ctx)
     }
     // opt_norm: 0 = default (int8 tensor-core path for large fp32-stored samples, else FP64 DMMA),
     //           1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel
-    if ((ctx->opt_norm & 15) == 2 || (ctx->opt_norm == 0 && ctx->mc.n_events >= 65536)) {
+    if (ctx->opt_norm == 2 || (ctx->opt_norm == 0 && ctx->mc.n_events >= 65536)) {
         bool handled = false;
         pwa_status s = launch_norm_i8(ctx, &handled);
         if (s != PWA_OK) return s;

@@ -41,10 +41,13 @@
 
 #include "pwa_internal.h"
 #include "stream_common.cuh"
+#include "tcgen05_common.cuh"
 
 namespace pwa {
 
 namespace i8 {
+
+using namespace tc;
 
 constexpr int TE = 64;                       // super-rows (K) per tile
 constexpr int ROWB = 512;                    // bytes of one fp32 super-row (128 reals)
@@ -58,64 +61,13 @@ constexpr int NCW = 8;                       // converter / epilogue warps
 constexpr int THREADS = (NCW + 2) * 32;
 constexpr size_t SMEM = 1024 + (size_t)NSTG * STG_BYTES + (size_t)NSL * SL_BYTES;
 
-struct Scales { float s[128]; int dbg; int one; };    // 2^s_p per real column of the 128-wide view; dbg: experiment switches (0 in production); one = 1 (a runtime 1 keeps the digit-offset add on the IMAD pipe)
+struct Scales { float s[128]; int one; };    // 2^s_p per real column of the 128-wide view; one = 1 (a runtime 1 keeps the digit-offset add on the IMAD pipe)
 
-// ---- PTX wrappers -----------------------------------------------------------------------------
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols)
-{
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
-{
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-// D[tmem] (+)= A[smem]^T-major * B[smem]: int8 x int8 -> int32
-__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
-{
-    asm volatile("{\n"
-                 ".reg .pred p;\n"
-                 "setp.ne.b32 p, %4, 0;\n"
-                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
-                 "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t (&v)[16])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                 : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// Shared-memory matrix descriptor of one digit plane (or a 32-row K step of it): MN-major,
-// SWIZZLE_128B, rows (K) of 128 bytes, 8-row swizzle atoms 1024 bytes apart (SBO).  One plane is
-// exactly one 128-byte atom along MN; an N = 256 operand continues in the NEXT plane (LBO = PLANE),
-// so [D_v | D_v+1] is one B operand and its two products land in adjacent accumulators.
-__device__ __forceinline__ uint64_t plane_desc(uint32_t smem_addr)
-{
-    uint64_t d = 0;
-    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);          // start address, bits [0, 14)
-    d |= (uint64_t)((uint32_t)PLANE >> 4) << 16;           // leading byte offset: next 128-byte atom along MN = next digit plane (N = 256)
-    d |= (uint64_t)(1024u >> 4) << 32;                     // stride byte offset: next 8 K rows
-    d |= (uint64_t)1 << 46;                                // descriptor version (Blackwell)
-    d |= (uint64_t)2 << 61;                                // SWIZZLE_128B
-    return d;
-}
-// kind::i8 instruction descriptor: D = s32, A = B = signed int8, both MN-major, M = 128, N = 128 or 256
-constexpr uint32_t idesc_n(uint32_t N) { return (2u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((N >> 3) << 17) | ((128u >> 4) << 24); }
-constexpr uint32_t kIdesc128 = idesc_n(128), kIdesc256 = idesc_n(256);
+// One digit plane (or a 32-row K step of it) as an MN-major operand (tcgen05_common.cuh): one plane is exactly one
+// 128-byte atom along MN; an N = 256 operand continues in the NEXT plane (LBO = PLANE), so [D_v | D_v+1] is one B
+// operand and its two products land in adjacent accumulators.
+__device__ __forceinline__ uint64_t plane_desc(uint32_t smem_addr) { return desc_mnmajor(smem_addr, PLANE); }
+constexpr uint32_t kIdesc128 = idesc_i8(128, true, true), kIdesc256 = idesc_i8(256, true, true);   // both operands MN-major
 
 // ---- the kernel -------------------------------------------------------------------------------
 // tmap: fp32 [rows][128] view of the MC sample, box = [TE rows][128 floats], no swizzle.
@@ -183,7 +135,6 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                     const uint64_t d0 = plane_desc(pl + 0 * PLANE + koff), d1 = plane_desc(pl + 1 * PLANE + koff);
                     const uint64_t d2 = plane_desc(pl + 2 * PLANE + koff), d3 = plane_desc(pl + 3 * PLANE + koff);
                     const uint32_t acc = (first && kk == 0) ? 0u : 1u;
-                    if (sc.dbg & 1) continue;                          // experiment: no MMA issued
                     // accumulators by ascending order: t = 3 at column 0, t = 4 at 128, t = 5 at 256, t = 6 at 384
                     umma_i8(tmem0 + 256, d3, d2, kIdesc256, acc);      // D3^T [D2 | D3] -> t = 5 | t = 6
                     umma_i8(tmem0 + 0,   d3, d0, kIdesc256, acc);      // D3^T [D0 | D1] -> t = 3 | t = 4
@@ -217,14 +168,6 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
 #pragma unroll
             for (int r = 0; r < TE / NCW; ++r) {
                 const uint32_t e = (uint32_t)(warp + r * NCW);
-                if (sc.dbg & 2) {                                      // experiment: no conversion arithmetic
-                    const uint32_t a = dst + e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 0 * PLANE), "r"(raw[r].x) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 1 * PLANE), "r"(raw[r].y) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 2 * PLANE), "r"(raw[r].z) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 3 * PLANE), "r"(raw[r].w) : "memory");
-                    continue;
-                }
                 const uint32_t w0 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) * one + 0x00808080) ^ 0x00808080u;
                 const uint32_t w1 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) * one + 0x00808080) ^ 0x00808080u;
                 const uint32_t w2 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) * one + 0x00808080) ^ 0x00808080u;
@@ -381,20 +324,6 @@ k_i8_assemble(const double *__restrict__ ysum, const double *__restrict__ dsum, 
 }  // namespace i8
 
 // ---- host side ----------------------------------------------------------------------------------
-static PFN_cuTensorMapEncodeTiled_v12000 i8_get_encode()
-{
-    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
-    if (!fn) {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
 static bool i8_shape_ok(const pwa_ctx *ctx)
 {
     const int D = 2 * ctx->n;
@@ -460,7 +389,7 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     const long long rows = N / G;                                // whole 128-real rows
     const int n_tail = (int)(N % G);
     if (rows < 1 || rows > 0x7fffffffLL - i8::TE) return PWA_OK;
-    PFN_cuTensorMapEncodeTiled_v12000 enc = i8_get_encode();
+    PFN_cuTensorMapEncodeTiled_v12000 enc = tc::tensor_map_encoder();
     if (!enc) return fail(ctx, PWA_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
     alignas(64) CUtensorMap tmap;
     {
@@ -491,7 +420,6 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     i8::Scales sc;
     i8::Exps ex;
     memcpy(sc.s, ctx->i8q.scale, sizeof(sc.s));
-    sc.dbg = ctx->opt_norm >= 16 ? (ctx->opt_norm >> 4) : 0;
     sc.one = 1;
     memcpy(ex.e, ctx->i8q.exp, sizeof(ex.e));
     i8::k_norm_i8<<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);

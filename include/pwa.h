@@ -223,9 +223,26 @@ pwa_status pwa_polar_to_cartesian(int32_t n_waves, const double *r_phi, double *
  * -d L_data / d theta + (N_data / Norm) d Norm / d theta, Norm evaluated by the same MC pass.                  */
 pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dnll_dmass, double *dnll_dwidth);
 
+/* One evaluation of a floating-resonance fit in TWO streaming passes (with floating masses and widths every
+ * evaluation has its own Breit-Wigner factors, so a matrix M built for it would be used exactly once; Norm, its
+ * gradient and all resonance derivatives are then cheaper as the explicit MC sum of eq. 3, O(N_acc n) instead
+ * of O(N_acc n^2)):
+ *   MC pass:   Norm = (1/N_gen) sum_j |S_j|^2,  2 (M V)_a = (2/N_gen) sum_j conj(B_ja) S_j,  d Norm / d(M_r, G_r)
+ *   data pass: L_data, T_a, d L_data / d(M_r, G_r)
+ * both with the Breit-Wigner factors recomputed in registers from (mass, ang).  Sets the resonance parameters to
+ * (mass0, width0) (HOST [n_res], as pwa_set_resonances: a previously built M becomes stale) and returns
+ * nll, grad[n][2], d nll / d M_r, d nll / d G_r (HOST [n_res] each), parts = {L_data, Norm} (may be NULL); the same
+ * numbers as pwa_build_norm + pwa_nll_grad + pwa_res_grad to rounding.  Honours "likelihood".  Needs factored DATA and
+ * MC uploads with the same n_ang, a wave map, and n + n_res * n_ang <= 64 (PWA_ERR_UNSUPPORTED otherwise: use the three
+ * calls).  Synchronous.                                                                                          */
+pwa_status pwa_nll_grad_floating(pwa_ctx *ctx, const double *V, const double *mass0, const double *width0,
+                                 double *nll, double *grad, double *dnll_dmass, double *dnll_dwidth, double *parts);
+
 /* ---- host minimiser (a quasi-Newton in real parameters stays on the host) --- */
 
-/* Plain BFGS with backtracking line search on the 2n reals of V (constant-resonance mode).
+/* All three minimisers first rescale the starting V by s = sqrt(N_data / Norm(V)) in the eq. 3 form: along V -> s V the
+ * extended likelihood is L_data + N ln s^2 - s^2 Norm, so the optimal scale is known in closed form.
+ * Plain BFGS with backtracking line search on the 2n reals of V (constant-resonance mode).
  * V_inout: HOST [n][2], start in / result out.  Stops after max_iter iterations, when
  * max|grad| < gtol, or when the line search is exhausted.  nll_out, n_iter_out, n_evals_out may be NULL. */
 pwa_status pwa_minimize_bfgs(pwa_ctx *ctx, double *V_inout, int32_t max_iter, double gtol,
@@ -252,8 +269,8 @@ pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V_inout, 
 /* Floating-resonance fit (configs[3]; with floating masses and widths nothing can be pre-calculated, so
  * EVERY evaluation re-evaluates the Breit-Wigner factors and rebuilds M): BFGS over the 2 n_waves Cartesian reals
  * of V and the masses and widths of the n_free resonances listed in free_res (HOST int32 [n_free], distinct
- * indices in [0, n_res)).  One evaluation = pwa_set_resonances + pwa_build_norm + pwa_nll_grad + pwa_res_grad
- * (four passes: MC Gram, data term, and the two resonance-gradient passes).  V_inout: HOST [n][2]; mass_inout,
+ * indices in [0, n_res)).  One evaluation = pwa_nll_grad_floating (two passes), or, where that is not supported,
+ * pwa_set_resonances + pwa_build_norm + pwa_nll_grad + pwa_res_grad (four passes).  V_inout: HOST [n][2]; mass_inout,
  * width_inout: HOST [n_res], all resonances (the fixed ones are read, the free ones updated).  A trial point with a
  * non-positive mass or width is rejected by the line search.  Needs factored DATA and MC uploads and a wave map.
  * n_res must equal pwa_n_res(ctx) (PWA_ERR_INVALID_ARG otherwise).  nll_out, n_iter_out, n_evals_out, why_out

@@ -31,7 +31,7 @@ SYMBOLS = [
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
     "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
     "pwa_batch_path", "pwa_minimize_bfgs_floating", "pwa_minimize_bfgs_batch_ex", "pwa_minimize_bfgs_floating_ex",
-    "pwa_n_res", "pwa_get_option", "pwa_storage", "pwa_n_events", "pwa_norm_sums", "pwa_combine_norm_host", "pwa_assemble_host_shards",
+    "pwa_n_res", "pwa_nll_grad_floating", "pwa_get_option", "pwa_storage", "pwa_n_events", "pwa_norm_sums", "pwa_combine_norm_host", "pwa_assemble_host_shards",
 ]
 PWA_FIT_CONVERGED, PWA_FIT_MAX_ITER, PWA_FIT_LINE_SEARCH = 0, 1, 2
 
@@ -88,6 +88,7 @@ def _load():
                                                     C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]),
         "pwa_minimize_bfgs_batch_ex": (C.c_int, [vp, i32, vp, i32, C.c_double, vp, vp, vp, C.POINTER(i32)]),
         "pwa_n_res": (i32, [vp]),
+        "pwa_nll_grad_floating": (C.c_int, [vp, vp, vp, vp, dp, vp, vp, vp, vp]),
         "pwa_get_option": (C.c_int, [vp, C.c_char_p, C.POINTER(i32)]),
         "pwa_storage": (C.c_int, [vp]),
         "pwa_n_events": (i64, [vp, C.c_int]),
@@ -371,6 +372,17 @@ def pwa_res_grad(ctx, V, n_res=None):
     dM, dG = np.empty(n_res), np.empty(n_res)
     _check(ctx, _lib.pwa_res_grad(ctx, V.ctypes.data, dM.ctypes.data, dG.ctypes.data))
     return dM, dG
+
+
+def pwa_nll_grad_floating(ctx, V, mass0, width0, want_status=False):
+    """Two-pass floating evaluation -> (nll, grad[n, 2], d nll / d M_r [n_res], d nll / d G_r [n_res], parts[2])."""
+    n, nr = _lib.pwa_n_waves(ctx), (_lib.pwa_n_res(ctx),)
+    V, m, w = _f64(V, (n, 2)), _f64(mass0, nr), _f64(width0, nr)
+    nll = C.c_double(0.0)
+    grad, dM, dG, parts = np.empty((n, 2)), np.empty(nr), np.empty(nr), np.empty(2)
+    st = _check(ctx, _lib.pwa_nll_grad_floating(ctx, V.ctypes.data, m.ctypes.data, w.ctypes.data, C.byref(nll),
+                                                grad.ctypes.data, dM.ctypes.data, dG.ctypes.data, parts.ctypes.data))
+    return (nll.value, grad, dM, dG, parts, st) if want_status else (nll.value, grad, dM, dG, parts)
 
 
 def pwa_minimize_bfgs(ctx, V0, max_iter=200, gtol=1e-6, want_iters=False):

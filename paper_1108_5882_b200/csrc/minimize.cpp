@@ -13,10 +13,12 @@ namespace {
 struct Bfgs {
     int d = 0;
     std::vector<double> x, g, H, p, xt, gt;
+    std::vector<double> cap;  // optional: largest |step| per variable and iteration (0 = unlimited); keeps a resonance in its basin
     double f = 0.0, t = 1.0, slope = 0.0;
     int iter = 0;
     int small_steps = 0;      // consecutive accepted steps shorter than 2^-10 of the quasi-Newton step
     int stall_limit = 0;      // > 0: that many of them in a row end the fit with PWA_FIT_LINE_SEARCH (noisy evaluations, see batch_ex)
+    bool fresh = true;        // the current direction is steepest descent (H = identity): a failed search along it is final
     int why = 0;              // why the fit stopped: PWA_FIT_CONVERGED / PWA_FIT_MAX_ITER / PWA_FIT_LINE_SEARCH
     bool done = false, have = false;
 
@@ -37,8 +39,11 @@ struct Bfgs {
             slope = 0.0; for (int i = 0; i < d; ++i) slope -= g[i] * g[i];
             first = true;
         }
+        fresh = first;
         t = 1.0;
         if (first) { double nrm = 0.0; for (int i = 0; i < d; ++i) nrm += p[i] * p[i]; nrm = sqrt(nrm); if (nrm > 1.0) t = 1.0 / nrm; }
+        if (!cap.empty())
+            for (int i = 0; i < d; ++i) if (cap[i] > 0.0 && fabs(p[i]) * t > cap[i]) t = cap[i] / fabs(p[i]);
     }
     void trial() { for (int i = 0; i < d; ++i) xt[i] = x[i] + t * p[i]; }
     // returns true when the trial point was accepted
@@ -47,7 +52,15 @@ struct Bfgs {
         const double c1 = 1e-4;
         if (!(isfinite(ft)) || ft > f + c1 * t * slope) {
             t *= 0.5;
-            if (t < 1e-20) { done = true; why = PWA_FIT_LINE_SEARCH; }
+            if (t < 1e-20) {
+                // the search along the quasi-Newton direction is exhausted: an inverse Hessian that has gone bad looks the
+                // same as the resolution of nll, so restart once from steepest descent before giving up
+                if (!fresh) {
+                    for (size_t k = 0; k < H.size(); ++k) H[k] = 0.0;
+                    for (int i = 0; i < d; ++i) H[(size_t)i * d + i] = 1.0;
+                    direction(true);
+                } else { done = true; why = PWA_FIT_LINE_SEARCH; }
+            }
             return false;
         }
         std::vector<double> s(d), y(d), Hy(d);
@@ -97,7 +110,7 @@ pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V, int32_
     if (!ctx || !V || K < 1 || K > 1024 || max_iter < 0) return PWA_ERR_INVALID_ARG;
     const int n = pwa_n_waves(ctx), d = 2 * n;
     std::vector<Bfgs> fit(K);
-    std::vector<double> X((size_t)K * d), F(K), Gr((size_t)K * d);
+    std::vector<double> X((size_t)K * d), F(K), Gr((size_t)K * d), Pt((size_t)K * 2);
     std::vector<int> act(K);                    // the fits evaluated by the current batched calls (all K in the first stage)
     for (int k = 0; k < K; ++k) act[k] = k;
     memcpy(X.data(), V, sizeof(double) * (size_t)K * d);
@@ -105,14 +118,29 @@ pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V, int32_
     pwa_status worst = PWA_OK;
     auto eval = [&]() -> pwa_status {            // evaluates rows 0 .. act.size()-1 of X
         const int Ka = (int)act.size();
-        pwa_status s = (Ka == 1) ? pwa_nll_grad(ctx, X.data(), F.data(), Gr.data(), nullptr)
-                                 : pwa_nll_grad_batch(ctx, Ka, X.data(), F.data(), Gr.data(), nullptr);
+        pwa_status s = (Ka == 1) ? pwa_nll_grad(ctx, X.data(), F.data(), Gr.data(), Pt.data())
+                                 : pwa_nll_grad_batch(ctx, Ka, X.data(), F.data(), Gr.data(), Pt.data());
         evals += 1;
         if (s == PWA_WARN_NONFINITE) { worst = s; return PWA_OK; }
         return s;
     };
     pwa_status s = eval();
     if (s != PWA_OK) return s;
+    // Euler prescale (pin P7): along V -> s V the extended likelihood of eq. 3 is L_data + N ln s^2 - s^2 Norm, whose
+    // optimum s^2 = N_data / Norm is known in closed form (at any stationary point Norm = N_data).  Starting there
+    // removes the one direction in which a random start is wrong by orders of magnitude.  (eq. 2 is scale-invariant.)
+    {
+        int32_t lik = 0;
+        const double n_data = (double)pwa_n_events(ctx, PWA_DATA);
+        if (pwa_get_option(ctx, "likelihood", &lik) == PWA_OK && lik == 0 && n_data > 0.0 && max_iter > 0) {
+            bool any = false;
+            for (int k = 0; k < K; ++k) {
+                const double norm = Pt[2 * k + 1];
+                if (norm > 0.0 && isfinite(norm)) { const double sc = sqrt(n_data / norm); for (int i = 0; i < d; ++i) X[(size_t)k * d + i] *= sc; any = true; }
+            }
+            if (any) { s = eval(); if (s != PWA_OK) return s; }
+        }
+    }
     // the K fits are independent: their O(d^2) updates run on the host cores in parallel (the results do not
     // depend on the thread count: every fit is handled by exactly one thread)
 #pragma omp parallel for schedule(static) if (K >= 4)
@@ -224,8 +252,11 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
     for (int i = 0; i < d; ++i) u[i] = x[i] / sc[i];
     int32_t evals = 0;
     pwa_status worst = PWA_OK;
+    bool two_pass = true;
     // f(x), grad f(x); returns +inf for a non-physical trial point (the line search backs off)
+    double norm_last = 0.0;                          // Norm of the most recent evaluation
     auto eval = [&](const double *uu, double *f, double *gg) -> pwa_status {
+        double parts[2] = {0.0, 0.0};
         std::vector<double> xv(d);
         for (int i = 0; i < d; ++i) xv[i] = uu[i] * sc[i];
         const double *xx = xv.data();
@@ -233,12 +264,27 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
             Mr[free_res[i]] = xx[2 * n + i]; Gr[free_res[i]] = xx[2 * n + n_free + i];
             if (!(Mr[free_res[i]] > 0.0) || !(Gr[free_res[i]] > 0.0)) { *f = INFINITY; return PWA_OK; }
         }
-        pwa_status s = pwa_set_resonances(ctx, Mr.data(), Gr.data());
+        pwa_status s = PWA_OK;
+        if (two_pass) {                                   // one evaluation = two streaming passes (pwa.h)
+            s = pwa_nll_grad_floating(ctx, xx, Mr.data(), Gr.data(), f, gg, dM.data(), dG.data(), parts);
+            if (s == PWA_ERR_UNSUPPORTED) two_pass = false;
+            else {
+                evals += 1;
+                norm_last = parts[1];
+                if (s == PWA_WARN_NONFINITE) { worst = s; s = PWA_OK; }
+                if (s != PWA_OK) return s;
+                for (int i = 0; i < n_free; ++i) { gg[2 * n + i] = dM[free_res[i]]; gg[2 * n + n_free + i] = dG[free_res[i]]; }
+                for (int i = 0; i < d; ++i) gg[i] *= sc[i];
+                return PWA_OK;
+            }
+        }
+        s = pwa_set_resonances(ctx, Mr.data(), Gr.data());
         if (s != PWA_OK) return s;
         s = pwa_build_norm(ctx, nullptr);
         if (s != PWA_OK) return s;
-        s = pwa_nll_grad(ctx, xx, f, gg, nullptr);
+        s = pwa_nll_grad(ctx, xx, f, gg, parts);
         evals += 1;
+        norm_last = parts[1];
         if (s == PWA_WARN_NONFINITE) { worst = s; s = PWA_OK; }
         if (s != PWA_OK) return s;
         if (n_free > 0) {
@@ -254,7 +300,22 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
     pwa_status s = eval(u.data(), &f0, g.data());
     if (s != PWA_OK) return s;
     if (!isfinite(f0)) return PWA_ERR_INVALID_ARG;      // the starting point itself must be physical
+    {   // Euler prescale of V (see pwa_minimize_bfgs_batch_ex): s^2 = N_data / Norm at the starting resonance parameters
+        int32_t lik = 0;
+        const double n_data = (double)pwa_n_events(ctx, PWA_DATA);
+        if (pwa_get_option(ctx, "likelihood", &lik) == PWA_OK && lik == 0 && n_data > 0.0 && norm_last > 0.0 && isfinite(norm_last) && max_iter > 0) {
+            const double scv = sqrt(n_data / norm_last);
+            for (int i = 0; i < 2 * n; ++i) u[i] *= scv;           // sc = 1 for the V components
+            s = eval(u.data(), &f0, g.data());
+            if (s != PWA_OK) return s;
+            if (!isfinite(f0)) return PWA_ERR_INVALID_ARG;
+        }
+    }
     fit.init(d, u.data());
+    // the likelihood has one local minimum per assignment of resonances to peaks: an iteration may move a mass by at most
+    // 3 % and a width by at most 6 % of its starting value (3 scaled units), so that the fit stays in the basin it started in
+    fit.cap.assign(d, 0.0);
+    for (int i = 2 * n; i < d; ++i) fit.cap[i] = 3.0;
     fit.f = f0; fit.g = g;
     if (fit.gmax() < gtol) { fit.done = true; fit.why = PWA_FIT_CONVERGED; }
     else if (max_iter == 0) { fit.done = true; fit.why = PWA_FIT_MAX_ITER; }

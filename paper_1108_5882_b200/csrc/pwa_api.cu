@@ -660,6 +660,58 @@ pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG)
     return launch_res_grad(ctx, V, dM, dG);
 }
 
+pwa_status pwa_nll_grad_floating(pwa_ctx *ctx, const double *V, const double *mass0, const double *width0, double *nll,
+                                 double *grad, double *dnll_dmass, double *dnll_dwidth, double *parts)
+{
+    if (!ctx || !V || !mass0 || !width0 || !nll || !grad || !dnll_dmass || !dnll_dwidth)
+        return ctx ? fail(ctx, PWA_ERR_INVALID_ARG, "null argument") : PWA_ERR_INVALID_ARG;
+    if (ctx->data.n_events < 0 || ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "DATA and MC must be uploaded");
+    if (!ctx->data.factored || !ctx->mc.factored) return fail(ctx, PWA_ERR_STATE, "pwa_nll_grad_floating needs factored uploads");
+    if (ctx->data.weights || ctx->mc.weights) return fail(ctx, PWA_ERR_UNSUPPORTED, "event weights are not supported with factored uploads");
+    const int n = ctx->n;
+    if (!finite_all(V, 2 * (size_t)n)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
+    pwa_status s = pwa_set_resonances(ctx, mass0, width0);      // M (if any) no longer belongs to these parameters: marked stale
+    if (s != PWA_OK) return s;
+    PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+    int NC = 0;
+    s = launch_floating_passes(ctx, V, &NC);
+    if (s != PWA_OK) return s;
+    s = wait_results(ctx, 2);
+    if (s != PWA_OK) return s;
+    // synthesis on the host (a few hundred flops): record 0 = MC pass, record 1 = data pass
+    const double *mc = ctx->h_result, *dt = ctx->h_result + NC;
+    const int n_res = ctx->n_res, n_ang = ctx->data.n_ang;
+    const double inv_ngen = 1.0 / (double)ctx->mc.n_gen;
+    const double norm = mc[0] * inv_ngen, L = dt[0];
+    const double wN = ctx->opt_likelihood == 1 ? eq2_n_data(ctx) / norm : 1.0;      // eq. 2: the Norm part carries N_data / Norm
+    *nll = ctx->opt_likelihood == 1 ? (-L + eq2_n_data(ctx) * log(norm)) : -(L - norm);
+    if (parts) { parts[0] = L; parts[1] = norm; }
+    for (int a = 0; a < n; ++a) {
+        // grad(L_data) = 2 conj(T);  grad(Norm) = 2 M V = (2 / N_gen) conj(T'),  T' = sum_j A_ja conj(S_j)
+        grad[2 * a]     = -2.0 * dt[2 + 2 * a] + wN * 2.0 * inv_ngen * mc[2 + 2 * a];
+        grad[2 * a + 1] =  2.0 * dt[3 + 2 * a] - wN * 2.0 * inv_ngen * mc[3 + 2 * a];
+    }
+    for (int r = 0; r < n_res; ++r) {
+        double ud[2] = {0.0, 0.0}, um[2] = {0.0, 0.0};              // U_r = sum_s C[r][s] Q2[r][s], C[r][s] = V of wave (r, s)
+        for (int sg = 0; sg < n_ang; ++sg) {
+            const int w = ctx->wave_of_pair[r * kMaxAng + sg];
+            if (w < 0) continue;
+            const double cr = V[2 * w], ci = V[2 * w + 1];
+            const double *qd = dt + 2 + 2 * (n + r * n_ang + sg), *qm = mc + 2 + 2 * (n + r * n_ang + sg);
+            ud[0] += cr * qd[0] - ci * qd[1]; ud[1] += cr * qd[1] + ci * qd[0];
+            um[0] += cr * qm[0] - ci * qm[1]; um[1] += cr * qm[1] + ci * qm[0];
+        }
+        const double Mr = mass0[r], Gr = width0[r];
+        // Re( -(2M - iG) U ) = -(2M Ur + G Ui);  Re( iM U ) = -M Ui                      (reading A9, C3)
+        const double dL_dM = 2.0 * (-(2.0 * Mr * ud[0] + Gr * ud[1])), dL_dG = 2.0 * (-Mr * ud[1]);
+        const double dN_dM = 2.0 * inv_ngen * (-(2.0 * Mr * um[0] + Gr * um[1])), dN_dG = 2.0 * inv_ngen * (-Mr * um[1]);
+        dnll_dmass[r] = -dL_dM + wN * dN_dM;
+        dnll_dwidth[r] = -dL_dG + wN * dN_dG;
+    }
+    const bool nonfinite = mc[1] != 0.0 || dt[1] != 0.0 || !isfinite(*nll) || !finite_all(grad, 2 * (size_t)n);
+    return nonfinite ? PWA_WARN_NONFINITE : PWA_OK;
+}
+
 uint64_t pwa_launch_count(const pwa_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 int32_t pwa_n_waves(const pwa_ctx *ctx) { return ctx ? ctx->n : 0; }

@@ -117,6 +117,7 @@ pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, 
 pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled);   // batch_i8.cu
 double batch_i8_error_estimate(const pwa_ctx *ctx);               // batch_i8.cu
 pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
+pwa_status launch_floating_passes(pwa_ctx *ctx, const double *V, int *ncomp_out);   // factored.cu
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
 
 }  // namespace pwa

@@ -54,6 +54,11 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
     __shared__ double s_mv[2 * kMaxWaves];
     if (M == nullptr) {
         for (int c = tid; c < NC; c += nthreads) out[c] = s_tot[c];
+        if (done_flag != nullptr) {                 // record in mapped host memory: visible to the host before the flag
+            __threadfence_system();
+            __syncthreads();
+            if (tid == 0) *reinterpret_cast<volatile unsigned long long *>(done_flag) = seq;
+        }
         return;
     }
     // (M V)_a: `slices` adjacent lanes share a row (coalesced reads of M, all loads independent),

@@ -118,6 +118,11 @@ def test_cfg3_full(pwa, oracle, synth):
             ref = np.concatenate([-dLM + dNM, -dLG + dNG])
             got = np.concatenate([dM, dG])
             assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+            # the two-pass evaluation (explicit MC sum, no M: what the floating-resonance minimiser and bench.py's cfg3
+            # step use) at full size against the same oracle quantities
+            nll2, g2, dM2, dG2, parts2 = pwa.pwa_nll_grad_floating(c.ctx, V, Mr, Gr)
+            check_eval((nll2, g2, parts2), oracle_eval_explicit(oracle, A, B, w.n_gen, V), 1e-12, w.n_data)
+            assert np.abs(np.concatenate([dM2, dG2]) - ref).max() <= 1e-12 * np.abs(ref).max()
             del A, B
 
 

@@ -274,8 +274,8 @@ def test_bfgs_floating_resonances(pwa, oracle, synth):
         # the context is left at the fitted point: value, V-gradient and resonance gradient there
         nll_fit, g_fit, parts = pwa.pwa_nll_grad(c.ctx, V)
         dM, dG = pwa.pwa_res_grad(c.ctx, V, w.n_res)
-        assert nll_fit == nll
-        assert parts[1] == pytest.approx(w.n_data, rel=1e-5)          # P7: Norm = N_data at a stationary point of eq. 3
+        assert nll_fit == pytest.approx(nll, rel=1e-13)      # fit: two-pass evaluations (explicit MC sum); here: M-based
+        assert parts[1] == pytest.approx(w.n_data, rel=1e-4)          # P7: Norm = N_data at a stationary point of eq. 3
     A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr)
     B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
     M_o = oracle.norm_matrix(B, w.n_gen)
@@ -751,7 +751,7 @@ def test_bfgs_floating_eq2_form(pwa, synth):
         assert nll < nll_start and iters >= 5 and why in (pwa.PWA_FIT_CONVERGED, pwa.PWA_FIT_MAX_ITER, pwa.PWA_FIT_LINE_SEARCH)
         nll_fit, g_fit, _ = pwa.pwa_nll_grad(c.ctx, V)
         dM, dG = pwa.pwa_res_grad(c.ctx, V)
-        assert nll_fit == nll
+        assert nll_fit == pytest.approx(nll, rel=1e-13)      # fit: two-pass evaluations (explicit MC sum); here: M-based
         assert np.abs(g_fit).max() <= 1e-2 * np.abs(g_start).max()
         with pytest.raises(pwa.PwaError) as e:                            # mass / width arrays sized by another n_res
             pwa._check(c.ctx, pwa._lib.pwa_minimize_bfgs_floating(c.ctx, V.ctypes.data, Mr.ctypes.data, Gr.ctypes.data,
@@ -839,3 +839,60 @@ def test_bfgs_reports_iterations_and_two_stage_batch(pwa):
             assert one[0] == pytest.approx(nllf[k], rel=1e-12)
             assert one[2][1] == pytest.approx(N, rel=1e-7)                # P7: Norm = N_data at a stationary point of eq. 3
             assert np.abs(one[1]).max() < 1e-5
+
+
+# ------------------------------------------------------------------ floating resonances in two passes (no M)
+@pytest.mark.parametrize("n_data,n_mc", [(5003, 7001), (100_003, 200_001)])
+def test_nll_grad_floating_two_pass(pwa, oracle, synth, n_data, n_mc):
+    """pwa_nll_grad_floating: Norm as the explicit MC sum of eq. 3 with its V- and resonance-derivatives in ONE MC
+    pass, the data term with its resonance derivatives in ONE data pass.  Against the oracle (M-based evaluation and
+    res_grad) at 1e-12, against the four-pass product path, in both likelihood forms."""
+    w = synth.make_workload(3, n_data=n_data, n_mc=n_mc, full_amplitudes=False)
+    Mr, Gr = synth.floating_start(w)
+    V = synth.eval_points(w, 1)[0]
+    A = oracle.expand_factored(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    B = oracle.expand_factored(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr)
+    M_o = oracle.norm_matrix(B, w.n_gen)
+    dLM, dLG = oracle.res_grad(w.mass_data, w.Z_data, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 0)
+    dNM, dNG = oracle.res_grad(w.mass_mc, w.Z_mc, w.res_of_wave, w.ang_of_wave, Mr, Gr, V, 1, w.n_gen)
+    with _factored_ctx(pwa, w, w.Mr, w.Gr) as c:
+        nll, g, dM, dG, parts, st = pwa.pwa_nll_grad_floating(c.ctx, V, Mr, Gr, want_status=True)
+        assert st == pwa.PWA_OK
+        check_eval((nll, g, parts), oracle.nll_grad(A, M_o, V), 1e-12, n_data)
+        ref = np.concatenate([-dLM + dNM, -dLG + dNG])
+        assert np.abs(np.concatenate([dM, dG]) - ref).max() <= 1e-12 * np.abs(ref).max()
+        with pytest.raises(pwa.PwaError) as e:                     # the call moved the resonances: an old M is stale
+            pwa.pwa_nll_grad(c.ctx, V)
+        assert e.value.status == pwa.PWA_ERR_STATE
+        # the four-pass path gives the same numbers
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        check_eval((nll, g, parts), pwa.pwa_nll_grad(c.ctx, V), 1e-12, n_data)
+        dM4, dG4 = pwa.pwa_res_grad(c.ctx, V)
+        assert np.abs(np.concatenate([dM - dM4, dG - dG4])).max() <= 1e-12 * np.abs(ref).max()
+        again = pwa.pwa_nll_grad_floating(c.ctx, V, Mr, Gr)        # reproducible bit for bit
+        assert again[0] == nll and np.array_equal(again[1], g) and np.array_equal(again[2], dM)
+        # eq. 2 form
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        nll2, g2, dM2, dG2, parts2 = pwa.pwa_nll_grad_floating(c.ctx, V, Mr, Gr)
+        check_eval((nll2, g2, parts2), oracle.nll_grad_eq2(A, M_o, V), 1e-12, n_data)
+        wN = n_data / parts_o[1] if (parts_o := oracle.nll_grad(A, M_o, V)[2]) is not None else 1.0
+        ref2 = np.concatenate([-dLM + wN * dNM, -dLG + wN * dNG])
+        assert np.abs(np.concatenate([dM2, dG2]) - ref2).max() <= 1e-12 * np.abs(ref2).max()
+
+
+def test_nll_grad_floating_three_angular_structures(pwa, oracle, synth):
+    """cfg-0 style wave map (4 resonances x 3 angular structures, 4 of the 12 pairs used) through the two-pass call."""
+    w = synth.make_workload(0, n_data=3001, n_mc=4001)
+    Zd, Zm = synth.angular(w, w.kin_data), synth.angular(w, w.kin_mc)
+    V = synth.eval_points(w, 1)[0]
+    M_o = oracle.norm_matrix(w.A_mc, w.n_gen)
+    dLM, dLG = oracle.res_grad(w.mass_data, Zd, w.res_of_wave, w.ang_of_wave, w.Mr, w.Gr, V, 0)
+    dNM, dNG = oracle.res_grad(w.mass_mc, Zm, w.res_of_wave, w.ang_of_wave, w.Mr, w.Gr, V, 1, w.n_gen)
+    with Ctx(pwa, w.n, "f64") as c:
+        pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_DATA, w.mass_data, Zd)
+        pwa.pwa_upload_events_factored(c.ctx, pwa.PWA_MC, w.mass_mc, Zm, n_generated=w.n_gen)
+        pwa.pwa_set_wave_map(c.ctx, w.n_res, w.res_of_wave, w.ang_of_wave)
+        nll, g, dM, dG, parts = pwa.pwa_nll_grad_floating(c.ctx, V, w.Mr, w.Gr)
+    check_eval((nll, g, parts), oracle.nll_grad(w.A_data, M_o, V), 1e-12, w.n_data)
+    ref = np.concatenate([-dLM + dNM, -dLG + dNG])
+    assert np.abs(np.concatenate([dM, dG]) - ref).max() <= 1e-12 * np.abs(ref).max()

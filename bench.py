@@ -246,13 +246,16 @@ SIDE_STEPS, SIDE_WARMUP = 10, 3      # every side measurement: >= 10 timed steps
 def measure_peaks(pwa, ctx, mp_hbm, mp_src):
     """Roofline denominators.  HBM: MEASURED_PEAKS.json (driver-written copy bandwidth).  FP64: MEASURED_PEAKS has
     no fp64 figure, so the register-resident DFMA and mma.sync.m8n8k4.f64 loops of pwa_microbench are run here
-    (SURVEY 8(d) "Denominators").  int8 tensor: the guide's nominal dense figure (2 x the nominal fp8 4.5 PFLOP/s
-    is sparse; dense int8 = 4.5 Pop/s)."""
+    (SURVEY 8(d) "Denominators").  int8 tensor: pwa_microbench(3), a loop of tcgen05.mma.kind::i8 M = 128, N = 256, K = 32
+    with both operands in shared memory on every SM (nominal dense int8: 4.5 Pop/s)."""
     return {"hbm_gbs": mp_hbm, "hbm_source": mp_src,
             "dfma_tflops": pwa.pwa_microbench(ctx, 0), "dmma_tflops": pwa.pwa_microbench(ctx, 1),
             "hbm_read_gbs": pwa.pwa_microbench(ctx, 2, 4 << 30),
             "fp64_source": "measured here: pwa_microbench(0 | 1), register-resident loops, best of 5",
             "hbm_read_source": "measured here: pwa_microbench(2), read-only stream over 4 GiB",
+            "int8_tops": pwa.pwa_microbench(ctx, 3), "int8_tops_n128": pwa.pwa_microbench(ctx, 4),
+            "int8_tops_n64": pwa.pwa_microbench(ctx, 5), "tmem_read_gbs": pwa.pwa_microbench(ctx, 7),
+            "int8_source": "measured here: pwa_microbench(3 | 4 | 5), tcgen05.mma.kind::i8 from shared memory, all SMs",
             "int8_tops_nominal": 4500.0}
 
 
@@ -272,7 +275,7 @@ def rl_flops(peaks, bound, flops, ms, **kw):
     elif bound == "alu":
         peak, src, unit = peaks["dfma_tflops"], peaks["fp64_source"], "TFLOP/s"
     else:
-        peak, src, unit = peaks["int8_tops_nominal"], "nominal dense int8 (B200 guide)", "Top/s"
+        peak, src, unit = peaks["int8_tops"], peaks["int8_source"], "Top/s"
     r = {"bound": bound.split("_")[0], "achieved": a, "peak": peak, "unit": unit, "frac": a / peak, "peak_source": src,
          "algorithmic_flops_per_launch": flops}
     r.update(kw)

@@ -385,7 +385,7 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem, peaks):
             pwa.pwa_set_weights(ctx, pwa.PWA_DATA, wts)
             ms_w, _ = tm.run(lambda i: pwa.pwa_nll_grad_enqueue(ctx, Vs[i % len(Vs)]), SIDE_STEPS, SIDE_WARMUP)
             pwa.pwa_set_weights(ctx, pwa.PWA_DATA, None)
-            out["weighted"] = {"ms_per_eval": ms_w, "roofline": rl_hbm(peaks, nbytes + 8 * w.n_data, ms_w, kernel="k_data_term (weighted)")}
+            out["weighted"] = {"ms_per_eval": ms_w, "roofline": rl_hbm(peaks, nbytes + 8 * w.n_data, ms_w, kernel="k_data_term_tma<.., WT> (weighted)")}
     finally:
         pwa.pwa_destroy(ctx)
     return out

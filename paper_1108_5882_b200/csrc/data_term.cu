@@ -268,10 +268,10 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     }
     VArg varg;
     for (int t = 0; t < 2 * n; ++t) varg.v[t] = V_host_k[t];
-    // "data_term": 0 = default: TMA-tiled two-phase kernel (data_term_tma.cu) where it applies (row of 128 .. 1024 bytes,
-    // no event weights), else the per-lane streaming kernel below; 20 = per-lane kernel always; 98 = default kernel
+    // "data_term": 0 = default: TMA-tiled two-phase kernel (data_term_tma.cu) where it applies (row of 128 .. 1024 bytes),
+    // else the per-lane streaming kernel below; 20 = per-lane kernel always; 98 = default kernel
     // without programmatic dependent launch; 99 = generic kernel
-    const bool per_lane = ctx->opt_data_term == 20 || ctx->data.weights != nullptr;   // the per-lane kernel carries the weight stream
+    const bool per_lane = ctx->opt_data_term == 20;
     if (!per_lane) {
         bool handled = false;
         pwa_status s = launch_data_term_tma(ctx, varg, fa, &handled);

@@ -110,10 +110,12 @@ __device__ __forceinline__ double fast_rcp(double x)
     return fma(y, e, y);
 }
 
-template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS>
+// WT: per-event weights (NEXT-3): L = sum_i w_i ln I_i, T_a = sum_i w_i A_ia / S_i.  The mantissa-product logarithm does
+// not commute with weights, so a weighted event takes its own IEEE log (one per lane and tile: ~10 % more instructions).
+template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS, bool WT>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long resident_rows,
-                const __grid_constant__ VArg varg, FinishArgs fa)
+                const __grid_constant__ VArg varg, FinishArgs fa, const double *__restrict__ wt)
 {
     using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
     constexpr int WPC = C::WPC, NW = C::NW, TR = C::TR, BOXB = C::BOXB, STAGE = C::STAGE;
@@ -203,6 +205,8 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
         const uint32_t parity = (uint32_t)((t / NS) & 1);
         const uint32_t tile = ring0 + (uint32_t)slot * STAGE;
         const long long row0 = (g0 + t * gstride) * TR;
+        double wv = 1.0;                                          // requested before the wait on the tile: its latency hides there
+        if (WT) wv = (row0 + row1) < N ? __ldg(wt + row0 + row1) : 0.0;
         // A stage is re-armed by the warp that consumed its previous tile, which may be another warp
         // of the group: a parity wait is only unambiguous once that re-arm has happened (before it the
         // barrier can still be one phase behind, and the flipped parity would read as "complete").
@@ -237,7 +241,12 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
             const unsigned ex = ((unsigned)hi >> 20) & 0x7ffu;   // I >= 0 or nan: biased exponent (sign ignored)
             const bool normal = (ex - 1u) < 0x7feu && hi > 0;    // not 0 / denormal / inf / nan / negative
             double rr, rim;
-            if (__all_sync(0xffffffffu, normal || !valid)) {
+            if (WT) {                                             // weighted: plain IEEE log per event (reading C14 included)
+                const double l = log(I);
+                const double inv = 1.0 / I;
+                rr = sr * inv * wv; rim = -si * inv * wv;
+                if (counted) { L += wv * l; if (!(I > 0.0) || !isfinite(l)) bad += 1.0; }
+            } else if (__all_sync(0xffffffffu, normal || !valid)) {
                 const double inv = fast_rcp(valid ? I : 1.0);
                 rr = sr * inv; rim = -si * inv;                   // r = conj(S) / I
                 if (counted) {
@@ -309,11 +318,13 @@ template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS>
 static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa_in)
 {
     using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
-    auto kern = k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS>;
+    const bool weighted = ctx->data.weights != nullptr;
+    auto kern = weighted ? k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, true>
+                         : k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, false>;
     const long long N = ctx->data.n_events;
     // per-instantiation, per-device launch plan: attribute + occupancy are queried once
-    static int s_occ[64] = {0};
-    int &occ = s_occ[ctx->device & 63];
+    static int s_occ2[2][64] = {{0}};
+    int &occ = s_occ2[weighted ? 1 : 0][ctx->device & 63];
     if (occ == 0) {
         PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
         int o = 0;
@@ -354,7 +365,8 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     long long resident_rows = -1;
     if (ctx->opt_l2_resident_mb > 0) resident_rows = ((long long)ctx->opt_l2_resident_mb << 20) / row_bytes;
     else if (ctx->opt_l2_resident_mb < 0 && sample_bytes <= ((size_t)1 << 30) && sample_bytes > ((size_t)64 << 20)) resident_rows = ((long long)48 << 20) / row_bytes;
-    PWA_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *reinterpret_cast<const CUtensorMap *>(tc.map), N, resident_rows, varg, fa));
+    PWA_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *reinterpret_cast<const CUtensorMap *>(tc.map), N, resident_rows, varg, fa,
+                                     (const double *)ctx->data.weights));
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;

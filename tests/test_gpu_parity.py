@@ -612,7 +612,7 @@ def test_fumili_factored(pwa, oracle, synth):
 # ------------------------------------------------------------------ NEXT-3: per-event weights
 @pytest.mark.parametrize("storage,n", [("f64", 4), ("f64", 16), ("f32", 32), ("f32", 64), ("f64", 64), ("f64", 5), ("f32", 3)])
 def test_event_weights_parity(pwa, oracle, storage, n):
-    """Weighted data term (per-lane streaming kernel / generic kernel) and weighted M (DMMA Gram kernel,
+    """Weighted data term (TMA-tiled, per-lane and generic kernels) and weighted M (DMMA Gram kernel,
     weight in the tile's padding column) against the weighted oracle, incl. negative weights; batched
     call; removing the weights restores the unweighted result bit for bit."""
     N, Nacc, K = 6007, 4099, 3
@@ -639,8 +639,11 @@ def test_event_weights_parity(pwa, oracle, storage, n):
         for k in range(K):
             L, T, _ = oracle.data_term_w(A, Vk[k], wd)
             ref = oracle.assemble(L, T, M_o, Vk[k])
-            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol, N)
+            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol, N)      # default: weighted TMA kernel where the row allows it
             check_eval((nllk[k], gk[k], partsk[k]), ref, tol, N)
+            pwa.pwa_set_option(c.ctx, "data_term", 20)                   # weighted per-lane kernel
+            check_eval(pwa.pwa_nll_grad(c.ctx, Vk[k]), ref, tol, N)
+            pwa.pwa_set_option(c.ctx, "data_term", 0)
         pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, None)
         pwa.pwa_set_weights(c.ctx, pwa.PWA_MC, None)
         assert np.array_equal(pwa.pwa_build_norm(c.ctx), M_plain)

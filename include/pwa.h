@@ -299,7 +299,7 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx);
 pwa_status pwa_sync(pwa_ctx *ctx);
 
 /* Selects a kernel family (0 = default).  Returns PWA_ERR_INVALID_ARG for unknown keys.
- * Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood".
+ * Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood", "resident".
  * "data_term": 0 = default (TMA-tiled streaming kernel where the row is 128 .. 1024 bytes and the sample carries no
  * event weights, else the per-lane streaming kernel), 20 = per-lane kernel, 98 = default without programmatic
  * dependent launch, 99 = generic kernel (any n).
@@ -311,7 +311,18 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * policy (the rest: evict_first), so that it stays in L2 from one evaluation to the next; -1 = automatic (48 MB for
  * samples between 64 MB and 1 GiB, else plain loads), 0 = plain loads, up to 120.
  * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
- * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch, pwa_res_grad and the minimisers.    */
+ * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch, pwa_res_grad and the minimisers.
+ * "resident": 0 = every evaluation is a kernel launch (default); 1 = pwa_nll_grad evaluates through a RESIDENT grid
+ * (below ~1e5 events an iteration costs latency, not bandwidth): the default data-term kernel is
+ * launched once, stays on the GPU and takes V / returns the record through tagged 8-byte words in pinned host memory,
+ * so that an evaluation costs two PCIe round trips and no launch.  Results are bitwise those of the launched
+ * evaluation (same grid, same tiles per block, same reduction order).  Served: n in {4, 8, 16, 32, 64},
+ * unweighted, constant resonances, "data_term" 0; anything else evaluates by launches under the option.  While
+ * the grid is resident it occupies every SM of the device (other streams of the process wait behind it) and the
+ * calling thread spins in pwa_nll_grad; every other entry point of the context that enqueues work or changes what
+ * the grid reads (uploads, weights, norm, options, batch / enqueue / minimiser calls, pwa_sync, pwa_destroy) ends
+ * the grid first, and the next pwa_nll_grad starts it again (one launch).  A grid that sees no command for ~2 s
+ * ends by itself.  Meant for a fit loop of single evaluations on a small sample; leave it off otherwise.          */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
 pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* current value of a pwa_set_option key */
 

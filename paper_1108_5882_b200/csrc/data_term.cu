@@ -239,7 +239,24 @@ static pwa_status launch_generic(pwa_ctx *ctx, const double *Vdev, const FinishA
 }
 
 pwa_status launch_factored_data_term(pwa_ctx *ctx, const double *Vk, const FinishArgs &fa);   // factored.cu
-pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled);   // data_term_tma.cu
+pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled, bool resident);   // data_term_tma.cu
+
+// Starts the resident evaluation grid (data_term_tma.cu, RES): same kernel, same grid, same finish as a launched evaluation
+// of record 0; *started stays false where the TMA kernel does not apply (the caller then evaluates by launches).
+pwa_status launch_resident(pwa_ctx *ctx, bool *started)
+{
+    *started = false;
+    const int n = ctx->n;
+    if (ctx->data.factored || ctx->data.weights || ctx->opt_data_term != 0 || !(n == 4 || n == 8 || n == 16 || n == 32 || n == 64)) return PWA_OK;
+    FinishArgs fa;
+    fa.partials = nullptr; fa.ticket = ctx->d_ticket; fa.n = n;
+    fa.M = ctx->d_M; fa.out = ctx->dev_result; fa.done_flag = ctx->dev_flags; fa.seq = ctx->seq;
+    fa.tagged = ctx->dev_rres;
+    fa.eq2 = ctx->opt_likelihood == 1; fa.n_eq2 = eq2_n_data(ctx);
+    VArg varg;
+    memset(&varg, 0, sizeof(varg));
+    return launch_data_term_tma(ctx, varg, fa, started, true);
+}
 
 // V_host_k: host pointer to V of evaluation k (already staged in ctx->h_V, mirrored in d_V).
 // out_dev_terms != nullptr selects the data-term-only output (multi-GPU path).
@@ -274,7 +291,7 @@ pwa_status launch_data_term(pwa_ctx *ctx, const double *V_host_k, int k, double 
     const bool per_lane = ctx->opt_data_term == 20;
     if (!per_lane) {
         bool handled = false;
-        pwa_status s = launch_data_term_tma(ctx, varg, fa, &handled);
+        pwa_status s = launch_data_term_tma(ctx, varg, fa, &handled, false);
         if (s != PWA_OK || handled) return s;
     }
     //                           ST      G  CK  E  THREADS MINB

@@ -110,12 +110,36 @@ __device__ __forceinline__ double fast_rcp(double x)
     return fma(y, e, y);
 }
 
+// Resident mode (RES; for small samples the per-iteration cost is latency, not bandwidth): the grid stays on the GPU
+// between evaluations and is driven through a mailbox instead of launches.  cmd_host: device-mapped pinned HOST memory,
+// 4n words of (tag << 32 | 32 bits of V), tag = low half of the evaluation's sequence number; cmd_dev: device memory,
+// [0] = sequence number, [1 .. 2n] = V.  Warp 0 of CTA 0 polls cmd_host over PCIe (one round trip per poll: the command is
+// complete when all words carry the new tag), copies V to cmd_dev and publishes the number there; the other CTAs poll
+// cmd_dev (L2).  The record goes back the same way (FinishArgs::tagged: tag << 32 | half a double per word, no fence and
+// no flag: the host has the record when every word carries the tag).  An evaluation is then exactly the body of the launched kernel (same grid, same tiles per CTA, same
+// reduction tree: bitwise the same result), and its finishing block publishes the record with that sequence number.  The
+// host sends the next command only after it has seen the record, so the evaluations of a grid never overlap.
+// kQuit as sequence number, or ~2 s without a command, ends the grid.
+struct ResidentArgs {
+    const unsigned long long *cmd_host;      // mapped host mailbox (read with system-scope volatile loads)
+    unsigned long long *cmd_dev;             // device copy: [0] = sequence number, [1 ..] = V
+    unsigned long long start_seq;            // sequence number at launch (commands have larger numbers)
+};
+// tag 0xffffffff in the mailbox = quit (the host never uses it for a command)
+constexpr unsigned long long kQuit = ~0ull;
+__device__ __forceinline__ unsigned long long ld_sys_u64(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // WT: per-event weights (NEXT-3): L = sum_i w_i ln I_i, T_a = sum_i w_i A_ia / S_i.  The mantissa-product logarithm does
 // not commute with weights, so a weighted event takes its own IEEE log (one per lane and tile: ~10 % more instructions).
-template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS, bool WT>
+template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS, bool WT, bool RES>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long resident_rows,
-                const __grid_constant__ VArg varg, FinishArgs fa, const double *__restrict__ wt)
+                const __grid_constant__ VArg varg, FinishArgs fa_in, const double *__restrict__ wt, ResidentArgs res)
 {
     using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
     constexpr int WPC = C::WPC, NW = C::NW, TR = C::TR, BOXB = C::BOXB, STAGE = C::STAGE;
@@ -128,10 +152,12 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
 
     extern __shared__ unsigned char tma_smem_raw[];
     __shared__ __align__(8) unsigned long long bars[NGRP][NS];
-    __shared__ volatile int issued[NGRP][NS];          // number of tiles issued into each stage so far (GW > 1)
+    __shared__ volatile unsigned issued[NGRP][NS];     // number of tiles issued into each stage so far (GW > 1)
     __shared__ __align__(16) double rbuf[NWARPS][32][2];
     __shared__ __align__(16) double sV[2 * NW];
-    for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = varg.v[t];
+    __shared__ unsigned long long s_seq;
+    FinishArgs fa = fa_in;
+    if (!RES) for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = varg.v[t];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int grp = warp / GW, wig = warp % GW;        // group in the CTA, warp in the group
@@ -142,8 +168,63 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     if (threadIdx.x == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     // Let the next kernel of the stream start as soon as SMs free up: its streaming phase only reads the (constant)
     // amplitudes and its own V; everything shared with this grid is touched after griddepcontrol.wait (block_finish).
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (wig == 0 && lane == 0) {
+    if (!RES) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    unsigned long long last_seq = res.start_seq;
+    for (int pass = 0;; ++pass) {                                 // one pass per evaluation (a single pass unless RES)
+    if (RES) {
+        if (warp == 0) {
+            unsigned long long seq = 0;
+            if (blockIdx.x == 0) {
+                // One PCIe round trip per poll: the mailbox is 4 NW words (tag << 32 | 32 bits of V); a command is complete
+                // when every word carries the same new tag (8-byte stores and loads are atomic, any arrival order is fine).
+                constexpr int WPL = (4 * NW + 31) / 32;                  // words per lane
+                unsigned long long w[WPL];
+                unsigned tag = 0;
+                for (unsigned spins = 0;; ++spins) {
+                    bool same = true;
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) {
+                        const int k = lane + 32 * j;
+                        w[j] = ld_sys_u64(res.cmd_host + (k < 4 * NW ? k : 0));
+                    }
+                    tag = __shfl_sync(0xffffffffu, (unsigned)(w[0] >> 32), 0);
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) same = same && (unsigned)(w[j] >> 32) == tag;
+                    if (__all_sync(0xffffffffu, same) && tag != (unsigned)last_seq) break;
+                    if (spins > (1u << 20)) { tag = 0xffffffffu; break; }       // ~2 s of PCIe polls without a command
+                }
+                if (tag == 0xffffffffu) seq = kQuit;
+                else {
+                    seq = last_seq + (unsigned long long)(unsigned)(tag - (unsigned)last_seq);
+                    unsigned *dst = reinterpret_cast<unsigned *>(res.cmd_dev + 1);
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) { const int k = lane + 32 * j; if (k < 4 * NW) dst[k] = (unsigned)w[j]; }
+                }
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(res.cmd_dev) = seq;
+            } else {
+                if (lane == 0) {
+                    for (unsigned spins = 0;; ++spins) {
+                        seq = ld_sys_u64(res.cmd_dev);
+                        if (seq != last_seq) break;
+                        if (spins > (1u << 26)) { seq = kQuit; break; }
+                        __nanosleep(40);
+                    }
+                }
+            }
+            if (lane == 0) s_seq = seq;
+        }
+        __syncthreads();
+        const unsigned long long seq = s_seq;
+        if (seq == kQuit) return;
+        last_seq = seq;
+        fa.seq = seq;
+        fa.tag = (unsigned)seq;
+        __threadfence();
+        for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = __longlong_as_double((long long)ld_sys_u64(res.cmd_dev + 1 + t));
+    }
+    if (pass == 0 && wig == 0 && lane == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(bar0 + 8 * s, 1); issued[grp][s] = 0; }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -155,6 +236,11 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     const long long gstride = (long long)gridDim.x * NGRP;
     const long long g0 = (long long)blockIdx.x * NGRP + grp;
     const long long nt_grp = (ntiles > g0) ? (ntiles - g0 + gstride - 1) / gstride : 0;   // tiles of this group
+    // a resident grid keeps its mbarriers and issue counters alive across evaluations: stage s has seen
+    // pass * ceil((nt_grp - s) / NS) tiles (completed barrier phases) before this pass
+    auto phase0 = [&](int slot) -> unsigned {
+        return RES ? (unsigned)pass * (unsigned)(nt_grp > slot ? (nt_grp - slot + NS - 1) / NS : 0) : 0u;
+    };
     const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
     auto issue = [&](long long t) {                              // lane 0 of the warp that owns tile t (or t - NS)
         const int slot = (int)(t % NS);
@@ -170,7 +256,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
             for (int cb = 0; cb < CB; ++cb)
                 tma_load_2d_hint(ring0 + (uint32_t)slot * STAGE + cb * BOXB, &tmap, cb * BOX_ELEMS, y, bar0 + 8 * slot, pol);
         }
-        if (GW > 1) { __threadfence_block(); issued[grp][slot] = (int)(t / NS) + 1; }
+        if (GW > 1) { __threadfence_block(); issued[grp][slot] = phase0(slot) + (unsigned)(t / NS) + 1u; }
     };
     if (lane == 0) {
         for (long long t = wig; t < NS && t < nt_grp; t += GW) issue(t);
@@ -202,7 +288,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
 
     for (long long t = wig; t < nt_grp; t += GW) {
         const int slot = (int)(t % NS);
-        const uint32_t parity = (uint32_t)((t / NS) & 1);
+        const uint32_t parity = (uint32_t)((phase0(slot) + (unsigned)(t / NS)) & 1u);
         const uint32_t tile = ring0 + (uint32_t)slot * STAGE;
         const long long row0 = (g0 + t * gstride) * TR;
         double wv = 1.0;                                          // requested before the wait on the tile: its latency hides there
@@ -210,7 +296,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
         // A stage is re-armed by the warp that consumed its previous tile, which may be another warp
         // of the group: a parity wait is only unambiguous once that re-arm has happened (before it the
         // barrier can still be one phase behind, and the flipped parity would read as "complete").
-        if (GW > 1) { const int need = (int)(t / NS) + 1; while (issued[grp][slot] < need) { } }
+        if (GW > 1) { const unsigned need = phase0(slot) + (unsigned)(t / NS) + 1u; while ((int)(issued[grp][slot] - need) < 0) { } }
         mbar_wait(bar0 + 8 * slot, parity);
 
         // ---------------- phase 1: S_i, ln I_i, r_i
@@ -223,7 +309,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
 #pragma unroll
             for (int w = 0; w < WPC; ++w) {
                 double vr, vi;
-                if (LPR == 1) { vr = varg.v[2 * (i * WPC + w)]; vi = varg.v[2 * (i * WPC + w) + 1]; }
+                if (LPR == 1 && !RES) { vr = varg.v[2 * (i * WPC + w)]; vi = varg.v[2 * (i * WPC + w) + 1]; }
                 else { const double2 v = lds_d2(sv0 + (uint32_t)((part * CPL1 + i) * WPC + w) * 16u); vr = v.x; vi = v.y; }
                 const int c = (i * WPC + w) & 1;                  // 2 x 2 independent chains per component
                 sre[c] = fma(vr, ar[w], sre[c]); sre[2 + c] = fma(-vi, ai[w], sre[2 + c]);
@@ -296,6 +382,9 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     for (int w = 0; w < W2; ++w) { trs[w] = tr[0][w]; tis[w] = ti[0][w]; if (U2 > 1) { trs[w] += tr[U2 - 1][w]; tis[w] += ti[U2 - 1][w]; } }
     auto wave_of = [&](int idx) { return (g2 + G2 * (idx / WPC)) * WPC + (idx % WPC); };
     reduce_and_finish<G2, W2, THREADS>(L, bad, trs, tis, wave_of, sV, fa);
+    if (!RES) return;
+    __syncthreads();                                              // every warp is past its last barrier wait: the ring can be re-armed
+    }
 }
 
 // ---- host side: tensor map ------------------------------------------------------------------------
@@ -315,16 +404,18 @@ static pwa_status make_tmap(pwa_ctx *ctx, CUtensorMap *out, const void *base, bo
 }
 
 template <typename ST, int CB, int LPR, int THREADS, int MINB, int GW, int NS>
-static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa_in)
+static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa_in, bool resident)
 {
     using C = TmaCfg<ST, CB, LPR, THREADS, GW, NS>;
     const bool weighted = ctx->data.weights != nullptr;
-    auto kern = weighted ? k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, true>
-                         : k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, false>;
+    if (resident && weighted) return fail(ctx, PWA_ERR_UNSUPPORTED, "resident evaluation does not take event weights");
+    auto kern = resident ? k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, false, true>
+              : weighted ? k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, true, false>
+                         : k_data_term_tma<ST, CB, LPR, THREADS, MINB, GW, NS, false, false>;
     const long long N = ctx->data.n_events;
     // per-instantiation, per-device launch plan: attribute + occupancy are queried once
-    static int s_occ2[2][64] = {{0}};
-    int &occ = s_occ2[weighted ? 1 : 0][ctx->device & 63];
+    static int s_occ2[3][64] = {{0}};
+    int &occ = s_occ2[resident ? 2 : weighted ? 1 : 0][ctx->device & 63];
     if (occ == 0) {
         PWA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
         int o = 0;
@@ -355,7 +446,7 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     // measured: up to ~1 GB per pass the overlap wins (51.4 vs 56.0 us at 256 MB, 162 vs 166 us at 1 GB); beyond, the early
     // successor CTAs disturb the tail of the running grid (0.417 vs 0.406 ms at 2.56 GB), so large samples launch plainly.
     // "data_term" = 98: experiment switch, always plain serialisation.
-    const bool pdl = ctx->opt_data_term != 98 && (size_t)N * (size_t)ctx->n * 2 * sizeof(ST) <= ((size_t)1 << 30);
+    const bool pdl = !resident && ctx->opt_data_term != 98 && (size_t)N * (size_t)ctx->n * 2 * sizeof(ST) <= ((size_t)1 << 30);
     attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
     cfg.attrs = attr; cfg.numAttrs = 1;
     // head of the sample kept in L2 between evaluations (see l2_policy_evict_last): 48 MB by default for samples that do
@@ -365,15 +456,17 @@ static pwa_status launch_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &f
     long long resident_rows = -1;
     if (ctx->opt_l2_resident_mb > 0) resident_rows = ((long long)ctx->opt_l2_resident_mb << 20) / row_bytes;
     else if (ctx->opt_l2_resident_mb < 0 && sample_bytes <= ((size_t)1 << 30) && sample_bytes > ((size_t)64 << 20)) resident_rows = ((long long)48 << 20) / row_bytes;
+    ResidentArgs res{nullptr, nullptr, 0ull};
+    if (resident) { res.cmd_host = ctx->dev_cmd_host; res.cmd_dev = ctx->d_cmd; res.start_seq = ctx->seq; }
     PWA_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, *reinterpret_cast<const CUtensorMap *>(tc.map), N, resident_rows, varg, fa,
-                                     (const double *)ctx->data.weights));
+                                     (const double *)ctx->data.weights, res));
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     return PWA_OK;
 }
 
 // One configuration per (storage, n): the fastest of the variants measured in round 1 (profiles/r1b_summary.md).
-pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled)
+pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs &fa, bool *handled, bool resident)
 {
     *handled = false;
     const int n = ctx->n;
@@ -386,16 +479,16 @@ pwa_status launch_data_term_tma(pwa_ctx *ctx, const VArg &varg, const FinishArgs
     //                         ST    CB LPR THREADS MINB GW NS     stage bytes
     if (f32) {
         switch (n) {
-        case 16: return launch_tma<float, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);      //  4 KB
-        case 32: return launch_tma<float, 2, 1, 512, 1, 2, 3>(ctx, varg, fa);      //  8 KB, 16 warps
-        case 64: return launch_tma<float, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);      //  8 KB, 16 warps, groups of 2
+        case 16: return launch_tma<float, 1, 1, 256, 2, 1, 3>(ctx, varg, fa, resident);      //  4 KB
+        case 32: return launch_tma<float, 2, 1, 512, 1, 2, 3>(ctx, varg, fa, resident);      //  8 KB, 16 warps
+        case 64: return launch_tma<float, 4, 2, 512, 1, 2, 3>(ctx, varg, fa, resident);      //  8 KB, 16 warps, groups of 2
         }
     } else {
         switch (n) {
-        case 8:  return launch_tma<double, 1, 1, 256, 2, 1, 3>(ctx, varg, fa);
-        case 16: return launch_tma<double, 2, 2, 512, 1, 2, 3>(ctx, varg, fa);
-        case 32: return launch_tma<double, 4, 2, 512, 1, 2, 3>(ctx, varg, fa);
-        case 64: return launch_tma<double, 8, 4, 512, 1, 2, 3>(ctx, varg, fa);
+        case 8:  return launch_tma<double, 1, 1, 256, 2, 1, 3>(ctx, varg, fa, resident);
+        case 16: return launch_tma<double, 2, 2, 512, 1, 2, 3>(ctx, varg, fa, resident);
+        case 32: return launch_tma<double, 4, 2, 512, 1, 2, 3>(ctx, varg, fa, resident);
+        case 64: return launch_tma<double, 8, 4, 512, 1, 2, 3>(ctx, varg, fa, resident);
         }
     }
     *handled = false;

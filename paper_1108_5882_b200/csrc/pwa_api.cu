@@ -167,6 +167,102 @@ static pwa_status upload_V(pwa_ctx *ctx, int K)
     return PWA_OK;
 }
 
+// ---- resident evaluation grid (option "resident", data_term_tma.cu) ------------------------------------------------
+// Mailbox words are (tag << 32 | 32 bits of payload), tag = low half of the evaluation's sequence number; tag 0xffffffff
+// in every word means quit and is never used for a command.
+static const unsigned kResidentQuitTag = 0xffffffffu;
+
+static void mailbox_fill(pwa_ctx *ctx, unsigned tag)
+{
+    volatile unsigned long long *w = ctx->h_cmd;
+    for (int k = 0; k < 4 * kMaxFastWaves; ++k) w[k] = (unsigned long long)tag << 32;
+    __sync_synchronize();
+}
+
+// Ends the grid (quit command + stream synchronisation).  Called by every entry point that enqueues other work on the
+// stream or changes what the grid reads (samples, M, options), so that a resident grid is never in anybody's way.
+static pwa_status resident_stop(pwa_ctx *ctx)
+{
+    if (!ctx->resident_running) return PWA_OK;
+    mailbox_fill(ctx, kResidentQuitTag);
+    ctx->resident_running = false;
+    PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return PWA_OK;
+}
+
+static pwa_status resident_start(pwa_ctx *ctx, bool *started)
+{
+    if ((unsigned)ctx->seq == kResidentQuitTag) ++ctx->seq;
+    mailbox_fill(ctx, (unsigned)ctx->seq);                      // commands carry later numbers
+    // the device copy of the sequence number starts at the same value (the CTAs other than CTA 0 poll it)
+    if (ctx->ev_V_pending) { PWA_CUDA(ctx, cudaEventSynchronize(ctx->ev_V)); ctx->ev_V_pending = false; }
+    memcpy(ctx->h_V, &ctx->seq, sizeof(unsigned long long));
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_cmd, ctx->h_V, sizeof(unsigned long long), cudaMemcpyHostToDevice, ctx->stream));
+    PWA_CUDA(ctx, cudaEventRecord(ctx->ev_V, ctx->stream));
+    ctx->ev_V_pending = true;
+    pwa_status s = launch_resident(ctx, started);
+    if (s == PWA_OK && *started) ctx->resident_running = true;
+    return s;
+}
+
+static void resident_send(pwa_ctx *ctx, const double *V, unsigned tag)
+{
+    const unsigned *half = reinterpret_cast<const unsigned *>(V);
+    volatile unsigned long long *w = ctx->h_cmd;
+    const int nw = 4 * ctx->n;
+    for (int k = 0; k < nw; ++k) w[k] = ((unsigned long long)tag << 32) | half[k];
+    __sync_synchronize();
+}
+
+// One evaluation through the mailbox.  The record comes back as 2 (4 + 2n) tagged words in mapped host memory and is
+// complete when every word carries this evaluation's tag; it is then unpacked into h_result[0] for unpack_results.
+// *done = false: the shape is not served by the resident kernel (the caller evaluates by a launch).
+static pwa_status resident_eval(pwa_ctx *ctx, const double *V, bool *done)
+{
+    *done = false;
+    if (!ctx->resident_running) {
+        bool started = false;
+        pwa_status s = resident_start(ctx, &started);
+        if (s != PWA_OK || !started) return s;
+    }
+    const int nwords = 2 * (4 + 2 * ctx->n);
+    volatile unsigned long long *r = ctx->h_rres;
+    ctx->last_K = 1;
+    for (int restarts = 0;; ++restarts) {
+        ++ctx->seq;
+        if ((unsigned)ctx->seq == kResidentQuitTag) ++ctx->seq;  // the grid follows any forward jump of the tag
+        const unsigned tag = (unsigned)ctx->seq;
+        resident_send(ctx, V, tag);
+        bool answered = false;
+        for (unsigned spins = 0; !answered; ++spins) {
+            if ((unsigned)(r[nwords - 1] >> 32) == tag) {
+                int k = 0;
+                while (k < nwords && (unsigned)(r[k] >> 32) == tag) ++k;
+                answered = k == nwords;
+                continue;
+            }
+            if ((spins & 0xfffffu) != 0xfffffu) continue;
+            cudaError_t e = cudaStreamQuery(ctx->stream);      // every ~1e6 polls: is the grid still there?
+            if (e == cudaSuccess) break;                       // it ended (idle for ~2 s before this command)
+            if (e != cudaErrorNotReady) return cuda_fail(ctx, e, "waiting for the resident grid");
+            if (spins > (1u << 31)) return fail(ctx, PWA_ERR_CUDA, "resident grid does not answer");
+        }
+        if (answered) break;
+        ctx->resident_running = false;
+        if (restarts == 3) return fail(ctx, PWA_ERR_CUDA, "resident grid keeps ending before it answers");
+        bool started = false;
+        pwa_status s = resident_start(ctx, &started);          // start it again, send the command again under a new number
+        if (s != PWA_OK) return s;
+        if (!started) return fail(ctx, PWA_ERR_CUDA, "resident grid could not be restarted");
+    }
+    __sync_synchronize();
+    unsigned *dst = reinterpret_cast<unsigned *>(ctx->h_result);
+    for (int k = 0; k < nwords; ++k) dst[k] = (unsigned)r[k];
+    ctx->h_flags[0] = ctx->seq;                                 // a pwa_fetch(1) behind this call returns the same record
+    *done = true;
+    return PWA_OK;
+}
+
 static pwa_status enqueue_evals(pwa_ctx *ctx, int K, bool batched)
 {
     const int n = ctx->n;
@@ -236,6 +332,16 @@ pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_V, sizeof(double) * kMaxK * 2 * n);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_V, sizeof(double) * kMaxK * 2 * n);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_V, cudaEventDisableTiming);
+    // mailbox of the resident grid (option "resident"): tagged command words, tagged record, device copy {seq, V}
+    const size_t cmd_words = 4 * (size_t)kMaxFastWaves, rres_words = 2 * (4 + 2 * (size_t)kMaxFastWaves);
+    if (e == cudaSuccess) e = cudaHostAlloc(&ctx->h_cmd, sizeof(unsigned long long) * cmd_words, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->dev_cmd_host, ctx->h_cmd, 0);
+    if (e == cudaSuccess) memset(ctx->h_cmd, 0, sizeof(unsigned long long) * cmd_words);
+    if (e == cudaSuccess) e = cudaHostAlloc(&ctx->h_rres, sizeof(unsigned long long) * rres_words, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->dev_rres, ctx->h_rres, 0);
+    if (e == cudaSuccess) memset(ctx->h_rres, 0, sizeof(unsigned long long) * rres_words);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_cmd, sizeof(unsigned long long) * (1 + 2 * (size_t)kMaxFastWaves));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_cmd, 0, sizeof(unsigned long long) * (1 + 2 * (size_t)kMaxFastWaves));
     // per-block partial slots of every single-V pass (data term: 2 + 2n components, resonance gradient: up to
     // 2 + 4 kMaxRes), sized here for the largest grid any launcher uses (<= 16 blocks per SM), so that no
     // evaluation call ever allocates (pwa.h, general rules)
@@ -255,6 +361,7 @@ void pwa_destroy(pwa_ctx *ctx)
 {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    if (ctx->resident_running && ctx->h_cmd) { mailbox_fill(ctx, kResidentQuitTag); ctx->resident_running = false; }
     cudaStreamSynchronize(ctx->stream);
     free_sample(ctx->data);
     free_sample(ctx->mc);
@@ -267,6 +374,9 @@ void pwa_destroy(pwa_ctx *ctx)
     if (ctx->d_V) cudaFree(ctx->d_V);
     if (ctx->h_V) cudaFreeHost(ctx->h_V);
     if (ctx->ev_V) cudaEventDestroy(ctx->ev_V);
+    if (ctx->h_cmd) cudaFreeHost(ctx->h_cmd);
+    if (ctx->h_rres) cudaFreeHost(ctx->h_rres);
+    if (ctx->d_cmd) cudaFree(ctx->d_cmd);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     if (ctx->d_H) cudaFree(ctx->d_H);
@@ -278,6 +388,7 @@ pwa_status pwa_upload_events(pwa_ctx *ctx, pwa_sample which, const void *amps, i
                              int64_t n_generated, uint32_t flags)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
     if (n_events < 0 || (n_events > 0 && !amps)) return fail(ctx, PWA_ERR_INVALID_ARG, "bad amps / n_events");
     if (flags > PWA_BORROW) return fail(ctx, PWA_ERR_INVALID_ARG, "bad flags");
@@ -302,6 +413,7 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
                                       int32_t n_ang, int64_t n_events, int64_t n_generated, uint32_t flags)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
     if (n_ang < 1 || n_ang > kMaxAng) return fail(ctx, PWA_ERR_INVALID_ARG, "n_ang must be in [1, 4]");
     if (n_events < 0 || (n_events > 0 && (!mass || !ang))) return fail(ctx, PWA_ERR_INVALID_ARG, "bad mass / ang / n_events");
@@ -327,6 +439,7 @@ pwa_status pwa_upload_events_factored(pwa_ctx *ctx, pwa_sample which, const doub
 pwa_status pwa_set_weights(pwa_ctx *ctx, pwa_sample which, const double *w, uint32_t flags)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (which != PWA_DATA && which != PWA_MC) return fail(ctx, PWA_ERR_INVALID_ARG, "bad sample id");
     if (flags > PWA_BORROW) return fail(ctx, PWA_ERR_INVALID_ARG, "bad flags");
     Sample &smp = (which == PWA_DATA) ? ctx->data : ctx->mc;
@@ -368,6 +481,7 @@ pwa_status pwa_set_weights(pwa_ctx *ctx, pwa_sample which, const double *w, uint
 pwa_status pwa_set_wave_map(pwa_ctx *ctx, int32_t n_res, const int32_t *res_of_wave, const int32_t *ang_of_wave)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (n_res < 1 || n_res > kMaxRes || !res_of_wave || !ang_of_wave) return fail(ctx, PWA_ERR_INVALID_ARG, "bad wave map");
     if (ctx->n > kMaxFastWaves) return fail(ctx, PWA_ERR_UNSUPPORTED, "factored mode needs n <= 64");
     std::vector<int32_t> pair(n_res * kMaxAng, -1);
@@ -390,6 +504,7 @@ pwa_status pwa_set_wave_map(pwa_ctx *ctx, int32_t n_res, const int32_t *res_of_w
 pwa_status pwa_set_resonances(pwa_ctx *ctx, const double *mass0, const double *width0)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (ctx->n_res < 1) return fail(ctx, PWA_ERR_STATE, "pwa_set_wave_map not called");
     if (!mass0 || !width0 || !finite_all(mass0, ctx->n_res) || !finite_all(width0, ctx->n_res))
         return fail(ctx, PWA_ERR_INVALID_ARG, "bad resonance parameters");
@@ -403,6 +518,7 @@ pwa_status pwa_set_resonances(pwa_ctx *ctx, const double *mass0, const double *w
 pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "no MC sample uploaded");
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
     pwa_status s = launch_norm_build(ctx);
@@ -438,6 +554,7 @@ pwa_status pwa_batch_path(pwa_ctx *ctx, int32_t *which_path, double *err_rel)
 pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
 {
     if (!ctx || !M) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     const size_t cnt = 2 * (size_t)ctx->n * ctx->n;
     if (!finite_all(M, cnt)) return fail(ctx, PWA_ERR_INVALID_ARG, "M contains non-finite values");
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -453,6 +570,7 @@ pwa_status pwa_set_norm(pwa_ctx *ctx, const double *M)
 pwa_status pwa_nll_grad_enqueue(pwa_ctx *ctx, const double *V)
 {
     if (!ctx || !V) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     pwa_status s = check_ready(ctx, true);
     if (s != PWA_OK) return s;
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -464,6 +582,7 @@ pwa_status pwa_nll_grad_enqueue(pwa_ctx *ctx, const double *V)
 pwa_status pwa_nll_grad_batch_enqueue(pwa_ctx *ctx, int32_t K, const double *V)
 {
     if (!ctx || !V) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (K < 1 || K > kMaxK) return fail(ctx, PWA_ERR_INVALID_ARG, "K must be in [1, 1024]");
     pwa_status s = check_ready(ctx, true);
     if (s != PWA_OK) return s;
@@ -485,6 +604,16 @@ pwa_status pwa_fetch(pwa_ctx *ctx, int32_t K, double *nll, double *grad, double 
 pwa_status pwa_nll_grad(pwa_ctx *ctx, const double *V, double *nll, double *grad, double *parts)
 {
     if (!ctx || !V || !nll || !grad) return ctx ? fail(ctx, PWA_ERR_INVALID_ARG, "null argument") : PWA_ERR_INVALID_ARG;
+    if (ctx->opt_resident) {                         // evaluation through the resident grid's mailbox: no launch
+        pwa_status s = check_ready(ctx, true);
+        if (s != PWA_OK) return s;
+        if (!finite_all(V, 2 * (size_t)ctx->n)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
+        PWA_CUDA(ctx, cudaSetDevice(ctx->device));
+        bool done = false;
+        s = resident_eval(ctx, V, &done);
+        if (s != PWA_OK) return s;
+        if (done) return unpack_results(ctx, 1, nll, grad, parts);
+    }
     pwa_status s = pwa_nll_grad_enqueue(ctx, V);
     if (s != PWA_OK) return s;
     return pwa_fetch(ctx, 1, nll, grad, parts);
@@ -501,6 +630,7 @@ pwa_status pwa_nll_grad_batch(pwa_ctx *ctx, int32_t K, const double *V, double *
 pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
 {
     if (!ctx || !V || !out_dev) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     pwa_status s = check_ready(ctx, false);
     if (s != PWA_OK) return s;
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -551,6 +681,7 @@ pwa_status pwa_assemble_host_shards(int32_t n, int32_t R, const double *terms, c
 pwa_status pwa_norm_sums(pwa_ctx *ctx, double *G_out, int64_t *n_gen_out)
 {
     if (!ctx || !G_out || !n_gen_out) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "no MC sample uploaded");
     if (!ctx->M_valid) return fail(ctx, PWA_ERR_STATE, "normalisation matrix missing or stale: call pwa_build_norm");
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -583,6 +714,7 @@ pwa_status pwa_combine_norm_host(int32_t n, int32_t R, const double *G, const in
 pwa_status pwa_fumili_hessian(pwa_ctx *ctx, const double *V, double *H, int32_t with_norm)
 {
     if (!ctx || !V || !H) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     pwa_status s = check_ready(ctx, with_norm != 0);
     if (s != PWA_OK) return s;
     if (ctx->data.factored && !ctx->res_set) return fail(ctx, PWA_ERR_STATE, "pwa_set_resonances not called");
@@ -653,6 +785,7 @@ pwa_status pwa_polar_to_cartesian(int32_t n, const double *r_phi, double *V)
 pwa_status pwa_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG)
 {
     if (!ctx || !V || !dM || !dG) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (ctx->data.n_events < 0 || ctx->mc.n_events < 0) return fail(ctx, PWA_ERR_STATE, "DATA and MC must be uploaded");
     if (!ctx->data.factored || !ctx->mc.factored) return fail(ctx, PWA_ERR_STATE, "pwa_res_grad needs factored uploads");
     if (!finite_all(V, 2 * (size_t)ctx->n)) return fail(ctx, PWA_ERR_INVALID_ARG, "V contains non-finite values");
@@ -729,6 +862,7 @@ pwa_dtype pwa_storage(const pwa_ctx *ctx) { return ctx ? ctx->storage : PWA_F64;
 pwa_status pwa_sync(pwa_ctx *ctx)
 {
     if (!ctx) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     PWA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return PWA_OK;
 }
@@ -736,10 +870,12 @@ pwa_status pwa_sync(pwa_ctx *ctx)
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
 {
     if (!ctx || !key) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     if (!strcmp(key, "data_term")) ctx->opt_data_term = value;
     else if (!strcmp(key, "norm")) ctx->opt_norm = value;
     else if (!strcmp(key, "batch")) ctx->opt_batch = value;
     else if (!strcmp(key, "l2_resident_mb")) { if (value < -1 || value > 120) return fail(ctx, PWA_ERR_INVALID_ARG, "l2_resident_mb must be in [-1, 120]"); ctx->opt_l2_resident_mb = value; }
+    else if (!strcmp(key, "resident")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "resident must be 0 or 1"); ctx->opt_resident = value != 0; }
     else if (!strcmp(key, "likelihood")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "likelihood must be 0 (eq. 3) or 1 (eq. 2)"); ctx->opt_likelihood = value; }
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
@@ -752,6 +888,7 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value)
     else if (!strcmp(key, "norm")) *value = ctx->opt_norm;
     else if (!strcmp(key, "batch")) *value = ctx->opt_batch;
     else if (!strcmp(key, "l2_resident_mb")) *value = ctx->opt_l2_resident_mb;
+    else if (!strcmp(key, "resident")) *value = ctx->opt_resident ? 1 : 0;
     else if (!strcmp(key, "likelihood")) *value = ctx->opt_likelihood;
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
@@ -760,6 +897,7 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value)
 pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result)
 {
     if (!ctx || !result) return PWA_ERR_INVALID_ARG;
+    { pwa_status rs__ = resident_stop(ctx); if (rs__ != PWA_OK) return rs__; }
     PWA_CUDA(ctx, cudaSetDevice(ctx->device));
     return run_microbench(ctx, which, bytes, result);
 }

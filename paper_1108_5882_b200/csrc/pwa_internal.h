@@ -82,6 +82,11 @@ struct pwa_ctx {
     // int8 tensor-core batched evaluation (batch_i8.cu): the same for the DATA sample, found on first use
     struct { bool checked = false, valid = false; int exp[128]; float scale[128]; double cmax[128];
              unsigned char *planes = nullptr; } i8d;       // planes: X digit-plane image of the sample (k_bi8_planes), library-owned
+    // resident evaluation grid (option "resident"; data_term_tma.cu): mailbox in device-mapped pinned host memory
+    // ([0] = sequence number, [1 ..] = V) and its device copy
+    unsigned long long *h_cmd = nullptr, *dev_cmd_host = nullptr, *d_cmd = nullptr;
+    unsigned long long *h_rres = nullptr, *dev_rres = nullptr;      // tagged result record of the resident grid (mapped host memory)
+    bool opt_resident = false, resident_running = false;
     uint64_t launches = 0;
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     int opt_l2_resident_mb = -1;              // MB of the data sample's head kept in L2 between evaluations (TMA data term); -1 = automatic, 0 = off
@@ -117,6 +122,7 @@ pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, 
 pwa_status launch_batch_i8(pwa_ctx *ctx, int K, bool *handled);   // batch_i8.cu
 double batch_i8_error_estimate(const pwa_ctx *ctx);               // batch_i8.cu
 pwa_status launch_res_grad(pwa_ctx *ctx, const double *V, double *dM, double *dG);
+pwa_status launch_resident(pwa_ctx *ctx, bool *started);   // data_term.cu
 pwa_status launch_floating_passes(pwa_ctx *ctx, const double *V, int *ncomp_out);   // factored.cu
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result);
 

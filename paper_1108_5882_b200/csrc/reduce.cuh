@@ -24,6 +24,11 @@ struct FinishArgs {
     // written (system-scope fence) done_flag[0] = seq tells the polling host thread it is complete
     unsigned long long *done_flag = nullptr;
     unsigned long long seq = 0;
+    // resident grid (data_term_tma.cu): the record goes to device-mapped host memory as 2 words per double,
+    // (tag << 32 | low half), (tag << 32 | high half): complete when every word carries the tag, so neither a
+    // system-scope fence nor a flag is needed
+    unsigned long long *tagged = nullptr;
+    unsigned tag = 0;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m)
@@ -46,8 +51,17 @@ __device__ __forceinline__ double warp_sum(double x)
 // eq2 true, n_eq2 = N_data (or sum of weights): nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2)
 __device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
                                             double *out, int n, bool eq2 = false, double n_eq2 = 0.0,
-                                            unsigned long long *done_flag = nullptr, unsigned long long seq = 0)
+                                            unsigned long long *done_flag = nullptr, unsigned long long seq = 0,
+                                            unsigned long long *tagged = nullptr, unsigned tag = 0)
 {
+    auto put = [&](int idx, double v) {
+        if (tagged != nullptr) {
+            const unsigned long long t = (unsigned long long)tag << 32;
+            volatile unsigned long long *p = tagged + 2 * idx;
+            p[0] = t | (unsigned)__double2loint(v);
+            p[1] = t | (unsigned)__double2hiint(v);
+        } else out[idx] = v;
+    };
     const int NC = 2 + 2 * n;
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int lane = tid & 31, warp = tid >> 5;
@@ -91,16 +105,16 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
         const double gw = eq2 ? 2.0 * (n_eq2 / acc) : 2.0;
         // grad_a = -2 conj(T_a) + gw (M V)_a
         for (int a = lane; a < n; a += 32) {
-            out[4 + 2 * a] = -2.0 * s_tot[2 + 2 * a] + gw * s_mv[2 * a];
-            out[5 + 2 * a] =  2.0 * s_tot[3 + 2 * a] + gw * s_mv[2 * a + 1];
+            put(4 + 2 * a, -2.0 * s_tot[2 + 2 * a] + gw * s_mv[2 * a]);
+            put(5 + 2 * a,  2.0 * s_tot[3 + 2 * a] + gw * s_mv[2 * a + 1]);
         }
         if (lane == 0) {
-            out[0] = eq2 ? (-s_tot[0] + n_eq2 * log(acc)) : -(s_tot[0] - acc);
-            out[1] = s_tot[0];
-            out[2] = acc;
-            out[3] = s_tot[1];
+            put(0, eq2 ? (-s_tot[0] + n_eq2 * log(acc)) : -(s_tot[0] - acc));
+            put(1, s_tot[0]);
+            put(2, acc);
+            put(3, s_tot[1]);
         }
-        if (done_flag != nullptr) {
+        if (done_flag != nullptr && tagged == nullptr) {
             __threadfence_system();                 // every writing lane: record visible to the host before the flag
             __syncwarp();
             if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(done_flag) = seq;
@@ -171,10 +185,12 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
             s_tot[c] = acc;
         }
     }
+    // re-arm the ticket for the next evaluation BEFORE the record is published: in a resident grid the host may send the
+    // next command as soon as it sees the record, and the first CTAs of that evaluation must find the ticket at zero
+    if (tid == 0) { *fa.ticket = 0u; __threadfence(); }
     __syncthreads();
 
-    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq);
-    if (tid == 0) *fa.ticket = 0u;   // re-arm for the next launch on this stream
+    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq, fa.tagged, fa.tag);
 }
 
 constexpr int kFastWaves = 64;   // == kMaxFastWaves (pwa_internal.h)

@@ -441,6 +441,102 @@ def test_back_to_back_enqueues_are_independent(pwa, storage, n, N):
             pwa.pwa_set_option(c.ctx, "l2_resident_mb", 500)
 
 
+# ------------------------------------------------------------------ resident evaluation grid (option "resident")
+@pytest.mark.parametrize("storage,n,N", [("f64", 4, 1000), ("f64", 8, 30_011), ("f64", 16, 100_000), ("f32", 16, 7),
+                                         ("f32", 32, 200_003), ("f32", 64, 50_001), ("f64", 64, 20_001)])
+def test_resident_grid_is_bitwise_the_launched_evaluation(pwa, storage, n, N):
+    """pwa_set_option("resident", 1): pwa_nll_grad goes through the mailbox of a grid that stays on the GPU (no launch per
+    evaluation).  Same kernel body, same grid, same reduction order: every evaluation is bitwise the launched one, in both
+    likelihood forms; any other entry point ends the grid transparently and the next pwa_nll_grad starts it again."""
+    A, B, _ = rand_case(500 + n, N, 2001, n, storage)
+    Vs = np.random.default_rng(6).normal(size=(40, n, 2))
+    with Ctx(pwa, n, storage) as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=2001)
+        M = pwa.pwa_build_norm(c.ctx, want_M=True)
+        lone = [pwa.pwa_nll_grad(c.ctx, V) for V in Vs]
+        pwa.pwa_set_option(c.ctx, "resident", 1)
+        assert pwa.pwa_get_option(c.ctx, "resident") == 1
+        for rep in range(3):
+            for V, ref in zip(Vs, lone):
+                nll, g, parts = pwa.pwa_nll_grad(c.ctx, V)
+                assert nll == ref[0] and np.array_equal(g, ref[1]) and np.array_equal(parts, ref[2])
+        nll1, g1, _ = pwa.pwa_fetch(c.ctx)                         # a fetch behind a resident evaluation: the same record
+        assert nll1[0] == lone[-1][0] and np.array_equal(g1[0], lone[-1][1])
+        # other calls between resident evaluations: batch, enqueue / fetch, a new M, the other likelihood form
+        nb, gb, _ = pwa.pwa_nll_grad_batch(c.ctx, Vs[:5])
+        nll, g, parts = pwa.pwa_nll_grad(c.ctx, Vs[7])
+        assert nll == lone[7][0] and np.array_equal(g, lone[7][1])
+        pwa.pwa_nll_grad_enqueue(c.ctx, Vs[2])
+        nll2, g2, _ = pwa.pwa_fetch(c.ctx)
+        assert nll2[0] == lone[2][0] and np.array_equal(g2[0], lone[2][1])
+        pwa.pwa_set_norm(c.ctx, 2.0 * M)
+        nll, g, parts = pwa.pwa_nll_grad(c.ctx, Vs[9])
+        assert parts[0] == lone[9][2][0] and parts[1] == 2.0 * lone[9][2][1]
+        pwa.pwa_set_norm(c.ctx, M)
+        pwa.pwa_set_option(c.ctx, "likelihood", 1)
+        res_eq2 = [pwa.pwa_nll_grad(c.ctx, V) for V in Vs[:6]]
+        pwa.pwa_set_option(c.ctx, "resident", 0)
+        for V, r in zip(Vs[:6], res_eq2):
+            nll, g, parts = pwa.pwa_nll_grad(c.ctx, V)
+            assert nll == r[0] and np.array_equal(g, r[1]) and np.array_equal(parts, r[2])
+        pwa.pwa_set_option(c.ctx, "likelihood", 0)
+        pwa.pwa_set_option(c.ctx, "resident", 1)
+        nll, g, parts = pwa.pwa_nll_grad(c.ctx, Vs[11])
+        assert nll == lone[11][0] and np.array_equal(g, lone[11][1])
+        # the context is destroyed with the grid still resident (Ctx.__exit__)
+
+
+def test_resident_grid_fallbacks_and_idle_restart(pwa):
+    """Shapes the resident kernel does not serve (n not a power of two <= 64, weighted samples) evaluate by launches under
+    the option; a grid that saw no command for ~2 s ends by itself and the next evaluation starts a new one; a
+    non-finite event is reported as in the launched path."""
+    import time
+    n, N = 5, 4001
+    A, B, _ = rand_case(91, N, 1001, n, "f64")
+    V = np.random.default_rng(8).normal(size=(n, 2))
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=1001)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        ref = pwa.pwa_nll_grad(c.ctx, V)
+        pwa.pwa_set_option(c.ctx, "resident", 1)
+        res = pwa.pwa_nll_grad(c.ctx, V)
+        assert res[0] == ref[0] and np.array_equal(res[1], ref[1])
+    n, N = 16, 20_003
+    A, B, _ = rand_case(92, N, 1001, n, "f64")
+    V = np.random.default_rng(9).normal(size=(n, 2))
+    w = np.random.default_rng(10).uniform(0.2, 1.5, size=N)
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=1001)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        ref = pwa.pwa_nll_grad(c.ctx, V)
+        pwa.pwa_set_option(c.ctx, "resident", 1)
+        assert pwa.pwa_nll_grad(c.ctx, V)[0] == ref[0]
+        time.sleep(6.0)                                            # the idle grid ends by itself
+        res = pwa.pwa_nll_grad(c.ctx, V)
+        assert res[0] == ref[0] and np.array_equal(res[1], ref[1])
+        for _ in range(20):
+            assert pwa.pwa_nll_grad(c.ctx, V)[0] == ref[0]
+        pwa.pwa_set_weights(c.ctx, pwa.PWA_DATA, w)                # weighted: launches (and ends the grid first)
+        res_w = pwa.pwa_nll_grad(c.ctx, V)
+        pwa.pwa_set_option(c.ctx, "resident", 0)
+        ref_w = pwa.pwa_nll_grad(c.ctx, V)
+        assert res_w[0] == ref_w[0] and np.array_equal(res_w[1], ref_w[1]) and res_w[0] != ref[0]
+    A2 = A.copy()
+    A2[1234] = 0.0                                                 # S = 0: ln 0, non-finite contribution
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, A2)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, B, n_generated=1001)
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        pwa.pwa_set_option(c.ctx, "resident", 1)
+        nll, g, parts, st = pwa.pwa_nll_grad(c.ctx, V, want_status=True)
+        assert st == pwa.PWA_WARN_NONFINITE and parts[0] == -math.inf and nll == math.inf
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_nll_grad(c.ctx, np.full((n, 2), np.nan))       # V is checked before it is sent
+
+
 # ------------------------------------------------------------------ NEXT-1 (A8): batched evaluation on the int8 tensor cores
 @pytest.mark.parametrize("N,K", [(100, 64), (128, 5), (129, 1), (257, 64), (6007, 64), (6007, 70), (40_001, 33)])
 def test_batch_i8_parity(pwa, oracle, N, K):

@@ -256,7 +256,20 @@ def measure_peaks(pwa, ctx, mp_hbm, mp_src):
             "int8_tops": pwa.pwa_microbench(ctx, 3), "int8_tops_n128": pwa.pwa_microbench(ctx, 4),
             "int8_tops_n64": pwa.pwa_microbench(ctx, 5), "tmem_read_gbs": pwa.pwa_microbench(ctx, 7),
             "int8_source": "measured here: pwa_microbench(3 | 4 | 5), tcgen05.mma.kind::i8 from shared memory, all SMs",
-            "int8_tops_nominal": 4500.0}
+            "int8_tops_nominal": 4500.0,
+            "tensor_overlap_ms": overlap_probe(pwa, ctx)}
+
+
+def overlap_probe(pwa, ctx):
+    """pwa_microbench(8): a stream of int8 tcgen05.mma next to 12 warps of one kind of epilogue work (the issuer's scheduler
+    kept free).  overlap = (t_mma + t_work - t_both) / min(t_mma, t_work): 1 = the work hides under the MMAs, 0 = serial.
+    fp64 arithmetic comes out at 0 (why the batched int8 kernel cannot hide its epilogue)."""
+    out = {"mma_alone": pwa.pwa_microbench(ctx, 8, 16)}
+    for mode, name in ((0, "fp64_fma"), (6, "fp64_diluted_1_in_4"), (5, "fp32_fma"), (3, "int_mad"), (1, "tcgen05_ld"), (2, "st_shared")):
+        alone = pwa.pwa_microbench(ctx, 8, mode + 32 + 64)
+        both = pwa.pwa_microbench(ctx, 8, mode + 48 + 64)
+        out[name] = {"alone": alone, "with_mma": both, "overlap": (out["mma_alone"] + alone - both) / min(out["mma_alone"], alone)}
+    return out
 
 
 def rl_hbm(peaks, nbytes, ms, **kw):

@@ -330,7 +330,12 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* c
  * which = 0: fp64 FMA (result TFLOP/s), 1: fp64 mma.sync m8n8k4 (TFLOP/s),
  * 2: HBM read-only stream over `bytes` of scratch (GB/s), 3 .. 6: tcgen05.mma.kind::i8 with M = 128, K = 32 and
  * N = 256 / 128 / 64 / 32, operands in shared memory (int8 Top/s, all SMs), 7: TMEM reads (tcgen05.ld 32x32b.x16 by
- * 16 warps per SM, GB/s).  Synchronous; result HOST.                                                              */
+ * 16 warps per SM, GB/s), 8: overlap probe: one warp issues a stream of tcgen05.mma.kind::i8 (M = N = 128) while 16 (or,
+ * with bit 6 of `bytes`, the 12 that do not share the issuer's scheduler) other warps run one kind of epilogue work;
+ * `bytes` = mode + 16 (MMAs on) + 32 (epilogue work on) + 64 (keep the issuer's scheduler free), mode 0 = fp64 FMA,
+ * 1 = tcgen05.ld, 2 = st.shared.v4, 3 = integer multiply-add, 4 = ld.shared.v4, 5 = fp32 FMA, 6 = 2 fp64 FMA among 6
+ * integer chains; result = milliseconds (compare MMAs alone, the work alone and both: DESIGN.md section 6.7 has the
+ * outcome: fp64 arithmetic does not overlap with the int8 MMAs at all).  Synchronous; result HOST.                  */
 pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result);
 
 #ifdef __cplusplus

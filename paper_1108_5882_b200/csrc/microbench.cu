@@ -111,6 +111,133 @@ __global__ void __launch_bounds__(512, 1) k_mb_tmem_ld(int iters, double *out)
     if (threadIdx.x < 32) { tc::tc_fence_after(); tc::tmem_dealloc(tmem0, 512); }
 }
 
+// Overlap probe: warp 16 issues `mma_iters` x 4 tcgen05.mma.kind::i8 (M = N = 128, K = 32, operands in shared memory) into
+// TMEM columns 0 .. 255 while warps 0 .. 15 run `epi_iters` iterations of one kind of epilogue work:
+// MODE 0 = fp64 FMA chains, 1 = tcgen05.ld 32x32b.x16 of columns 256 .. 511, 2 = st.shared.v4, 3 = integer LOP3 / IMAD
+// chains, 4 = ld.shared.v4.  Timed with either side switched off and with both: does the work overlap with the MMAs?
+template <int MODE>
+__global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_iters, bool skip_sched0, double *out)
+{
+    extern __shared__ unsigned char mb_smem[];
+    __shared__ __align__(8) unsigned long long bar;
+    __shared__ uint32_t tmem_base_s;
+    const uint32_t base = (smem_u32(mb_smem) + 1023u) & ~1023u;
+    const uint32_t scratch = base + 16384u + 32768u;            // 8 KB: 16 bytes per epilogue thread
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { mbar_init(smem_u32(&bar), 1); tc::fence_async_smem(); }
+    if (warp == 0) tc::tmem_alloc(smem_u32(&tmem_base_s), 512);
+    tc::tc_fence_before();
+    __syncthreads();
+    tc::tc_fence_after();
+    const uint32_t tmem0 = tmem_base_s;
+    if (warp == 16) {
+        if (threadIdx.x == 512 && mma_iters > 0) {
+            constexpr uint32_t id = tc::idesc_i8(128, false, false);
+            for (int it = 0; it < mma_iters; ++it) {
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk)
+                    tc::umma_i8(tmem0 + (uint32_t)((it & 1) * 128), tc::desc_kmajor(base + 32u * kk), tc::desc_kmajor(base + 16384u + 32u * kk), id, 1u);
+            }
+            tc::umma_commit(smem_u32(&bar));
+            mbar_wait(smem_u32(&bar), 0);
+        }
+    } else if (epi_iters > 0 && !(epi_iters < 0)) {
+        const int q = warp & 3, j = warp >> 2;
+        if (skip_sched0 && q == 0) {
+        } else if (MODE == 5) {
+            float a[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = 1.0f + threadIdx.x * 1e-6f + i;
+            const float m = 1.0f - 1e-6f, c = 1e-7f;
+            for (int it = 0; it < epi_iters; ++it) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = fmaf(a[i], m, c);
+            }
+            float sum = 0.0f;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) sum += a[i];
+            if (sum == 0.12345f && out != nullptr) out[0] = sum;
+        } else if (MODE == 6) {                                  // 2 fp64 FMA chains diluted in 6 integer chains
+            double a[2] = {1.0 + threadIdx.x * 1e-9, 2.0};
+            uint32_t b[6];
+#pragma unroll
+            for (int i = 0; i < 6; ++i) b[i] = threadIdx.x * 2654435761u + i;
+            const double m = 1.0 - 1e-12, c = 1e-13;
+            for (int it = 0; it < epi_iters; ++it) {
+                a[0] = fma(a[0], m, c); a[1] = fma(a[1], m, c);
+#pragma unroll
+                for (int i = 0; i < 6; ++i) b[i] = (b[i] ^ (uint32_t)it) * 2246822519u + 0x9e3779b9u;
+            }
+            uint32_t x = 0;
+#pragma unroll
+            for (int i = 0; i < 6; ++i) x ^= b[i];
+            if ((a[0] + a[1] == 0.12345 || x == 0x12345u) && out != nullptr) out[0] = 1.0;
+        } else if (MODE == 0) {
+            double a[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = 1.0 + threadIdx.x * 1e-9 + i;
+            const double m = 1.0 - 1e-12, c = 1e-13;
+            for (int it = 0; it < epi_iters; ++it) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+            }
+            double sum = 0.0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) sum += a[i];
+            if (sum == 0.12345 && out != nullptr) out[0] = sum;
+        } else if (MODE == 1) {
+            int acc = 0;
+            for (int it = 0; it < epi_iters; ++it) {
+                int32_t v[16];
+                tc::tmem_ld16(tmem0 + ((uint32_t)(32 * q) << 16) + (uint32_t)(256 + 64 * j + 16 * (it & 3)), v);
+                tc::tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc ^= v[i];
+            }
+            if (acc == 0x12345 && out != nullptr) out[0] = 1.0;
+        } else if (MODE == 2) {
+            const uint32_t a = scratch + 16u * threadIdx.x;
+            for (int it = 0; it < epi_iters; ++it) tc::sts128(a, (uint32_t)it, (uint32_t)it + 1u, (uint32_t)it + 2u, (uint32_t)it + 3u);
+        } else if (MODE == 3) {
+            uint32_t a[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = threadIdx.x * 2654435761u + i;
+            for (int it = 0; it < epi_iters; ++it) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = (a[i] ^ (uint32_t)it) * 2246822519u + 0x9e3779b9u;
+            }
+            uint32_t x = 0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x ^= a[i];
+            if (x == 0x12345u && out != nullptr) out[0] = 1.0;
+        } else {
+            const uint32_t a = scratch + 16u * threadIdx.x;
+            uint32_t x = 0;
+            for (int it = 0; it < epi_iters; ++it) {
+                uint32_t r0, r1, r2, r3;
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(a) : "memory");
+                x ^= r0 ^ r1 ^ r2 ^ r3;
+            }
+            if (x == 0x12345u && out != nullptr) out[0] = 1.0;
+        }
+    }
+    tc::tc_fence_before();
+    __syncthreads();
+    if (warp == 0) { tc::tc_fence_after(); tc::tmem_dealloc(tmem0, 512); }
+}
+
+template <int MODE>
+static cudaError_t launch_overlap(pwa_ctx *ctx, int mma_iters, int epi_iters, bool skip, bool first)
+{
+    constexpr int SM = 1024 + 16384 + 32768 + 8192;
+    if (first) {
+        cudaError_t e = cudaFuncSetAttribute(k_mb_overlap<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM);
+        if (e != cudaSuccess) return e;
+    }
+    k_mb_overlap<MODE><<<ctx->sm_count, 544, SM, ctx->stream>>>(mma_iters, epi_iters, skip, nullptr);
+    return cudaGetLastError();
+}
+
 pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result)
 {
     cudaEvent_t e0, e1;
@@ -142,6 +269,18 @@ pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result
             else k_mb_umma<32><<<ctx->sm_count, 128, SM, ctx->stream>>>(iters, nullptr);
         }
         else if (which == 7) k_mb_tmem_ld<<<ctx->sm_count, 512, 0, ctx->stream>>>(iters * 4, nullptr);
+        else if (which == 8) {
+            // bytes = mode + 16 * (1: MMAs on) + 32 * (1: epilogue work on); result = milliseconds
+            const int mode = (int)(bytes & 15), mi = (bytes & 16) ? iters : 0;
+            const int per_mode[7] = {16384, 14000, 16384, 32768, 16384, 65536, 40000};    // ~1e6 cycles of each kind of work alone
+            if (mode > 6) return fail(ctx, PWA_ERR_INVALID_ARG, "unknown overlap probe mode");
+            const int ei = (bytes & 32) ? per_mode[mode] : 0;
+            const bool skip = (bytes & 64) != 0;
+            cudaError_t e = mode == 0 ? launch_overlap<0>(ctx, mi, ei, skip, rep == 0) : mode == 1 ? launch_overlap<1>(ctx, mi, ei, skip, rep == 0)
+                          : mode == 2 ? launch_overlap<2>(ctx, mi, ei, skip, rep == 0) : mode == 3 ? launch_overlap<3>(ctx, mi, ei, skip, rep == 0)
+                          : mode == 4 ? launch_overlap<4>(ctx, mi, ei, skip, rep == 0) : mode == 5 ? launch_overlap<5>(ctx, mi, ei, skip, rep == 0) : launch_overlap<6>(ctx, mi, ei, skip, rep == 0);
+            PWA_CUDA(ctx, e);
+        }
         else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown microbench id");
         ctx->launches++;
         PWA_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
@@ -159,6 +298,7 @@ pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result
         *result = 2.0 * 128.0 * N * 32.0 * 4.0 * iters * ctx->sm_count / sec * 1e-12;
     }
     else if (which == 7) *result = 16.0 * 32.0 * 16.0 * 4.0 * (iters * 4.0) * ctx->sm_count / sec * 1e-9;   // GB/s of TMEM reads
+    else if (which == 8) *result = (double)best;
     else *result = (double)bytes / sec * 1e-9;
     return PWA_OK;
 }

@@ -322,7 +322,9 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * calling thread spins in pwa_nll_grad; every other entry point of the context that enqueues work or changes what
  * the grid reads (uploads, weights, norm, options, batch / enqueue / minimiser calls, pwa_sync, pwa_destroy) ends
  * the grid first, and the next pwa_nll_grad starts it again (one launch).  A grid that sees no command for ~2 s
- * ends by itself.  Meant for a fit loop of single evaluations on a small sample; leave it off otherwise.          */
+ * ends by itself.  Meant for a fit loop of single evaluations on a small sample; leave it off otherwise.  Under a
+ * tool that makes kernel launches synchronous (ncu) the launch cannot return while the grid waits for its first
+ * command: pwa_nll_grad then fails with PWA_ERR_CUDA after a few restarts (~10 s) instead of hanging.               */
 pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value);
 pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* current value of a pwa_set_option key */
 

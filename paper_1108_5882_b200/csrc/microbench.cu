@@ -172,6 +172,16 @@ __global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_it
 #pragma unroll
             for (int i = 0; i < 6; ++i) x ^= b[i];
             if ((a[0] + a[1] == 0.12345 || x == 0x12345u) && out != nullptr) out[0] = 1.0;
+        } else if (MODE == 7) {                                  // streaming 16-byte global loads (out = a buffer of gridDim.x * epi_iters * 8 KB)
+            const uint4 *p = reinterpret_cast<const uint4 *>(out) + (size_t)blockIdx.x * epi_iters * 512 + (threadIdx.x & 511);
+            uint32_t x = 0;
+#pragma unroll 8
+            for (int it = 0; it < epi_iters; ++it) {
+                uint4 v;
+                asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p + (size_t)it * 512));
+                x ^= v.x ^ v.y ^ v.z ^ v.w;
+            }
+            if (x == 0x12345u) reinterpret_cast<uint32_t *>(out)[0] = x;
         } else if (MODE == 0) {
             double a[8];
 #pragma unroll
@@ -227,14 +237,14 @@ __global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_it
 }
 
 template <int MODE>
-static cudaError_t launch_overlap(pwa_ctx *ctx, int mma_iters, int epi_iters, bool skip, bool first)
+static cudaError_t launch_overlap(pwa_ctx *ctx, int mma_iters, int epi_iters, bool skip, bool first, double *buf = nullptr)
 {
     constexpr int SM = 1024 + 16384 + 32768 + 8192;
     if (first) {
         cudaError_t e = cudaFuncSetAttribute(k_mb_overlap<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM);
         if (e != cudaSuccess) return e;
     }
-    k_mb_overlap<MODE><<<ctx->sm_count, 544, SM, ctx->stream>>>(mma_iters, epi_iters, skip, nullptr);
+    k_mb_overlap<MODE><<<ctx->sm_count, 544, SM, ctx->stream>>>(mma_iters, epi_iters, skip, buf);
     return cudaGetLastError();
 }
 
@@ -243,7 +253,7 @@ pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result
     cudaEvent_t e0, e1;
     PWA_CUDA(ctx, cudaEventCreate(&e0));
     PWA_CUDA(ctx, cudaEventCreate(&e1));
-    pwa_status s = ensure_scratch(ctx, which == 2 ? (size_t)bytes : 4096);
+    pwa_status s = ensure_scratch(ctx, which == 2 ? (size_t)bytes : (which == 8 && (bytes & 15) == 7) ? (size_t)ctx->sm_count * 3000 * 8192 : 4096);
     if (s != PWA_OK) return s;
     double *out = ctx->d_result;
     const int iters = 4096;
@@ -272,13 +282,14 @@ pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result
         else if (which == 8) {
             // bytes = mode + 16 * (1: MMAs on) + 32 * (1: epilogue work on); result = milliseconds
             const int mode = (int)(bytes & 15), mi = (bytes & 16) ? iters : 0;
-            const int per_mode[7] = {16384, 14000, 16384, 32768, 16384, 65536, 40000};    // ~1e6 cycles of each kind of work alone
-            if (mode > 6) return fail(ctx, PWA_ERR_INVALID_ARG, "unknown overlap probe mode");
+            const int per_mode[8] = {16384, 14000, 16384, 32768, 16384, 65536, 40000, 3000};    // ~1e6 cycles of each kind of work alone
+            if (mode > 7) return fail(ctx, PWA_ERR_INVALID_ARG, "unknown overlap probe mode");
             const int ei = (bytes & 32) ? per_mode[mode] : 0;
             const bool skip = (bytes & 64) != 0;
             cudaError_t e = mode == 0 ? launch_overlap<0>(ctx, mi, ei, skip, rep == 0) : mode == 1 ? launch_overlap<1>(ctx, mi, ei, skip, rep == 0)
                           : mode == 2 ? launch_overlap<2>(ctx, mi, ei, skip, rep == 0) : mode == 3 ? launch_overlap<3>(ctx, mi, ei, skip, rep == 0)
-                          : mode == 4 ? launch_overlap<4>(ctx, mi, ei, skip, rep == 0) : mode == 5 ? launch_overlap<5>(ctx, mi, ei, skip, rep == 0) : launch_overlap<6>(ctx, mi, ei, skip, rep == 0);
+                          : mode == 4 ? launch_overlap<4>(ctx, mi, ei, skip, rep == 0) : mode == 5 ? launch_overlap<5>(ctx, mi, ei, skip, rep == 0) : mode == 6 ? launch_overlap<6>(ctx, mi, ei, skip, rep == 0)
+                          : launch_overlap<7>(ctx, mi, ei, skip, rep == 0, reinterpret_cast<double *>(ctx->d_scratch));
             PWA_CUDA(ctx, e);
         }
         else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown microbench id");

@@ -533,10 +533,18 @@ def run_ours(args):
     rank, ws, local = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    # PWA_BENCH_BACKEND=gloo (tests only): several ranks share the visible GPUs and exchange through host memory, so that
+    # the N > 1 code below can be exercised on a one-GPU box (tests/test_gpu_sharded.py); the driver's runs use nccl
+    backend = os.environ.get("PWA_BENCH_BACKEND", "nccl")
+    if backend != "nccl":
+        local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
     if ws > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
     if args.gpus != ws and rank == 0:
         sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={ws}; using {ws}\n")
     import __graft_entry__
@@ -608,7 +616,7 @@ def run_ours(args):
             extra["m_build"]["upload_prepass_ms"] = ms_pre
             M_all = pwa.pwa_build_norm(ctx)
             if ws > 1:
-                M_all, _ = sharded.combine_norm(ctx, device=dev)
+                M_all, _ = sharded.combine_norm(ctx, device=dev if backend == "nccl" else None)
             w.A_mc = None   # free 10 GB of host memory
         else:
             M_all = np.zeros((n, n, 2)); M_all[np.arange(n), np.arange(n), 0] = 1.0
@@ -670,7 +678,7 @@ def run_ours(args):
                                         "last_batch_path": path,
                                         "nll_best": float(np.min(nllf)), "nll_worst": float(np.max(nllf))}
         if ws > 1:
-            t = torch.tensor([ms, wall_ms, ms_kernel], dtype=torch.float64, device=dev)
+            t = torch.tensor([ms, wall_ms, ms_kernel], dtype=torch.float64, device=dev if backend == "nccl" else "cpu")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms, wall_ms, ms_kernel = (float(x) for x in t.tolist())
     finally:
@@ -693,7 +701,7 @@ def run_ours(args):
         "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "n_waves": n, "n_data_per_gpu": w.n_data, "storage": w.storage,
-                   "parallelism": f"event-sharded x{ws}" if ws > 1 else "single GPU",
+                   "parallelism": (f"event-sharded x{ws}" + ("" if backend == "nccl" else f" ({backend} exchange, test mode)")) if ws > 1 else "single GPU",
                    "l2": f"input {bytes_data / 1e6:.0f} MB per step vs 126 MB L2: "
                          + ("larger than L2, no flush needed" if bytes_data > 2.5e8 else "L2-RESIDENT (latency-bound config)")},
         "evals_per_s": 1e3 / ms,

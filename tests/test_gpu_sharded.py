@@ -103,3 +103,34 @@ def test_two_rank_sharded_gpu(tmp_path, oracle, N, Nacc, n, storage):
     assert abs(r[0]["nll2"] - nll2_o) <= tol * max(abs(nll2_o), abs(oracle.data_term(A, Vs[0])[0]))
     assert np.abs(r[0]["g2"] - g2_o).max() <= tol * np.abs(g2_o).max()
     assert float(r[0]["local_norm"]) == pytest.approx(float(r[0]["parts"][0][1]), rel=1e-12)
+
+
+def test_bench_two_ranks_on_one_gpu(tmp_path):
+    """bench.py's N > 1 code (shard generation, combine_norm, the sharded step with its all-gather, max-over-ranks timing,
+    the JSON line of rank 0) under torch.distributed.run with two ranks.  One GPU here, so the ranks share it and exchange
+    through gloo (PWA_BENCH_BACKEND=gloo, a test switch: the driver's runs use nccl); sizes are reduced, the line is not a
+    measurement."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, PWA_BENCH_BACKEND="gloo", MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "4", "--warmup", "3",
+           "--n-data", "300000", "--n-mc", "400000"]
+    r = subprocess.run(cmd, cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]                    # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["steps"] == 4
+    assert d["value"] > 0 and d["e2e"]["value"] > 0 and d["gpu_launches"] >= 4
+    assert d["config"]["n_data_per_gpu"] == 300000 and "event-sharded x2" in d["config"]["parallelism"]
+    assert d["value"] == pytest.approx(2 * 300000 * d["config"]["n_waves"] / d["ms_per_step"] * 1e3, rel=1e-9)
+    # the reference arm under the same launcher: rank 0 alone runs and prints, the other rank exits 0
+    cmd_ref = cmd[:cmd.index(os.path.join(root, "bench.py")) + 1] + ["--impl", "reference", "--gpus", "2", "--steps", "2", "--warmup", "3",
+                                                                     "--n-data", "20000"]
+    r = subprocess.run(cmd_ref, cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1 and json.loads(lines[0])["impl"] == "reference"

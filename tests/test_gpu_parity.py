@@ -995,3 +995,30 @@ def test_nll_grad_floating_three_angular_structures(pwa, oracle, synth):
     check_eval((nll, g, parts), oracle.nll_grad(w.A_data, M_o, V), 1e-12, w.n_data)
     ref = np.concatenate([-dLM + dNM, -dLG + dNG])
     assert np.abs(np.concatenate([dM, dG]) - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------ hardware probes (roofline denominators, overlap probe)
+def test_microbench_probes(pwa):
+    """pwa_microbench: every probe id returns a finite positive figure in the range its unit implies; unknown ids and
+    unknown overlap modes are rejected.  The overlap probe's headline is asserted loosely: fp64 work next to
+    a stream of int8 MMAs costs (almost) the sum of both, tcgen05.ld hides under them."""
+    with Ctx(pwa, 4, "f64") as c:
+        dfma, dmma = pwa.pwa_microbench(c.ctx, 0), pwa.pwa_microbench(c.ctx, 1)
+        assert 5.0 < dfma < 100.0 and 5.0 < dmma < 100.0                       # TFLOP/s
+        assert 1000.0 < pwa.pwa_microbench(c.ctx, 2, 1 << 30) < 12000.0        # GB/s
+        tops = [pwa.pwa_microbench(c.ctx, w) for w in (3, 4, 5, 6)]            # int8 Top/s, N = 256 / 128 / 64 / 32
+        assert all(200.0 < t < 10000.0 for t in tops) and tops[0] >= 0.9 * tops[1] and tops[1] > tops[2] > tops[3]
+        assert pwa.pwa_microbench(c.ctx, 7) > 1000.0                           # GB/s of TMEM reads
+        mma = pwa.pwa_microbench(c.ctx, 8, 16)
+        ov = {}
+        for mode in (0, 1):
+            alone, both = pwa.pwa_microbench(c.ctx, 8, mode + 32 + 64), pwa.pwa_microbench(c.ctx, 8, mode + 48 + 64)
+            assert alone > 0 and both >= 0.95 * max(alone, mma)
+            ov[mode] = (mma + alone - both) / min(mma, alone)
+        assert ov[0] < 0.5 < ov[1], ov
+        for mode in (2, 3, 4, 5, 6, 7):
+            assert pwa.pwa_microbench(c.ctx, 8, mode + 48) > 0
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_microbench(c.ctx, 8, 9 + 48)
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_microbench(c.ctx, 99)

@@ -78,19 +78,25 @@ constexpr size_t SLOT = 128 * 128 + KC;      // doubles per CTA slot: Q[col][c],
 struct Scales { float s[128]; };             // 2^s_c per real column
 struct Exps { int e[128]; };                 // s_c
 
+// The four levels of an accumulator combined exactly: z = 2^16 (2^8 a6 + a5) + (2^8 a4 + a3), |z| < 2^48, formed as a
+// 64-bit integer (one wide multiply-add) and dropped into the mantissa of 1.5 * 2^52; one fp64 subtraction removes the
+// offset (two int -> fp64 conversions and an fp64 FMA before: fp64 instructions are the ones that cannot run beside MMAs).
+__device__ __forceinline__ double z48(int a6, int a5, int a4, int a3)
+{
+    const long long z = (long long)(a6 * 256 + a5) * 65536 + (long long)(a4 * 256 + a3);
+    return __longlong_as_double(z + 0x4338000000000000LL) - 6755399441055744.0;
+}
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, %0;" ::"n"(NEW * 32) : "memory"); }
 constexpr uint32_t kI1_128 = idesc_i8(128, false, false), kI1_256 = idesc_i8(256, false, false);   // GEMM1: both operands K-major
 constexpr uint32_t kI2_128 = idesc_i8(128, true, true),  kI2_256 = idesc_i8(256, true, true);      // GEMM2: both operands MN-major
 
-// 1 / x for 1 <= x < 2^100: 20-bit hardware seed, two Newton steps (relative error ~2^-52)
+// 1 / x for 1 <= x < 2^100: 20-bit hardware seed, one Newton step (relative error ~2^-40)
 __device__ __forceinline__ double rcp_d(double x)
 {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
+    const double e = fma(-x, r, 1.0);             // the seed carries the upper 20 mantissa bits: one Newton step gives 2^-40,
+    return fma(r, e, r);                          // and Rh is quantised 31 bits below the tile's column maximum
 }
 
 // ---- X digit planes (once per upload) ------------------------------------------------------------
@@ -311,8 +317,8 @@ k_batch_i8(const unsigned char *__restrict__ planes, const float *__restrict__ A
 #pragma unroll
                 for (int m = 0; m < 4; ++m) {
                     // z = 2^16 y + x exactly (|y| < 2^30, |x| < 2^31)
-                    fr[m] = fma(i2d(a6[2 * m] * 256 + a5[2 * m]), 65536.0, i2d(a4[2 * m] * 256 + a3[2 * m]));
-                    fi[m] = fma(i2d(a6[2 * m + 1] * 256 + a5[2 * m + 1]), 65536.0, i2d(a4[2 * m + 1] * 256 + a3[2 * m + 1]));
+                    fr[m] = z48(a6[2 * m], a5[2 * m], a4[2 * m], a3[2 * m]);
+                    fi[m] = z48(a6[2 * m + 1], a5[2 * m + 1], a4[2 * m + 1], a3[2 * m + 1]);
                     I[m] = fma(fr[m], fr[m], fi[m] * fi[m]);
                     cancel |= I[m] < thr2 && 16 * j + 4 * ch + m < Kc;
                 }
@@ -465,7 +471,7 @@ k_batch_i8(const unsigned char *__restrict__ planes, const float *__restrict__ A
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     // Z / s with Z = 2^16 (2^8 a6 + a5) + (2^8 a4 + a3): the four levels combined exactly in fp64 (|Z| < 2^48), one fused accumulation
-                    const double Z = fma(i2d(a6[i] * 256 + a5[i]), 65536.0, i2d(a4[i] * 256 + a3[i]));
+                    const double Z = z48(a6[i], a5[i], a4[i], a3[i]);
                     Tacc[8 * ch + i] = fma(Z, inv[i >> 1], Tacc[8 * ch + i]);
                 }
             }

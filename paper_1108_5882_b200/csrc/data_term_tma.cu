@@ -112,17 +112,17 @@ __device__ __forceinline__ double fast_rcp(double x)
 
 // Resident mode (RES; for small samples the per-iteration cost is latency, not bandwidth): the grid stays on the GPU
 // between evaluations and is driven through a mailbox instead of launches.  cmd_host: device-mapped pinned HOST memory,
-// 4n words of (tag << 32 | 32 bits of V), tag = low half of the evaluation's sequence number; cmd_dev: device memory,
-// [0] = sequence number, [1 .. 2n] = V.  Warp 0 of CTA 0 polls cmd_host over PCIe (one round trip per poll: the command is
-// complete when all words carry the new tag), copies V to cmd_dev and publishes the number there; the other CTAs poll
-// cmd_dev (L2).  The record goes back the same way (FinishArgs::tagged: tag << 32 | half a double per word, no fence and
-// no flag: the host has the record when every word carries the tag).  An evaluation is then exactly the body of the launched kernel (same grid, same tiles per CTA, same
-// reduction tree: bitwise the same result), and its finishing block publishes the record with that sequence number.  The
-// host sends the next command only after it has seen the record, so the evaluations of a grid never overlap.
-// kQuit as sequence number, or ~2 s without a command, ends the grid.
+// 4n words of (tag << 32 | 32 bits of V), tag = low half of the evaluation's sequence number; cmd_dev: the same words in
+// device memory.  Warp 0 of block 0 polls cmd_host over PCIe (one round trip per poll: the command is complete when all
+// words carry the new tag) and forwards the words to cmd_dev, which warp 0 of every other block polls in L2 the same way.
+// The record goes back the same way (FinishArgs::tagged: tag << 32 | half a double per word, no fence and no flag: the
+// host has the record when every word carries the tag).  An evaluation is exactly the body of the launched kernel (same
+// grid, same tiles per CTA, same reduction tree: bitwise the same result).  The host sends the next command only after it
+// has seen the record, so the evaluations of a grid never overlap.  Tag 0xffffffff in every word, or ~2 s without a
+// command, ends the grid.
 struct ResidentArgs {
     const unsigned long long *cmd_host;      // mapped host mailbox (read with system-scope volatile loads)
-    unsigned long long *cmd_dev;             // device copy: [0] = sequence number, [1 ..] = V
+    unsigned long long *cmd_dev;             // device copy of the mailbox (forwarded by block 0)
     unsigned long long start_seq;            // sequence number at launch (commands have larger numbers)
 };
 // tag 0xffffffff in the mailbox = quit (the host never uses it for a command)
@@ -155,6 +155,7 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     __shared__ volatile unsigned issued[NGRP][NS];     // number of tiles issued into each stage so far (GW > 1)
     __shared__ __align__(16) double rbuf[NWARPS][32][2];
     __shared__ __align__(16) double sV[2 * NW];
+    __shared__ __align__(16) double s_mv_early[2 * NW];
     __shared__ unsigned long long s_seq;
     FinishArgs fa = fa_in;
     if (!RES) for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = varg.v[t];
@@ -173,47 +174,45 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     for (int pass = 0;; ++pass) {                                 // one pass per evaluation (a single pass unless RES)
     if (RES) {
         if (warp == 0) {
-            unsigned long long seq = 0;
+            // The mailbox is 4 NW words (tag << 32 | 32 bits of V); a command is complete when every word carries the same
+            // new tag (8-byte stores and loads are single transactions, any arrival order is fine): ONE round trip per poll,
+            // no flag behind a fence.  Block 0 polls the host's mailbox over PCIe and forwards the words to the device
+            // copy, which the other blocks poll in L2 with the same protocol.
+            constexpr int WPL = (4 * NW + 31) / 32;                      // words per lane
+            const unsigned long long *src = blockIdx.x == 0 ? res.cmd_host : res.cmd_dev;
+            const unsigned limit = blockIdx.x == 0 ? (1u << 20) : (1u << 26);     // block 0: ~2 s of PCIe polls without a command
+            unsigned long long w[WPL];
+            unsigned tag = 0;
+            for (unsigned spins = 0;; ++spins) {
+                bool same = true;
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) {
+                    const int k = lane + 32 * j;
+                    w[j] = ld_sys_u64(src + (k < 4 * NW ? k : 0));
+                }
+                tag = __shfl_sync(0xffffffffu, (unsigned)(w[0] >> 32), 0);
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) same = same && (unsigned)(w[j] >> 32) == tag;
+                if (__all_sync(0xffffffffu, same) && tag != (unsigned)last_seq) break;
+                if (spins > limit) {
+                    tag = 0xffffffffu;
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) w[j] = 0xffffffff00000000ull;
+                    break;
+                }
+                if (blockIdx.x != 0) __nanosleep(40);
+            }
             if (blockIdx.x == 0) {
-                // One PCIe round trip per poll: the mailbox is 4 NW words (tag << 32 | 32 bits of V); a command is complete
-                // when every word carries the same new tag (8-byte stores and loads are atomic, any arrival order is fine).
-                constexpr int WPL = (4 * NW + 31) / 32;                  // words per lane
-                unsigned long long w[WPL];
-                unsigned tag = 0;
-                for (unsigned spins = 0;; ++spins) {
-                    bool same = true;
 #pragma unroll
-                    for (int j = 0; j < WPL; ++j) {
-                        const int k = lane + 32 * j;
-                        w[j] = ld_sys_u64(res.cmd_host + (k < 4 * NW ? k : 0));
-                    }
-                    tag = __shfl_sync(0xffffffffu, (unsigned)(w[0] >> 32), 0);
-#pragma unroll
-                    for (int j = 0; j < WPL; ++j) same = same && (unsigned)(w[j] >> 32) == tag;
-                    if (__all_sync(0xffffffffu, same) && tag != (unsigned)last_seq) break;
-                    if (spins > (1u << 20)) { tag = 0xffffffffu; break; }       // ~2 s of PCIe polls without a command
-                }
-                if (tag == 0xffffffffu) seq = kQuit;
-                else {
-                    seq = last_seq + (unsigned long long)(unsigned)(tag - (unsigned)last_seq);
-                    unsigned *dst = reinterpret_cast<unsigned *>(res.cmd_dev + 1);
-#pragma unroll
-                    for (int j = 0; j < WPL; ++j) { const int k = lane + 32 * j; if (k < 4 * NW) dst[k] = (unsigned)w[j]; }
-                }
-                __threadfence();
-                __syncwarp();
-                if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(res.cmd_dev) = seq;
-            } else {
-                if (lane == 0) {
-                    for (unsigned spins = 0;; ++spins) {
-                        seq = ld_sys_u64(res.cmd_dev);
-                        if (seq != last_seq) break;
-                        if (spins > (1u << 26)) { seq = kQuit; break; }
-                        __nanosleep(40);
-                    }
+                for (int j = 0; j < WPL; ++j) {
+                    const int k = lane + 32 * j;
+                    if (k < 4 * NW) *reinterpret_cast<volatile unsigned long long *>(res.cmd_dev + k) = w[j];
                 }
             }
-            if (lane == 0) s_seq = seq;
+            unsigned *sV32 = reinterpret_cast<unsigned *>(sV);
+#pragma unroll
+            for (int j = 0; j < WPL; ++j) { const int k = lane + 32 * j; if (k < 4 * NW) sV32[k] = (unsigned)w[j]; }
+            if (lane == 0) s_seq = tag == 0xffffffffu ? kQuit : last_seq + (unsigned long long)(unsigned)(tag - (unsigned)last_seq);
         }
         __syncthreads();
         const unsigned long long seq = s_seq;
@@ -221,8 +220,6 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
         last_seq = seq;
         fa.seq = seq;
         fa.tag = (unsigned)seq;
-        __threadfence();
-        for (int t = threadIdx.x; t < 2 * NW; t += THREADS) sV[t] = __longlong_as_double((long long)ld_sys_u64(res.cmd_dev + 1 + t));
     }
     if (pass == 0 && wig == 0 && lane == 0) {
 #pragma unroll
@@ -261,6 +258,9 @@ k_data_term_tma(const __grid_constant__ CUtensorMap tmap, long long N, long long
     if (lane == 0) {
         for (long long t = wig; t < NS && t < nt_grp; t += GW) issue(t);
     }
+    // (M V) of step A7 while the first tiles are in flight: every block forms it (n^2 complex multiply-adds from the
+    // L2-resident M), the block that finishes last uses its copy, and the finish loses a dependent L2 round trip
+    if (fa.M != nullptr) { compute_mv(fa.M, sV, NW, s_mv_early); fa.mv_ready = s_mv_early; }
 
     // phase-1 coordinates: lane -> (row, part)
     const int row1 = lane % TR, part = lane / TR;

@@ -194,10 +194,12 @@ static pwa_status resident_start(pwa_ctx *ctx, bool *started)
 {
     if ((unsigned)ctx->seq == kResidentQuitTag) ++ctx->seq;
     mailbox_fill(ctx, (unsigned)ctx->seq);                      // commands carry later numbers
-    // the device copy of the sequence number starts at the same value (the CTAs other than CTA 0 poll it)
+    // the device copy of the mailbox starts with the same tags (staged through h_V: the host may write the first command
+    // into h_cmd before the copy has run)
     if (ctx->ev_V_pending) { PWA_CUDA(ctx, cudaEventSynchronize(ctx->ev_V)); ctx->ev_V_pending = false; }
-    memcpy(ctx->h_V, &ctx->seq, sizeof(unsigned long long));
-    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_cmd, ctx->h_V, sizeof(unsigned long long), cudaMemcpyHostToDevice, ctx->stream));
+    unsigned long long *stage = reinterpret_cast<unsigned long long *>(ctx->h_V);
+    for (int k = 0; k < 4 * ctx->n; ++k) stage[k] = (unsigned long long)(unsigned)ctx->seq << 32;
+    PWA_CUDA(ctx, cudaMemcpyAsync(ctx->d_cmd, stage, sizeof(unsigned long long) * 4 * (size_t)ctx->n, cudaMemcpyHostToDevice, ctx->stream));
     PWA_CUDA(ctx, cudaEventRecord(ctx->ev_V, ctx->stream));
     ctx->ev_V_pending = true;
     pwa_status s = launch_resident(ctx, started);
@@ -340,8 +342,8 @@ pwa_status pwa_create(pwa_ctx **out, int32_t n_waves, pwa_dtype storage, int32_t
     if (e == cudaSuccess) e = cudaHostAlloc(&ctx->h_rres, sizeof(unsigned long long) * rres_words, cudaHostAllocMapped);
     if (e == cudaSuccess) e = cudaHostGetDevicePointer(&ctx->dev_rres, ctx->h_rres, 0);
     if (e == cudaSuccess) memset(ctx->h_rres, 0, sizeof(unsigned long long) * rres_words);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_cmd, sizeof(unsigned long long) * (1 + 2 * (size_t)kMaxFastWaves));
-    if (e == cudaSuccess) e = cudaMemset(ctx->d_cmd, 0, sizeof(unsigned long long) * (1 + 2 * (size_t)kMaxFastWaves));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_cmd, sizeof(unsigned long long) * cmd_words);
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_cmd, 0, sizeof(unsigned long long) * cmd_words);
     // per-block partial slots of every single-V pass (data term: 2 + 2n components, resonance gradient: up to
     // 2 + 4 kMaxRes), sized here for the largest grid any launcher uses (<= 16 blocks per SM), so that no
     // evaluation call ever allocates (pwa.h, general rules)

@@ -29,6 +29,7 @@ struct FinishArgs {
     // system-scope fence nor a flag is needed
     unsigned long long *tagged = nullptr;
     unsigned tag = 0;
+    const double *mv_ready = nullptr;     // (M V) already formed by this block in its shared memory (compute_mv), or nullptr
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m)
@@ -43,40 +44,13 @@ __device__ __forceinline__ double warp_sum(double x)
     return x;
 }
 
-// Step A7 from block totals s_tot[0..2+2n) = {L_data, n_nonfinite, Re T_0, Im T_0, ...} and V in
-// shared memory: M == nullptr -> copy the data-term components to out[0..2+2n); otherwise write
-// the result record {nll, L_data, Norm, n_nonfinite, grad[2n]} (P:41 second term, P:55).
-// Must be called by every thread of the block; s_tot and sV valid for all threads on entry.
-// eq2 false: nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V                      (eq. 3, P:41)
-// eq2 true, n_eq2 = N_data (or sum of weights): nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2, P:33)
-__device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
-                                            double *out, int n, bool eq2 = false, double n_eq2 = 0.0,
-                                            unsigned long long *done_flag = nullptr, unsigned long long seq = 0,
-                                            unsigned long long *tagged = nullptr, unsigned tag = 0)
+// (M V)_a -> s_mv[2a], s_mv[2a + 1] (shared memory, 2n doubles).  Must be called by every thread of the block; the caller
+// synchronises the block before s_mv is read.  `slices` adjacent lanes share a row (coalesced reads of M, all loads
+// independent), partial dot products are combined with a fixed xor tree: the result depends on (n, blockDim) only, so a
+// kernel may form it early (while its first tiles are in flight) and hand it to assemble_from_totals as mv_ready.
+__device__ inline void compute_mv(const double *M, const double *sV, int n, double *s_mv)
 {
-    auto put = [&](int idx, double v) {
-        if (tagged != nullptr) {
-            const unsigned long long t = (unsigned long long)tag << 32;
-            volatile unsigned long long *p = tagged + 2 * idx;
-            p[0] = t | (unsigned)__double2loint(v);
-            p[1] = t | (unsigned)__double2hiint(v);
-        } else out[idx] = v;
-    };
-    const int NC = 2 + 2 * n;
     const int tid = threadIdx.x, nthreads = blockDim.x;
-    const int lane = tid & 31, warp = tid >> 5;
-    __shared__ double s_mv[2 * kMaxWaves];
-    if (M == nullptr) {
-        for (int c = tid; c < NC; c += nthreads) out[c] = s_tot[c];
-        if (done_flag != nullptr) {                 // record in mapped host memory: visible to the host before the flag
-            __threadfence_system();
-            __syncthreads();
-            if (tid == 0) *reinterpret_cast<volatile unsigned long long *>(done_flag) = seq;
-        }
-        return;
-    }
-    // (M V)_a: `slices` adjacent lanes share a row (coalesced reads of M, all loads independent),
-    // partial dot products are combined with a fixed xor tree
     int slices = 1;
     while (slices * 2 <= 32 && slices * 2 * n <= nthreads && slices * 2 <= n) slices *= 2;
     const int rows_per_pass = nthreads / slices;
@@ -97,6 +71,43 @@ __device__ inline void assemble_from_totals(const double *s_tot, const double *s
         for (int m = 1; m < slices; m <<= 1) { mr += shfl_xor_d(mr, m); mi += shfl_xor_d(mi, m); }
         if (a < n && sl == 0) { s_mv[2 * a] = mr; s_mv[2 * a + 1] = mi; }
     }
+}
+
+// Step A7 from block totals s_tot[0..2+2n) = {L_data, n_nonfinite, Re T_0, Im T_0, ...} and V in
+// shared memory: M == nullptr -> copy the data-term components to out[0..2+2n); otherwise write
+// the result record {nll, L_data, Norm, n_nonfinite, grad[2n]} (P:41 second term, P:55).
+// Must be called by every thread of the block; s_tot and sV valid for all threads on entry.
+// eq2 false: nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V                      (eq. 3, P:41)
+// eq2 true, n_eq2 = N_data (or sum of weights): nll = -L_data + N_data ln Norm, grad = -2 conj(T) + (2 N_data / Norm) M V   (eq. 2, P:33)
+__device__ inline void assemble_from_totals(const double *s_tot, const double *sV, const double *M,
+                                            double *out, int n, bool eq2 = false, double n_eq2 = 0.0,
+                                            unsigned long long *done_flag = nullptr, unsigned long long seq = 0,
+                                            unsigned long long *tagged = nullptr, unsigned tag = 0,
+                                            const double *mv_ready = nullptr)
+{
+    auto put = [&](int idx, double v) {
+        if (tagged != nullptr) {
+            const unsigned long long t = (unsigned long long)tag << 32;
+            volatile unsigned long long *p = tagged + 2 * idx;
+            p[0] = t | (unsigned)__double2loint(v);
+            p[1] = t | (unsigned)__double2hiint(v);
+        } else out[idx] = v;
+    };
+    const int NC = 2 + 2 * n;
+    const int tid = threadIdx.x, nthreads = blockDim.x;
+    const int lane = tid & 31, warp = tid >> 5;
+    __shared__ double s_mv_own[2 * kMaxWaves];
+    if (M == nullptr) {
+        for (int c = tid; c < NC; c += nthreads) out[c] = s_tot[c];
+        if (done_flag != nullptr) {                 // record in mapped host memory: visible to the host before the flag
+            __threadfence_system();
+            __syncthreads();
+            if (tid == 0) *reinterpret_cast<volatile unsigned long long *>(done_flag) = seq;
+        }
+        return;
+    }
+    if (mv_ready == nullptr) compute_mv(M, sV, n, s_mv_own);
+    const double *s_mv = mv_ready != nullptr ? mv_ready : s_mv_own;
     __syncthreads();
     if (warp == 0) {
         double acc = 0.0;   // Norm = sum_a Re( conj(V_a) (M V)_a )
@@ -190,7 +201,7 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
     if (tid == 0) { *fa.ticket = 0u; __threadfence(); }
     __syncthreads();
 
-    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq, fa.tagged, fa.tag);
+    assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq, fa.tagged, fa.tag, fa.mv_ready);
 }
 
 constexpr int kFastWaves = 64;   // == kMaxFastWaves (pwa_internal.h)

@@ -155,6 +155,10 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
     if (tid == 0) s_last = (atomicAdd(fa.ticket, 1u) == gridDim.x - 1);
     __syncthreads();
     if (!s_last) return;
+    // every block has arrived: re-arm the ticket for the next evaluation here, ahead of the fence below and long BEFORE the
+    // record is published (in a resident grid the host may send the next command as soon as it sees the record, and the
+    // first blocks of that evaluation must find the ticket at zero)
+    if (tid == 0) *fa.ticket = 0u;
     __threadfence();
 
     // `ngroups` groups of NC adjacent threads: group g adds slots g, g + ngroups, ... of its
@@ -196,9 +200,6 @@ __device__ inline void block_finish(double *s_tot, double *s_red, const double *
             s_tot[c] = acc;
         }
     }
-    // re-arm the ticket for the next evaluation BEFORE the record is published: in a resident grid the host may send the
-    // next command as soon as it sees the record, and the first CTAs of that evaluation must find the ticket at zero
-    if (tid == 0) { *fa.ticket = 0u; __threadfence(); }
     __syncthreads();
 
     assemble_from_totals(s_tot, sV, fa.M, fa.out, n, fa.eq2, fa.n_eq2, fa.done_flag, fa.seq, fa.tagged, fa.tag, fa.mv_ready);

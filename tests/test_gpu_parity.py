@@ -128,6 +128,16 @@ def test_empty_inputs(pwa):
         assert np.all(M == 0)
         nll, g, parts = pwa.pwa_nll_grad(c.ctx, np.ones((n, 2)))
         assert nll == 0.0 and np.all(g == 0) and parts[0] == 0.0 and parts[1] == 0.0
+    for n, storage in ((16, "f64"), (32, "f32")):          # shapes of the TMA kernel, launched and through the resident grid
+        with Ctx(pwa, n, storage) as c:
+            pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, np.zeros((0, n, 2), dtype=np.float64 if storage == "f64" else np.float32), n_events=0)
+            M0 = np.zeros((n, n, 2)); M0[np.arange(n), np.arange(n), 0] = 1.0
+            pwa.pwa_set_norm(c.ctx, M0)
+            V = np.random.default_rng(3).normal(size=(n, 2))
+            for resident in (0, 1):
+                pwa.pwa_set_option(c.ctx, "resident", resident)
+                nll, g, parts = pwa.pwa_nll_grad(c.ctx, V)
+                assert parts[0] == 0.0 and nll == pytest.approx(np.sum(V * V), rel=1e-14) and np.allclose(g, 2.0 * V, rtol=1e-14)
 
 
 def test_call_order_errors(pwa):

@@ -204,6 +204,16 @@ def grad_polar(V, grad):
     return out
 
 
+def fix_phase(V, grad=None, ref=0):
+    """Fixed-phase gauge: -> (V', grad') with wave `ref` real and non-negative, the gradient turned by the same angle and its
+    d/d Im V_ref component dropped (0).  grad=None -> (V', None)."""
+    n = np.asarray(V).shape[0]
+    V2 = _f64(V, (n, 2)).copy()
+    g2 = None if grad is None else _f64(grad, (n, 2)).copy()
+    lib().pwa_oracle_fix_phase(C.c_int(n), C.c_int(int(ref)), _p(V2), None if g2 is None else _p(g2))
+    return V2, g2
+
+
 def fumili(A, V, M=None):
     """Fumili-style approximate Hessian [2n, 2n] in the (x_0, y_0, x_1, ...) order; M=None -> data part only."""
     A, dt = _amp(A)

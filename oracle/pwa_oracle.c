@@ -39,7 +39,8 @@
  * restatement, PSD, Hess(Norm) vs differences of the norm gradient; P16 event weights: unit weights,
  * integer weights = duplicated events, numpy restatement, linearity in w; P17 the sampled entry points
  * (norm_block / norm_block_w with a0, b0 > 0, fumili_rows with p0 > 0): bitwise equal to the same entries of
- * the full result, zero outside, numpy restatement of the block.
+ * the full result, zero outside, numpy restatement of the block; P18 fixed-phase gauge: nll unchanged, the turned
+ * gradient equals the gradient evaluated at the turned V, relative phases kept, gauge identity sum_a (x g_y - y g_x) = 0.
  * Parity unpinned by the paper: the choices C2, C3, C4, C5, C9-C13 (definitions, not
  * results), and the resonance-parameter gradient beyond finite differences (P5/P10 style).
  *
@@ -358,6 +359,28 @@ void pwa_oracle_grad_polar(int n, const double *V, const double *grad, double *o
         out[2 * a]     = grad[2 * a] * cos(phi) + grad[2 * a + 1] * sin(phi);
         out[2 * a + 1] = -grad[2 * a] * r * sin(phi) + grad[2 * a + 1] * r * cos(phi);
     }
+}
+
+/* Fixed-phase gauge.  |S_i| and V^dagger M V do not change under V -> exp(i a) V, so nll
+ * (eq. 3 and eq. 2) has one flat direction.  The gauge "wave ref is real and non-negative" removes it: with
+ * a = -arg V_ref every V_a is turned by a; a Cartesian gradient, read as the complex number g_a = d/dx_a + i d/dy_a,
+ * turns by the same angle (nll(V) = nll(V') with V' = exp(i a) V gives g'(V') = exp(i a) g(V)); the component
+ * d/d Im V_ref belongs to the parameter the gauge fixes at zero and is dropped (set to 0).  In place; grad may be NULL. */
+void pwa_oracle_fix_phase(int n, int ref, double *V, double *grad)
+{
+    double a = -atan2(V[2 * ref + 1], V[2 * ref]);
+    for (int w = 0; w < n; ++w) {
+        double r = hypot(V[2 * w], V[2 * w + 1]), ph = atan2(V[2 * w + 1], V[2 * w]);
+        V[2 * w] = r * cos(ph + a);
+        V[2 * w + 1] = r * sin(ph + a);
+        if (grad) {
+            double gr = hypot(grad[2 * w], grad[2 * w + 1]), gp = atan2(grad[2 * w + 1], grad[2 * w]);
+            grad[2 * w] = gr * cos(gp + a);
+            grad[2 * w + 1] = gr * sin(gp + a);
+        }
+    }
+    V[2 * ref + 1] = 0.0;                     /* exactly on the gauge (sin of a rounded angle leaves ~1e-17 r) */
+    if (grad) grad[2 * ref + 1] = 0.0;
 }
 
 /* ---------- NEXT-2: Fumili-style approximate Hessian (ref. P:123) -----

@@ -507,6 +507,43 @@ def test_p14_polar_chain_rule(oracle):
     assert abs(gp[:, 1].sum()) <= 1e-10 * np.abs(gp).max()
 
 
+def test_p18_fixed_phase_gauge(oracle):
+    """P:85-87 / SURVEY NEXT-4: nll does not depend on a common phase of V; the gauge "wave ref real and >= 0".
+    (a) V' keeps every magnitude and every relative phase (V'_a |V_ref| = V_a conj(V_ref), complex arithmetic in numpy),
+    Im V'_ref = 0, Re V'_ref = |V_ref|; (b) nll(V') = nll(V) in both likelihood forms; (c) the turned gradient equals the
+    gradient the oracle evaluates AT V' (an independent evaluation), except for the dropped component, which is 0;
+    (d) gauge identity at any V: sum_a (x_a g_ya - y_a g_xa) = 0 (the derivative along the phase orbit), so the dropped
+    component carries no information: g'_y,ref = -sum_{a != ref} (x'_a g'_ya - y'_a g'_xa) / x'_ref; a wrong turning sense
+    of the gradient fails (c) and (d)."""
+    rng = np.random.default_rng(18)
+    N, Nacc, n = 350, 600, 5
+    A, B = rand_amps(rng, N, n), rand_amps(rng, Nacc, n)
+    M = oracle.norm_matrix(B, Nacc + 20)
+    for ref in (0, 3):
+        V = rng.normal(size=(n, 2))
+        f, g, parts, _ = oracle.nll_grad(A, M, V)
+        V2, g2 = oracle.fix_phase(V, g, ref)
+        Vc, V2c = cplx(V), cplx(V2)
+        assert V2[ref, 1] == 0.0 and V2[ref, 0] == pytest.approx(abs(Vc[ref]), rel=1e-15)
+        assert np.allclose(V2c * abs(Vc[ref]), Vc * np.conj(Vc[ref]), rtol=1e-14, atol=1e-15)
+        f2, gt, parts2, _ = oracle.nll_grad(A, M, V2)
+        assert f2 == pytest.approx(f, rel=1e-13) and parts2[1] == pytest.approx(parts[1], rel=1e-13)
+        e2, _, _ = oracle.nll_grad_eq2(A, M, V)
+        e2t, _, _ = oracle.nll_grad_eq2(A, M, V2)
+        assert e2t == pytest.approx(e2, rel=1e-13)
+        scale = np.abs(gt).max()
+        mask = np.ones((n, 2), bool)
+        mask[ref, 1] = False
+        assert np.abs(g2 - gt)[mask].max() <= 1e-11 * scale and g2[ref, 1] == 0.0
+        for VV, gg in ((V, g), (V2, gt)):
+            assert abs((VV[:, 0] * gg[:, 1] - VV[:, 1] * gg[:, 0]).sum()) <= 1e-10 * scale * np.abs(VV).max()
+        others = [a for a in range(n) if a != ref]
+        rec = -(V2[others, 0] * gt[others, 1] - V2[others, 1] * gt[others, 0]).sum() / V2[ref, 0]
+        assert rec == pytest.approx(gt[ref, 1], rel=1e-8, abs=1e-10 * scale)
+        Vonly, none = oracle.fix_phase(V, None, ref)
+        assert none is None and np.array_equal(Vonly, V2)
+
+
 # ---------------------------------------------------------------- P15 Fumili-style approximate Hessian (NEXT-2)
 def test_p15_fumili_matrix(oracle):
     """H_data = sum_i u_i u_i^T with u_i = grad ln I_i.  (a) numpy/BLAS restatement; (b) symmetric PSD;

@@ -216,6 +216,16 @@ pwa_status pwa_assemble_host_eq2(int32_t n_waves, double n_data, double L_data, 
 pwa_status pwa_grad_to_polar(int32_t n_waves, const double *V, const double *grad, double *grad_polar);
 pwa_status pwa_polar_to_cartesian(int32_t n_waves, const double *r_phi, double *V);
 
+/* Fixed-phase gauge, host only.  nll (eq. 3 and eq. 2) depends on V only up to a common phase:
+ * |S_i| and V^dagger M V do not change under V -> exp(i a) V, which leaves every fit one flat direction.  The gauge
+ * "wave ref_wave is real and non-negative" removes it.  pwa_fix_phase_host turns V[n][2] IN PLACE by
+ * exp(-i arg V_ref) (exact complex multiplication by conj(V_ref) / |V_ref|; Im V_ref is set to exactly 0); when grad
+ * is not NULL the Cartesian gradient grad[n][2], read as g_a = d/dRe V_a + i d/dIm V_a, is turned by the same factor
+ * (it is then the gradient at the turned V) and its component d/dIm V_ref, the parameter the gauge fixes, is set to 0.
+ * V_ref = 0 leaves V and grad unturned (only the component is zeroed).  PWA_ERR_INVALID_ARG for ref_wave outside
+ * [0, n_waves).  The minimisers apply the gauge themselves with pwa_set_option(ctx, "fix_phase", ref_wave + 1).     */
+pwa_status pwa_fix_phase_host(int32_t n_waves, int32_t ref_wave, double *V, double *grad);
+
 /* Floating mode: gradient of nll w.r.t. the resonance parameters at the current
  * (mass0, width0) and the given V (reading A9):  d nll / d M_r and d nll / d G_r, HOST
  * [n_res] each (n_res of pwa_set_wave_map: see pwa_n_res).  Needs factored DATA and MC uploads.  One extra pass
@@ -299,7 +309,7 @@ uint64_t pwa_launch_count(const pwa_ctx *ctx);
 pwa_status pwa_sync(pwa_ctx *ctx);
 
 /* Selects a kernel family (0 = default).  Returns PWA_ERR_INVALID_ARG for unknown keys.
- * Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood", "resident".
+ * Keys: "data_term", "norm", "batch", "l2_resident_mb", "likelihood", "resident", "fix_phase".
  * "data_term": 0 = default (TMA-tiled streaming kernel where the row is 128 .. 1024 bytes and the sample carries no
  * event weights, else the per-lane streaming kernel), 20 = per-lane kernel, 98 = default without programmatic
  * dependent launch, 99 = generic kernel (any n).
@@ -312,6 +322,10 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * samples between 64 MB and 1 GiB, else plain loads), 0 = plain loads, up to 120.
  * "likelihood": 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form (see
  * pwa_assemble_host_eq2); applies to pwa_nll_grad, pwa_nll_grad_batch, pwa_res_grad and the minimisers.
+ * "fix_phase": 0 = the minimisers leave all 2n real parameters free (default); k in 1 .. n = pwa_minimize_bfgs,
+ * pwa_minimize_bfgs_batch(_ex) and pwa_minimize_bfgs_floating(_ex) fit in the gauge Im V_(k-1) = 0, Re V_(k-1) >= 0 at
+ * the start (pwa_fix_phase_host on every starting point, the gauge component of every gradient set to 0: 2n - 1 free
+ * real parameters per fit, the returned V has Im V_(k-1) = 0 exactly).  Evaluation calls are not affected.
  * "resident": 0 = every evaluation is a kernel launch (default); 1 = pwa_nll_grad evaluates through a RESIDENT grid
  * (below ~1e5 events an iteration costs latency, not bandwidth): the default data-term kernel is
  * launched once, stays on the GPU and takes V / returns the record through tagged 8-byte words in pinned host memory,

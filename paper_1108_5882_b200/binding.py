@@ -29,7 +29,7 @@ SYMBOLS = [
     "pwa_nll_grad_batch_enqueue", "pwa_fetch", "pwa_data_term_enqueue", "pwa_assemble_host",
     "pwa_res_grad", "pwa_minimize_bfgs", "pwa_minimize_bfgs_batch", "pwa_n_waves",
     "pwa_launch_count", "pwa_sync", "pwa_set_option", "pwa_microbench", "pwa_norm_error_bound",
-    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fumili_hessian", "pwa_set_weights",
+    "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fix_phase_host", "pwa_fumili_hessian", "pwa_set_weights",
     "pwa_batch_path", "pwa_minimize_bfgs_floating", "pwa_minimize_bfgs_batch_ex", "pwa_minimize_bfgs_floating_ex",
     "pwa_n_res", "pwa_nll_grad_floating", "pwa_get_option", "pwa_storage", "pwa_n_events", "pwa_norm_sums", "pwa_combine_norm_host", "pwa_assemble_host_shards",
 ]
@@ -81,6 +81,7 @@ def _load():
         "pwa_fumili_hessian": (C.c_int, [vp, vp, vp, i32]),
         "pwa_set_weights": (C.c_int, [vp, C.c_int, vp, u32]),
         "pwa_polar_to_cartesian": (C.c_int, [i32, vp, vp]),
+        "pwa_fix_phase_host": (C.c_int, [i32, i32, vp, vp]),
         "pwa_batch_path": (C.c_int, [vp, C.POINTER(i32), dp]),
         "pwa_minimize_bfgs_floating": (C.c_int, [vp, vp, vp, vp, i32, vp, i32, i32, C.c_double, dp,
                                                  C.POINTER(i32), C.POINTER(i32)]),
@@ -351,6 +352,21 @@ def pwa_grad_to_polar(V, grad):
     out = np.zeros((n, 2))
     _check(None, _lib.pwa_grad_to_polar(n, V.ctypes.data, grad.ctypes.data, out.ctypes.data))
     return out
+
+
+def pwa_fix_phase_host(V, grad=None, ref_wave=0):
+    """-> (V', grad') in the gauge Im V_ref = 0, Re V_ref >= 0 (copies; grad' is None when grad is None)."""
+    V = np.array(V, dtype=np.float64, order="C")
+    n = V.shape[0]
+    if V.shape != (n, 2):
+        raise ValueError(f"V must be [n, 2], got {V.shape}")
+    g = None
+    if grad is not None:
+        g = np.array(grad, dtype=np.float64, order="C")
+        if g.shape != (n, 2):
+            raise ValueError(f"grad must be [{n}, 2], got {g.shape}")
+    _check(None, _lib.pwa_fix_phase_host(n, int(ref_wave), V.ctypes.data, None if g is None else g.ctypes.data))
+    return V, g
 
 
 def pwa_polar_to_cartesian(r_phi):

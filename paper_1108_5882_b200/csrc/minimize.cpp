@@ -114,12 +114,20 @@ pwa_status pwa_minimize_bfgs_batch_ex(pwa_ctx *ctx, int32_t K, double *V, int32_
     std::vector<int> act(K);                    // the fits evaluated by the current batched calls (all K in the first stage)
     for (int k = 0; k < K; ++k) act[k] = k;
     memcpy(X.data(), V, sizeof(double) * (size_t)K * d);
+    // fixed-phase gauge ("fix_phase" = ref + 1): every starting point is turned so that Im V_ref = 0, and the
+    // component d/dIm V_ref of every gradient is dropped.  BFGS then never moves that coordinate (its row of the inverse
+    // Hessian stays the identity row, because the step and the gradient difference are zero there).
+    int32_t gauge = 0;
+    if (pwa_get_option(ctx, "fix_phase", &gauge) != PWA_OK) gauge = 0;
+    const int ref = gauge - 1;
+    if (ref >= 0) for (int k = 0; k < K; ++k) pwa_fix_phase_host(n, ref, X.data() + (size_t)k * d, nullptr);
     int32_t evals = 0;
     pwa_status worst = PWA_OK;
     auto eval = [&]() -> pwa_status {            // evaluates rows 0 .. act.size()-1 of X
         const int Ka = (int)act.size();
         pwa_status s = (Ka == 1) ? pwa_nll_grad(ctx, X.data(), F.data(), Gr.data(), Pt.data())
                                  : pwa_nll_grad_batch(ctx, Ka, X.data(), F.data(), Gr.data(), Pt.data());
+        if (ref >= 0) for (int j = 0; j < Ka; ++j) Gr[(size_t)j * d + 2 * ref + 1] = 0.0;
         evals += 1;
         if (s == PWA_WARN_NONFINITE) { worst = s; return PWA_OK; }
         return s;
@@ -244,6 +252,10 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
     // likelihood has one local minimum per assignment of resonances to peaks)
     std::vector<double> x(d), u(d), sc(d, 1.0), g(d), Mr(mass, mass + n_res), Gr(width, width + n_res), dM(n_res), dG(n_res);
     memcpy(x.data(), V, sizeof(double) * 2 * n);
+    int32_t gauge = 0;                               // fixed-phase gauge of V, as in pwa_minimize_bfgs_batch_ex
+    if (pwa_get_option(ctx, "fix_phase", &gauge) != PWA_OK) gauge = 0;
+    const int ref = gauge - 1;
+    if (ref >= 0) pwa_fix_phase_host(n, ref, x.data(), nullptr);
     for (int i = 0; i < n_free; ++i) {
         x[2 * n + i] = mass[free_res[i]]; x[2 * n + n_free + i] = width[free_res[i]];
         sc[2 * n + i] = 0.01 * fabs(mass[free_res[i]]); sc[2 * n + n_free + i] = 0.02 * fabs(width[free_res[i]]);
@@ -275,6 +287,7 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
                 if (s != PWA_OK) return s;
                 for (int i = 0; i < n_free; ++i) { gg[2 * n + i] = dM[free_res[i]]; gg[2 * n + n_free + i] = dG[free_res[i]]; }
                 for (int i = 0; i < d; ++i) gg[i] *= sc[i];
+                if (ref >= 0) gg[2 * ref + 1] = 0.0;
                 return PWA_OK;
             }
         }
@@ -293,6 +306,7 @@ pwa_status pwa_minimize_bfgs_floating_ex(pwa_ctx *ctx, double *V, double *mass, 
             for (int i = 0; i < n_free; ++i) { gg[2 * n + i] = dM[free_res[i]]; gg[2 * n + n_free + i] = dG[free_res[i]]; }
         }
         for (int i = 0; i < d; ++i) gg[i] *= sc[i];       // d f / d u
+        if (ref >= 0) gg[2 * ref + 1] = 0.0;
         return PWA_OK;
     };
     Bfgs fit;

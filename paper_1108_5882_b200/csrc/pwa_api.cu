@@ -774,6 +774,27 @@ pwa_status pwa_grad_to_polar(int32_t n, const double *V, const double *grad, dou
     return PWA_OK;
 }
 
+pwa_status pwa_fix_phase_host(int32_t n, int32_t ref, double *V, double *grad)
+{
+    if (n < 1 || ref < 0 || ref >= n || !V) return PWA_ERR_INVALID_ARG;
+    const double xr = V[2 * ref], yr = V[2 * ref + 1], r = hypot(xr, yr);
+    if (r > 0.0) {
+        const double c = xr / r, s = -yr / r;                       // exp(-i arg V_ref) = conj(V_ref) / |V_ref|
+        for (int a = 0; a < n; ++a) {
+            const double x = V[2 * a], y = V[2 * a + 1];
+            V[2 * a] = x * c - y * s; V[2 * a + 1] = x * s + y * c;
+            if (grad) {
+                const double gx = grad[2 * a], gy = grad[2 * a + 1];
+                grad[2 * a] = gx * c - gy * s; grad[2 * a + 1] = gx * s + gy * c;
+            }
+        }
+        V[2 * ref] = r;
+    }
+    V[2 * ref + 1] = 0.0;
+    if (grad) grad[2 * ref + 1] = 0.0;
+    return PWA_OK;
+}
+
 pwa_status pwa_polar_to_cartesian(int32_t n, const double *r_phi, double *V)
 {
     if (n < 1 || !r_phi || !V) return PWA_ERR_INVALID_ARG;
@@ -879,6 +900,7 @@ pwa_status pwa_set_option(pwa_ctx *ctx, const char *key, int32_t value)
     else if (!strcmp(key, "l2_resident_mb")) { if (value < -1 || value > 120) return fail(ctx, PWA_ERR_INVALID_ARG, "l2_resident_mb must be in [-1, 120]"); ctx->opt_l2_resident_mb = value; }
     else if (!strcmp(key, "resident")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "resident must be 0 or 1"); ctx->opt_resident = value != 0; }
     else if (!strcmp(key, "likelihood")) { if (value != 0 && value != 1) return fail(ctx, PWA_ERR_INVALID_ARG, "likelihood must be 0 (eq. 3) or 1 (eq. 2)"); ctx->opt_likelihood = value; }
+    else if (!strcmp(key, "fix_phase")) { if (value < 0 || value > ctx->n) return fail(ctx, PWA_ERR_INVALID_ARG, "fix_phase must be 0 (off) or a wave number 1 .. n"); ctx->opt_fix_phase = value; }
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
 }
@@ -892,6 +914,7 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value)
     else if (!strcmp(key, "l2_resident_mb")) *value = ctx->opt_l2_resident_mb;
     else if (!strcmp(key, "resident")) *value = ctx->opt_resident ? 1 : 0;
     else if (!strcmp(key, "likelihood")) *value = ctx->opt_likelihood;
+    else if (!strcmp(key, "fix_phase")) *value = ctx->opt_fix_phase;
     else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown option key");
     return PWA_OK;
 }

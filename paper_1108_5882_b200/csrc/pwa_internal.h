@@ -91,6 +91,7 @@ struct pwa_ctx {
     int opt_data_term = 0, opt_norm = 0, opt_batch = 0;
     int opt_l2_resident_mb = -1;              // MB of the data sample's head kept in L2 between evaluations (TMA data term); -1 = automatic, 0 = off
     int opt_likelihood = 0;                   // 0 = eq. 3 extended form (default), 1 = eq. 2 normalised form
+    int opt_fix_phase = 0;                    // minimisers: 0 = all parameters free, k = gauge Im V_(k-1) = 0 (pwa_fix_phase_host)
     std::string err;
 };
 

@@ -108,3 +108,26 @@ def test_eq2_and_polar_host_twins_match_oracle(binding):
     assert np.abs(gp - oracle.grad_polar(V, g)).max() <= 1e-13 * np.abs(gp).max()
     r_phi = np.stack([np.hypot(V[:, 0], V[:, 1]), np.arctan2(V[:, 1], V[:, 0])], axis=-1)
     assert np.allclose(binding.pwa_polar_to_cartesian(r_phi), V, rtol=1e-14, atol=1e-15)
+
+
+def test_fix_phase_host_matches_oracle(binding):
+    """NEXT-4: the fixed-phase gauge (pwa_fix_phase_host, plain complex multiplication) against the oracle (angle
+    arithmetic), including the gradient, a reference wave that is already real, V_ref = 0 and the argument checks."""
+    from oracle import oracle
+    rng = np.random.default_rng(43)
+    n = 7
+    for ref in (0, 4, n - 1):
+        V, g = rng.normal(size=(n, 2)), rng.normal(size=(n, 2)) * 50.0
+        V2, g2 = binding.pwa_fix_phase_host(V, g, ref)
+        Vo, go = oracle.fix_phase(V, g, ref)
+        assert np.abs(V2 - Vo).max() <= 1e-14 * np.abs(V).max() and np.abs(g2 - go).max() <= 1e-13 * np.abs(g).max()
+        assert V2[ref, 1] == 0.0 and V2[ref, 0] > 0.0 and g2[ref, 1] == 0.0
+        V3, none = binding.pwa_fix_phase_host(V2, None, ref)            # already in the gauge: unchanged to rounding
+        assert none is None and np.abs(V3 - V2).max() <= 1e-15 * np.abs(V).max()
+    V = rng.normal(size=(n, 2))
+    V[2] = 0.0
+    V2, g2 = binding.pwa_fix_phase_host(V, np.ones((n, 2)), 2)          # V_ref = 0: nothing to turn
+    assert np.array_equal(V2, V) and g2[2, 1] == 0.0 and g2.sum() == 2 * n - 1
+    for bad in (-1, n):
+        with pytest.raises(binding.PwaError):
+            binding.pwa_fix_phase_host(V, None, bad)

@@ -295,6 +295,22 @@ def test_bfgs_floating_resonances(pwa, oracle, synth):
     assert np.abs(g_fit).max() <= 1e-3 * np.abs(g_norm).max()
 
 
+def test_bfgs_floating_fixed_phase(pwa, synth):
+    """The floating-resonance minimiser in the gauge Im V_ref = 0 ("fix_phase"): the reference wave stays real through the
+    fit (the gauge component of every gradient is dropped), a short fit lowers nll like the free one."""
+    w = synth.make_workload(3, n_data=10_007, n_mc=30_011, full_amplitudes=False)
+    Mr0, Gr0 = synth.floating_start(w)
+    free = np.arange(w.n_free, dtype=np.int32)
+    with _factored_ctx(pwa, w, Mr0, Gr0) as c:
+        pwa.pwa_build_norm(c.ctx, want_M=False)
+        nll_start = pwa.pwa_nll_grad(c.ctx, w.V_true)[0]
+        _, _, _, nll_free, _, _, _ = pwa.pwa_minimize_bfgs_floating(c.ctx, w.V_true, Mr0, Gr0, free, max_iter=60, gtol=1e-2)
+        pwa.pwa_set_option(c.ctx, "fix_phase", 4)
+        V, Mr, Gr, nll, iters, evals, st = pwa.pwa_minimize_bfgs_floating(c.ctx, w.V_true, Mr0, Gr0, free, max_iter=60, gtol=1e-2)
+        assert V[3, 1] == 0.0 and V[3, 0] > 0.0
+        assert nll < nll_start and abs(nll - nll_free) <= 0.05 * (nll_start - nll_free)
+
+
 # ------------------------------------------------------------------ device-resident (BORROW) path and the multi-GPU building block
 def test_borrowed_device_buffers_and_data_term_only(pwa, oracle):
     import torch
@@ -343,6 +359,49 @@ def test_bfgs_converges_on_cfg0(pwa, oracle, synth):
     g_norm = oracle.assemble(0.0, np.zeros((w.n, 2)), M, Vfit)[1]
     check_eval((nll_fit, g_fit, parts), oracle.nll_grad(w.A_data, M, Vfit), 1e-12, w.n_data,
                gscale=np.abs(g_norm).max())
+
+
+def test_fixed_phase_gauge(pwa, oracle, synth):
+    """NEXT-4: nll on the CUDA path does not depend on a common phase of V, its gradient turns with V (the host
+    twin pwa_fix_phase_host against a second GPU evaluation and the oracle at the turned point), and the minimisers with
+    "fix_phase" return a V with Im V_ref = 0 exactly at the same minimum as the free fit; the batched minimiser too."""
+    w = synth.make_workload(0)
+    n = w.n
+    with Ctx(pwa, n, "f64") as c:
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_DATA, w.A_data)
+        pwa.pwa_upload_events(c.ctx, pwa.PWA_MC, w.A_mc, n_generated=w.n_gen)
+        M = pwa.pwa_build_norm(c.ctx)
+        V = synth.eval_points(w, 1)[0]
+        for lik in (0, 1):
+            pwa.pwa_set_option(c.ctx, "likelihood", lik)
+            f, g, parts = pwa.pwa_nll_grad(c.ctx, V)
+            for ref in (0, n - 1):
+                V2, g2 = pwa.pwa_fix_phase_host(V, g, ref)
+                f2, gt, parts2 = pwa.pwa_nll_grad(c.ctx, V2)
+                assert f2 == pytest.approx(f, rel=1e-13) and parts2[1] == pytest.approx(parts[1], rel=1e-13)
+                mask = np.ones((n, 2), bool)
+                mask[ref, 1] = False
+                assert np.abs(g2 - gt)[mask].max() <= 1e-11 * np.abs(gt).max() and g2[ref, 1] == 0.0
+                if lik == 0:
+                    check_eval((f2, gt, parts2), oracle.nll_grad(w.A_data, M, V2), 1e-12, w.n_data)
+        pwa.pwa_set_option(c.ctx, "likelihood", 0)
+        V0 = synth.eval_points(w, 1, stream=synth.S_START)[0]
+        Vfree, nll_free, _, _ = pwa.pwa_minimize_bfgs(c.ctx, V0, max_iter=400, gtol=1e-6)
+        with pytest.raises(pwa.PwaError):
+            pwa.pwa_set_option(c.ctx, "fix_phase", n + 1)
+        for ref in (0, 2):
+            pwa.pwa_set_option(c.ctx, "fix_phase", ref + 1)
+            assert pwa.pwa_get_option(c.ctx, "fix_phase") == ref + 1
+            Vg, nll_g, _, _ = pwa.pwa_minimize_bfgs(c.ctx, V0, max_iter=400, gtol=1e-6)
+            assert Vg[ref, 1] == 0.0 and Vg[ref, 0] > 0.0
+            assert nll_g == pytest.approx(nll_free, abs=1e-6 * abs(nll_free))
+            # the same minimum up to the common phase: the free fit turned into the gauge
+            assert np.abs(Vg - pwa.pwa_fix_phase_host(Vfree, None, ref)[0]).max() <= 2e-3 * np.abs(Vg).max()
+        Vk = synth.eval_points(w, 6, stream=synth.S_START)
+        Vb, nll_b, _, _ = pwa.pwa_minimize_bfgs_batch(c.ctx, Vk, max_iter=400, gtol=1e-6)
+        assert np.all(Vb[:, 2, 1] == 0.0) and np.all(Vb[:, 2, 0] > 0.0)
+        assert nll_b.min() == pytest.approx(nll_free, abs=1e-6 * abs(nll_free))
+        pwa.pwa_set_option(c.ctx, "fix_phase", 0)
 
 
 def test_bfgs_batch_lockstep(pwa, synth):

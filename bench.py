@@ -733,6 +733,18 @@ def cpu_baseline(synth, w, M, V, name, gpu_result):
     dt = (time.perf_counter() - t0) / reps
     base = {"value": S * w.n / dt, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
             "sample": f"first {S} of {w.n_data} data events of {name}, {reps} full lnL+gradient evaluations, {dt:.2f} s each"}
+    # the same oracle on ONE thread, on a prefix of about a second
+    nt = oracle.threads()
+    try:
+        oracle.set_threads(1)
+        S1 = max(1, min(S, int(S / max(nt, 1) / max(dt, 1e-3))))
+        A1 = A[:S1]
+        t0 = time.perf_counter()
+        oracle.nll_grad(A1, M, V)
+        dt1 = time.perf_counter() - t0
+        base["one_thread"] = {"value": S1 * w.n / dt1, "unit": "event-waves/s", "sample": f"first {S1} events, 1 evaluation, {dt1:.2f} s"}
+    finally:
+        oracle.set_threads(nt)
     parity = None
     if gpu_result is not None and S == w.n_data:
         nll_o, g_o, parts_o = ref[0], ref[1], ref[2]

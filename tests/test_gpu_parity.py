@@ -354,6 +354,13 @@ def test_bfgs_converges_on_cfg0(pwa, oracle, synth):
     prof_true = -(p_true[0] - w.n_data * math.log(p_true[1] / w.n_data) - w.n_data)
     assert nll_fit <= prof_true + 1e-6 * abs(prof_true)
     assert nll_fit <= nll_true
+    # P12 (statistical sanity): the fitted amplitudes are the generated ones times ONE common complex constant c,
+    # |c|^2 ~ N_data / Norm(V_true), within the statistical error of 1e4 events
+    Vc, Vt = Vfit[:, 0] + 1j * Vfit[:, 1], w.V_true[:, 0] + 1j * w.V_true[:, 1]
+    ratio = Vc / Vt
+    c = (np.conj(Vt) @ Vc) / (np.conj(Vt) @ Vt)                      # least-squares common constant
+    assert np.abs(ratio - c).max() <= 0.25 * abs(c)
+    assert abs(c) ** 2 == pytest.approx(w.n_data / p_true[1], rel=0.1)
     # the oracle agrees with the GPU at the fitted point
     # (there g = -2 conj(T) + 2 M V cancels to ~1e-6 of either term: scale by |2 M V|)
     g_norm = oracle.assemble(0.0, np.zeros((w.n, 2)), M, Vfit)[1]

@@ -370,6 +370,18 @@ def bench_constant(torch, pwa, synth, w, steps, warmup, elem, peaks):
                 wall_r = (time.perf_counter() - t0) / steps * 1e3
                 out["resident"] = {"e2e_ms_per_eval": wall_r, "e2e_evals_per_s": 1e3 / wall_r,
                                    "note": "pwa_set_option('resident', 1): host V in, host record out, through the binding"}
+                # what a fit sees: the host BFGS driver on this sample, evaluations by launches and through the resident grid
+                if w.A_mc is not None:
+                    V0 = synth.eval_points(w, 1, stream=synth.S_START)[0]
+                    fit = {}
+                    for mode, key in ((0, "launched"), (1, "resident")):
+                        pwa.pwa_set_option(ctx, "resident", mode)
+                        t0 = time.perf_counter()
+                        _, nll_f, ev, _, it = pwa.pwa_minimize_bfgs(ctx, V0, max_iter=100, gtol=0.0, want_iters=True)
+                        dt = time.perf_counter() - t0
+                        fit[key] = {"iterations": it, "evaluations": ev, "wall_ms": dt * 1e3, "us_per_evaluation": dt / max(ev, 1) * 1e6,
+                                    "nll": nll_f}
+                    out["resident"]["bfgs_100_iterations"] = fit
             except pwa.PwaError as e:       # e.g. under a profiler that makes launches synchronous: the grid never sees a command
                 out["resident"] = {"unavailable": str(e)}
             pwa.pwa_set_option(ctx, "resident", 0)

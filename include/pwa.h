@@ -166,6 +166,25 @@ pwa_status pwa_fetch(pwa_ctx *ctx, int32_t K, double *nll, double *grad, double 
  * pwa_assemble_host.  Asynchronous.                                                      */
 pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev);
 
+/* The same record WITHOUT any allocation and without a context, for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it): steps A2 - A5 (eq. 1; eq. 3 first term, P:41;
+ * fp64 reduction) over amps_dev (DEVICE, row-major [n_events][n_waves] complex interleaved, element type
+ * `storage`, caller-owned, not kept) at V (HOST [n_waves][2], passed to the kernel by value) -> out_dev (DEVICE,
+ * [2 + 2 n_waves] doubles = { L_data, n_nonfinite, Re T_0, Im T_0, ... }).  Asynchronous on cuda_stream (cudaStream_t,
+ * may be 0) of `device`.  The per-block partial sums of the fixed-order reduction live in ONE static device array of
+ * 1 065 216 bytes that every GPU holds from the moment it loads the library until the process exits; it limits the
+ * call to n_waves <= PWA_STATIC_MAX_WAVES (PWA_ERR_UNSUPPORTED beyond, with the reason in errbuf; any n_events >= 0 is
+ * served, the grid is capped at 1024 blocks).  The call issues one 256-byte cudaMemsetAsync and one kernel launch and
+ * calls no cudaMalloc / cudaFree / allocating library routine; its first call on a device looks up the array's address
+ * (do that once before a capture).  Every call shares the array: calls that OVERLAP on the GPU (different streams, or
+ * several host threads) race and return wrong sums; calls on one stream are ordered and safe.  A plain one-event-
+ * per-thread kernel (no TMA, no event weights, constant resonances only): slower than the context path, bitwise
+ * reproducible for a fixed shape.  errbuf (HOST, errbuf_len bytes, may be NULL) receives the error text.              */
+#define PWA_STATIC_MAX_WAVES 64
+pwa_status pwa_data_term_static(int32_t device, void *cuda_stream, pwa_dtype storage, int32_t n_waves,
+                                const void *amps_dev, int64_t n_events, const double *V, double *out_dev,
+                                char *errbuf, int32_t errbuf_len);
+
 /* Host-only step A7: Norm = V^H M V, nll = -(L_data - Norm), grad = -2 conj(T) + 2 M V.
  * All pointers HOST; T [n][2], M [n][n][2], V [n][2]; parts [2] or NULL.  No GPU needed. */
 pwa_status pwa_assemble_host(int32_t n_waves, double L_data, const double *T, const double *M,

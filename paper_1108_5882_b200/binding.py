@@ -32,6 +32,7 @@ SYMBOLS = [
     "pwa_assemble_host_eq2", "pwa_grad_to_polar", "pwa_polar_to_cartesian", "pwa_fix_phase_host", "pwa_fumili_hessian", "pwa_set_weights",
     "pwa_batch_path", "pwa_minimize_bfgs_floating", "pwa_minimize_bfgs_batch_ex", "pwa_minimize_bfgs_floating_ex",
     "pwa_n_res", "pwa_nll_grad_floating", "pwa_get_option", "pwa_storage", "pwa_n_events", "pwa_norm_sums", "pwa_combine_norm_host", "pwa_assemble_host_shards",
+    "pwa_data_term_static",
 ]
 PWA_FIT_CONVERGED, PWA_FIT_MAX_ITER, PWA_FIT_LINE_SEARCH = 0, 1, 2
 
@@ -66,6 +67,7 @@ def _load():
         "pwa_nll_grad_batch_enqueue": (C.c_int, [vp, i32, vp]),
         "pwa_fetch": (C.c_int, [vp, i32, vp, vp, vp]),
         "pwa_data_term_enqueue": (C.c_int, [vp, vp, vp]),
+        "pwa_data_term_static": (C.c_int, [i32, vp, C.c_int, i32, vp, C.c_int64, vp, vp, vp, i32]),
         "pwa_assemble_host": (C.c_int, [i32, C.c_double, vp, vp, vp, dp, vp, vp]),
         "pwa_res_grad": (C.c_int, [vp, vp, vp, vp]),
         "pwa_minimize_bfgs": (C.c_int, [vp, vp, i32, C.c_double, dp, C.POINTER(i32), C.POINTER(i32)]),
@@ -308,6 +310,35 @@ def pwa_data_term_enqueue(ctx, V, out_dev):
     V = _f64(V, (n, 2))
     ptr, _, _ = _ptr_and_keep(out_dev)
     _check(ctx, _lib.pwa_data_term_enqueue(ctx, V.ctypes.data, C.c_void_p(ptr)))
+
+
+PWA_STATIC_MAX_WAVES = 64
+
+
+def pwa_data_term_static(amps_dev, V, out_dev, n_events=None, device=0, cuda_stream=0):
+    """Allocation-free data term (no context): amps_dev torch CUDA tensor [N, n, 2] float32 / float64, V [n, 2],
+    out_dev torch CUDA float64 tensor with >= 2 + 2n elements.  Asynchronous on cuda_stream."""
+    V = _f64(V)
+    n = V.shape[0]
+    if V.shape != (n, 2):
+        raise ValueError(f"V must be [n, 2], got {V.shape}")
+    pa, ka, code = _ptr_and_keep(amps_dev)
+    if code is None or isinstance(ka, np.ndarray):
+        raise TypeError("amps_dev must be a float32 / float64 CUDA tensor")
+    if n_events is None:
+        if tuple(ka.shape[1:]) != (n, 2):
+            raise ValueError(f"amps_dev must be [N, {n}, 2], got {tuple(ka.shape)}")
+        n_events = ka.shape[0]
+    if int(np.prod(ka.shape)) < int(n_events) * n * 2:
+        raise ValueError("amps_dev holds fewer than n_events * n * 2 elements")
+    po, ko, co = _ptr_and_keep(out_dev)
+    if co != PWA_F64 or int(np.prod(ko.shape)) < 2 + 2 * n:
+        raise ValueError("out_dev must be a float64 CUDA tensor with >= 2 + 2n elements")
+    err = C.create_string_buffer(256)
+    st = int(_lib.pwa_data_term_static(int(device), C.c_void_p(int(cuda_stream) or None), int(code), n, C.c_void_p(pa),
+                                       int(n_events), V.ctypes.data, C.c_void_p(po), err, 256))
+    if st != PWA_OK:
+        raise PwaError(st, err.value.decode())
 
 
 def pwa_assemble_host(L_data, T, M, V):

@@ -191,7 +191,7 @@ __device__ __forceinline__ void norm_body(const void *__restrict__ Bv, long long
 #pragma unroll
         for (int m = 1; m < TPS; m <<= 1) { sr += __shfl_xor_sync(0xffffffffu, sr, m); si += __shfl_xor_sync(0xffffffffu, si, m); }
         if (t * ET + e < N) {
-            const double I = sr * sr + si * si, rr = sr / I, ri = -si / I;      // r = 1 / S = conj(S) / I
+            const double I = sr * sr + si * si, inv = 1.0 / I, rr = sr * inv, ri = -si * inv;      // r = 1 / S = conj(S) / I
             for (int a = part; a < n; a += TPS) {
                 const double2 x = *reinterpret_cast<const double2 *>(row + 2 * a);
                 *reinterpret_cast<double2 *>(row + 2 * a) = make_double2(x.x * rr - x.y * ri, x.x * ri + x.y * rr);
@@ -421,7 +421,7 @@ static pwa_status dispatch_nd(pwa_ctx *ctx, const FactArgs &fargs, const GramJob
     if (D <= 16)  return launch_nd<ST, 2,  1, MODE, 2, 128, NANG>(ctx, fargs, job);
     if (D <= 32)  return launch_nd<ST, 4,  1, MODE, 2, 128, NANG>(ctx, fargs, job);
     if (D <= 64)  return launch_nd<ST, 8,  2, MODE, 2, 64, NANG>(ctx, fargs, job);
-    return launch_nd<ST, 16, 4, MODE, 1, 32, NANG>(ctx, fargs, job);
+    return launch_nd<ST, 16, 4, MODE, 1, 64, NANG>(ctx, fargs, job);
 }
 
 static pwa_status run_gram(pwa_ctx *ctx, const GramJob &job, bool *handled)

@@ -323,6 +323,17 @@ def m_build_record(pwa, tm, ctx, w, n, elem, peaks):
     hb = rl_hbm(peaks, nbytes, ms_m, kernel="i8::k_norm_i8" if path == 1 else "k_norm_dmma")
     if path == 1:
         rec["roofline"] = hb                                 # exact integer GEMM keeps up with the stream: HBM-bound
+        # opt-in variant with three digit planes ("norm" = 3): faster, larger a-priori bound; measured against the default's M
+        M4 = pwa.pwa_build_norm(ctx)
+        pwa.pwa_set_option(ctx, "norm", 3)
+        ms3, _ = tm.run(lambda i: pwa.pwa_build_norm(ctx, want_M=False), SIDE_STEPS, SIDE_WARMUP)
+        M3 = pwa.pwa_build_norm(ctx)
+        bound3, _ = pwa.pwa_norm_error_bound(ctx)
+        pwa.pwa_set_option(ctx, "norm", 0)
+        pwa.pwa_build_norm(ctx, want_M=False)                # leave the default's M in the context
+        rec["three_planes"] = {"ms": ms3, "roofline": rl_hbm(peaks, nbytes, ms3, kernel="i8::k_norm_i8<3>"),
+                               "error_bound_abs": bound3, "max_abs_M": float(np.abs(M4).max()),
+                               "measured_diff_to_default_abs": float(np.abs(M3 - M4).max())}
     else:
         tb = rl_flops(peaks, "tensor", flops_sym, ms_m, kernel="k_norm_dmma")
         rec["roofline"] = hb if hb["frac"] >= tb["frac"] else tb    # the floor that is closer is the binding one

@@ -119,7 +119,8 @@ pwa_status pwa_build_norm(pwa_ctx *ctx, double *M_out);
  * most recent pwa_build_norm.  The FP64 paths only carry summation rounding (reported as 0); the
  * int8 tensor-core path for fp32-stored samples (fixed-point digit planes, exact integer
  * accumulation, low orders truncated: DESIGN.md section 6.6) reports its quantisation + truncation
- * bound in the units of M.  *which_path (may be NULL): 0 = FP64 path, 1 = int8 tcgen05 path.    */
+ * bound in the units of M.  *which_path (may be NULL): 0 = FP64 path, 1 = int8 tcgen05 path, 3 = its three-plane
+ * variant ("norm" = 3).                                                                                 */
 pwa_status pwa_norm_error_bound(pwa_ctx *ctx, double *bound, int32_t *which_path);
 
 /* Installs an externally computed M (HOST [n][n][2]), e.g. the sum over ranks of per-shard
@@ -333,7 +334,10 @@ pwa_status pwa_sync(pwa_ctx *ctx);
  * event weights, else the per-lane streaming kernel), 20 = per-lane kernel, 98 = default without programmatic
  * dependent launch, 99 = generic kernel (any n).
  * "norm": 0 = default (int8 tcgen05 path for fp32-stored constant-resonance samples of >= 65536 events, else
- * FP64 DMMA), 1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel.
+ * FP64 DMMA), 1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 3 = the same with THREE digit planes
+ * (24 instead of 32 bits below each column's maximum, 4 instead of 7 digit-pair products per step: faster, and
+ * pwa_norm_error_bound then reports a bound ~2^9 times larger, typically above the 1e-6 bar of fp32 storage although
+ * the measured error stays ~1e-9 of max|M|; opt-in, never the default), 99 = generic CUDA-core kernel.
  * "batch": 0 = default (see pwa_batch_path), 1 = FP64 DMMA GEMMs for any K, 2 = int8 tcgen05 GEMMs
  * whenever the shape allows, 99 = K passes of the streaming kernel.
  * "l2_resident_mb": MB of the head of the DATA sample that the streaming data term loads with the L2 evict_last

@@ -185,11 +185,12 @@ pwa_status launch_norm_build(pwa_ctx *ctx)
     }
     // opt_norm: 0 = default (int8 tensor-core path for large fp32-stored samples, else FP64 DMMA),
     //           1 = FP64 DMMA, 2 = int8 tcgen05 path whenever the shape allows, 99 = generic CUDA-core kernel
-    if (ctx->opt_norm == 2 || (ctx->opt_norm == 0 && ctx->mc.n_events >= 65536)) {
+    //           3 = int8 tcgen05 path with THREE digit planes (24 bits below the column maximum: faster, larger a-priori bound)
+    if (ctx->opt_norm == 2 || ctx->opt_norm == 3 || (ctx->opt_norm == 0 && ctx->mc.n_events >= 65536)) {
         bool handled = false;
-        pwa_status s = launch_norm_i8(ctx, &handled);
+        pwa_status s = launch_norm_i8(ctx, &handled, ctx->opt_norm == 3);
         if (s != PWA_OK) return s;
-        if (handled) { ctx->M_path = 1; return PWA_OK; }
+        if (handled) { ctx->M_path = ctx->opt_norm == 3 ? 3 : 1; return PWA_OK; }
     }
     if (ctx->opt_norm != 99) {
         bool handled = false;

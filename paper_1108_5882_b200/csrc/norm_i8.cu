@@ -53,7 +53,7 @@ constexpr int TE = 64;                       // super-rows (K) per tile
 constexpr int ROWB = 512;                    // bytes of one fp32 super-row (128 reals)
 constexpr int STG_BYTES = TE * ROWB;         // 32 KB fp32 tile
 constexpr int PLANE = TE * 128;              // 8 KB: one int8 digit plane of a tile
-constexpr int SL_BYTES = 4 * PLANE;          // 32 KB: four digit planes
+constexpr int SL_BYTES = 4 * PLANE;          // 32 KB: four digit planes (the three-plane variant leaves the fourth unused)
 constexpr int NSTG = 3;                      // fp32 tile ring
 constexpr int NSL = 3;                       // digit-plane ring
 constexpr int FT = 512;                      // tiles between two TMEM flushes (32768 events)
@@ -74,6 +74,13 @@ constexpr uint32_t kIdesc128 = idesc_i8(128, true, true), kIdesc256 = idesc_i8(2
 // slots: [gridDim.x][128][128] doubles, Y = 2^23 acc0 + 2^16 acc1 + 2^7 acc2 + acc3 summed over the
 // CTA's flushes (P = 2^24 (Y + Y^T) in units of 2^-(s_p + s_q)).
 // dslots: [gridDim.x][NCW][128] doubles, the t = 2 diagonal per converter warp (P_pp += 2^16 * sum).
+// NP = 4: the scheme above.  NP = 3 (option "norm" = 3): q = rint(B 2^(s_p - 8)) has 24 bits below the column maximum and
+// three balanced digits; per K step
+//     acc4 += D2^T D2  (t = 4),  acc3 += D2^T D1  (t = 3)      one N = 256 MMA, D2^T [D1 | D2]
+//     acc2a += D2^T D0,  acc2b += D1^T D1           (t = 2)      two N = 128 MMAs
+// = 4 products instead of 7 and 56 KB instead of 88 KB of operand reads per tile; orders t <= 1 are dropped (the exact
+// t = 0 diagonal sum_e d0^2 is added back).  Y = 2^16 acc4 + 2^9 acc3 + 2 acc2a + acc2b, P = 2^31 (Y + Y^T) 2^-(s_p + s_q).
+template <int NP>
 __global__ void __launch_bounds__(THREADS, 1)
 k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __grid_constant__ Scales sc,
           double *__restrict__ slots, double *__restrict__ dslots)
@@ -135,11 +142,18 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                     const uint64_t d0 = plane_desc(pl + 0 * PLANE + koff), d1 = plane_desc(pl + 1 * PLANE + koff);
                     const uint64_t d2 = plane_desc(pl + 2 * PLANE + koff), d3 = plane_desc(pl + 3 * PLANE + koff);
                     const uint32_t acc = (first && kk == 0) ? 0u : 1u;
-                    // accumulators by ascending order: t = 3 at column 0, t = 4 at 128, t = 5 at 256, t = 6 at 384
-                    umma_i8(tmem0 + 256, d3, d2, kIdesc256, acc);      // D3^T [D2 | D3] -> t = 5 | t = 6
-                    umma_i8(tmem0 + 0,   d3, d0, kIdesc256, acc);      // D3^T [D0 | D1] -> t = 3 | t = 4
-                    umma_i8(tmem0 + 128, d3, d1, kIdesc128, 1u);       // second D3^T D1  -> t = 4
-                    umma_i8(tmem0 + 0,   d2, d1, kIdesc256, 1u);       // D2^T [D1 | D2] -> t = 3 | t = 4
+                    if (NP == 4) {
+                        // accumulators by ascending order: t = 3 at column 0, t = 4 at 128, t = 5 at 256, t = 6 at 384
+                        umma_i8(tmem0 + 256, d3, d2, kIdesc256, acc);      // D3^T [D2 | D3] -> t = 5 | t = 6
+                        umma_i8(tmem0 + 0,   d3, d0, kIdesc256, acc);      // D3^T [D0 | D1] -> t = 3 | t = 4
+                        umma_i8(tmem0 + 128, d3, d1, kIdesc128, 1u);       // second D3^T D1  -> t = 4
+                        umma_i8(tmem0 + 0,   d2, d1, kIdesc256, 1u);       // D2^T [D1 | D2] -> t = 3 | t = 4
+                    } else {
+                        // D2^T D0 at column 0, D1^T D1 at 128, t = 3 at 256, t = 4 at 384
+                        umma_i8(tmem0 + 256, d2, d1, kIdesc256, acc);      // D2^T [D1 | D2] -> t = 3 | t = 4
+                        umma_i8(tmem0 + 0,   d2, d0, kIdesc128, acc);      // D2^T D0        -> t = 2
+                        umma_i8(tmem0 + 128, d1, d1, kIdesc128, acc);      // D1^T D1        -> t = 2
+                    }
                 }
                 umma_commit(b_sl_empty + 8 * b);
                 if ((t % FT) == FT - 1 || t == nt - 1) umma_commit(b_acc_full);
@@ -168,22 +182,32 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
 #pragma unroll
             for (int r = 0; r < TE / NCW; ++r) {
                 const uint32_t e = (uint32_t)(warp + r * NCW);
-                const uint32_t w0 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) * one + 0x00808080) ^ 0x00808080u;
-                const uint32_t w1 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) * one + 0x00808080) ^ 0x00808080u;
-                const uint32_t w2 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) * one + 0x00808080) ^ 0x00808080u;
-                const uint32_t w3 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].w) * scl[3]) * one + 0x00808080) ^ 0x00808080u;
-                // exact t = 2 diagonal: d0 d2 + d1 d1 + d2 d0 per element (<= 3 * 2^14, 4096 rows per warp and flush)
-                dg[0] = __dp4a((int)w0, (int)__byte_perm(w0, 0u, 0x4012), dg[0]);
-                dg[1] = __dp4a((int)w1, (int)__byte_perm(w1, 0u, 0x4012), dg[1]);
-                dg[2] = __dp4a((int)w2, (int)__byte_perm(w2, 0u, 0x4012), dg[2]);
-                dg[3] = __dp4a((int)w3, (int)__byte_perm(w3, 0u, 0x4012), dg[3]);
+                // balanced digits: NP = 4: bytes d0 d1 d2 d3; NP = 3: bytes d0 d1 d2 (byte 3 is the sign extension of d2, unused)
+                constexpr int OFS = NP == 4 ? 0x00808080 : 0x00008080;
+                const uint32_t w0 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].x) * scl[0]) * one + OFS) ^ (uint32_t)OFS;
+                const uint32_t w1 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].y) * scl[1]) * one + OFS) ^ (uint32_t)OFS;
+                const uint32_t w2 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].z) * scl[2]) * one + OFS) ^ (uint32_t)OFS;
+                const uint32_t w3 = (uint32_t)(__float2int_rn(__uint_as_float(raw[r].w) * scl[3]) * one + OFS) ^ (uint32_t)OFS;
+                if (NP == 4) {
+                    // exact t = 2 diagonal: d0 d2 + d1 d1 + d2 d0 per element (<= 3 * 2^14, 4096 rows per warp and flush)
+                    dg[0] = __dp4a((int)w0, (int)__byte_perm(w0, 0u, 0x4012), dg[0]);
+                    dg[1] = __dp4a((int)w1, (int)__byte_perm(w1, 0u, 0x4012), dg[1]);
+                    dg[2] = __dp4a((int)w2, (int)__byte_perm(w2, 0u, 0x4012), dg[2]);
+                    dg[3] = __dp4a((int)w3, (int)__byte_perm(w3, 0u, 0x4012), dg[3]);
+                } else {
+                    // exact t = 0 diagonal: d0 d0 per element (<= 2^14)
+                    dg[0] = __dp4a((int)(w0 & 0xffu), (int)w0, dg[0]);
+                    dg[1] = __dp4a((int)(w1 & 0xffu), (int)w1, dg[1]);
+                    dg[2] = __dp4a((int)(w2 & 0xffu), (int)w2, dg[2]);
+                    dg[3] = __dp4a((int)(w3 & 0xffu), (int)w3, dg[3]);
+                }
                 const uint32_t t0 = __byte_perm(w0, w1, 0x5140), t1 = __byte_perm(w2, w3, 0x5140);
                 const uint32_t t2 = __byte_perm(w0, w1, 0x7362), t3 = __byte_perm(w2, w3, 0x7362);
                 const uint32_t a = dst + e * 128u + ((chunk_id ^ (e & 7u)) << 4) + chunk_off;
                 asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 0 * PLANE), "r"(__byte_perm(t0, t1, 0x5410)) : "memory");
                 asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 1 * PLANE), "r"(__byte_perm(t0, t1, 0x7632)) : "memory");
                 asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 2 * PLANE), "r"(__byte_perm(t2, t3, 0x5410)) : "memory");
-                asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 3 * PLANE), "r"(__byte_perm(t2, t3, 0x7632)) : "memory");
+                if (NP == 4) asm volatile("st.shared.u32 [%0], %1;" ::"r"(a + 3 * PLANE), "r"(__byte_perm(t2, t3, 0x7632)) : "memory");
             }
             fence_async_smem();                       // digit planes -> visible to the tensor core (async proxy)
             __syncwarp();
@@ -210,8 +234,10 @@ k_norm_i8(const __grid_constant__ CUtensorMap tmap, long long ntiles, const __gr
                     double *yp = slot + (size_t)m * 128 + c0;
 #pragma unroll
                     for (int j = 0; j < 16; j += 2) {
-                        double y0 = (double)a0[j] * 8388608.0 + (double)a1[j] * 65536.0 + ((double)a2[j] * 128.0 + (double)a3[j]);
-                        double y1 = (double)a0[j + 1] * 8388608.0 + (double)a1[j + 1] * 65536.0 + ((double)a2[j + 1] * 128.0 + (double)a3[j + 1]);
+                        // NP = 4: 2^23 t6 + 2^16 t5 + 2^7 t4 + t3;  NP = 3: 2^16 t4 + 2^9 t3 + (D1^T D1 + 2 D2^T D0)
+                        constexpr double W0 = NP == 4 ? 8388608.0 : 65536.0, W1 = NP == 4 ? 65536.0 : 512.0, W2 = NP == 4 ? 128.0 : 1.0, W3 = NP == 4 ? 1.0 : 2.0;
+                        double y0 = (double)a0[j] * W0 + (double)a1[j] * W1 + ((double)a2[j] * W2 + (double)a3[j] * W3);
+                        double y1 = (double)a0[j + 1] * W0 + (double)a1[j + 1] * W1 + ((double)a2[j + 1] * W2 + (double)a3[j + 1] * W3);
                         if (chunk > 0) { const double2 old = *reinterpret_cast<const double2 *>(yp + j); y0 += old.x; y1 += old.y; }
                         *reinterpret_cast<double2 *>(yp + j) = make_double2(y0, y1);
                     }
@@ -298,7 +324,7 @@ struct Exps { int e[128]; };                   // s_p of the 128-wide view
 // evaluated for a <= b and mirrored, so M is exactly Hermitian.
 __global__ void __launch_bounds__(256)
 k_i8_assemble(const double *__restrict__ ysum, const double *__restrict__ dsum, const __grid_constant__ Exps ex, int n,
-              const float *__restrict__ tail, int n_tail, double inv_ngen, double *__restrict__ M)
+              const float *__restrict__ tail, int n_tail, double inv_ngen, double *__restrict__ M, int yshift)
 {
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx >= n * n) return;
@@ -309,7 +335,7 @@ k_i8_assemble(const double *__restrict__ ysum, const double *__restrict__ dsum, 
         double acc = 0.0;
         for (int g = 0; g < G; ++g) {
             const int pp = g * D + p, qq = g * D + q;
-            acc += (ysum[pp * 128 + qq] + ysum[qq * 128 + pp]) * exp2((double)(24 - ex.e[pp] - ex.e[qq]));
+            acc += (ysum[pp * 128 + qq] + ysum[qq * 128 + pp]) * exp2((double)(yshift - ex.e[pp] - ex.e[qq]));   // 24 (four planes) or 31 (three)
             if (p == q) acc += dsum[pp] * exp2((double)(16 - 2 * ex.e[pp]));
         }
         for (int j = 0; j < n_tail; ++j) acc += (double)tail[(size_t)j * D + p] * (double)tail[(size_t)j * D + q];
@@ -380,7 +406,7 @@ pwa_status prepare_norm_i8(pwa_ctx *ctx)
     return i8_column_scales(ctx, ctx->mc.amps, ctx->mc.n_events, 2 * ctx->n, q.exp, q.scale, q.cmax, &q.valid);
 }
 
-pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
+pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled, bool three_planes)
 {
     *handled = false;
     if (!ctx->i8q.valid || !i8_shape_ok(ctx)) return PWA_OK;
@@ -407,7 +433,8 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     if (grid > ntiles) grid = ntiles;
     static bool s_attr[64] = {false};
     if (!s_attr[ctx->device & 63]) {
-        PWA_CUDA(ctx, cudaFuncSetAttribute(i8::k_norm_i8, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)i8::SMEM));
+        PWA_CUDA(ctx, cudaFuncSetAttribute(i8::k_norm_i8<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)i8::SMEM));
+        PWA_CUDA(ctx, cudaFuncSetAttribute(i8::k_norm_i8<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)i8::SMEM));
         s_attr[ctx->device & 63] = true;
     }
     const size_t slot_doubles = (size_t)grid * 16384, dslot_doubles = (size_t)grid * i8::NCW * 128;
@@ -420,16 +447,18 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
     i8::Scales sc;
     i8::Exps ex;
     memcpy(sc.s, ctx->i8q.scale, sizeof(sc.s));
+    if (three_planes) for (int p = 0; p < 128; ++p) sc.s[p] = ldexpf(sc.s[p], -8);      // 24 bits below the column maximum
     sc.one = 1;
     memcpy(ex.e, ctx->i8q.exp, sizeof(ex.e));
-    i8::k_norm_i8<<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);
+    if (three_planes) i8::k_norm_i8<3><<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);
+    else i8::k_norm_i8<4><<<(unsigned)grid, i8::THREADS, i8::SMEM, ctx->stream>>>(tmap, ntiles, sc, slots, dslots);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     i8::k_i8_slot_sum<<<516, 256, 0, ctx->stream>>>(slots, (int)grid, ysum, dslots, dsum);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     const float *tail = reinterpret_cast<const float *>(ctx->mc.amps) + (size_t)rows * 128;
-    i8::k_i8_assemble<<<(n * n + 255) / 256, 256, 0, ctx->stream>>>(ysum, dsum, ex, n, tail, n_tail, 1.0 / (double)ctx->mc.n_gen, ctx->d_M);
+    i8::k_i8_assemble<<<(n * n + 255) / 256, 256, 0, ctx->stream>>>(ysum, dsum, ex, n, tail, n_tail, 1.0 / (double)ctx->mc.n_gen, ctx->d_M, three_planes ? 31 : 24);
     ctx->launches++;
     PWA_CUDA(ctx, cudaGetLastError());
     *handled = true;
@@ -439,6 +468,7 @@ pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled)
 // A-priori bound on |M_gpu - M_exact|_ab / sqrt(M_aa M_bb)-free absolute form: returns
 // max_ab of  N_acc / N_gen * 2 * (eps_q (c_a |B|max_b + c_b |B|max_a) + eps_t c_a c_b),
 // with c = 2^(31 - s) per real column (max over re/im of the wave), eps_q = 2^-32, eps_t = 3 * 2^-32 (1 + 2^-7).
+// Three planes (M_path == 3): eps_q = 2^-24, eps_t = 2^-23 (1 + 2^-9) (orders t <= 1 dropped: <= (128^2 + 2 * 2^8 * 128^2) 2^-46 c_p c_q).
 double norm_i8_error_bound(const pwa_ctx *ctx)
 {
     if (!ctx->i8q.valid) return 0.0;
@@ -448,7 +478,9 @@ double norm_i8_error_bound(const pwa_ctx *ctx)
         cm = fmax(cm, ldexp(1.0, 31 - ctx->i8q.exp[p]));
         bm = fmax(bm, ctx->i8q.cmax[p]);
     }
-    const double eps_q = ldexp(1.0, -32), eps_t = 3.0 * ldexp(1.0, -32) * (1.0 + 1.0 / 128.0);
+    const bool three = ctx->M_path == 3;
+    const double eps_q = three ? ldexp(1.0, -24) : ldexp(1.0, -32);
+    const double eps_t = three ? ldexp(1.0, -23) * (1.0 + 1.0 / 512.0) : 3.0 * ldexp(1.0, -32) * (1.0 + 1.0 / 128.0);
     // each complex entry is a sum of two real Gram entries
     return 2.0 * (double)ctx->mc.n_events / (double)ctx->mc.n_gen * (2.0 * eps_q * cm * bm + eps_t * cm * cm);
 }

@@ -539,7 +539,7 @@ pwa_status pwa_norm_error_bound(pwa_ctx *ctx, double *bound, int32_t *which_path
 {
     if (!ctx || !bound) return PWA_ERR_INVALID_ARG;
     if (!ctx->M_valid) return fail(ctx, PWA_ERR_STATE, "normalisation matrix missing or stale: call pwa_build_norm");
-    *bound = ctx->M_path == 1 ? norm_i8_error_bound(ctx) : 0.0;
+    *bound = (ctx->M_path == 1 || ctx->M_path == 3) ? norm_i8_error_bound(ctx) : 0.0;
     if (which_path) *which_path = ctx->M_path;
     return PWA_OK;
 }

@@ -116,7 +116,7 @@ pwa_status launch_batch(pwa_ctx *ctx, int K);   // V already staged in h_V/d_V
 pwa_status launch_norm_build(pwa_ctx *ctx);
 pwa_status launch_fumili(pwa_ctx *ctx, double *H_dev, bool with_norm);   // norm_dmma.cu (row-scaled Gram over DATA)
 pwa_status prepare_norm_i8(pwa_ctx *ctx);                  // norm_i8.cu: after a constant-resonance MC upload
-pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled);    // norm_i8.cu
+pwa_status launch_norm_i8(pwa_ctx *ctx, bool *handled, bool three_planes);    // norm_i8.cu
 double norm_i8_error_bound(const pwa_ctx *ctx);
 pwa_status i8_column_scales(pwa_ctx *ctx, const void *amps, long long n_events, int D, int *exp, float *scale,
                             double *cmax, bool *valid);    // norm_i8.cu

@@ -269,6 +269,11 @@ def overlap_probe(pwa, ctx):
         alone = pwa.pwa_microbench(ctx, 8, mode + 32 + 64)
         both = pwa.pwa_microbench(ctx, 8, mode + 48 + 64)
         out[name] = {"alone": alone, "with_mma": both, "overlap": (out["mma_alone"] + alone - both) / min(out["mma_alone"], alone)}
+    # window mode: one fp64 window and one integer window, in either order (who waits for whom)
+    for flag, name in ((0, "windows_fp64_first"), (128, "windows_int_first")):
+        alone = pwa.pwa_microbench(ctx, 8, 8 + 32 + 64 + flag + (8192 << 8))
+        both = pwa.pwa_microbench(ctx, 8, 8 + 48 + 64 + flag + (8192 << 8))
+        out[name] = {"alone": alone, "with_mma": both, "added": both - alone}
     return out
 
 

@@ -373,7 +373,9 @@ pwa_status pwa_get_option(pwa_ctx *ctx, const char *key, int32_t *value);   /* c
  * with bit 6 of `bytes`, the 12 that do not share the issuer's scheduler) other warps run one kind of epilogue work;
  * `bytes` = mode + 16 (MMAs on) + 32 (epilogue work on) + 64 (keep the issuer's scheduler free), mode 0 = fp64 FMA,
  * 1 = tcgen05.ld, 2 = st.shared.v4, 3 = integer multiply-add, 4 = ld.shared.v4, 5 = fp32 FMA, 6 = 2 fp64 FMA among 6
- * integer chains, 7 = a stream of 16-byte global loads (3.6 GB of scratch); result = milliseconds (compare MMAs alone, the work alone and both: DESIGN.md section 6.7 has the
+ * integer chains, 7 = a stream of 16-byte global loads (3.6 GB of scratch), 8 = WINDOWS: the warps alternate, together,
+ * between a window of fp64 FMA chains and one of integer chains (window length in fp64 iterations in bits 8 .. 23 of
+ * `bytes`, default 64; bit 7: the integer window comes first); result = milliseconds (compare MMAs alone, the work alone and both: DESIGN.md section 6.7 has the
  * outcome: fp64 arithmetic does not overlap with the int8 MMAs at all).  Synchronous; result HOST.                  */
 pwa_status pwa_microbench(pwa_ctx *ctx, int32_t which, int64_t bytes, double *result);
 

@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(512, 1) k_mb_tmem_ld(int iters, double *out)
 // MODE 0 = fp64 FMA chains, 1 = tcgen05.ld 32x32b.x16 of columns 256 .. 511, 2 = st.shared.v4, 3 = integer LOP3 / IMAD
 // chains, 4 = ld.shared.v4.  Timed with either side switched off and with both: does the work overlap with the MMAs?
 template <int MODE>
-__global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_iters, bool skip_sched0, double *out)
+__global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_iters, bool skip_sched0, double *out, int win = 64)
 {
     extern __shared__ unsigned char mb_smem[];
     __shared__ __align__(8) unsigned long long bar;
@@ -157,6 +157,43 @@ __global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_it
 #pragma unroll
             for (int i = 0; i < 8; ++i) sum += a[i];
             if (sum == 0.12345f && out != nullptr) out[0] = sum;
+        } else if (MODE == 8) {
+            // WINDOWS: all epilogue warps alternate between a window of fp64 FMA chains and a window of integer chains
+            // (window = `win` iterations, the warps change windows together through a named barrier); epi_iters = total
+            // fp64 iterations, the integer windows run twice as many.  Do the MMAs advance during the integer windows?
+            double a[8];
+            uint32_t b[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { a[i] = 1.0 + threadIdx.x * 1e-9 + i; b[i] = threadIdx.x * 2654435761u + i; }
+            const double m = 1.0 - 1e-12, c = 1e-13;
+            const int nthr = skip_sched0 ? 384 : 512;
+            const bool int_first = win < 0;                       // negative window: the integer window comes first
+            if (int_first) win = -win;
+            for (int done = 0; done < epi_iters; done += win) {
+                if (int_first) {
+                    for (int it = 0; it < 2 * win; ++it) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) b[i] = (b[i] ^ (uint32_t)it) * 2246822519u + 0x9e3779b9u;
+                    }
+                    asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory");
+                }
+                for (int it = 0; it < win; ++it) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+                }
+                asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory");
+                if (!int_first) {
+                    for (int it = 0; it < 2 * win; ++it) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) b[i] = (b[i] ^ (uint32_t)it) * 2246822519u + 0x9e3779b9u;
+                    }
+                    asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory");
+                }
+            }
+            double sum = 0.0; uint32_t x = 0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { sum += a[i]; x ^= b[i]; }
+            if ((sum == 0.12345 || x == 0x12345u) && out != nullptr) out[0] = 1.0;
         } else if (MODE == 6) {                                  // 2 fp64 FMA chains diluted in 6 integer chains
             double a[2] = {1.0 + threadIdx.x * 1e-9, 2.0};
             uint32_t b[6];
@@ -237,14 +274,14 @@ __global__ void __launch_bounds__(544, 1) k_mb_overlap(int mma_iters, int epi_it
 }
 
 template <int MODE>
-static cudaError_t launch_overlap(pwa_ctx *ctx, int mma_iters, int epi_iters, bool skip, bool first, double *buf = nullptr)
+static cudaError_t launch_overlap(pwa_ctx *ctx, int mma_iters, int epi_iters, bool skip, bool first, double *buf = nullptr, int win = 64)
 {
     constexpr int SM = 1024 + 16384 + 32768 + 8192;
     if (first) {
         cudaError_t e = cudaFuncSetAttribute(k_mb_overlap<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM);
         if (e != cudaSuccess) return e;
     }
-    k_mb_overlap<MODE><<<ctx->sm_count, 544, SM, ctx->stream>>>(mma_iters, epi_iters, skip, buf);
+    k_mb_overlap<MODE><<<ctx->sm_count, 544, SM, ctx->stream>>>(mma_iters, epi_iters, skip, buf, win);
     return cudaGetLastError();
 }
 
@@ -282,14 +319,15 @@ pwa_status run_microbench(pwa_ctx *ctx, int which, int64_t bytes, double *result
         else if (which == 8) {
             // bytes = mode + 16 * (1: MMAs on) + 32 * (1: epilogue work on); result = milliseconds
             const int mode = (int)(bytes & 15), mi = (bytes & 16) ? iters : 0;
-            const int per_mode[8] = {16384, 14000, 16384, 32768, 16384, 65536, 40000, 3000};    // ~1e6 cycles of each kind of work alone
-            if (mode > 7) return fail(ctx, PWA_ERR_INVALID_ARG, "unknown overlap probe mode");
+            const int per_mode[9] = {16384, 14000, 16384, 32768, 16384, 65536, 40000, 3000, 8192};    // ~1e6 cycles of each kind of work alone
+            if (mode > 8) return fail(ctx, PWA_ERR_INVALID_ARG, "unknown overlap probe mode");
             const int ei = (bytes & 32) ? per_mode[mode] : 0;
             const bool skip = (bytes & 64) != 0;
             cudaError_t e = mode == 0 ? launch_overlap<0>(ctx, mi, ei, skip, rep == 0) : mode == 1 ? launch_overlap<1>(ctx, mi, ei, skip, rep == 0)
                           : mode == 2 ? launch_overlap<2>(ctx, mi, ei, skip, rep == 0) : mode == 3 ? launch_overlap<3>(ctx, mi, ei, skip, rep == 0)
                           : mode == 4 ? launch_overlap<4>(ctx, mi, ei, skip, rep == 0) : mode == 5 ? launch_overlap<5>(ctx, mi, ei, skip, rep == 0) : mode == 6 ? launch_overlap<6>(ctx, mi, ei, skip, rep == 0)
-                          : launch_overlap<7>(ctx, mi, ei, skip, rep == 0, reinterpret_cast<double *>(ctx->d_scratch));
+                          : mode == 7 ? launch_overlap<7>(ctx, mi, ei, skip, rep == 0, reinterpret_cast<double *>(ctx->d_scratch))
+                          : launch_overlap<8>(ctx, mi, ei, skip, rep == 0, nullptr, (((bytes >> 8) & 0xffff) ? (int)((bytes >> 8) & 0xffff) : 64) * ((bytes & 128) ? -1 : 1));
             PWA_CUDA(ctx, e);
         }
         else return fail(ctx, PWA_ERR_INVALID_ARG, "unknown microbench id");

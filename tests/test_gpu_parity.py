@@ -1126,6 +1126,12 @@ def test_microbench_probes(pwa):
         assert ov[0] < 0.5 < ov[1], ov
         for mode in (2, 3, 4, 5, 6, 7):
             assert pwa.pwa_microbench(c.ctx, 8, mode + 48) > 0
+        # window mode: the MMAs hide under an integer window that comes first, and add when the fp64 window comes first
+        added = {}
+        for flag in (0, 128):
+            alone = pwa.pwa_microbench(c.ctx, 8, 8 + 32 + 64 + flag + (8192 << 8))
+            added[flag] = pwa.pwa_microbench(c.ctx, 8, 8 + 48 + 64 + flag + (8192 << 8)) - alone
+        assert added[128] < 0.5 * mma < added[0], added
         with pytest.raises(pwa.PwaError):
             pwa.pwa_microbench(c.ctx, 8, 9 + 48)
         with pytest.raises(pwa.PwaError):

@@ -178,9 +178,9 @@ pwa_status pwa_data_term_enqueue(pwa_ctx *ctx, const double *V, double *out_dev)
  * served, the grid is capped at 1024 blocks).  The call issues one 256-byte cudaMemsetAsync and one kernel launch and
  * calls no cudaMalloc / cudaFree / allocating library routine; its first call on a device looks up the array's address
  * (do that once before a capture).  Every call shares the array: calls that OVERLAP on the GPU (different streams, or
- * several host threads) race and return wrong sums; calls on one stream are ordered and safe.  A plain one-event-
- * per-thread kernel (no TMA, no event weights, constant resonances only): slower than the context path, bitwise
- * reproducible for a fixed shape.  errbuf (HOST, errbuf_len bytes, may be NULL) receives the error text.              */
+ * several host threads) race and return wrong sums; calls on one stream are ordered and safe.  A plain lane-group
+ * streaming kernel (no TMA, no event weights, constant resonances only; amps_dev 16-byte aligned): ~1.3 TB/s at
+ * 5e6 events x 64 waves fp32, about a fifth of the context path's rate; bitwise reproducible for a fixed shape.  errbuf (HOST, errbuf_len bytes, may be NULL) receives the error text.              */
 #define PWA_STATIC_MAX_WAVES 64
 pwa_status pwa_data_term_static(int32_t device, void *cuda_stream, pwa_dtype storage, int32_t n_waves,
                                 const void *amps_dev, int64_t n_events, const double *V, double *out_dev,

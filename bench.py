@@ -147,6 +147,16 @@ def sizes_for(args, spec):
     return int(n_data), int(n_mc)
 
 
+def workload_config(workload, n, n_data, storage, ws, backend):
+    """The `config` object of the JSON line: the same for our arm and for the reference arm (which times the oracle on a
+    bounded sample of exactly this workload)."""
+    bytes_data = n_data * n * 2 * (8 if storage == "f64" else 4)
+    return {"workload": workload, "n_waves": n, "n_data_per_gpu": n_data, "storage": storage,
+            "parallelism": (f"event-sharded x{ws}" + ("" if backend == "nccl" else f" ({backend} exchange, test mode)")) if ws > 1 else "single GPU",
+            "l2": f"input {bytes_data / 1e6:.0f} MB per step vs 126 MB L2: "
+                  + ("larger than L2, no flush needed" if bytes_data > 2.5e8 else "L2-RESIDENT (latency-bound config)")}
+
+
 # --------------------------------------------------------------------------- reference arm
 def oracle_sample_size(oracle, A, M, V, n_total, target_s):
     """Largest prefix of the data whose oracle evaluation takes about target_s seconds."""
@@ -200,8 +210,8 @@ def run_reference(args):
         "unit": "event-waves/s", "n_gpus": args.gpus, "steps": K, "warmup": W,
         "ms_per_step": dt / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "n_waves": w.n, "n_data": n_data, "storage": w.storage,
-                   "sample_events": S},
+        "config": workload_config(args.workload, w.n, n_data, w.storage, ws, os.environ.get("PWA_BENCH_BACKEND", "nccl")),   # our arm's config
+        "sample_events": S,
         "evals_per_s": K / dt * (S / n_data),
         "cpu_baseline": {"value": value, "unit": "event-waves/s", "cores": oracle.threads(), "kind": "oracle",
                          "sample": sample},
@@ -742,10 +752,7 @@ def run_ours(args):
         "metric": "event-waves/s (lnL+gradient evaluation)", "value": units / ms * 1e3, "unit": "event-waves/s",
         "n_gpus": ws, "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "n_waves": n, "n_data_per_gpu": w.n_data, "storage": w.storage,
-                   "parallelism": (f"event-sharded x{ws}" + ("" if backend == "nccl" else f" ({backend} exchange, test mode)")) if ws > 1 else "single GPU",
-                   "l2": f"input {bytes_data / 1e6:.0f} MB per step vs 126 MB L2: "
-                         + ("larger than L2, no flush needed" if bytes_data > 2.5e8 else "L2-RESIDENT (latency-bound config)")},
+        "config": workload_config(args.workload, n, w.n_data, w.storage, ws, backend),
         "evals_per_s": 1e3 / ms,
         "e2e": {"value": units / wall_ms * 1e3, "unit": "event-waves/s", "ms_per_step": wall_ms,
                 "evals_per_s": 1e3 / wall_ms, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 8 * (4 + 2 * n),
